@@ -1,0 +1,205 @@
+"""oracle — CPU oracle of the GALE relation hot path. TEST INFRASTRUCTURE ONLY.
+
+ctypes wrapper over oracle/gale_oracle.cpp (plain single-threaded C++; see its header for the
+definitions, citations and pins). Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference leg may import this package. It never imports the CUDA package
+(paper_2507_15230_b200) and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gale_oracle.cpp")
+_LIB = os.path.join(_HERE, "libgale_oracle.so")
+_lib = None
+
+REL_VT, REL_VV, REL_TT = 1, 2, 4
+
+
+def build(force: bool = False) -> str:
+    """Compile gale_oracle.cpp -> libgale_oracle.so (g++ -O2, host only, no SIMD tricks)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        vp, i64, c_int, u32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_uint32
+        i32p, i64p = ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int64)
+        lib.go_compute_global.restype = vp
+        lib.go_compute_global.argtypes = [c_int, i64, i64, i32p, u32]
+        lib.go_status.restype = c_int
+        lib.go_status.argtypes = [vp]
+        lib.go_free.restype = None
+        lib.go_free.argtypes = [vp]
+        for name, rt in [("go_vt_offsets", i64p), ("go_vt_indices", i32p), ("go_vv_offsets", i64p),
+                         ("go_vv_indices", i32p), ("go_tt", i32p), ("go_first_tet", i64p)]:
+            getattr(lib, name).restype = rt
+            getattr(lib, name).argtypes = [vp]
+        lib.go_vv_nnz.restype = i64
+        lib.go_vv_nnz.argtypes = [vp]
+        lib.go_compute_restricted.restype = vp
+        lib.go_compute_restricted.argtypes = [c_int, i64, i64, i32p, ctypes.c_int32, i32p, ctypes.c_int32, i32p, u32]
+        lib.go_sub_relations.restype = vp
+        lib.go_sub_relations.argtypes = [vp]
+        lib.go_sub_gid.restype = i32p
+        lib.go_sub_gid.argtypes = [vp]
+        lib.go_sub_size.restype = i64
+        lib.go_sub_size.argtypes = [vp]
+        lib.go_sub_free.restype = None
+        lib.go_sub_free.argtypes = [vp]
+        lib.go_slice_rows.restype = i64
+        lib.go_slice_rows.argtypes = [i64p, i32p, i64, i64, i32p, i32p, i32p]
+        lib.go_slice_tt.restype = None
+        lib.go_slice_tt.argtypes = [i32p, c_int, i64, i64, i32p, i32p]
+        lib.go_brute_vt.restype = None
+        lib.go_brute_vt.argtypes = [c_int, i64, i64, i32p, i64p, i32p]
+        lib.go_brute_vv.restype = None
+        lib.go_brute_vv.argtypes = [c_int, i64, i64, i32p, i64p, i32p]
+        lib.go_brute_tt.restype = c_int
+        lib.go_brute_tt.argtypes = [c_int, i64, i32p, i32p]
+        _lib = lib
+    return _lib
+
+
+def _i32(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+
+
+def _i64(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))
+
+
+def _np(ptr, n, dtype):
+    if n == 0:
+        return np.empty(0, dtype)
+    return np.ctypeslib.as_array(ptr, shape=(n,)).astype(dtype, copy=True)
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def _canon(T):
+    T = np.ascontiguousarray(T, dtype=np.int32)
+    assert T.ndim == 2 and T.shape[1] in (3, 4)
+    return T
+
+
+def relations_global(dim: int, num_vertices: int, simplices: np.ndarray, mask: int = 7) -> dict:
+    """Global VT / VV (CSR, int64 offsets) and TT ([nT, D]) straight from the definitions."""
+    lib = _load()
+    T = _canon(simplices)
+    D, nT, nV = dim + 1, T.shape[0], int(num_vertices)
+    h = lib.go_compute_global(dim, nV, nT, _i32(T), mask)
+    try:
+        st = lib.go_status(h)
+        if st != 0:
+            raise OracleError(f"oracle input contract violated: status {st}")
+        out = dict(first_tet=_np(lib.go_first_tet(h), nV + 1, np.int64))
+        if mask & REL_VT:
+            out["vt_off"] = _np(lib.go_vt_offsets(h), nV + 1, np.int64)
+            out["vt_idx"] = _np(lib.go_vt_indices(h), nT * D, np.int32)
+        if mask & REL_VV:
+            out["vv_off"] = _np(lib.go_vv_offsets(h), nV + 1, np.int64)
+            out["vv_idx"] = _np(lib.go_vv_indices(h), int(lib.go_vv_nnz(h)), np.int32)
+        if mask & REL_TT:
+            out["tt"] = _np(lib.go_tt(h), nT * D, np.int32).reshape(nT, D)
+        return out
+    finally:
+        lib.go_free(h)
+
+
+def _slice_clusters(lib, h, D, offsets, clusters, mask, first_tet, gid, gid_first_tet):
+    """Per-cluster results: VT/VV rows of the cluster's vertices, TT rows of its
+    internal simplices; ids global; CSR offsets int32 starting at 0."""
+    res = []
+    gp = _i32(gid) if gid is not None else None
+    for c in clusters:
+        lo, hi = int(offsets[c]), int(offsets[c + 1])
+        r = dict(cluster=int(c), v_lo=lo, v_hi=hi)
+        for key, bit, fo, fi in (("vt", REL_VT, lib.go_vt_offsets, lib.go_vt_indices),
+                                 ("vv", REL_VV, lib.go_vv_offsets, lib.go_vv_indices)):
+            if not mask & bit:
+                continue
+            off = np.empty(hi - lo + 1, np.int32)
+            nnz = int(lib.go_slice_rows(fo(h), fi(h), lo, hi, None, _i32(off), None))
+            idx = np.empty(nnz, np.int32)
+            lib.go_slice_rows(fo(h), fi(h), lo, hi, gp if key == "vt" else None, _i32(off), _i32(idx))
+            r[key] = (off, idx)
+        # internal simplices: contiguous range by C2 (I_T)
+        t_lo, t_hi = int(first_tet[lo]), int(first_tet[hi])          # ids in the handle's mesh
+        r["t_lo"] = int(gid_first_tet[lo])                           # global id of the first internal simplex
+        r["t_hi"] = r["t_lo"] + (t_hi - t_lo)
+        if mask & REL_TT:
+            tt = np.empty((t_hi - t_lo, D), np.int32)
+            lib.go_slice_tt(lib.go_tt(h), D, t_lo, t_hi, gp, _i32(tt))
+            r["tt"] = tt
+        res.append(r)
+    return res
+
+
+def cluster_results(dim: int, num_vertices: int, simplices: np.ndarray, cluster_offsets: np.ndarray,
+                    clusters, mask: int = 7, restricted: bool = False) -> list:
+    """Oracle output for each cluster id in `clusters`, in that order.
+
+    restricted=False: global pass then slice. restricted=True: the definitions on the sub-mesh of
+    simplices meeting the selection's vertex closure (exact; see gale_oracle.cpp) — for meshes too
+    large for a global pass.
+    """
+    lib = _load()
+    T = _canon(simplices)
+    D, nT, nV = dim + 1, T.shape[0], int(num_vertices)
+    offsets = np.ascontiguousarray(cluster_offsets, dtype=np.int32)
+    clusters = [int(c) for c in clusters]
+    # first_tet of the *global* mesh (needed to name the internal range in global ids)
+    gfirst = np.searchsorted(T[:, 0], np.arange(nV + 1), side="left").astype(np.int64) if nT else np.zeros(nV + 1, np.int64)
+    if not restricted:
+        h = lib.go_compute_global(dim, nV, nT, _i32(T), mask)
+        try:
+            if lib.go_status(h) != 0:
+                raise OracleError(f"oracle input contract violated: status {lib.go_status(h)}")
+            first = _np(lib.go_first_tet(h), nV + 1, np.int64)
+            return _slice_clusters(lib, h, D, offsets, clusters, mask, first, None, gfirst)
+        finally:
+            lib.go_free(h)
+    sel = np.asarray(sorted(set(clusters)), np.int32)
+    s = lib.go_compute_restricted(dim, nV, nT, _i32(T), len(offsets) - 1, _i32(offsets), len(sel), _i32(sel), mask)
+    try:
+        h = lib.go_sub_relations(s)
+        if lib.go_status(h) != 0:
+            raise OracleError(f"oracle input contract violated: status {lib.go_status(h)}")
+        gid = _np(lib.go_sub_gid(s), int(lib.go_sub_size(s)), np.int32)
+        first = _np(lib.go_first_tet(h), nV + 1, np.int64)
+        return _slice_clusters(lib, h, D, offsets, clusters, mask, first, gid, gfirst)
+    finally:
+        lib.go_sub_free(s)
+
+
+def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:
+    """Brute-force enumeration of VT, VV, TT for tiny meshes (membership scans only)."""
+    lib = _load()
+    T = _canon(simplices)
+    D, nT, nV = dim + 1, T.shape[0], int(num_vertices)
+    vt_off = np.empty(nV + 1, np.int64)
+    vt_idx = np.empty(nT * D, np.int32)
+    lib.go_brute_vt(dim, nV, nT, _i32(T), _i64(vt_off), _i32(vt_idx))
+    vv_off = np.empty(nV + 1, np.int64)
+    vv_idx = np.empty(nT * D * (D - 1), np.int32)
+    lib.go_brute_vv(dim, nV, nT, _i32(T), _i64(vv_off), _i32(vv_idx))
+    tt = np.empty((nT, D), np.int32)
+    st = lib.go_brute_tt(dim, nT, _i32(T), _i32(tt))
+    if st != 0:
+        raise OracleError(f"non-manifold facet (status {st})")
+    return dict(vt_off=vt_off, vt_idx=vt_idx[:vt_off[-1]].copy(), vv_off=vv_off,
+                vv_idx=vv_idx[:vv_off[-1]].copy(), tt=tt)

@@ -1,0 +1,257 @@
+"""Pins of the CPU oracle against things other than itself (SURVEY.md §8(c) pin table).
+
+Each test is chosen so that a plausible mistake in oracle/gale_oracle.cpp (dropped term, wrong
+index, transposed operand, self not excluded, wrong facet <-> opposite-vertex order) fails it.
+All CPU-only.
+"""
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+
+import meshgen
+import oracle
+
+
+def rows(off, idx):
+    return [idx[off[i]:off[i + 1]].tolist() for i in range(len(off) - 1)]
+
+
+# ---------------------------------------------------------------- golden: Fig. 1 toy
+def _read_fig1(golden_dir):
+    simp, exp = [], {"VV": {}, "VT": {}, "TT": {}}
+    for line in open(os.path.join(golden_dir, "fig1_toy.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        head, vals = line.split(":")
+        head = head.split()
+        vals = [int(x) for x in vals.split()]
+        if head[0] == "simplices":
+            simp.append(vals)
+        else:
+            exp[head[1]][int(head[2])] = vals
+    return np.array(simp, np.int32), exp
+
+
+def test_fig1_toy_golden(golden_dir):
+    T, exp = _read_fig1(golden_dir)
+    R = oracle.relations_global(3, 5, T)
+    vv, vt = rows(R["vv_off"], R["vv_idx"]), rows(R["vt_off"], R["vt_idx"])
+    assert vv[0] == [1, 2, 3]                      # the value the paper prints
+    for v, e in exp["VV"].items():
+        assert vv[v] == e
+    for v, e in exp["VT"].items():
+        assert vt[v] == e
+    for t, e in exp["TT"].items():
+        assert R["tt"][t].tolist() == e
+
+
+# ---------------------------------------------------------------- brute force on tiny meshes
+TINY = [
+    dict(dim=3, n=4),
+    dict(dim=3, n=5, drop_frac=0.15),
+    dict(dim=3, n=5, clustering="octree", capacity=20, permute=True),
+    dict(dim=3, n=5, clustering="octree", capacity=16, warp=True, drop_frac=0.3),
+    dict(dim=2, n=8, clustering="morton", block=4),
+    dict(dim=2, n=9, clustering="octree", capacity=10, permute=True, drop_frac=0.2),
+]
+
+
+@pytest.mark.parametrize("spec", TINY)
+def test_brute_force(spec):
+    spec = dict(spec)
+    if spec.get("clustering", "morton") == "morton":
+        spec.setdefault("block", 2 if spec["n"] % 2 == 0 else 1)
+        if spec["n"] & (spec["n"] - 1):
+            spec.update(clustering="octree", capacity=12)
+    m = meshgen.make_mesh(seed=1234, **spec)
+    R = oracle.relations_global(m.dim, m.num_vertices, m.simplices)
+    B = oracle.brute_force(m.dim, m.num_vertices, m.simplices)
+    for k in ("vt_off", "vt_idx", "vv_off", "vv_idx", "tt"):
+        assert np.array_equal(R[k], B[k]), k
+
+
+# ---------------------------------------------------------------- library pins (scipy.sparse)
+@pytest.mark.parametrize("dim,n", [(3, 9), (2, 20)])
+def test_scipy_incidence(dim, n):
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=64, permute=True, drop_frac=0.1, seed=77)
+    T, nV, nT, D = m.simplices, m.num_vertices, m.num_simplices, dim + 1
+    R = oracle.relations_global(dim, nV, T)
+    # B = V x T incidence matrix
+    B = sp.csr_matrix((np.ones(nT * D, np.int32), (T.ravel(), np.repeat(np.arange(nT), D))), shape=(nV, nT))
+    B.sort_indices()
+    # VT = CSR of B (= transpose of the T x V list)
+    assert np.array_equal(B.indptr, R["vt_off"]) and np.array_equal(B.indices, R["vt_idx"])
+    # VV = pattern of B B^T minus the diagonal
+    A = (B @ B.T).tolil()
+    A.setdiag(0)
+    A = A.tocsr()
+    A.eliminate_zeros()
+    A.sort_indices()
+    assert np.array_equal(A.indptr, R["vv_off"]) and np.array_equal(A.indices, R["vv_idx"])
+    # TT neighbour *sets* = pairs of simplices sharing exactly D-1 vertices
+    S = (B.T @ B).tocoo()
+    keep = (S.data == D - 1) & (S.row != S.col)
+    N = sp.csr_matrix((np.ones(keep.sum(), np.int8), (S.row[keep], S.col[keep])), shape=(nT, nT))
+    N.sort_indices()
+    for t in range(nT):
+        got = sorted(x for x in R["tt"][t].tolist() if x >= 0)
+        assert got == N.indices[N.indptr[t]:N.indptr[t + 1]].tolist()
+
+
+# ---------------------------------------------------------------- closed forms, Euler, degrees
+def _closed_forms(golden_dir):
+    out = []
+    for line in open(os.path.join(golden_dir, "kuhn_closed_forms.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        d, n, V, T, E, F, b = line.split()
+        out.append((int(d), int(n), int(V), int(T), int(E), None if F == "-" else int(F), int(b)))
+    return out
+
+
+def test_kuhn_closed_forms_and_euler(golden_dir):
+    for dim, n, V, nT, E, F, bnd in _closed_forms(golden_dir):
+        D = dim + 1
+        m = meshgen.make_mesh(dim, n, clustering="octree", capacity=50, seed=5)
+        assert (m.num_vertices, m.num_simplices) == (V, nT)
+        R = oracle.relations_global(dim, V, m.simplices)
+        assert R["vt_off"][-1] == D * nT                      # sum |VT| = D * #simplices
+        assert R["vv_off"][-1] == 2 * E                       # sum |VV| = 2 E
+        nb = int((R["tt"] < 0).sum())
+        assert nb == bnd                                      # boundary facets
+        if dim == 3:
+            assert (D * nT + nb) // 2 == F
+            assert V - E + F - nT == 1                        # Euler characteristic of a ball
+        else:
+            assert (D * nT + nb) // 2 == E                    # facets of a 2-D mesh are its edges
+            assert V - E + nT == 1
+        # no -1 inside VT / VV rows, self never in VV
+        assert R["vt_idx"].min() >= 0 and R["vv_idx"].min() >= 0
+        src = np.repeat(np.arange(V), np.diff(R["vv_off"]))
+        assert not np.any(src == R["vv_idx"])
+
+
+@pytest.mark.parametrize("dim,n,dvt,dvv", [(3, 7, 24, 14), (2, 12, 6, 6)])
+def test_interior_kuhn_degrees(dim, n, dvt, dvv):
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=40, permute=True, seed=9)
+    R = oracle.relations_global(dim, m.num_vertices, m.simplices)
+    g2f = m.meta["grid_to_final"]
+    g = np.arange(n ** dim)
+    coords = np.stack([(g // n ** a) % n for a in range(dim)], 1)
+    interior = np.all((coords > 0) & (coords < n - 1), axis=1)
+    vs = g2f[interior]
+    assert np.all(np.diff(R["vt_off"])[vs] == dvt)
+    assert np.all(np.diff(R["vv_off"])[vs] == dvv)
+
+
+# ---------------------------------------------------------------- structural invariants of TT
+@pytest.mark.parametrize("dim,n,drop", [(3, 10, 0.0), (3, 10, 0.15), (2, 30, 0.15)])
+def test_tt_symmetry_and_shared_facet(dim, n, drop):
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=100, drop_frac=drop, seed=3)
+    T, D = m.simplices, dim + 1
+    tt = oracle.relations_global(dim, m.num_vertices, T, mask=oracle.REL_TT)["tt"]
+    for k in range(D):
+        t = np.nonzero(tt[:, k] >= 0)[0]
+        s = tt[t, k]
+        assert np.all(s != t)
+        facet = np.delete(T[t], k, axis=1)                    # T[t] minus its k-th vertex
+        # every facet vertex lies in the neighbour, and the neighbour points back through the same facet
+        for j in range(D - 1):
+            assert np.all((T[s] == facet[:, j:j + 1]).any(axis=1))
+        back = (tt[s] == t[:, None])
+        assert np.all(back.sum(axis=1) == 1)
+        kk = back.argmax(axis=1)
+        other = np.stack([np.delete(T[si], ki) for si, ki in zip(s, kk)]) if len(s) else facet
+        assert np.array_equal(other, facet)
+        # |T[t] ∩ T[s]| = D-1 exactly
+        inter = sum((T[t][:, a:a + 1] == T[s]).any(axis=1).astype(int) for a in range(D))
+        assert np.all(inter == D - 1)
+
+
+def test_vv_symmetry_and_star_union():
+    m = meshgen.make_mesh(3, 8, clustering="octree", capacity=64, warp=True, drop_frac=0.1, seed=11)
+    R = oracle.relations_global(3, m.num_vertices, m.simplices)
+    vv, vt = rows(R["vv_off"], R["vv_idx"]), rows(R["vt_off"], R["vt_idx"])
+    pairs = {(v, u) for v in range(m.num_vertices) for u in vv[v]}
+    assert all((u, v) in pairs for (v, u) in pairs)
+    for v in range(m.num_vertices):                          # VV(v) = union of VT(v)'s vertices minus v
+        star = set(m.simplices[vt[v]].ravel().tolist()) - {v}
+        assert sorted(star) == vv[v]
+
+
+# ---------------------------------------------------------------- clustering independence
+def test_clustering_independence():
+    a = meshgen.make_mesh(3, 8, clustering="morton", block=4, seed=21, keep_fields=True)
+    b = meshgen.make_mesh(3, 8, clustering="octree", capacity=30, permute=True, seed=22, keep_fields=True)
+    Ra = oracle.relations_global(3, a.num_vertices, a.simplices)
+    Rb = oracle.relations_global(3, b.num_vertices, b.simplices)
+    ga, gb = a.meta["grid_to_final"], b.meta["grid_to_final"]
+    a2b = np.empty_like(ga)
+    a2b[ga] = gb                                              # vertex id in a -> vertex id in b
+    # simplex id in a -> simplex id in b via the canonical row
+    key = lambda T: [tuple(r) for r in T.tolist()]
+    where_b = {r: i for i, r in enumerate(key(b.simplices))}
+    ta2b = np.array([where_b[tuple(sorted(a2b[r].tolist()))] for r in a.simplices])
+    vva, vvb = rows(Ra["vv_off"], Ra["vv_idx"]), rows(Rb["vv_off"], Rb["vv_idx"])
+    vta, vtb = rows(Ra["vt_off"], Ra["vt_idx"]), rows(Rb["vt_off"], Rb["vt_idx"])
+    for v in range(a.num_vertices):
+        assert sorted(a2b[vva[v]].tolist()) == vvb[a2b[v]]
+        assert sorted(ta2b[vta[v]].tolist()) == vtb[a2b[v]]
+    for t in range(a.num_simplices):
+        na = {int(ta2b[x]) for x in Ra["tt"][t] if x >= 0}
+        nb = {int(x) for x in Rb["tt"][ta2b[t]] if x >= 0}
+        assert na == nb
+
+
+# ---------------------------------------------------------------- per-cluster slices
+def test_cluster_slices_cover_global_once():
+    m = meshgen.make_config(4, n=20)
+    G = oracle.relations_global(3, m.num_vertices, m.simplices)
+    res = oracle.cluster_results(3, m.num_vertices, m.simplices, m.cluster_offsets, range(m.num_clusters))
+    vt_i = np.concatenate([r["vt"][1] for r in res])
+    vv_i = np.concatenate([r["vv"][1] for r in res])
+    tt = np.concatenate([r["tt"] for r in res])
+    assert np.array_equal(vt_i, G["vt_idx"]) and np.array_equal(vv_i, G["vv_idx"]) and np.array_equal(tt, G["tt"])
+    t_next = 0
+    for r in res:                                            # internal ranges tile [0, nT) in order
+        assert r["t_lo"] == t_next and r["tt"].shape[0] == r["t_hi"] - r["t_lo"]
+        t_next = r["t_hi"]
+        assert r["vt"][0][0] == 0 and r["vt"][0][-1] == len(r["vt"][1])
+        if r["t_hi"] > r["t_lo"]:                            # internal iff lowest vertex in the cluster
+            v0 = m.simplices[r["t_lo"]:r["t_hi"], 0]
+            assert v0.min() >= r["v_lo"] and v0.max() < r["v_hi"]
+    assert t_next == m.num_simplices
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 24), (4, 24), (2, 96), (1, None)])
+def test_restricted_equals_global_slice(cfg, n):
+    m = meshgen.make_config(cfg, n=n)
+    rng = np.random.default_rng(cfg)
+    sel = rng.choice(m.num_clusters, size=min(5, m.num_clusters), replace=False).tolist()
+    a = oracle.cluster_results(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, sel)
+    b = oracle.cluster_results(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, sel, restricted=True)
+    for ra, rb in zip(a, b):
+        assert (ra["t_lo"], ra["t_hi"]) == (rb["t_lo"], rb["t_hi"])
+        for k in ("vt", "vv"):
+            assert np.array_equal(ra[k][0], rb[k][0]) and np.array_equal(ra[k][1], rb[k][1])
+        assert np.array_equal(ra["tt"], rb["tt"])
+
+
+# ---------------------------------------------------------------- contract violations are refused
+def test_rejects_bad_input():
+    m = meshgen.make_mesh(3, 4, seed=2, block=2)
+    T = m.simplices.copy()
+    T[[3, 4]] = T[[4, 3]]                                     # rows out of lexicographic order
+    with pytest.raises(oracle.OracleError):
+        oracle.relations_global(3, m.num_vertices, T)
+    T = m.simplices.copy()
+    T[0, 0], T[0, 1] = T[0, 1], T[0, 0]                       # row not ascending
+    with pytest.raises(oracle.OracleError):
+        oracle.relations_global(3, m.num_vertices, T)
+    # three triangles on one edge: non-manifold facet
+    T = np.array([[0, 1, 2], [0, 1, 3], [0, 1, 4]], np.int32)
+    with pytest.raises(oracle.OracleError):
+        oracle.relations_global(2, 5, T)
