@@ -1,0 +1,159 @@
+/* gale.h — C ABI of the B200-native GALE relation hot path.
+ *
+ * What it computes (PAPER.md = /root/reference/PAPER.md, arXiv 2507.15230):
+ *   GALE's "worker producers" (PAPER.md:160 §4.2, :226-280 §4.6, Alg. 1 :232-250): for a batch of
+ *   mesh segments ("clusters"), the coboundary relation VT and the adjacency relations VV and TT
+ *   (§2.2, Table 1 :53-58), delivered to the consumer side through a bounded queue of
+ *   pre-allocated buffers (PAPER.md:158 leader producer; :208 "pre-allocates sufficient GPU memory").
+ *   Readings of everything the paper leaves open are listed in DESIGN.md §Readings.
+ *
+ * Input contract ("canonical mesh"): D = dim+1 vertex ids per simplex, int32;
+ *   (C1) each row strictly ascending, (C2) rows strictly ascending lexicographically,
+ *   (C3) ids in [0, num_vertices), (C4) every facet has at most two cofaces.
+ *   Cluster c owns the vertices [o[c], o[c+1]) (I_V, Alg. 1 line 3 :243) and the
+ *   *internal* simplices {t : o[c] <= T[t][0] < o[c+1]}, a contiguous id range by C2.
+ *
+ * Output per cluster, canonical sorted CSR, all stored ids GLOBAL:
+ *   VT rows v = o[c]..o[c+1]-1 : ascending ids of the simplices containing v (internal + external);
+ *   VV rows v                  : ascending ids of the distinct vertices u != v sharing a simplex with v;
+ *   TT rows t in I_T[c]        : D entries; entry k = the simplex sharing the facet opposite the k-th
+ *                                smallest vertex of t, or -1 on the boundary.
+ *
+ * No CPU fallback exists: without an sm_100 CUDA device every compute entry returns
+ * GALE_ERR_UNSUPPORTED / GALE_ERR_CUDA. No exception crosses this boundary.
+ * Thread-safety: one producer thread (compute) + one consumer thread (pop/release) per handle.
+ */
+#ifndef GALE_H_
+#define GALE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gale_mesh gale_mesh_t; /* opaque; owned by the library, freed by gale_destroy */
+
+enum { GALE_REL_VT = 1, GALE_REL_VV = 2, GALE_REL_TT = 4, GALE_REL_ALL = 7 };
+
+enum {
+  GALE_OK = 0,
+  GALE_ERR_INVALID_ARG = -1,   /* null pointer, bad dim, relation_mask == 0, ...                      */
+  GALE_ERR_NOT_CANONICAL = -2, /* C1-C3 violated (checked when GALE_VALIDATE is set)                  */
+  GALE_ERR_DEGENERATE = -3,    /* reserved                                                            */
+  GALE_ERR_NONMANIFOLD = -4,   /* C4 violated (checked when GALE_VALIDATE_MANIFOLD is set)            */
+  GALE_ERR_BAD_CLUSTER = -5,   /* cluster id out of range, or n_clusters > max_batch_clusters         */
+  GALE_ERR_WOULD_BLOCK = -6,   /* every queue slot is un-released (compute), or timeout (pop)         */
+  GALE_ERR_EMPTY = -7,         /* pop with nothing in flight                                          */
+  GALE_ERR_WORKSPACE = -8,     /* workspace too small / misaligned, or a device capacity guard fired  */
+  GALE_ERR_CUDA = -9,          /* a CUDA call failed; see gale_last_error()                           */
+  GALE_ERR_UNSUPPORTED = -10   /* no sm_100 device, or a vertex star too large for shared memory      */
+};
+
+enum {
+  GALE_VALIDATE = 1u,          /* check C1-C3 and the cluster offsets at create (one pass)            */
+  GALE_VALIDATE_MANIFOLD = 2u  /* also check C4 (facet pass, slower)                                  */
+};
+
+typedef struct {
+  int32_t dim;                      /* 3 = tetrahedra, 2 = triangles                                  */
+  int32_t num_vertices;
+  int64_t num_simplices;            /* every simplex id must fit int32                                */
+  const int32_t *d_simplices;       /* DEVICE, [num_simplices*(dim+1)], canonical, 16-byte aligned;
+                                       caller-owned, must outlive the handle, never written          */
+  int32_t num_clusters;
+  const int32_t *h_cluster_offsets; /* HOST, [num_clusters+1], I_V: 0 = o[0] <= ... <= o[nC] = nV;
+                                       read during create only                                       */
+  int32_t max_batch_clusters;       /* largest n_clusters of one compute call (e.g. 64)               */
+  int32_t queue_depth;              /* > 0: that many pinned HOST result slots, results are copied
+                                       D2H on a library-owned side stream;
+                                       0: results stay in a ring of device slots (benchmark mode)     */
+  int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4);
+                                       a popped view stays valid until device_ring-1 later batches
+                                       have been submitted                                            */
+  int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = default)           */
+  void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
+                                       must outlive the handle                                       */
+  size_t workspace_bytes;
+  uint32_t flags;                   /* GALE_VALIDATE | GALE_VALIDATE_MANIFOLD                         */
+} gale_mesh_desc_t;
+
+/* One finished batch. cluster_ids and *_row_begin are HOST arrays owned by the library; offsets and
+ * indices live in the slot: pinned HOST memory when queue_depth > 0, DEVICE memory when 0
+ * (on_device tells which). Everything stays valid until gale_queue_release (queue_depth > 0) or
+ * until device_ring-1 later batches are submitted (queue_depth == 0).
+ * Rows of the i-th requested cluster are [row_begin[i], row_begin[i+1]); offsets are batch-relative
+ * (offsets[0] = 0, non-decreasing, offsets[rows] = nnz). TT rows have constant length dim+1. */
+typedef struct {
+  int64_t sequence;              /* submission order, from 0                                         */
+  int32_t n_clusters;
+  uint32_t relation_mask;
+  int32_t dim;
+  int32_t on_device;
+  const int32_t *cluster_ids;    /* HOST [n_clusters], as passed to compute                          */
+  const int32_t *vt_row_begin;   /* HOST [n_clusters+1] (also the VV row partition)                  */
+  const int32_t *tt_row_begin;   /* HOST [n_clusters+1]                                              */
+  int64_t vt_rows, vt_nnz;
+  const int32_t *vt_offsets;     /* [vt_rows+1] or NULL when VT was not requested                    */
+  const int32_t *vt_indices;     /* [vt_nnz]                                                         */
+  int64_t vv_rows, vv_nnz;
+  const int32_t *vv_offsets;     /* [vv_rows+1] or NULL                                              */
+  const int32_t *vv_indices;     /* [vv_nnz]                                                         */
+  int64_t tt_rows;
+  const int32_t *tt_indices;     /* [tt_rows*(dim+1)] or NULL                                        */
+  float kernel_ms;               /* CUDA-event time of this batch's kernel                           */
+  int32_t slot;                  /* internal: pass the view back unchanged to gale_queue_release     */
+} gale_batch_view_t;
+
+/* Init statistics ("Initialization"), for reporting. */
+typedef struct {
+  int32_t tile_vertices, num_tiles;
+  int64_t num_external_refs;     /* total length of the per-tile T_ex lists                          */
+  int64_t vt_nnz, vv_nnz;        /* whole-mesh totals                                                */
+  int32_t smem_bytes;            /* dynamic shared memory per thread block of the batch kernel       */
+  int32_t max_staged;            /* largest per-tile staged simplex count                            */
+  size_t slot_bytes;             /* bytes of one result slot                                         */
+  size_t workspace_used;
+  double create_ms;
+} gale_mesh_info_t;
+
+/* Upper bound of the device workspace gale_mesh_create needs for this descriptor
+ * (d_workspace / workspace_bytes are ignored). Cheap: reads the counts only. */
+int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t *desc, size_t *out_bytes);
+
+/* Initialization: validates, builds I_T (first simplex of every vertex), the
+ * per-tile external lists T_ex, the index used to resolve cross-cluster facets, the per-tile output
+ * sizes, and uploads them into the workspace. Work is enqueued on cuda_stream (a cudaStream_t,
+ * 0 = default stream) and finished (synchronised) on return. *out is set on GALE_OK only. */
+int32_t gale_mesh_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_mesh_t **out);
+
+int32_t gale_mesh_info(const gale_mesh_t *mesh, gale_mesh_info_t *out);
+
+/* Producer side: enqueue the relation kernels for the clusters
+ * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) on cuda_stream and,
+ * when queue_depth > 0, the D2H copy into a pinned slot on the library's side stream.
+ * Asynchronous w.r.t. the host. Returns GALE_ERR_WOULD_BLOCK when all slots are un-released. */
+int32_t gale_cluster_batch_compute(gale_mesh_t *mesh, uint32_t relation_mask, const int32_t *h_cluster_ids,
+                                   int32_t n_clusters, void *cuda_stream);
+
+/* Consumer side: wait (up to timeout_ms; < 0 = forever) for the oldest submitted batch and
+ * describe it in *out. Batches pop in submission order. GALE_ERR_EMPTY if nothing is in flight,
+ * GALE_ERR_WOULD_BLOCK on timeout, GALE_ERR_WORKSPACE if a device-side capacity guard fired. */
+int32_t gale_queue_pop(gale_mesh_t *mesh, gale_batch_view_t *out, int32_t timeout_ms);
+
+/* Give a popped slot back to the queue (no-op when queue_depth == 0). */
+int32_t gale_queue_release(gale_mesh_t *mesh, const gale_batch_view_t *view);
+
+/* Drains in-flight work, frees pinned memory, streams and events. The workspace and the simplex
+ * array stay the caller's. */
+int32_t gale_destroy(gale_mesh_t *mesh);
+
+const char *gale_status_string(int32_t status);
+/* Text of the last CUDA failure seen by this thread's calls ("" if none). */
+const char *gale_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GALE_H_ */

@@ -1,0 +1,272 @@
+"""paper_2507_15230_b200 — Python binding of the B200-native GALE relation hot path.
+
+Thin ctypes marshalling over the C ABI in include/gale.h (csrc/libgale.so): every relation entry is
+computed by the CUDA kernels in csrc/gale_kernels.cuh. PyTorch only provides device memory and
+streams. There is no CPU fallback: if libgale.so is missing or no sm_100 device is present the calls
+raise GaleError.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from .build import LIB, build_library
+
+REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
+VALIDATE, VALIDATE_MANIFOLD = 1, 2
+OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
+ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
+
+_i32p = ctypes.POINTER(ctypes.c_int32)
+
+
+class gale_mesh_desc_t(ctypes.Structure):
+    _fields_ = [("dim", ctypes.c_int32), ("num_vertices", ctypes.c_int32), ("num_simplices", ctypes.c_int64),
+                ("d_simplices", ctypes.c_void_p), ("num_clusters", ctypes.c_int32),
+                ("h_cluster_offsets", _i32p), ("max_batch_clusters", ctypes.c_int32),
+                ("queue_depth", ctypes.c_int32), ("device_ring", ctypes.c_int32), ("tile_vertices", ctypes.c_int32),
+                ("d_workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t), ("flags", ctypes.c_uint32)]
+
+
+class gale_batch_view_t(ctypes.Structure):
+    _fields_ = [("sequence", ctypes.c_int64), ("n_clusters", ctypes.c_int32), ("relation_mask", ctypes.c_uint32),
+                ("dim", ctypes.c_int32), ("on_device", ctypes.c_int32),
+                ("cluster_ids", _i32p), ("vt_row_begin", _i32p), ("tt_row_begin", _i32p),
+                ("vt_rows", ctypes.c_int64), ("vt_nnz", ctypes.c_int64),
+                ("vt_offsets", ctypes.c_void_p), ("vt_indices", ctypes.c_void_p),
+                ("vv_rows", ctypes.c_int64), ("vv_nnz", ctypes.c_int64),
+                ("vv_offsets", ctypes.c_void_p), ("vv_indices", ctypes.c_void_p),
+                ("tt_rows", ctypes.c_int64), ("tt_indices", ctypes.c_void_p),
+                ("kernel_ms", ctypes.c_float), ("slot", ctypes.c_int32)]
+
+
+class gale_mesh_info_t(ctypes.Structure):
+    _fields_ = [("tile_vertices", ctypes.c_int32), ("num_tiles", ctypes.c_int32),
+                ("num_external_refs", ctypes.c_int64), ("vt_nnz", ctypes.c_int64), ("vv_nnz", ctypes.c_int64),
+                ("smem_bytes", ctypes.c_int32), ("max_staged", ctypes.c_int32),
+                ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double)]
+
+
+EXPORTS = ["gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
+           "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
+
+
+class GaleError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} ({status}) {detail}".rstrip())
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
+    """dlopen csrc/libgale.so (fails loudly when it was not built: there is no fallback path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        build_library()
+    if not os.path.exists(LIB):
+        raise RuntimeError(f"{LIB} not built (no fallback path exists); run "
+                           "`python -c 'import __graft_entry__ as g; g.build()'`")
+    lib = ctypes.CDLL(LIB)
+    vp = ctypes.c_void_p
+    lib.gale_mesh_workspace_bytes.restype = ctypes.c_int32
+    lib.gale_mesh_workspace_bytes.argtypes = [ctypes.POINTER(gale_mesh_desc_t), ctypes.POINTER(ctypes.c_size_t)]
+    lib.gale_mesh_create.restype = ctypes.c_int32
+    lib.gale_mesh_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
+    lib.gale_mesh_info.restype = ctypes.c_int32
+    lib.gale_mesh_info.argtypes = [vp, ctypes.POINTER(gale_mesh_info_t)]
+    lib.gale_cluster_batch_compute.restype = ctypes.c_int32
+    lib.gale_cluster_batch_compute.argtypes = [vp, ctypes.c_uint32, _i32p, ctypes.c_int32, vp]
+    lib.gale_queue_pop.restype = ctypes.c_int32
+    lib.gale_queue_pop.argtypes = [vp, ctypes.POINTER(gale_batch_view_t), ctypes.c_int32]
+    lib.gale_queue_release.restype = ctypes.c_int32
+    lib.gale_queue_release.argtypes = [vp, ctypes.POINTER(gale_batch_view_t)]
+    lib.gale_destroy.restype = ctypes.c_int32
+    lib.gale_destroy.argtypes = [vp]
+    lib.gale_status_string.restype = ctypes.c_char_p
+    lib.gale_status_string.argtypes = [ctypes.c_int32]
+    lib.gale_last_error.restype = ctypes.c_char_p
+    lib.gale_last_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load_library().gale_status_string(int(status)).decode()
+
+
+def _check(status: int, where: str):
+    if status != OK:
+        raise GaleError(status, where, load_library().gale_last_error().decode())
+
+
+# ---- the C-ABI calls, same names, marshalling only ----------------------------------------------------
+def gale_mesh_workspace_bytes(desc: gale_mesh_desc_t) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().gale_mesh_workspace_bytes(ctypes.byref(desc), ctypes.byref(out)), "gale_mesh_workspace_bytes")
+    return int(out.value)
+
+
+def gale_mesh_create(desc: gale_mesh_desc_t, cuda_stream: int = 0) -> ctypes.c_void_p:
+    h = ctypes.c_void_p()
+    _check(load_library().gale_mesh_create(ctypes.byref(desc), ctypes.c_void_p(cuda_stream), ctypes.byref(h)),
+           "gale_mesh_create")
+    return h
+
+
+def gale_mesh_info(handle) -> gale_mesh_info_t:
+    info = gale_mesh_info_t()
+    _check(load_library().gale_mesh_info(handle, ctypes.byref(info)), "gale_mesh_info")
+    return info
+
+
+def gale_cluster_batch_compute(handle, relation_mask: int, cluster_ids, cuda_stream: int = 0) -> int:
+    """Returns the status (OK or ERR_WOULD_BLOCK); other errors raise."""
+    ids = np.ascontiguousarray(cluster_ids, dtype=np.int32)
+    st = load_library().gale_cluster_batch_compute(handle, relation_mask, ids.ctypes.data_as(_i32p), len(ids),
+                                                   ctypes.c_void_p(cuda_stream))
+    if st not in (OK, ERR_WOULD_BLOCK):
+        _check(st, "gale_cluster_batch_compute")
+    return st
+
+
+def gale_queue_pop(handle, timeout_ms: int = -1):
+    """Returns (status, view); status is OK, ERR_EMPTY or ERR_WOULD_BLOCK; other errors raise."""
+    view = gale_batch_view_t()
+    st = load_library().gale_queue_pop(handle, ctypes.byref(view), timeout_ms)
+    if st not in (OK, ERR_EMPTY, ERR_WOULD_BLOCK):
+        _check(st, "gale_queue_pop")
+    return st, view
+
+
+def gale_queue_release(handle, view: gale_batch_view_t) -> None:
+    _check(load_library().gale_queue_release(handle, ctypes.byref(view)), "gale_queue_release")
+
+
+def gale_destroy(handle) -> None:
+    _check(load_library().gale_destroy(handle), "gale_destroy")
+
+
+# ---- convenience holder (keeps the torch tensors alive; still marshalling only) ----------------------
+class GaleMesh:
+    """Owns the device tensors (simplices, workspace) behind one gale_mesh_t handle."""
+
+    def __init__(self, dim: int, num_vertices: int, simplices, cluster_offsets, *, max_batch_clusters: int = 64,
+                 queue_depth: int = 0, device_ring: int = 0, tile_vertices: int = 0, flags: int = VALIDATE,
+                 device="cuda:0"):
+        import torch
+
+        load_library()
+        if not torch.cuda.is_available():
+            raise GaleError(ERR_UNSUPPORTED, "GaleMesh", "no CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        if isinstance(simplices, torch.Tensor):
+            self.simplices = simplices.to(device=self.device, dtype=torch.int32).contiguous()
+        else:
+            self.simplices = torch.from_numpy(np.ascontiguousarray(simplices, dtype=np.int32)).to(self.device)
+        self.dim, self.D = dim, dim + 1
+        self.offsets = np.ascontiguousarray(cluster_offsets, dtype=np.int32)
+        d = gale_mesh_desc_t()
+        d.dim, d.num_vertices, d.num_simplices = dim, int(num_vertices), int(self.simplices.shape[0])
+        d.d_simplices = self.simplices.data_ptr() if d.num_simplices else None
+        d.num_clusters = len(self.offsets) - 1
+        d.h_cluster_offsets = self.offsets.ctypes.data_as(_i32p)
+        d.max_batch_clusters, d.queue_depth, d.device_ring = max_batch_clusters, queue_depth, device_ring
+        d.tile_vertices, d.flags = tile_vertices, flags
+        self.desc = d
+        nbytes = gale_mesh_workspace_bytes(d)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        d.d_workspace, d.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.handle = gale_mesh_create(d, torch.cuda.current_stream(self.device).cuda_stream)
+        self.info = gale_mesh_info(self.handle)
+
+    def compute(self, cluster_ids, relation_mask: int = REL_ALL, stream=None) -> int:
+        s = (stream or self.torch.cuda.current_stream(self.device)).cuda_stream
+        return gale_cluster_batch_compute(self.handle, relation_mask, cluster_ids, s)
+
+    def pop(self, timeout_ms: int = -1):
+        return gale_queue_pop(self.handle, timeout_ms)
+
+    def release(self, view) -> None:
+        gale_queue_release(self.handle, view)
+
+    def _array(self, view, ptr, n):
+        """int32 array over slot memory: a torch view of the workspace (device) or numpy (pinned host)."""
+        if not ptr or n == 0:
+            return self.torch.empty(0, dtype=self.torch.int32, device=self.device) if view.on_device else np.empty(0, np.int32)
+        if view.on_device:
+            off = ptr - self.workspace.data_ptr()
+            return self.workspace[off:off + 4 * n].view(self.torch.int32)
+        return np.ctypeslib.as_array(ctypes.cast(ptr, _i32p), shape=(n,))
+
+    def view_arrays(self, view) -> dict:
+        """Expose a popped view as arrays (no copies of the slot data)."""
+        n = view.n_clusters
+        out = dict(sequence=view.sequence, n_clusters=n, relation_mask=view.relation_mask, kernel_ms=view.kernel_ms,
+                   cluster_ids=np.ctypeslib.as_array(view.cluster_ids, shape=(n,)).copy() if n else np.empty(0, np.int32),
+                   vt_row_begin=np.ctypeslib.as_array(view.vt_row_begin, shape=(n + 1,)).copy(),
+                   tt_row_begin=np.ctypeslib.as_array(view.tt_row_begin, shape=(n + 1,)).copy())
+        if view.relation_mask & REL_VT:
+            out["vt_offsets"] = self._array(view, view.vt_offsets, view.vt_rows + 1)
+            out["vt_indices"] = self._array(view, view.vt_indices, view.vt_nnz)
+        if view.relation_mask & REL_VV:
+            out["vv_offsets"] = self._array(view, view.vv_offsets, view.vv_rows + 1)
+            out["vv_indices"] = self._array(view, view.vv_indices, view.vv_nnz)
+        if view.relation_mask & REL_TT:
+            out["tt_indices"] = self._array(view, view.tt_indices, view.tt_rows * self.D)
+        return out
+
+    def run_batch(self, cluster_ids, relation_mask: int = REL_ALL) -> dict:
+        """compute + pop + copy to host numpy + release (test helper; the arithmetic is all on the GPU)."""
+        st = self.compute(cluster_ids, relation_mask)
+        if st != OK:
+            raise GaleError(st, "run_batch")
+        st, view = self.pop(-1)
+        if st != OK:
+            raise GaleError(st, "run_batch/pop")
+        arr = self.view_arrays(view)
+        host = {}
+        for k, v in arr.items():
+            if hasattr(v, "cpu"):
+                host[k] = v.cpu().numpy()
+            elif isinstance(v, np.ndarray):
+                host[k] = np.array(v, copy=True)
+            else:
+                host[k] = v
+        self.release(view)
+        return host
+
+    def destroy(self) -> None:
+        if getattr(self, "handle", None):
+            gale_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def split_batch(host: dict, D: int) -> list:
+    """Cut a host copy of a batch (run_batch) into per-cluster CSR pieces, offsets restarted at 0."""
+    res = []
+    for i in range(host["n_clusters"]):
+        r0, r1 = int(host["vt_row_begin"][i]), int(host["vt_row_begin"][i + 1])
+        t0, t1 = int(host["tt_row_begin"][i]), int(host["tt_row_begin"][i + 1])
+        item = dict(cluster=int(host["cluster_ids"][i]))
+        for k in ("vt", "vv"):
+            if k + "_offsets" in host:
+                off = host[k + "_offsets"][r0:r1 + 1]
+                item[k] = ((off - off[0]).astype(np.int32), host[k + "_indices"][off[0]:off[-1]])
+        if "tt_indices" in host:
+            item["tt"] = host["tt_indices"][t0 * D:t1 * D].reshape(-1, D)
+        res.append(item)
+    return res

@@ -1,0 +1,662 @@
+// gale_lib.cu — C-ABI boundary of the GALE relation hot path (include/gale.h).
+//
+// Host side of the paper's producer: initialization (I_T, T_ex, interval arrays),
+// the leader producer's batch set-up and launch and the bounded queue of
+// pre-allocated result buffers handed to consumers. Every relation entry is
+// computed by the kernels in gale_kernels.cuh; nothing here computes VT/VV/TT on the CPU.
+#include "gale_kernels.cuh"
+
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <mutex>
+#include <string>
+#include <thread>
+#include <vector>
+
+#include "../../include/gale.h"
+
+namespace {
+
+using gale::DeviceMesh;
+using gale::SmemCfg;
+
+thread_local std::string g_last_error;
+
+#define GALE_CUDA(call)                                                                                  \
+  do {                                                                                                   \
+    cudaError_t e_ = (call);                                                                             \
+    if (e_ != cudaSuccess) {                                                                             \
+      g_last_error = std::string(#call) + ": " + cudaGetErrorString(e_);                                 \
+      return GALE_ERR_CUDA;                                                                              \
+    }                                                                                                    \
+  } while (0)
+
+constexpr size_t kAlign = 256;
+inline size_t up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
+inline int pow2_at_least(long long x) {
+  int p = 64;
+  while (p < x) p <<= 1;
+  return p;
+}
+constexpr int kSmemLimit = 227 * 1024;  // opt-in dynamic shared memory per block on sm_100
+
+// ---- result of the create-time analysis ----------------------------------------------------------
+struct Plan {
+  // key
+  const int32_t* dT = nullptr;
+  int dim = 0, nV = 0, nC = 0, tv_req = 0;
+  long long nT = 0;
+  uint32_t flags = 0;
+  std::vector<int32_t> cl_off;
+  // index (host copies)
+  int tv = 0, nTiles = 0;
+  std::vector<int32_t> first_tet, opp_first, opp_perm, tile_vlo, cl_tile_begin, tex;
+  std::vector<long long> tex_off, vt_pref, vv_pref;
+  SmemCfg cfg{};
+  int smem_bytes = 0;
+  // per-cluster sizes
+  std::vector<long long> cl_vt, cl_vv;   // nnz per cluster
+  std::vector<int32_t> cl_t_lo;          // [nC+1] first internal simplex of cluster c (I_T)
+  long long max_rows = 0, max_vt = 0, max_vv = 0, max_tt = 0;
+  double analyse_ms = 0;
+
+  size_t index_bytes() const {
+    size_t b = 0;
+    b += up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) + up(tile_vlo.size() * 4);
+    b += up(cl_tile_begin.size() * 4) + up(tex.size() * 4 + 16) + up(tex_off.size() * 8) + up(vt_pref.size() * 8) +
+         up(vv_pref.size() * 8);
+    return b;
+  }
+};
+
+struct SlotLayout {
+  size_t vt_off = 0, vt_idx = 0, vv_off = 0, vv_idx = 0, tt = 0, total = 0;
+};
+SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
+  const int D = p.dim + 1;
+  SlotLayout L;
+  size_t o = 0;
+  L.vt_off = o; o = up(o + (size_t(maxB) * p.max_rows + 1) * 4);
+  L.vt_idx = o; o = up(o + size_t(maxB) * p.max_vt * 4);
+  L.vv_off = o; o = up(o + (size_t(maxB) * p.max_rows + 1) * 4);
+  L.vv_idx = o; o = up(o + size_t(maxB) * p.max_vv * 4);
+  L.tt = o;     o = up(o + size_t(maxB) * p.max_tt * D * 4);
+  L.total = o;
+  return L;
+}
+
+int validate_host(const Plan& p, const std::vector<int32_t>& T) {
+  const int D = p.dim + 1;
+  for (long long t = 0; t < p.nT; ++t) {
+    const int32_t* r = T.data() + t * D;
+    if (r[0] < 0 || r[D - 1] >= p.nV) return GALE_ERR_NOT_CANONICAL;
+    for (int k = 1; k < D; ++k)
+      if (r[k] <= r[k - 1]) return GALE_ERR_NOT_CANONICAL;
+    if (t > 0 && !std::lexicographical_compare(r - D, r, r, r + D)) return GALE_ERR_NOT_CANONICAL;
+  }
+  return GALE_OK;
+}
+
+// C4: every facet has at most two cofaces (sorted facet list, like the paper's sorted F list, :178).
+template <int D>
+int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
+  struct F { int32_t v[D - 1]; };
+  std::vector<F> f(size_t(p.nT) * D);
+  for (long long t = 0; t < p.nT; ++t)
+    for (int k = 0; k < D; ++k) {
+      int o = 0;
+      for (int j = 0; j < D; ++j)
+        if (j != k) f[t * D + k].v[o++] = T[t * D + j];
+    }
+  auto less = [](const F& a, const F& b) { return std::lexicographical_compare(a.v, a.v + D - 1, b.v, b.v + D - 1); };
+  std::sort(f.begin(), f.end(), less);
+  for (size_t i = 2; i < f.size(); ++i)
+    if (!less(f[i - 2], f[i])) return GALE_ERR_NONMANIFOLD;
+  return GALE_OK;
+}
+
+// Tiles, T_ex per tile, maxima. Returns false if a tile exceeds the staging limits for this tv.
+bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
+  const int D = p.dim + 1;
+  p.tv = tv;
+  p.tile_vlo.clear();
+  p.cl_tile_begin.assign(p.nC + 1, 0);
+  for (int c = 0; c < p.nC; ++c) {
+    p.cl_tile_begin[c] = int(p.tile_vlo.size());
+    for (int v = p.cl_off[c]; v < p.cl_off[c + 1]; v += tv) p.tile_vlo.push_back(v);
+  }
+  p.cl_tile_begin[p.nC] = int(p.tile_vlo.size());
+  p.nTiles = int(p.tile_vlo.size());
+  p.tile_vlo.push_back(p.nV);
+  std::vector<int32_t> tile_of(p.nV);
+  for (int i = 0; i < p.nTiles; ++i)
+    for (int v = p.tile_vlo[i]; v < p.tile_vlo[i + 1]; ++v) tile_of[v] = i;
+  // T_ex: simplex t is external to every tile it touches other than the tile of its lowest vertex
+  p.tex_off.assign(p.nTiles + 1, 0);
+  for (int pass = 0; pass < 2; ++pass) {
+    std::vector<long long> cur;
+    if (pass == 1) {
+      for (int i = 0; i < p.nTiles; ++i) p.tex_off[i + 1] += p.tex_off[i];
+      p.tex.resize(size_t(p.tex_off[p.nTiles]));
+      cur.assign(p.tex_off.begin(), p.tex_off.end() - 1);
+    }
+    for (long long t = 0; t < p.nT; ++t) {
+      const int32_t* r = T.data() + t * D;
+      const int t0 = tile_of[r[0]];
+      int seen[3], ns = 0;
+      for (int k = 1; k < D; ++k) {
+        const int tk = tile_of[r[k]];
+        if (tk == t0) continue;
+        bool dup = false;
+        for (int s = 0; s < ns; ++s) dup |= seen[s] == tk;
+        if (dup) continue;
+        seen[ns++] = tk;
+        if (pass == 0) ++p.tex_off[tk + 1]; else p.tex[size_t(cur[tk]++)] = int32_t(t);
+      }
+    }
+  }
+  long long smax = 0, sext = 0, sint = 0;
+  for (int i = 0; i < p.nTiles; ++i) {
+    const long long si = p.first_tet[p.tile_vlo[i + 1]] - p.first_tet[p.tile_vlo[i]];
+    const long long se = p.tex_off[i + 1] - p.tex_off[i];
+    smax = std::max(smax, si + se);
+    sext = std::max(sext, se);
+    sint = std::max(sint, si);
+  }
+  p.cfg = SmemCfg{};
+  p.cfg.tv = tv;
+  p.cfg.smax = int(std::max(1LL, smax));
+  p.cfg.sext = int(std::max(1LL, sext));
+  p.cfg.sint = int(std::max(1LL, sint));
+  p.cfg.bm_words = (tv + 31) / 32;
+  return smax <= gale::kMaxStaged;
+}
+
+template <int D>
+int run_count(const Plan& p, const DeviceMesh& dm, const gale::CountCfg& cc, int smem, long long* d_stats,
+              cudaStream_t st) {
+  GALE_CUDA(cudaFuncSetAttribute(gale::gale_count_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  gale::gale_count_kernel<D><<<std::max(1, p.nTiles), gale::kThreads, smem, st>>>(dm, cc, p.nTiles, d_stats);
+  GALE_CUDA(cudaGetLastError());
+  return GALE_OK;
+}
+
+struct DevBuf {  // temporary device memory of the analysis
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  int alloc(size_t n) { GALE_CUDA(cudaMalloc(&p, std::max<size_t>(n, 16))); return GALE_OK; }
+};
+
+int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& out) {
+  const auto t0 = std::chrono::steady_clock::now();
+  auto p = std::make_unique<Plan>();
+  p->dT = d.d_simplices; p->dim = d.dim; p->nV = d.num_vertices; p->nC = d.num_clusters; p->nT = d.num_simplices;
+  p->tv_req = d.tile_vertices; p->flags = d.flags;
+  p->cl_off.assign(d.h_cluster_offsets, d.h_cluster_offsets + d.num_clusters + 1);
+  const int D = d.dim + 1;
+  if (p->cl_off.front() != 0 || p->cl_off.back() != p->nV) return GALE_ERR_INVALID_ARG;
+  for (int c = 0; c < p->nC; ++c)
+    if (p->cl_off[c] > p->cl_off[c + 1]) return GALE_ERR_INVALID_ARG;
+
+  std::vector<int32_t> T(size_t(p->nT) * D);
+  if (p->nT) GALE_CUDA(cudaMemcpy(T.data(), d.d_simplices, T.size() * 4, cudaMemcpyDeviceToHost));
+  if (d.flags & (GALE_VALIDATE | GALE_VALIDATE_MANIFOLD)) {
+    int rc = validate_host(*p, T);
+    if (rc != GALE_OK) return rc;
+  }
+  if (d.flags & GALE_VALIDATE_MANIFOLD) {
+    int rc = D == 4 ? validate_manifold<4>(*p, T) : validate_manifold<3>(*p, T);
+    if (rc != GALE_OK) return rc;
+  }
+  // I_T: first simplex whose lowest vertex is >= v; and the same keyed by the second vertex
+  p->first_tet.assign(p->nV + 1, 0);
+  p->opp_first.assign(p->nV + 1, 0);
+  for (long long t = 0; t < p->nT; ++t) {
+    ++p->first_tet[T[t * D] + 1];
+    ++p->opp_first[T[t * D + 1] + 1];
+  }
+  for (int v = 0; v < p->nV; ++v) {
+    p->first_tet[v + 1] += p->first_tet[v];
+    p->opp_first[v + 1] += p->opp_first[v];
+  }
+  p->opp_perm.resize(size_t(p->nT));
+  {
+    std::vector<int32_t> cur(p->opp_first.begin(), p->opp_first.end() - 1);
+    for (long long t = 0; t < p->nT; ++t) p->opp_perm[cur[T[t * D + 1]]++] = int32_t(t);
+  }
+  p->cl_t_lo.resize(p->nC + 1);
+  for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
+
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kThreads) : (d.dim == 3 ? 128 : 256);
+  for (;; tv /= 2) {
+    if (tv < 1) return GALE_ERR_UNSUPPORTED;
+    if (!build_tiles(*p, T, tv)) continue;
+    // sizing run on the device (temporary copies of the index)
+    gale::CountCfg cc{tv, p->cfg.smax, p->cfg.sext, 8192, p->cfg.bm_words};
+    int csmem = gale::make_count_layout(cc, D).total;
+    while (csmem > kSmemLimit && cc.hcap > 256) { cc.hcap /= 2; csmem = gale::make_count_layout(cc, D).total; }
+    if (csmem > kSmemLimit) continue;
+    DevBuf b_ft, b_vlo, b_toff, b_tex, b_stats, b_err;
+    int rc;
+    if ((rc = b_ft.alloc(p->first_tet.size() * 4)) || (rc = b_vlo.alloc(p->tile_vlo.size() * 4)) ||
+        (rc = b_toff.alloc(p->tex_off.size() * 8)) || (rc = b_tex.alloc(p->tex.size() * 4)) ||
+        (rc = b_stats.alloc(size_t(p->nTiles) * 32)) || (rc = b_err.alloc(4)))
+      return rc;
+    GALE_CUDA(cudaMemcpyAsync(b_ft.p, p->first_tet.data(), p->first_tet.size() * 4, cudaMemcpyHostToDevice, st));
+    GALE_CUDA(cudaMemcpyAsync(b_vlo.p, p->tile_vlo.data(), p->tile_vlo.size() * 4, cudaMemcpyHostToDevice, st));
+    GALE_CUDA(cudaMemcpyAsync(b_toff.p, p->tex_off.data(), p->tex_off.size() * 8, cudaMemcpyHostToDevice, st));
+    if (!p->tex.empty())
+      GALE_CUDA(cudaMemcpyAsync(b_tex.p, p->tex.data(), p->tex.size() * 4, cudaMemcpyHostToDevice, st));
+    GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
+    DeviceMesh dm{};
+    dm.T = d.d_simplices;
+    dm.first_tet = static_cast<int32_t*>(b_ft.p);
+    dm.tile_vlo = static_cast<int32_t*>(b_vlo.p);
+    dm.tex_off = static_cast<long long*>(b_toff.p);
+    dm.tex = static_cast<int32_t*>(b_tex.p);
+    dm.err = static_cast<int32_t*>(b_err.p);
+    rc = D == 4 ? run_count<4>(*p, dm, cc, csmem, static_cast<long long*>(b_stats.p), st)
+                : run_count<3>(*p, dm, cc, csmem, static_cast<long long*>(b_stats.p), st);
+    if (rc != GALE_OK) return rc;
+    std::vector<long long> stats(size_t(p->nTiles) * 4);
+    int err = 0;
+    if (p->nTiles)
+      GALE_CUDA(cudaMemcpyAsync(stats.data(), b_stats.p, stats.size() * 8, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaMemcpyAsync(&err, b_err.p, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    if (err & gale::ERR_COUNT_ROW_TOO_BIG) return GALE_ERR_UNSUPPORTED;
+    if (err) { g_last_error = "device guard fired during sizing: " + std::to_string(err); return GALE_ERR_WORKSPACE; }
+
+    p->vt_pref.assign(p->nTiles + 1, 0);
+    p->vv_pref.assign(p->nTiles + 1, 0);
+    long long vt_max = 1, vv_max = 1, uniq_max = 1, rec_max = 1;
+    for (int i = 0; i < p->nTiles; ++i) {
+      p->vt_pref[i + 1] = p->vt_pref[i] + stats[i * 4 + 0];
+      p->vv_pref[i + 1] = p->vv_pref[i] + stats[i * 4 + 1];
+      vt_max = std::max(vt_max, stats[i * 4 + 0]);
+      vv_max = std::max(vv_max, stats[i * 4 + 1]);
+      uniq_max = std::max(uniq_max, stats[i * 4 + 2]);
+      rec_max = std::max(rec_max, stats[i * 4 + 3]);
+    }
+    p->cfg.vt_max = int(vt_max);
+    p->cfg.vv_max = int(vv_max);
+    p->cfg.vvh_cap = pow2_at_least(2 * uniq_max);
+    p->cfg.tth_cap = pow2_at_least(rec_max + 1);
+    p->smem_bytes = gale::make_layout(p->cfg, D).total;
+    if (p->smem_bytes > kSmemLimit) continue;
+    break;
+  }
+  // per-cluster sizes
+  p->cl_vt.resize(p->nC);
+  p->cl_vv.resize(p->nC);
+  for (int c = 0; c < p->nC; ++c) {
+    p->cl_vt[c] = p->vt_pref[p->cl_tile_begin[c + 1]] - p->vt_pref[p->cl_tile_begin[c]];
+    p->cl_vv[c] = p->vv_pref[p->cl_tile_begin[c + 1]] - p->vv_pref[p->cl_tile_begin[c]];
+    p->max_rows = std::max<long long>(p->max_rows, p->cl_off[c + 1] - p->cl_off[c]);
+    p->max_vt = std::max(p->max_vt, p->cl_vt[c]);
+    p->max_vv = std::max(p->max_vv, p->cl_vv[c]);
+    p->max_tt = std::max<long long>(p->max_tt, p->cl_t_lo[c + 1] - p->cl_t_lo[c]);
+  }
+  p->analyse_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  out = std::move(p);
+  return GALE_OK;
+}
+
+bool plan_matches(const Plan& p, const gale_mesh_desc_t& d) {
+  return p.dT == d.d_simplices && p.dim == d.dim && p.nV == d.num_vertices && p.nC == d.num_clusters &&
+         p.nT == d.num_simplices && p.tv_req == d.tile_vertices && p.flags == d.flags &&
+         std::equal(p.cl_off.begin(), p.cl_off.end(), d.h_cluster_offsets);
+}
+std::mutex g_plan_mutex;
+std::unique_ptr<Plan> g_plan_cache;  // handed from gale_mesh_workspace_bytes to gale_mesh_create
+
+int check_desc(const gale_mesh_desc_t* d) {
+  if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
+      !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
+      d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1)
+    return GALE_ERR_INVALID_ARG;
+  if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
+  return GALE_OK;
+}
+int check_device() {
+  int dev = 0;
+  cudaDeviceProp prop{};
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    g_last_error = "no CUDA device";
+    return GALE_ERR_UNSUPPORTED;
+  }
+  if (prop.major != 10) {
+    g_last_error = "device is not sm_100 (compute capability " + std::to_string(prop.major) + "." + std::to_string(prop.minor) + ")";
+    return GALE_ERR_UNSUPPORTED;
+  }
+  return GALE_OK;
+}
+size_t total_workspace(const Plan& p, const gale_mesh_desc_t& d) {
+  const int slots = d.queue_depth > 0 ? d.queue_depth : (d.device_ring > 0 ? d.device_ring : 4);
+  return p.index_bytes() + size_t(slots) * slot_capacity_layout(p, d.max_batch_clusters).total + kAlign;
+}
+
+enum SlotState { SLOT_FREE = 0, SLOT_SUBMITTED = 1, SLOT_POPPED = 2 };
+
+struct Slot {
+  char* dev = nullptr;
+  char* pinned = nullptr;
+  cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_ready = nullptr;
+  std::atomic<int> state{SLOT_FREE};
+  long long seq = 0;
+  int n = 0;
+  uint32_t mask = 0;
+  std::vector<int32_t> ids, row_begin, tt_row_begin;
+  long long rows = 0, vt_nnz = 0, vv_nnz = 0, tt_rows = 0;
+  SlotLayout used;  // section offsets of this batch
+};
+
+}  // namespace
+
+struct gale_mesh {
+  std::unique_ptr<Plan> plan;
+  int dim = 0, D = 0, maxB = 0, queue_depth = 0;
+  DeviceMesh dm{};
+  std::vector<std::unique_ptr<Slot>> slots;
+  SlotLayout cap;
+  cudaStream_t side = nullptr;
+  int32_t* h_err = nullptr;  // mapped pinned; the kernels write guard codes here
+  std::atomic<long long> submitted{0}, popped{0};
+  size_t workspace_used = 0;
+  double create_ms = 0;
+};
+
+extern "C" {
+
+const char* gale_status_string(int32_t s) {
+  switch (s) {
+    case GALE_OK: return "GALE_OK";
+    case GALE_ERR_INVALID_ARG: return "GALE_ERR_INVALID_ARG";
+    case GALE_ERR_NOT_CANONICAL: return "GALE_ERR_NOT_CANONICAL";
+    case GALE_ERR_DEGENERATE: return "GALE_ERR_DEGENERATE";
+    case GALE_ERR_NONMANIFOLD: return "GALE_ERR_NONMANIFOLD";
+    case GALE_ERR_BAD_CLUSTER: return "GALE_ERR_BAD_CLUSTER";
+    case GALE_ERR_WOULD_BLOCK: return "GALE_ERR_WOULD_BLOCK";
+    case GALE_ERR_EMPTY: return "GALE_ERR_EMPTY";
+    case GALE_ERR_WORKSPACE: return "GALE_ERR_WORKSPACE";
+    case GALE_ERR_CUDA: return "GALE_ERR_CUDA";
+    case GALE_ERR_UNSUPPORTED: return "GALE_ERR_UNSUPPORTED";
+    default: return "GALE_ERR_UNKNOWN";
+  }
+}
+const char* gale_last_error(void) { return g_last_error.c_str(); }
+
+int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t* desc, size_t* out_bytes) {
+  if (!out_bytes) return GALE_ERR_INVALID_ARG;
+  int rc = check_desc(desc);
+  if (rc != GALE_OK) return rc;
+  if ((rc = check_device()) != GALE_OK) return rc;
+  std::unique_ptr<Plan> p;
+  if ((rc = analyse(*desc, nullptr, p)) != GALE_OK) return rc;
+  *out_bytes = total_workspace(*p, *desc);
+  std::lock_guard<std::mutex> lk(g_plan_mutex);
+  g_plan_cache = std::move(p);
+  return GALE_OK;
+}
+
+int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_mesh_t** out) {
+  if (!out) return GALE_ERR_INVALID_ARG;
+  int rc = check_desc(desc);
+  if (rc != GALE_OK) return rc;
+  if ((rc = check_device()) != GALE_OK) return rc;
+  if (!desc->d_workspace || reinterpret_cast<uintptr_t>(desc->d_workspace) % kAlign) return GALE_ERR_WORKSPACE;
+  const auto t0 = std::chrono::steady_clock::now();
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  std::unique_ptr<Plan> p;
+  {
+    std::lock_guard<std::mutex> lk(g_plan_mutex);
+    if (g_plan_cache && plan_matches(*g_plan_cache, *desc)) p = std::move(g_plan_cache);
+    g_plan_cache.reset();
+  }
+  if (!p && (rc = analyse(*desc, st, p)) != GALE_OK) return rc;
+  if (total_workspace(*p, *desc) > desc->workspace_bytes) return GALE_ERR_WORKSPACE;
+
+  auto m = std::make_unique<gale_mesh>();
+  m->dim = desc->dim; m->D = desc->dim + 1; m->maxB = desc->max_batch_clusters; m->queue_depth = desc->queue_depth;
+  char* base = static_cast<char*>(desc->d_workspace);
+  size_t o = 0;
+  auto put = [&](const void* src, size_t bytes, size_t pad = 0) -> void* {
+    void* dst = base + o;
+    if (bytes) cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+    o = up(o + bytes + pad);
+    return dst;
+  };
+  m->dm.T = desc->d_simplices;
+  m->dm.first_tet = static_cast<int32_t*>(put(p->first_tet.data(), p->first_tet.size() * 4));
+  m->dm.opp_first = static_cast<int32_t*>(put(p->opp_first.data(), p->opp_first.size() * 4));
+  m->dm.opp_perm = static_cast<int32_t*>(put(p->opp_perm.data(), p->opp_perm.size() * 4));
+  m->dm.tile_vlo = static_cast<int32_t*>(put(p->tile_vlo.data(), p->tile_vlo.size() * 4));
+  m->dm.cluster_tile_begin = static_cast<int32_t*>(put(p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4));
+  m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
+  m->dm.tex_off = static_cast<long long*>(put(p->tex_off.data(), p->tex_off.size() * 8));
+  m->dm.vt_pref = static_cast<long long*>(put(p->vt_pref.data(), p->vt_pref.size() * 8));
+  m->dm.vv_pref = static_cast<long long*>(put(p->vv_pref.data(), p->vv_pref.size() * 8));
+  GALE_CUDA(cudaGetLastError());
+  // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
+  GALE_CUDA(cudaStreamSynchronize(st));
+  std::vector<int32_t>().swap(p->opp_perm);
+  std::vector<int32_t>().swap(p->tex);
+  std::vector<int32_t>().swap(p->opp_first);
+
+  GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
+  *m->h_err = 0;
+  GALE_CUDA(cudaHostGetDevicePointer(reinterpret_cast<void**>(&m->dm.err), m->h_err, 0));
+
+  m->cap = slot_capacity_layout(*p, m->maxB);
+  const int nslots = desc->queue_depth > 0 ? desc->queue_depth : (desc->device_ring > 0 ? desc->device_ring : 4);
+  for (int i = 0; i < nslots; ++i) {
+    auto s = std::make_unique<Slot>();
+    s->dev = base + o;
+    o += m->cap.total;
+    if (desc->queue_depth > 0) GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&s->pinned), m->cap.total, cudaHostAllocDefault));
+    GALE_CUDA(cudaEventCreate(&s->ev_start));
+    GALE_CUDA(cudaEventCreate(&s->ev_done));
+    GALE_CUDA(cudaEventCreateWithFlags(&s->ev_ready, cudaEventDisableTiming));
+    m->slots.push_back(std::move(s));
+  }
+  m->workspace_used = o;
+  if (desc->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
+  if (m->D == 4)
+    GALE_CUDA(cudaFuncSetAttribute(gale::gale_batch_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+  else
+    GALE_CUDA(cudaFuncSetAttribute(gale::gale_batch_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+  m->plan = std::move(p);
+  m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() +
+                 (m->plan->analyse_ms);
+  *out = m.release();
+  return GALE_OK;
+}
+
+int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
+  if (!m || !out) return GALE_ERR_INVALID_ARG;
+  const Plan& p = *m->plan;
+  out->tile_vertices = p.tv;
+  out->num_tiles = p.nTiles;
+  out->num_external_refs = p.tex_off.empty() ? 0 : p.tex_off.back();
+  out->vt_nnz = p.vt_pref.empty() ? 0 : p.vt_pref.back();
+  out->vv_nnz = p.vv_pref.empty() ? 0 : p.vv_pref.back();
+  out->smem_bytes = p.smem_bytes;
+  out->max_staged = p.cfg.smax;
+  out->slot_bytes = m->cap.total;
+  out->workspace_used = m->workspace_used;
+  out->create_ms = m->create_ms;
+  return GALE_OK;
+}
+
+int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const int32_t* h_cluster_ids,
+                                   int32_t n_clusters, void* cuda_stream) {
+  if (!m || (relation_mask & ~uint32_t(GALE_REL_ALL)) || relation_mask == 0 || n_clusters < 0 ||
+      (n_clusters > 0 && !h_cluster_ids))
+    return GALE_ERR_INVALID_ARG;
+  if (n_clusters > m->maxB) return GALE_ERR_BAD_CLUSTER;
+  const Plan& p = *m->plan;
+  for (int i = 0; i < n_clusters; ++i)
+    if (h_cluster_ids[i] < 0 || h_cluster_ids[i] >= p.nC) return GALE_ERR_BAD_CLUSTER;
+  const long long seq = m->submitted.load();
+  Slot& s = *m->slots[size_t(seq % (long long)m->slots.size())];
+  if (s.state.load(std::memory_order_acquire) != SLOT_FREE) return GALE_ERR_WOULD_BLOCK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int D = m->D;
+
+  // batch set-up (a0): row / nnz bases of every requested cluster, in request order
+  s.seq = seq; s.n = n_clusters; s.mask = relation_mask;
+  s.ids.assign(h_cluster_ids, h_cluster_ids + n_clusters);
+  s.row_begin.assign(n_clusters + 1, 0);
+  s.tt_row_begin.assign(n_clusters + 1, 0);
+  std::vector<long long> vtb(n_clusters + 1, 0), vvb(n_clusters + 1, 0);
+  for (int i = 0; i < n_clusters; ++i) {
+    const int c = s.ids[i];
+    const long long rows = p.cl_off[c + 1] - p.cl_off[c];
+    const long long ttr = p.cl_t_lo[c + 1] - p.cl_t_lo[c];
+    if (s.row_begin[i] + rows >= (1LL << 31) - 1 || vtb[i] + p.cl_vt[c] >= (1LL << 31) - 1 ||
+        (s.tt_row_begin[i] + ttr) * D >= (1LL << 31) - 1)
+      return GALE_ERR_INVALID_ARG;
+    s.row_begin[i + 1] = int32_t(s.row_begin[i] + rows);
+    s.tt_row_begin[i + 1] = int32_t(s.tt_row_begin[i] + ttr);
+    vtb[i + 1] = vtb[i] + p.cl_vt[c];
+    vvb[i + 1] = vvb[i] + p.cl_vv[c];
+  }
+  s.rows = s.row_begin[n_clusters]; s.vt_nnz = vtb[n_clusters]; s.vv_nnz = vvb[n_clusters];
+  s.tt_rows = s.tt_row_begin[n_clusters];
+  // compact section layout of this batch (one D2H copy of `used.total` bytes)
+  {
+    size_t o = 0;
+    s.used.vt_off = o; if (relation_mask & GALE_REL_VT) o = up(o + size_t(s.rows + 1) * 4, 16);
+    s.used.vt_idx = o; if (relation_mask & GALE_REL_VT) o = up(o + size_t(s.vt_nnz) * 4, 16);
+    s.used.vv_off = o; if (relation_mask & GALE_REL_VV) o = up(o + size_t(s.rows + 1) * 4, 16);
+    s.used.vv_idx = o; if (relation_mask & GALE_REL_VV) o = up(o + size_t(s.vv_nnz) * 4, 16);
+    s.used.tt = o;     if (relation_mask & GALE_REL_TT) o = up(o + size_t(s.tt_rows) * D * 4, 16);
+    s.used.total = o;
+    if (o > m->cap.total) return GALE_ERR_WORKSPACE;
+  }
+  gale::OutPtrs O{};
+  O.vt_offsets = reinterpret_cast<int32_t*>(s.dev + s.used.vt_off);
+  O.vt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.vt_idx);
+  O.vv_offsets = reinterpret_cast<int32_t*>(s.dev + s.used.vv_off);
+  O.vv_indices = reinterpret_cast<int32_t*>(s.dev + s.used.vv_idx);
+  O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
+
+  GALE_CUDA(cudaEventRecord(s.ev_start, st));
+  for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
+    gale::BatchParams P{};
+    const int nb = std::max(0, std::min(gale::kMaxBatch, n_clusters - b));
+    P.n_clusters = nb; P.mask = relation_mask;
+    P.total_rows = int(s.rows); P.total_vt_nnz = int(s.vt_nnz); P.total_vv_nnz = int(s.vv_nnz);
+    for (int i = 0; i < nb; ++i) {
+      const int c = s.ids[b + i];
+      P.tile_prefix[i + 1] = P.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
+      P.cluster[i] = c;
+      P.row_base[i] = s.row_begin[b + i];
+      P.vt_base[i] = int(vtb[b + i]);
+      P.vv_base[i] = int(vvb[b + i]);
+      P.tt_base[i] = s.tt_row_begin[b + i];
+    }
+    const int grid = std::max(1, P.tile_prefix[nb]);
+    if (D == 4)
+      gale::gale_batch_kernel<4><<<grid, gale::kThreads, p.smem_bytes, st>>>(m->dm, P, p.cfg, O);
+    else
+      gale::gale_batch_kernel<3><<<grid, gale::kThreads, p.smem_bytes, st>>>(m->dm, P, p.cfg, O);
+    GALE_CUDA(cudaGetLastError());
+  }
+  GALE_CUDA(cudaEventRecord(s.ev_done, st));
+  if (m->queue_depth > 0) {  // a7: D2H into the pinned slot on the side stream
+    GALE_CUDA(cudaStreamWaitEvent(m->side, s.ev_done, 0));
+    if (s.used.total) GALE_CUDA(cudaMemcpyAsync(s.pinned, s.dev, s.used.total, cudaMemcpyDeviceToHost, m->side));
+    GALE_CUDA(cudaEventRecord(s.ev_ready, m->side));
+  }
+  s.state.store(SLOT_SUBMITTED, std::memory_order_release);
+  m->submitted.store(seq + 1);
+  return GALE_OK;
+}
+
+int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_ms) {
+  if (!m || !out) return GALE_ERR_INVALID_ARG;
+  const long long seq = m->popped.load();
+  if (seq >= m->submitted.load()) return GALE_ERR_EMPTY;
+  Slot& s = *m->slots[size_t(seq % (long long)m->slots.size())];
+  if (s.state.load(std::memory_order_acquire) != SLOT_SUBMITTED) return GALE_ERR_EMPTY;
+  cudaEvent_t ev = m->queue_depth > 0 ? s.ev_ready : s.ev_done;
+  if (timeout_ms < 0) {
+    GALE_CUDA(cudaEventSynchronize(ev));
+  } else {
+    const auto deadline = std::chrono::steady_clock::now() + std::chrono::milliseconds(timeout_ms);
+    for (;;) {
+      cudaError_t q = cudaEventQuery(ev);
+      if (q == cudaSuccess) break;
+      if (q != cudaErrorNotReady) { g_last_error = cudaGetErrorString(q); return GALE_ERR_CUDA; }
+      if (std::chrono::steady_clock::now() >= deadline) return GALE_ERR_WOULD_BLOCK;
+      std::this_thread::yield();
+    }
+  }
+  if (*static_cast<volatile int32_t*>(m->h_err) != 0) {
+    g_last_error = "device capacity guard fired: code " + std::to_string(*m->h_err);
+    return GALE_ERR_WORKSPACE;
+  }
+  const char* b = m->queue_depth > 0 ? s.pinned : s.dev;
+  std::memset(out, 0, sizeof(*out));
+  out->sequence = s.seq; out->n_clusters = s.n; out->relation_mask = s.mask; out->dim = m->dim;
+  out->on_device = m->queue_depth > 0 ? 0 : 1;
+  out->cluster_ids = s.ids.data();
+  out->vt_row_begin = s.row_begin.data();
+  out->tt_row_begin = s.tt_row_begin.data();
+  if (s.mask & GALE_REL_VT) {
+    out->vt_rows = s.rows; out->vt_nnz = s.vt_nnz;
+    out->vt_offsets = reinterpret_cast<const int32_t*>(b + s.used.vt_off);
+    out->vt_indices = reinterpret_cast<const int32_t*>(b + s.used.vt_idx);
+  }
+  if (s.mask & GALE_REL_VV) {
+    out->vv_rows = s.rows; out->vv_nnz = s.vv_nnz;
+    out->vv_offsets = reinterpret_cast<const int32_t*>(b + s.used.vv_off);
+    out->vv_indices = reinterpret_cast<const int32_t*>(b + s.used.vv_idx);
+  }
+  if (s.mask & GALE_REL_TT) {
+    out->tt_rows = s.tt_rows;
+    out->tt_indices = reinterpret_cast<const int32_t*>(b + s.used.tt);
+  }
+  float ms = 0.f;
+  if (cudaEventElapsedTime(&ms, s.ev_start, s.ev_done) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }
+  out->kernel_ms = ms;
+  out->slot = int32_t(seq % (long long)m->slots.size());
+  s.state.store(SLOT_POPPED, std::memory_order_release);
+  m->popped.store(seq + 1);
+  return GALE_OK;
+}
+
+int32_t gale_queue_release(gale_mesh_t* m, const gale_batch_view_t* view) {
+  if (!m || !view || view->slot < 0 || view->slot >= int(m->slots.size())) return GALE_ERR_INVALID_ARG;
+  Slot& s = *m->slots[size_t(view->slot)];
+  if (s.state.load(std::memory_order_acquire) != SLOT_POPPED || s.seq != view->sequence) return GALE_ERR_INVALID_ARG;
+  s.state.store(SLOT_FREE, std::memory_order_release);
+  return GALE_OK;
+}
+
+int32_t gale_destroy(gale_mesh_t* m) {
+  if (!m) return GALE_ERR_INVALID_ARG;
+  for (auto& s : m->slots) {
+    if (s->ev_done) cudaEventSynchronize(s->ev_done);
+    if (m->queue_depth > 0 && s->ev_ready && s->state.load() != SLOT_FREE) cudaEventSynchronize(s->ev_ready);
+  }
+  if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
+  for (auto& s : m->slots) {
+    if (s->pinned) cudaFreeHost(s->pinned);
+    if (s->ev_start) cudaEventDestroy(s->ev_start);
+    if (s->ev_done) cudaEventDestroy(s->ev_done);
+    if (s->ev_ready) cudaEventDestroy(s->ev_ready);
+  }
+  if (m->h_err) cudaFreeHost(m->h_err);
+  cudaGetLastError();
+  delete m;
+  return GALE_OK;
+}
+
+}  // extern "C"
