@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py — tets/s through VT+VV+TT per cluster batch, and the HBM roofline fraction.
+
+A *step* is one pass of the whole hot path over the whole mesh: every
+cluster once, in batches of `--batch` clusters (config 5: 4,096 clusters -> 64 batches of 64), results
+kept in the device ring (queue_depth = 0). `value` = simplices / device time of a step.
+`e2e` is the same pass through the C ABI with HOST buffers: the simplex array is copied from pinned
+host memory each step and every batch is streamed D2H through the pinned result queue (a7) and
+popped/released on the host.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--n GRID] [--impl reference]
+
+Under torchrun (N > 1) every rank runs an independent replica of the same pass (the path has no
+exchange step: clusters are independent); rank 0 prints the one JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import meshgen  # noqa: E402
+
+METRIC = "tets/s through VT+VV+TT per cluster batch"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def algorithmic_bytes(dim, n_simplices, rows, vt_nnz, vv_nnz, tt_rows, n_batches):
+    """Compulsory bytes of a pass: each simplex row read once, each output
+    array written once (indices + offsets)."""
+    D = dim + 1
+    return 4 * D * n_simplices + 4 * (vt_nnz + vv_nnz) + 4 * D * tt_rows + 2 * 4 * (rows + n_batches)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        sel = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
+        sm, mx, reasons = [], [], set()
+        for r in sel:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(args):
+    t0 = time.time()
+    mesh = meshgen.make_config(args.config, n=args.n)
+    return mesh, time.time() - t0
+
+
+def oracle_sample(mesh, target_s=15.0, max_clusters=256):
+    """Time the CPU oracle (as it stands, single thread) on a bounded sample of the same mesh:
+    whole clusters, restricted evaluation (oracle/gale_oracle.cpp), one call whose cluster count is
+    calibrated to about target_s seconds. Returns (tets/s, description)."""
+    import oracle
+
+    first = np.searchsorted(mesh.simplices[:, 0], mesh.cluster_offsets)
+    nC = mesh.num_clusters
+
+    def run(k):
+        sel = np.linspace(0, nC - 1, num=k).astype(int).tolist() if k < nC else list(range(nC))
+        t0 = time.perf_counter()
+        oracle.cluster_results(mesh.dim, mesh.num_vertices, mesh.simplices, mesh.cluster_offsets, sel, restricted=True)
+        return time.perf_counter() - t0, int(sum(first[c + 1] - first[c] for c in set(sel)))
+
+    k = min(nC, 8)
+    dt, done = run(k)
+    if dt < target_s / 3 and k < min(nC, max_clusters):
+        dt1, _ = run(1)                                     # fixed cost of a call (whole-mesh scans)
+        per = max((dt - dt1) / max(k - 1, 1), 1e-6)
+        k = int(max(k, min(nC, max_clusters, (target_s - dt1) / per)))
+        dt, done = run(k)
+    desc = (f"{k} whole clusters of the same mesh ({done} internal simplices), VT+VV+TT, restricted oracle "
+            f"(includes its whole-mesh scan), one call, {dt:.1f} s")
+    return done / max(dt, 1e-9), desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    mesh, _ = make_workload(args)
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, sample = [], ""
+    for i in range(args.warmup + args.steps):
+        v, sample = oracle_sample(mesh, target_s=per_step, max_clusters=64)
+        if i >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "tets/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": workload_config(args, mesh),
+            "cpu_baseline": {"value": value, "unit": "tets/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "tets/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def workload_config(args, mesh, extra=None):
+    cfg = {"workload": mesh.meta["name"], "config_index": args.config, "dim": mesh.dim,
+           "num_vertices": mesh.num_vertices, "num_simplices": mesh.num_simplices,
+           "num_clusters": mesh.num_clusters, "batch_clusters": args.batch, "relations": "VT+VV+TT",
+           "l2_policy": "inputs+outputs of a step (GBs) far exceed the 126 MB L2; no flush needed"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--n", type=int, default=None, help="grid size override (smaller mesh of the same family)")
+    ap.add_argument("--batch", type=int, default=64)
+    ap.add_argument("--ring", type=int, default=8, help="device result slots in the device-timed run")
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--impl", default="gale", choices=["gale", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2507_15230_b200 as gale
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback exists)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    mesh, gen_s = make_workload(args)
+    D = mesh.dim + 1
+    nC, B = mesh.num_clusters, args.batch
+    batches = [np.arange(b, min(nC, b + B), dtype=np.int32) for b in range(0, nC, B)]
+
+    t0 = time.time()
+    gm = gale.GaleMesh(mesh.dim, mesh.num_vertices, mesh.simplices, mesh.cluster_offsets, max_batch_clusters=B,
+                       queue_depth=0, device_ring=args.ring, tile_vertices=args.tile, flags=0)
+    create_s = time.time() - t0
+    info = gm.info
+    stream = torch.cuda.current_stream()
+
+    kernel_ms = []
+
+    def one_pass(g, record=False):
+        """Submit every batch; pop/release lagging by the ring so the GPU always has work queued."""
+        inflight = 0
+        for ids in batches:
+            while g.compute(ids) == gale.ERR_WOULD_BLOCK:
+                st, v = g.pop(-1)
+                if record:
+                    kernel_ms.append(v.kernel_ms)
+                g.release(v)
+                inflight -= 1
+            inflight += 1
+        while inflight:
+            st, v = g.pop(-1)
+            if record:
+                kernel_ms.append(v.kernel_ms)
+            g.release(v)
+            inflight -= 1
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_pass(gm)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.1)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        one_pass(gm, record=True)
+    e1.record(stream)
+    barrier()
+    w1 = time.time()
+    clocks = sampler.stop(w0, w1)
+    ms = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = world * mesh.num_simplices / (ms_per_step * 1e-3)
+
+    # roofline of the dominant kernel (gale_batch_kernel): algorithmic bytes per launch / avg launch time
+    rows = mesh.num_vertices
+    alg_bytes = algorithmic_bytes(mesh.dim, mesh.num_simplices, rows, info.vt_nnz, info.vv_nnz, mesh.num_simplices,
+                                  len(batches))
+    launches = args.steps * len(batches)
+    avg_launch_ms = float(np.mean(kernel_ms)) if kernel_ms else ms_per_step / len(batches)
+    achieved = alg_bytes / len(batches) / (avg_launch_ms * 1e-3) / 1e9
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_kind = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_kind = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "kernel": f"gale_batch_kernel<{D}>", "peak_kind": peak_kind,
+                "bytes_per_launch": alg_bytes / len(batches), "avg_launch_ms": avg_launch_ms,
+                "step_gbs": alg_bytes / (ms_per_step * 1e-3) / 1e9,
+                "frac_of_8TBs_nominal": achieved / 8000.0}
+    gm.destroy()
+    del gm
+
+    # end to end through the C ABI with host buffers
+    e2e = None
+    if not args.no_e2e:
+        host_T = torch.from_numpy(mesh.simplices).pin_memory()
+        dev_T = torch.empty_like(host_T, device="cuda")
+        dev_T.copy_(host_T, non_blocking=True)
+        g2 = gale.GaleMesh(mesh.dim, mesh.num_vertices, dev_T, mesh.cluster_offsets, max_batch_clusters=B,
+                           queue_depth=3, tile_vertices=args.tile, flags=0)
+        d2h = 4 * (2 * (rows + len(batches)) + info.vt_nnz + info.vv_nnz + D * mesh.num_simplices)
+        h2d = host_T.numel() * 4
+        checksum = 0
+
+        def e2e_pass():
+            nonlocal checksum
+            g2.simplices.copy_(host_T, non_blocking=True)       # H2D of the step's input (same values)
+            inflight = 0
+
+            def drain_one():
+                nonlocal checksum
+                st, v = g2.pop(-1)
+                a = g2.view_arrays(v)
+                checksum += int(a["vt_offsets"][-1]) + int(a["vv_offsets"][-1]) + int(a["tt_indices"][-1])  # host reads
+                g2.release(v)
+
+            for ids in batches:
+                while g2.compute(ids) == gale.ERR_WOULD_BLOCK:
+                    drain_one(); inflight -= 1
+                inflight += 1
+            while inflight:
+                drain_one(); inflight -= 1
+
+        e2e_steps = max(1, min(args.steps, 3))
+        e2e_pass()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_pass()
+        barrier()
+        dt = (time.perf_counter() - t0) / e2e_steps
+        if dist:
+            t = torch.tensor([dt], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * mesh.num_simplices / dt, "unit": "tets/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": dt * 1e3, "steps": e2e_steps,
+               "what": "H2D of the simplex array from pinned memory + streamed pass, queue_depth=3, "
+                       "D2H of every CSR batch to pinned slots, pop+read+release on the host"}
+        g2.destroy()
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        v, sample = oracle_sample(mesh)
+        cpu = {"value": v, "unit": "tets/s", "cores": 1, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": "tets/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+                "config": workload_config(args, mesh, {"tile_vertices": info.tile_vertices, "num_tiles": info.num_tiles,
+                                                       "smem_bytes_per_block": info.smem_bytes,
+                                                       "device_ring": args.ring, "parallelism": f"replicas x{world}",
+                                                       "mesh_create_s": create_s, "mesh_generate_s": gen_s}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
