@@ -23,6 +23,7 @@ namespace {
 
 using gale::DeviceMesh;
 using gale::SmemCfg;
+using gale::TileDesc;
 
 thread_local std::string g_last_error;
 
@@ -37,11 +38,7 @@ thread_local std::string g_last_error;
 
 constexpr size_t kAlign = 256;
 inline size_t up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
-inline int pow2_at_least(long long x) {
-  int p = 64;
-  while (p < x) p <<= 1;
-  return p;
-}
+inline long long pad_to(long long x, long long a) { return (x + a - 1) / a * a; }
 constexpr int kSmemLimit = 227 * 1024;  // opt-in dynamic shared memory per block on sm_100
 
 // ---- result of the create-time analysis ----------------------------------------------------------
@@ -53,23 +50,23 @@ struct Plan {
   uint32_t flags = 0;
   std::vector<int32_t> cl_off;
   // index (host copies)
-  int tv = 0, nTiles = 0;
-  std::vector<int32_t> first_tet, opp_first, opp_perm, tile_vlo, cl_tile_begin, tex;
-  std::vector<long long> tex_off, vt_pref, vv_pref;
-  SmemCfg cfg{};
+  int tv = 0, nTiles = 0, NT = 0;
+  std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, halo;
+  std::vector<uint16_t> loc;            // 4 per staged simplex
+  std::vector<TileDesc> tiles;
+  SmemCfg cfg{};                        // capacities for the full relation mask
   int smem_bytes = 0;
+  long long ext_refs = 0, vt_total = 0, vv_total = 0;
   // per-cluster sizes
-  std::vector<long long> cl_vt, cl_vv;   // nnz per cluster
-  std::vector<int32_t> cl_t_lo;          // [nC+1] first internal simplex of cluster c (I_T)
+  std::vector<long long> cl_vt, cl_vv;  // nnz per cluster
+  std::vector<int32_t> cl_t_lo;         // [nC+1] first internal simplex of cluster c (I_T)
   long long max_rows = 0, max_vt = 0, max_vv = 0, max_tt = 0;
   double analyse_ms = 0;
 
   size_t index_bytes() const {
-    size_t b = 0;
-    b += up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) + up(tile_vlo.size() * 4);
-    b += up(cl_tile_begin.size() * 4) + up(tex.size() * 4 + 16) + up(tex_off.size() * 8) + up(vt_pref.size() * 8) +
-         up(vv_pref.size() * 8);
-    return b;
+    return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
+           up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
+           up(halo.size() * 4 + 16) + up(loc.size() * 2 + 16);
   }
 };
 
@@ -119,30 +116,55 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-// Tiles, T_ex per tile, maxima. Returns false if a tile exceeds the staging limits for this tv.
+inline int threads_for_tile(int tv) { return tv > 128 ? 512 : 256; }
+
+// Kernel capacities for one launch: regions the relation mask does not need are dropped.
+SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
+  SmemCfg c = full;
+  if (!(mask & gale::REL_VV)) { c.W = 0; c.vv_max = 0; }
+  if (!(mask & gale::REL_TT)) { c.cap = 0; c.nrec = 0; }
+  if (!(mask & gale::REL_VT)) c.vt_max = 0;
+  if (count_mode) { c.vt_max = 0; c.vv_max = 0; }
+  return c;
+}
+
+using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::OutPtrs);
+KernelFn kernel_for(int D, int NT) {
+  if (D == 4) return NT == 512 ? gale::gale_batch_kernel<4, 512> : gale::gale_batch_kernel<4, 256>;
+  return NT == 512 ? gale::gale_batch_kernel<3, 512> : gale::gale_batch_kernel<3, 256>;
+}
+
+// Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
+// simplices. Returns false if a tile exceeds a kernel limit for this tv (the caller retries smaller).
 bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   const int D = p.dim + 1;
   p.tv = tv;
-  p.tile_vlo.clear();
+  p.NT = threads_for_tile(tv);
+  std::vector<int32_t> tile_vlo;
   p.cl_tile_begin.assign(p.nC + 1, 0);
   for (int c = 0; c < p.nC; ++c) {
-    p.cl_tile_begin[c] = int(p.tile_vlo.size());
-    for (int v = p.cl_off[c]; v < p.cl_off[c + 1]; v += tv) p.tile_vlo.push_back(v);
+    p.cl_tile_begin[c] = int(tile_vlo.size());
+    for (int v = p.cl_off[c]; v < p.cl_off[c + 1]; v += tv) tile_vlo.push_back(v);
   }
-  p.cl_tile_begin[p.nC] = int(p.tile_vlo.size());
-  p.nTiles = int(p.tile_vlo.size());
-  p.tile_vlo.push_back(p.nV);
-  std::vector<int32_t> tile_of(p.nV);
-  for (int i = 0; i < p.nTiles; ++i)
-    for (int v = p.tile_vlo[i]; v < p.tile_vlo[i + 1]; ++v) tile_of[v] = i;
+  p.cl_tile_begin[p.nC] = int(tile_vlo.size());
+  p.nTiles = int(tile_vlo.size());
+  tile_vlo.push_back(p.nV);
+  const int nTiles = p.nTiles;
+  std::vector<int32_t> tile_of(p.nV), tile_vhi(nTiles);
+  for (int c = 0; c < p.nC; ++c)
+    for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) {
+      tile_vhi[i] = std::min(tile_vlo[i] + tv, p.cl_off[c + 1]);
+      for (int v = tile_vlo[i]; v < tile_vhi[i]; ++v) tile_of[v] = i;
+    }
   // T_ex: simplex t is external to every tile it touches other than the tile of its lowest vertex
-  p.tex_off.assign(p.nTiles + 1, 0);
+  std::vector<long long> raw_off(nTiles + 1, 0);
+  std::vector<int32_t> raw;
   for (int pass = 0; pass < 2; ++pass) {
     std::vector<long long> cur;
     if (pass == 1) {
-      for (int i = 0; i < p.nTiles; ++i) p.tex_off[i + 1] += p.tex_off[i];
-      p.tex.resize(size_t(p.tex_off[p.nTiles]));
-      cur.assign(p.tex_off.begin(), p.tex_off.end() - 1);
+      for (int i = 0; i < nTiles; ++i) raw_off[i + 1] += raw_off[i];
+      raw.resize(size_t(raw_off[nTiles]));
+      cur.assign(raw_off.begin(), raw_off.end() - 1);
     }
     for (long long t = 0; t < p.nT; ++t) {
       const int32_t* r = T.data() + t * D;
@@ -155,41 +177,194 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
         for (int s = 0; s < ns; ++s) dup |= seen[s] == tk;
         if (dup) continue;
         seen[ns++] = tk;
-        if (pass == 0) ++p.tex_off[tk + 1]; else p.tex[size_t(cur[tk]++)] = int32_t(t);
+        if (pass == 0) ++raw_off[tk + 1]; else raw[size_t(cur[tk]++)] = int32_t(t);
       }
     }
   }
-  long long smax = 0, sext = 0, sint = 0;
-  for (int i = 0; i < p.nTiles; ++i) {
-    const long long si = p.first_tet[p.tile_vlo[i + 1]] - p.first_tet[p.tile_vlo[i]];
-    const long long se = p.tex_off[i + 1] - p.tex_off[i];
-    smax = std::max(smax, si + se);
-    sext = std::max(sext, se);
-    sint = std::max(sint, si);
+  p.ext_refs = raw_off[nTiles];
+  // descriptors, padded offsets, limits that need no halo
+  p.tiles.assign(nTiles, TileDesc{});
+  long long stg = 0, texo = 0;
+  const int max_local = D == 4 ? gale::kMaxLocal4 : gale::kMaxLocal3;
+  for (int c = 0; c < p.nC; ++c)
+    for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) {
+      TileDesc& d = p.tiles[i];
+      d.v_lo = tile_vlo[i];
+      d.nrows = tile_vhi[i] - tile_vlo[i];
+      d.t_lo = p.first_tet[d.v_lo];
+      d.s_int = p.first_tet[tile_vhi[i]] - d.t_lo;
+      d.s_ext = int(raw_off[i + 1] - raw_off[i]);
+      d.row_rel = d.v_lo - p.cl_off[c];
+      d.tt_rel = d.t_lo - p.first_tet[p.cl_off[c]];
+      d.stg_off = stg;
+      d.tex_off = texo;
+      const long long S = (long long)d.s_int + d.s_ext;
+      if (S > (long long)gale::kItems * p.NT || 4LL * d.s_int + d.s_ext > gale::kMaxRec) return false;
+      stg += pad_to(S, 2);
+      texo += pad_to(d.s_ext, 4);
+    }
+  p.loc.assign(size_t(stg) * 4 + 8, 0);
+  p.tex.assign(size_t(texo) + 4, 0);
+  for (int i = 0; i < nTiles; ++i)
+    std::copy(raw.begin() + raw_off[i], raw.begin() + raw_off[i + 1], p.tex.begin() + p.tiles[i].tex_off);
+  // halo + local encoding, tiles split over host threads
+  const int nth = std::max(1, std::min<int>(32, std::min<int>(int(std::thread::hardware_concurrency()), nTiles / 64 + 1)));
+  std::vector<std::vector<int32_t>> halo_part(nth);
+  std::vector<int> tile_lo(nth + 1);
+  for (int w = 0; w <= nth; ++w) tile_lo[w] = int((long long)nTiles * w / nth);
+  std::atomic<bool> ok{true};
+  auto work = [&](int w) {
+    std::vector<uint16_t> map(size_t(p.nV), uint16_t(0xFFFF));
+    std::vector<int32_t>& hp = halo_part[w];
+    std::vector<int32_t> h;
+    for (int i = tile_lo[w]; i < tile_lo[w + 1] && ok.load(std::memory_order_relaxed); ++i) {
+      TileDesc& d = p.tiles[i];
+      const int v_lo = d.v_lo, v_hi = d.v_lo + d.nrows;
+      const int32_t* ex = p.tex.data() + d.tex_off;
+      auto simplex = [&](int s) { return T.data() + (long long)(s < d.s_ext ? ex[s] : d.t_lo + (s - d.s_ext)) * D; };
+      const int S = d.s_int + d.s_ext;
+      h.clear();
+      for (int s = 0; s < S; ++s) {
+        const int32_t* r = simplex(s);
+        for (int k = 0; k < D; ++k)
+          if ((r[k] < v_lo || r[k] >= v_hi) && map[r[k]] == 0xFFFF) { map[r[k]] = 0xFFFE; h.push_back(r[k]); }
+      }
+      std::sort(h.begin(), h.end());
+      const int nhalo = int(h.size());
+      const int nlo = int(std::lower_bound(h.begin(), h.end(), v_lo) - h.begin());
+      if (nhalo + d.nrows > max_local) {
+        for (int v : h) map[v] = 0xFFFF;
+        ok.store(false);
+        return;
+      }
+      for (int j = 0; j < nhalo; ++j) map[h[j]] = uint16_t(j < nlo ? j : j + d.nrows);
+      d.nlo = nlo;
+      d.nhalo = nhalo;
+      d.halo_off = (long long)hp.size();  // relative to this thread's part; rebased below
+      uint16_t* out = p.loc.data() + d.stg_off * 4;
+      for (int s = 0; s < S; ++s) {
+        const int32_t* r = simplex(s);
+        for (int k = 0; k < 4; ++k)
+          out[s * 4 + k] = k >= D ? uint16_t(0xFFFF)
+                                  : (r[k] >= v_lo && r[k] < v_hi) ? uint16_t(nlo + (r[k] - v_lo)) : map[r[k]];
+      }
+      hp.insert(hp.end(), h.begin(), h.end());
+      hp.resize(size_t(pad_to((long long)hp.size(), 4)), 0);
+      for (int v : h) map[v] = 0xFFFF;
+    }
+  };
+  {
+    std::vector<std::thread> th;
+    for (int w = 1; w < nth; ++w) th.emplace_back(work, w);
+    work(0);
+    for (auto& t : th) t.join();
+  }
+  if (!ok.load()) return false;
+  long long hoff = 0;
+  for (int w = 0; w < nth; ++w) {
+    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].halo_off += hoff;
+    hoff += (long long)halo_part[w].size();
+  }
+  p.halo.assign(size_t(hoff) + 4, 0);
+  hoff = 0;
+  for (int w = 0; w < nth; ++w) {
+    std::copy(halo_part[w].begin(), halo_part[w].end(), p.halo.begin() + hoff);
+    hoff += (long long)halo_part[w].size();
+    std::vector<int32_t>().swap(halo_part[w]);
+  }
+  // shared-memory capacities known so far
+  long long smax = 2, sext = 4, sint = 2, nhalo = 4, nloc = 1;
+  for (const TileDesc& d : p.tiles) {
+    smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 2));
+    sext = std::max(sext, pad_to(d.s_ext, 4));
+    sint = std::max<long long>(sint, d.s_int);
+    nhalo = std::max(nhalo, pad_to(d.nhalo, 4));
+    nloc = std::max<long long>(nloc, d.nhalo + d.nrows);
   }
   p.cfg = SmemCfg{};
   p.cfg.tv = tv;
-  p.cfg.smax = int(std::max(1LL, smax));
-  p.cfg.sext = int(std::max(1LL, sext));
-  p.cfg.sint = int(std::max(1LL, sint));
-  p.cfg.bm_words = (tv + 31) / 32;
-  return smax <= gale::kMaxStaged;
-}
-
-template <int D>
-int run_count(const Plan& p, const DeviceMesh& dm, const gale::CountCfg& cc, int smem, long long* d_stats,
-              cudaStream_t st) {
-  GALE_CUDA(cudaFuncSetAttribute(gale::gale_count_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  gale::gale_count_kernel<D><<<std::max(1, p.nTiles), gale::kThreads, smem, st>>>(dm, cc, p.nTiles, d_stats);
-  GALE_CUDA(cudaGetLastError());
-  return GALE_OK;
+  p.cfg.smax = int(smax);
+  p.cfg.sext = int(sext);
+  p.cfg.nhalo = int(nhalo);
+  p.cfg.W = int((nloc + 31) / 32) | 1;
+  p.cfg.nrec = int(pad_to(4 * sint, 8));
+  return true;
 }
 
 struct DevBuf {  // temporary device memory of the analysis
   void* p = nullptr;
   ~DevBuf() { if (p) cudaFree(p); }
   int alloc(size_t n) { GALE_CUDA(cudaMalloc(&p, std::max<size_t>(n, 16))); return GALE_OK; }
+  template <class V>
+  int upload(const V& v, cudaStream_t st) {
+    int rc = alloc(v.size() * sizeof(typename V::value_type));
+    if (rc != GALE_OK) return rc;
+    if (!v.empty())
+      GALE_CUDA(cudaMemcpyAsync(p, v.data(), v.size() * sizeof(typename V::value_type), cudaMemcpyHostToDevice, st));
+    return GALE_OK;
+  }
 };
+
+// Sizing run (count mode of the batch kernel) over all tiles: exact VT / VV entry counts and the
+// number of distinct facets per tile. Returns GALE_ERR_WORKSPACE-like codes via rc; `fits` tells
+// whether the count-mode shared memory fits at this tile size.
+int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long long>& stats, bool& fits) {
+  const int D = p.dim + 1;
+  fits = true;
+  stats.assign(size_t(p.nTiles) * 4, 0);
+  if (p.nTiles == 0) return GALE_OK;
+  long long rec_max = 1;
+  for (const TileDesc& d : p.tiles) rec_max = std::max(rec_max, 4LL * d.s_int + d.s_ext);
+  SmemCfg full = p.cfg;
+  full.cap = int(rec_max + 32);
+  // one launch for all three relations if the shared memory allows, else VT|VV and TT apart
+  std::vector<uint32_t> parts;
+  if (gale::make_layout(cfg_for_mask(full, 7, true)).total <= kSmemLimit) parts = {7u};
+  else parts = {3u, 4u};
+  for (uint32_t m : parts)
+    if (gale::make_layout(cfg_for_mask(full, m, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
+
+  DevBuf b_ft, b_tiles, b_tex, b_halo, b_loc, b_stats, b_err;
+  int rc;
+  if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
+      (rc = b_halo.upload(p.halo, st)) || (rc = b_loc.upload(p.loc, st)) ||
+      (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
+    return rc;
+  GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
+  DeviceMesh dm{};
+  dm.T = dT;
+  dm.first_tet = static_cast<int32_t*>(b_ft.p);
+  dm.tiles = static_cast<TileDesc*>(b_tiles.p);
+  dm.tex = static_cast<int32_t*>(b_tex.p);
+  dm.halo = static_cast<int32_t*>(b_halo.p);
+  dm.loc = static_cast<uint2*>(b_loc.p);
+  dm.err = static_cast<int32_t*>(b_err.p);
+  KernelFn fn = kernel_for(D, p.NT);
+  std::vector<long long> part_stats(stats.size());
+  for (uint32_t m : parts) {
+    const SmemCfg c = cfg_for_mask(full, m, true);
+    const int smem = gale::make_layout(c).total;
+    GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    gale::BatchParams P{};
+    P.mask = m | gale::MODE_COUNT;
+    gale::OutPtrs O{};
+    O.stats = static_cast<long long*>(b_stats.p);
+    fn<<<p.nTiles, p.NT, smem, st>>>(dm, P, c, O);
+    GALE_CUDA(cudaGetLastError());
+    GALE_CUDA(cudaMemcpyAsync(part_stats.data(), b_stats.p, stats.size() * 8, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    for (int i = 0; i < p.nTiles; ++i) {
+      if (m & 1) stats[i * 4 + 0] = part_stats[i * 4 + 0];
+      if (m & 2) stats[i * 4 + 1] = part_stats[i * 4 + 1];
+      if (m & 4) stats[i * 4 + 2] = part_stats[i * 4 + 2];
+    }
+  }
+  int err = 0;
+  GALE_CUDA(cudaMemcpyAsync(&err, b_err.p, 4, cudaMemcpyDeviceToHost, st));
+  GALE_CUDA(cudaStreamSynchronize(st));
+  if (err) { g_last_error = "device guard fired during sizing: " + std::to_string(err); return GALE_ERR_WORKSPACE; }
+  return GALE_OK;
+}
 
 int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& out) {
   const auto t0 = std::chrono::steady_clock::now();
@@ -215,9 +390,17 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   // I_T: first simplex whose lowest vertex is >= v; and the same keyed by the second vertex
   p->first_tet.assign(p->nV + 1, 0);
   p->opp_first.assign(p->nV + 1, 0);
-  for (long long t = 0; t < p->nT; ++t) {
-    ++p->first_tet[T[t * D] + 1];
-    ++p->opp_first[T[t * D + 1] + 1];
+  {
+    std::vector<int32_t> ranked(size_t(p->nV), 0);  // incidences of v in slots 1..D-1 (atomically ranked part of its VT row)
+    for (long long t = 0; t < p->nT; ++t) {
+      ++p->first_tet[T[t * D] + 1];
+      ++p->opp_first[T[t * D + 1] + 1];
+      for (int k = 1; k < D; ++k)
+        if (++ranked[T[t * D + k]] > gale::kMaxRowPart) {
+          g_last_error = "a vertex has more than 1023 incident simplices in which it is not the lowest vertex";
+          return GALE_ERR_UNSUPPORTED;
+        }
+    }
   }
   for (int v = 0; v < p->nV; ++v) {
     p->first_tet[v + 1] += p->first_tet[v];
@@ -231,74 +414,49 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   p->cl_t_lo.resize(p->nC + 1);
   for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
 
-  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kThreads) : (d.dim == 3 ? 128 : 256);
-  for (;; tv /= 2) {
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, 512) : (d.dim == 3 ? 256 : 512);
+  std::vector<long long> stats;
+  for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
-    if (!build_tiles(*p, T, tv)) continue;
-    // sizing run on the device (temporary copies of the index)
-    gale::CountCfg cc{tv, p->cfg.smax, p->cfg.sext, 8192, p->cfg.bm_words};
-    int csmem = gale::make_count_layout(cc, D).total;
-    while (csmem > kSmemLimit && cc.hcap > 256) { cc.hcap /= 2; csmem = gale::make_count_layout(cc, D).total; }
-    if (csmem > kSmemLimit) continue;
-    DevBuf b_ft, b_vlo, b_toff, b_tex, b_stats, b_err;
-    int rc;
-    if ((rc = b_ft.alloc(p->first_tet.size() * 4)) || (rc = b_vlo.alloc(p->tile_vlo.size() * 4)) ||
-        (rc = b_toff.alloc(p->tex_off.size() * 8)) || (rc = b_tex.alloc(p->tex.size() * 4)) ||
-        (rc = b_stats.alloc(size_t(p->nTiles) * 32)) || (rc = b_err.alloc(4)))
-      return rc;
-    GALE_CUDA(cudaMemcpyAsync(b_ft.p, p->first_tet.data(), p->first_tet.size() * 4, cudaMemcpyHostToDevice, st));
-    GALE_CUDA(cudaMemcpyAsync(b_vlo.p, p->tile_vlo.data(), p->tile_vlo.size() * 4, cudaMemcpyHostToDevice, st));
-    GALE_CUDA(cudaMemcpyAsync(b_toff.p, p->tex_off.data(), p->tex_off.size() * 8, cudaMemcpyHostToDevice, st));
-    if (!p->tex.empty())
-      GALE_CUDA(cudaMemcpyAsync(b_tex.p, p->tex.data(), p->tex.size() * 4, cudaMemcpyHostToDevice, st));
-    GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
-    DeviceMesh dm{};
-    dm.T = d.d_simplices;
-    dm.first_tet = static_cast<int32_t*>(b_ft.p);
-    dm.tile_vlo = static_cast<int32_t*>(b_vlo.p);
-    dm.tex_off = static_cast<long long*>(b_toff.p);
-    dm.tex = static_cast<int32_t*>(b_tex.p);
-    dm.err = static_cast<int32_t*>(b_err.p);
-    rc = D == 4 ? run_count<4>(*p, dm, cc, csmem, static_cast<long long*>(b_stats.p), st)
-                : run_count<3>(*p, dm, cc, csmem, static_cast<long long*>(b_stats.p), st);
-    if (rc != GALE_OK) return rc;
-    std::vector<long long> stats(size_t(p->nTiles) * 4);
-    int err = 0;
-    if (p->nTiles)
-      GALE_CUDA(cudaMemcpyAsync(stats.data(), b_stats.p, stats.size() * 8, cudaMemcpyDeviceToHost, st));
-    GALE_CUDA(cudaMemcpyAsync(&err, b_err.p, 4, cudaMemcpyDeviceToHost, st));
-    GALE_CUDA(cudaStreamSynchronize(st));
-    if (err & gale::ERR_COUNT_ROW_TOO_BIG) return GALE_ERR_UNSUPPORTED;
-    if (err) { g_last_error = "device guard fired during sizing: " + std::to_string(err); return GALE_ERR_WORKSPACE; }
-
-    p->vt_pref.assign(p->nTiles + 1, 0);
-    p->vv_pref.assign(p->nTiles + 1, 0);
-    long long vt_max = 1, vv_max = 1, uniq_max = 1, rec_max = 1;
-    for (int i = 0; i < p->nTiles; ++i) {
-      p->vt_pref[i + 1] = p->vt_pref[i] + stats[i * 4 + 0];
-      p->vv_pref[i + 1] = p->vv_pref[i] + stats[i * 4 + 1];
-      vt_max = std::max(vt_max, stats[i * 4 + 0]);
-      vv_max = std::max(vv_max, stats[i * 4 + 1]);
-      uniq_max = std::max(uniq_max, stats[i * 4 + 2]);
-      rec_max = std::max(rec_max, stats[i * 4 + 3]);
+    const bool last = tv == 1;
+    bool fits = build_tiles(*p, T, tv);
+    if (fits) {
+      int rc = run_sizing(*p, d.d_simplices, st, stats, fits);
+      if (rc != GALE_OK) return rc;
     }
-    p->cfg.vt_max = int(vt_max);
-    p->cfg.vv_max = int(vv_max);
-    p->cfg.vvh_cap = pow2_at_least(2 * uniq_max);
-    p->cfg.tth_cap = pow2_at_least(rec_max + 1);
-    p->smem_bytes = gale::make_layout(p->cfg, D).total;
-    if (p->smem_bytes > kSmemLimit) continue;
-    break;
+    if (fits) {
+      long long vt_max = 1, vv_max = 1, faces_max = 1;
+      for (int i = 0; i < p->nTiles; ++i) {
+        vt_max = std::max(vt_max, stats[i * 4 + 0]);
+        vv_max = std::max(vv_max, stats[i * 4 + 1]);
+        faces_max = std::max(faces_max, stats[i * 4 + 2]);
+      }
+      p->cfg.vt_max = int(pad_to(vt_max, 8));
+      p->cfg.vv_max = int(pad_to(vv_max, 8));
+      p->cfg.cap = int(pad_to(faces_max * 3 / 2 + 32, 4));   // load factor <= 2/3
+      p->smem_bytes = gale::make_layout(p->cfg).total;
+      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
+    }
+    if (fits) break;
+    if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
   }
-  // per-cluster sizes
-  p->cl_vt.resize(p->nC);
-  p->cl_vv.resize(p->nC);
+  // per-tile output placement inside its cluster, per-cluster sizes
+  p->cl_vt.assign(p->nC, 0);
+  p->cl_vv.assign(p->nC, 0);
   for (int c = 0; c < p->nC; ++c) {
-    p->cl_vt[c] = p->vt_pref[p->cl_tile_begin[c + 1]] - p->vt_pref[p->cl_tile_begin[c]];
-    p->cl_vv[c] = p->vv_pref[p->cl_tile_begin[c + 1]] - p->vv_pref[p->cl_tile_begin[c]];
+    long long vt = 0, vv = 0;
+    for (int i = p->cl_tile_begin[c]; i < p->cl_tile_begin[c + 1]; ++i) {
+      TileDesc& t = p->tiles[i];
+      if (vt > INT32_MAX || vv > INT32_MAX) return GALE_ERR_UNSUPPORTED;
+      t.vt_rel = int32_t(vt); t.vv_rel = int32_t(vv);
+      t.vt_nnz = int32_t(stats[i * 4 + 0]); t.vv_nnz = int32_t(stats[i * 4 + 1]);
+      vt += t.vt_nnz; vv += t.vv_nnz;
+    }
+    p->cl_vt[c] = vt; p->cl_vv[c] = vv;
+    p->vt_total += vt; p->vv_total += vv;
     p->max_rows = std::max<long long>(p->max_rows, p->cl_off[c + 1] - p->cl_off[c]);
-    p->max_vt = std::max(p->max_vt, p->cl_vt[c]);
-    p->max_vv = std::max(p->max_vv, p->cl_vv[c]);
+    p->max_vt = std::max(p->max_vt, vt);
+    p->max_vv = std::max(p->max_vv, vv);
     p->max_tt = std::max<long long>(p->max_tt, p->cl_t_lo[c + 1] - p->cl_t_lo[c]);
   }
   p->analyse_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
@@ -435,17 +593,18 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.first_tet = static_cast<int32_t*>(put(p->first_tet.data(), p->first_tet.size() * 4));
   m->dm.opp_first = static_cast<int32_t*>(put(p->opp_first.data(), p->opp_first.size() * 4));
   m->dm.opp_perm = static_cast<int32_t*>(put(p->opp_perm.data(), p->opp_perm.size() * 4));
-  m->dm.tile_vlo = static_cast<int32_t*>(put(p->tile_vlo.data(), p->tile_vlo.size() * 4));
   m->dm.cluster_tile_begin = static_cast<int32_t*>(put(p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4));
+  m->dm.tiles = static_cast<TileDesc*>(put(p->tiles.data(), p->tiles.size() * sizeof(TileDesc), 16));
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
-  m->dm.tex_off = static_cast<long long*>(put(p->tex_off.data(), p->tex_off.size() * 8));
-  m->dm.vt_pref = static_cast<long long*>(put(p->vt_pref.data(), p->vt_pref.size() * 8));
-  m->dm.vv_pref = static_cast<long long*>(put(p->vv_pref.data(), p->vv_pref.size() * 8));
+  m->dm.halo = static_cast<int32_t*>(put(p->halo.data(), p->halo.size() * 4, 16));
+  m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
   GALE_CUDA(cudaStreamSynchronize(st));
   std::vector<int32_t>().swap(p->opp_perm);
   std::vector<int32_t>().swap(p->tex);
+  std::vector<int32_t>().swap(p->halo);
+  std::vector<uint16_t>().swap(p->loc);
   std::vector<int32_t>().swap(p->opp_first);
 
   GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
@@ -466,10 +625,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   }
   m->workspace_used = o;
   if (desc->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
-  if (m->D == 4)
-    GALE_CUDA(cudaFuncSetAttribute(gale::gale_batch_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
-  else
-    GALE_CUDA(cudaFuncSetAttribute(gale::gale_batch_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
   m->plan = std::move(p);
   m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() +
                  (m->plan->analyse_ms);
@@ -482,9 +638,9 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   const Plan& p = *m->plan;
   out->tile_vertices = p.tv;
   out->num_tiles = p.nTiles;
-  out->num_external_refs = p.tex_off.empty() ? 0 : p.tex_off.back();
-  out->vt_nnz = p.vt_pref.empty() ? 0 : p.vt_pref.back();
-  out->vv_nnz = p.vv_pref.empty() ? 0 : p.vv_pref.back();
+  out->num_external_refs = p.ext_refs;
+  out->vt_nnz = p.vt_total;
+  out->vv_nnz = p.vv_total;
   out->smem_bytes = p.smem_bytes;
   out->max_staged = p.cfg.smax;
   out->slot_bytes = m->cap.total;
@@ -546,6 +702,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   O.vv_indices = reinterpret_cast<int32_t*>(s.dev + s.used.vv_idx);
   O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
 
+  const SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
+  const int smem = gale::make_layout(cfg).total;
   GALE_CUDA(cudaEventRecord(s.ev_start, st));
   for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
     gale::BatchParams P{};
@@ -562,10 +720,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.tt_base[i] = s.tt_row_begin[b + i];
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    if (D == 4)
-      gale::gale_batch_kernel<4><<<grid, gale::kThreads, p.smem_bytes, st>>>(m->dm, P, p.cfg, O);
-    else
-      gale::gale_batch_kernel<3><<<grid, gale::kThreads, p.smem_bytes, st>>>(m->dm, P, p.cfg, O);
+    kernel_for(D, p.NT)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, O);
     GALE_CUDA(cudaGetLastError());
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, st));
