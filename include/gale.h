@@ -72,7 +72,7 @@ typedef struct {
   int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4);
                                        a popped view stays valid until device_ring-1 later batches
                                        have been submitted                                            */
-  int32_t tile_vertices;            /* vertices per thread-block tile, <= 512 (0 = default)           */
+  int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = default)           */
   void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
                                        must outlive the handle                                       */
   size_t workspace_bytes;

@@ -51,7 +51,7 @@ struct Plan {
   std::vector<int32_t> cl_off;
   // index (host copies)
   int tv = 0, nTiles = 0, NT = 0;
-  std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, halo;
+  std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
   std::vector<uint16_t> loc;            // 4 per staged simplex
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
@@ -66,7 +66,7 @@ struct Plan {
   size_t index_bytes() const {
     return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
            up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(halo.size() * 4 + 16) + up(loc.size() * 2 + 16);
+           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16);
   }
 };
 
@@ -116,22 +116,24 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-inline int threads_for_tile(int tv) { return tv > 128 ? 512 : 256; }
+inline int threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : 128); }  // NT >= 2 * tv
 
 // Kernel capacities for one launch: regions the relation mask does not need are dropped.
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
   SmemCfg c = full;
-  if (!(mask & gale::REL_VV)) { c.W = 0; c.vv_max = 0; }
-  if (!(mask & gale::REL_TT)) { c.cap = 0; c.nrec = 0; }
-  if (!(mask & gale::REL_VT)) c.vt_max = 0;
+  if (!(mask & gale::REL_VV)) { c.WV = 0; c.vv_max = 0; }
+  if (!(mask & gale::REL_TT)) c.cap = 0;
+  if (!(mask & gale::REL_VT)) { c.WT = 0; c.vt_max = 0; }
   if (count_mode) { c.vt_max = 0; c.vv_max = 0; }
   return c;
 }
 
-using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::OutPtrs);
+using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::SmemLayout,
+                          const gale::OutPtrs);
 KernelFn kernel_for(int D, int NT) {
-  if (D == 4) return NT == 512 ? gale::gale_batch_kernel<4, 512> : gale::gale_batch_kernel<4, 256>;
-  return NT == 512 ? gale::gale_batch_kernel<3, 512> : gale::gale_batch_kernel<3, 256>;
+  if (D == 4)
+    return NT == 512 ? gale::gale_batch_kernel<4, 512> : (NT == 256 ? gale::gale_batch_kernel<4, 256> : gale::gale_batch_kernel<4, 128>);
+  return NT == 512 ? gale::gale_batch_kernel<3, 512> : (NT == 256 ? gale::gale_batch_kernel<3, 256> : gale::gale_batch_kernel<3, 128>);
 }
 
 // Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
@@ -199,7 +201,7 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       d.stg_off = stg;
       d.tex_off = texo;
       const long long S = (long long)d.s_int + d.s_ext;
-      if (S > (long long)gale::kItems * p.NT || 4LL * d.s_int + d.s_ext > gale::kMaxRec) return false;
+      if (S > gale::kMaxStaged || (long long)D * d.s_int + d.s_ext + 32 > gale::kMaxCap) return false;
       stg += pad_to(S, 2);
       texo += pad_to(d.s_ext, 4);
     }
@@ -209,13 +211,13 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     std::copy(raw.begin() + raw_off[i], raw.begin() + raw_off[i + 1], p.tex.begin() + p.tiles[i].tex_off);
   // halo + local encoding, tiles split over host threads
   const int nth = std::max(1, std::min<int>(32, std::min<int>(int(std::thread::hardware_concurrency()), nTiles / 64 + 1)));
-  std::vector<std::vector<int32_t>> halo_part(nth);
+  std::vector<std::vector<int32_t>> gid_part(nth);
   std::vector<int> tile_lo(nth + 1);
   for (int w = 0; w <= nth; ++w) tile_lo[w] = int((long long)nTiles * w / nth);
   std::atomic<bool> ok{true};
   auto work = [&](int w) {
     std::vector<uint16_t> map(size_t(p.nV), uint16_t(0xFFFF));
-    std::vector<int32_t>& hp = halo_part[w];
+    std::vector<int32_t>& hp = gid_part[w];
     std::vector<int32_t> h;
     for (int i = tile_lo[w]; i < tile_lo[w + 1] && ok.load(std::memory_order_relaxed); ++i) {
       TileDesc& d = p.tiles[i];
@@ -239,8 +241,8 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       }
       for (int j = 0; j < nhalo; ++j) map[h[j]] = uint16_t(j < nlo ? j : j + d.nrows);
       d.nlo = nlo;
-      d.nhalo = nhalo;
-      d.halo_off = (long long)hp.size();  // relative to this thread's part; rebased below
+      d.nloc = nhalo + d.nrows;
+      d.gid_off = (long long)hp.size();  // relative to this thread's part; rebased below
       uint16_t* out = p.loc.data() + d.stg_off * 4;
       for (int s = 0; s < S; ++s) {
         const int32_t* r = simplex(s);
@@ -248,7 +250,9 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
           out[s * 4 + k] = k >= D ? uint16_t(0xFFFF)
                                   : (r[k] >= v_lo && r[k] < v_hi) ? uint16_t(nlo + (r[k] - v_lo)) : map[r[k]];
       }
-      hp.insert(hp.end(), h.begin(), h.end());
+      hp.insert(hp.end(), h.begin(), h.begin() + nlo);  // local id -> global id, ascending
+      for (int v = v_lo; v < v_hi; ++v) hp.push_back(v);
+      hp.insert(hp.end(), h.begin() + nlo, h.end());
       hp.resize(size_t(pad_to((long long)hp.size(), 4)), 0);
       for (int v : h) map[v] = 0xFFFF;
     }
@@ -262,32 +266,32 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   if (!ok.load()) return false;
   long long hoff = 0;
   for (int w = 0; w < nth; ++w) {
-    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].halo_off += hoff;
-    hoff += (long long)halo_part[w].size();
+    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].gid_off += hoff;
+    hoff += (long long)gid_part[w].size();
   }
-  p.halo.assign(size_t(hoff) + 4, 0);
+  p.gid.assign(size_t(hoff) + 4, 0);
   hoff = 0;
   for (int w = 0; w < nth; ++w) {
-    std::copy(halo_part[w].begin(), halo_part[w].end(), p.halo.begin() + hoff);
-    hoff += (long long)halo_part[w].size();
-    std::vector<int32_t>().swap(halo_part[w]);
+    std::copy(gid_part[w].begin(), gid_part[w].end(), p.gid.begin() + hoff);
+    hoff += (long long)gid_part[w].size();
+    std::vector<int32_t>().swap(gid_part[w]);
   }
   // shared-memory capacities known so far
-  long long smax = 2, sext = 4, sint = 2, nhalo = 4, nloc = 1;
+  long long smax = 2, sext = 4, sint = 2, nloc = 4;
   for (const TileDesc& d : p.tiles) {
     smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 2));
     sext = std::max(sext, pad_to(d.s_ext, 4));
-    sint = std::max<long long>(sint, d.s_int);
-    nhalo = std::max(nhalo, pad_to(d.nhalo, 4));
-    nloc = std::max<long long>(nloc, d.nhalo + d.nrows);
+    sint = std::max(sint, pad_to(d.s_int, 2));
+    nloc = std::max(nloc, pad_to(d.nloc, 4));
   }
   p.cfg = SmemCfg{};
   p.cfg.tv = tv;
   p.cfg.smax = int(smax);
   p.cfg.sext = int(sext);
-  p.cfg.nhalo = int(nhalo);
-  p.cfg.W = int((nloc + 31) / 32) | 1;
-  p.cfg.nrec = int(pad_to(4 * sint, 8));
+  p.cfg.nloc = int(nloc);
+  p.cfg.sint = int(sint);
+  p.cfg.WT = int((smax + 31) / 32) | 1;
+  p.cfg.WV = int((nloc + 31) / 32) | 1;
   return true;
 }
 
@@ -314,9 +318,9 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   stats.assign(size_t(p.nTiles) * 4, 0);
   if (p.nTiles == 0) return GALE_OK;
   long long rec_max = 1;
-  for (const TileDesc& d : p.tiles) rec_max = std::max(rec_max, 4LL * d.s_int + d.s_ext);
+  for (const TileDesc& d : p.tiles) rec_max = std::max(rec_max, (long long)D * d.s_int + d.s_ext);
   SmemCfg full = p.cfg;
-  full.cap = int(rec_max + 32);
+  full.cap = int(rec_max + 32);  // distinct facets <= facet records
   // one launch for all three relations if the shared memory allows, else VT|VV and TT apart
   std::vector<uint32_t> parts;
   if (gale::make_layout(cfg_for_mask(full, 7, true)).total <= kSmemLimit) parts = {7u};
@@ -324,10 +328,10 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   for (uint32_t m : parts)
     if (gale::make_layout(cfg_for_mask(full, m, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
 
-  DevBuf b_ft, b_tiles, b_tex, b_halo, b_loc, b_stats, b_err;
+  DevBuf b_ft, b_tiles, b_tex, b_gid, b_loc, b_stats, b_err;
   int rc;
   if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
-      (rc = b_halo.upload(p.halo, st)) || (rc = b_loc.upload(p.loc, st)) ||
+      (rc = b_gid.upload(p.gid, st)) || (rc = b_loc.upload(p.loc, st)) ||
       (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
     return rc;
   GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
@@ -336,27 +340,28 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   dm.first_tet = static_cast<int32_t*>(b_ft.p);
   dm.tiles = static_cast<TileDesc*>(b_tiles.p);
   dm.tex = static_cast<int32_t*>(b_tex.p);
-  dm.halo = static_cast<int32_t*>(b_halo.p);
+  dm.gid = static_cast<int32_t*>(b_gid.p);
   dm.loc = static_cast<uint2*>(b_loc.p);
   dm.err = static_cast<int32_t*>(b_err.p);
   KernelFn fn = kernel_for(D, p.NT);
   std::vector<long long> part_stats(stats.size());
   for (uint32_t m : parts) {
     const SmemCfg c = cfg_for_mask(full, m, true);
-    const int smem = gale::make_layout(c).total;
+    const gale::SmemLayout lay = gale::make_layout(c);
+    const int smem = lay.total;
     GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     gale::BatchParams P{};
     P.mask = m | gale::MODE_COUNT;
     gale::OutPtrs O{};
     O.stats = static_cast<long long*>(b_stats.p);
-    fn<<<p.nTiles, p.NT, smem, st>>>(dm, P, c, O);
+    fn<<<p.nTiles, p.NT, smem, st>>>(dm, P, c, lay, O);
     GALE_CUDA(cudaGetLastError());
     GALE_CUDA(cudaMemcpyAsync(part_stats.data(), b_stats.p, stats.size() * 8, cudaMemcpyDeviceToHost, st));
     GALE_CUDA(cudaStreamSynchronize(st));
     for (int i = 0; i < p.nTiles; ++i) {
       if (m & 1) stats[i * 4 + 0] = part_stats[i * 4 + 0];
       if (m & 2) stats[i * 4 + 1] = part_stats[i * 4 + 1];
-      if (m & 4) stats[i * 4 + 2] = part_stats[i * 4 + 2];
+      if (m & 4) { stats[i * 4 + 2] = part_stats[i * 4 + 2]; stats[i * 4 + 3] = part_stats[i * 4 + 3]; }
     }
   }
   int err = 0;
@@ -390,17 +395,9 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   // I_T: first simplex whose lowest vertex is >= v; and the same keyed by the second vertex
   p->first_tet.assign(p->nV + 1, 0);
   p->opp_first.assign(p->nV + 1, 0);
-  {
-    std::vector<int32_t> ranked(size_t(p->nV), 0);  // incidences of v in slots 1..D-1 (atomically ranked part of its VT row)
-    for (long long t = 0; t < p->nT; ++t) {
-      ++p->first_tet[T[t * D] + 1];
-      ++p->opp_first[T[t * D + 1] + 1];
-      for (int k = 1; k < D; ++k)
-        if (++ranked[T[t * D + k]] > gale::kMaxRowPart) {
-          g_last_error = "a vertex has more than 1023 incident simplices in which it is not the lowest vertex";
-          return GALE_ERR_UNSUPPORTED;
-        }
-    }
+  for (long long t = 0; t < p->nT; ++t) {
+    ++p->first_tet[T[t * D] + 1];
+    ++p->opp_first[T[t * D + 1] + 1];
   }
   for (int v = 0; v < p->nV; ++v) {
     p->first_tet[v + 1] += p->first_tet[v];
@@ -414,7 +411,7 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   p->cl_t_lo.resize(p->nC + 1);
   for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
 
-  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, 512) : (d.dim == 3 ? 256 : 512);
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, 256) : (d.dim == 3 ? 128 : 256);
   std::vector<long long> stats;
   for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
@@ -433,9 +430,10 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
       }
       p->cfg.vt_max = int(pad_to(vt_max, 8));
       p->cfg.vv_max = int(pad_to(vv_max, 8));
-      p->cfg.cap = int(pad_to(faces_max * 3 / 2 + 32, 4));   // load factor <= 2/3
+      p->cfg.cap = int(std::min<long long>(pad_to(faces_max * 2 + 32, 4), gale::kMaxCap & ~3));   // load factor <= 1/2
       p->smem_bytes = gale::make_layout(p->cfg).total;
-      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
+      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit &&
+             faces_max + 32 <= p->cfg.cap;
     }
     if (fits) break;
     if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
@@ -596,14 +594,14 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.cluster_tile_begin = static_cast<int32_t*>(put(p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4));
   m->dm.tiles = static_cast<TileDesc*>(put(p->tiles.data(), p->tiles.size() * sizeof(TileDesc), 16));
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
-  m->dm.halo = static_cast<int32_t*>(put(p->halo.data(), p->halo.size() * 4, 16));
+  m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
   m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
   GALE_CUDA(cudaStreamSynchronize(st));
   std::vector<int32_t>().swap(p->opp_perm);
   std::vector<int32_t>().swap(p->tex);
-  std::vector<int32_t>().swap(p->halo);
+  std::vector<int32_t>().swap(p->gid);
   std::vector<uint16_t>().swap(p->loc);
   std::vector<int32_t>().swap(p->opp_first);
 
@@ -703,7 +701,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
 
   const SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
-  const int smem = gale::make_layout(cfg).total;
+  const gale::SmemLayout lay = gale::make_layout(cfg);
+  const int smem = lay.total;
   GALE_CUDA(cudaEventRecord(s.ev_start, st));
   for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
     gale::BatchParams P{};
@@ -720,7 +719,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.tt_base[i] = s.tt_row_begin[b + i];
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    kernel_for(D, p.NT)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, O);
+    kernel_for(D, p.NT)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, st));
