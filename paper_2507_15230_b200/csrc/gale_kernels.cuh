@@ -193,17 +193,18 @@ __device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t cap) {
 
 // a4: claim or find the slot of facet `key` for staged simplex `s`. The first arrival (claimer)
 // leaves s in the low half of the slot's pair word, the second (finder) in the high half; a facet
-// has at most two cofaces (C4). Returns the slot; `stat` accumulates claims (low 16 bits) and
-// probes (high bits) for the sizing run.
+// has at most two cofaces (C4). Returns the slot. COUNT (sizing run): `stat` accumulates claims
+// (low 16 bits) and probes (high bits).
+template <bool COUNT>
 __device__ __forceinline__ uint32_t tt_insert(uint32_t* keys, uint16_t* pair16, uint32_t cap, uint32_t key, int s,
                                               uint32_t& stat, int32_t* err) {
   uint32_t slot = hash_slot(key, cap);
   for (uint32_t probe = 0; probe < cap; ++probe) {
     const uint32_t prev = atomicCAS(&keys[slot], kEmpty32, key);
-    stat += 0x10000u;
+    if (COUNT) stat += 0x10000u;
     if (prev == kEmpty32) {
       pair16[2 * slot] = (uint16_t)s;
-      stat += 1u;
+      if (COUNT) stat += 1u;
       return slot;
     }
     if (prev == key) {
@@ -290,14 +291,14 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* s
 // The batch kernel: VT + VV + TT for every tile of the requested clusters (or, with MODE_COUNT,
 // the exact output sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer
 // likewise sizes its relation arrays before launch). NT >= 2 * rows per tile.
-template <int D, int NT>
+template <int D, int NT, bool COUNT>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2)))
 gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
                   const SmemLayout L, const OutPtrs O) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t mask = P.mask;
-  const bool count_only = (mask & MODE_COUNT) != 0;
+  constexpr bool count_only = COUNT;  // the host sets MODE_COUNT in the mask for this instantiation
   const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0, do_tt = (mask & REL_TT) != 0;
 
   // ---- block -> (cluster slot, tile) ----------------------------------------------------------
@@ -381,21 +382,53 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     uint16_t* pair16 = reinterpret_cast<uint16_t*>(pair);
     const uint32_t cap = (uint32_t)C.cap;
     uint32_t stat = 0u;
-    for (int i = tid; i < s_int; i += NT) {
-      int l[4];
-      unpack_local(tets[s_ext + i], l);
-      const int s = s_ext + i;
-      const uint32_t s0 = tt_insert(keys, pair16, cap, facet_key<D, 0>(l), s, stat, M.err);
-      const uint32_t s1 = tt_insert(keys, pair16, cap, facet_key<D, 1>(l), s, stat, M.err);
-      const uint32_t s2 = tt_insert(keys, pair16, cap, facet_key<D, 2>(l), s, stat, M.err);
-      uint32_t s3 = 0u;
-      if constexpr (D == 4) s3 = tt_insert(keys, pair16, cap, facet_key<D, 3>(l), s, stat, M.err);
-      slots[i] = make_uint2(s0 | (s1 << 16), s2 | (s3 << 16));
+    {
+      // A thread walks the facets of its internal simplices i = tid, tid + NT, ... in ONE flat probe
+      // loop: a lane whose facet settles goes on to its next facet while others still probe.
+      int i = tid, k = 0;
+      uint32_t kq[4] = {0u, 0u, 0u, 0u};  // keys of the facets of simplex i not yet placed; kq[0] is current
+      uint32_t sl_lo = 0u, sl_hi = 0u;    // the D slots of simplex i, 16 bits each, shifted in from the top
+      if (i < s_int) {
+        int l[4];
+        unpack_local(tets[s_ext + i], l);
+        kq[0] = facet_key<D, 0>(l); kq[1] = facet_key<D, 1>(l); kq[2] = facet_key<D, 2>(l);
+        if constexpr (D == 4) kq[3] = facet_key<D, 3>(l);
+      }
+      uint32_t slot = hash_slot(kq[0], cap), tries = 0u;
+      while (i < s_int) {
+        const uint32_t prev = atomicCAS(&keys[slot], kEmpty32, kq[0]);
+        if (COUNT) stat += 0x10000u;
+        if (prev == kEmpty32 || prev == kq[0]) {
+          pair16[2 * slot + (prev != kEmpty32 ? 1 : 0)] = (uint16_t)(s_ext + i);
+          if (COUNT) stat += prev == kEmpty32 ? 1u : 0u;
+          sl_lo = __funnelshift_r(sl_lo, sl_hi, 16);
+          sl_hi = (sl_hi >> 16) | (slot << 16);
+          if (++k == D) {
+            if constexpr (D == 3) { sl_lo = __funnelshift_r(sl_lo, sl_hi, 16); sl_hi >>= 16; }
+            slots[i] = make_uint2(sl_lo, sl_hi);
+            i += NT;
+            k = 0;
+            if (i < s_int) {
+              int l[4];
+              unpack_local(tets[s_ext + i], l);
+              kq[0] = facet_key<D, 0>(l); kq[1] = facet_key<D, 1>(l); kq[2] = facet_key<D, 2>(l);
+              if constexpr (D == 4) kq[3] = facet_key<D, 3>(l);
+            }
+          } else {
+            kq[0] = kq[1]; kq[1] = kq[2]; kq[2] = kq[3];
+          }
+          slot = hash_slot(kq[0], cap);
+          tries = 0u;
+        } else {
+          slot = slot + 1 == cap ? 0u : slot + 1;
+          if (++tries > cap) { raise_err(M.err, ERR_TT_TABLE_FULL); break; }
+        }
+      }
     }
     for (int e = tid; e < s_ext; e += NT) {
       int l[4];
       unpack_local(tets[e], l);
-      if ((unsigned)(l[1] - nlo) < (unsigned)nrows) tt_insert(keys, pair16, cap, facet_key<D, 0>(l), e, stat, M.err);
+      if ((unsigned)(l[1] - nlo) < (unsigned)nrows) tt_insert<COUNT>(keys, pair16, cap, facet_key<D, 0>(l), e, stat, M.err);
     }
     if (count_only) {
       atomicAdd(&scan[37], stat & 0xFFFFu);
@@ -499,18 +532,19 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     const int vrow = tid - NT / 2;
     const bool vv_thread = do_vv && vrow >= 0 && vrow < nrows;
     const int wT = (S + 31) >> 5, wV = (td.nloc + 31) >> 5;
+    int nbits = 0;  // set bits of this thread's row
     {
       uint32_t deg = 0u;
       if (vt_thread) {
         const uint32_t* row = bmT + tid * WT;
 #pragma unroll 4
-        for (int w = 0; w < wT; ++w) deg += __popc(row[w]);
-        deg += (uint32_t)(ft[tid + 1] - ft[tid]);
+        for (int w = 0; w < wT; ++w) nbits += __popc(row[w]);
+        deg = (uint32_t)(nbits + ft[tid + 1] - ft[tid]);
       } else if (vv_thread) {
         const uint32_t* row = bmV + vrow * WV;
 #pragma unroll 4
-        for (int w = 0; w < wV; ++w) deg += __popc(row[w]);
-        deg <<= 16;
+        for (int w = 0; w < wV; ++w) nbits += __popc(row[w]);
+        deg = (uint32_t)nbits << 16;
       }
       const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);
       if (vt_thread) off_vt[tid] = (int)(ex & 0xFFFFu);
@@ -530,30 +564,30 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
 
     // ---- expand the rows into the staging areas, ids translated back to global ------------------
+    // One loop iteration per set bit (not per word): lanes of a warp run in step however their
+    // bits are spread over the words of their rows.
     if (vt_thread) {
       O.vt_offsets[row0 + tid] = vt0 + (int)off_vt[tid];
       const uint32_t* row = bmT + tid * WT;
-      int p = off_vt[tid];
-      for (int w = 0; w < wT; ++w) {
-        uint32_t bits = row[w];
-        while (bits) {
-          const int s = w * 32 + __ffs(bits) - 1;
-          bits &= bits - 1;
-          st_vt[p++] = s < s_ext ? texid[s] : t_lo + (s - s_ext);
-        }
+      int p = off_vt[tid], sbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nbits; ++n) {
+        while (bits == 0u) { bits = *row++; sbase += 32; }
+        const int s = sbase + __ffs(bits) - 1;
+        bits &= bits - 1;
+        st_vt[p++] = s < s_ext ? texid[s] : t_lo + (s - s_ext);
       }
       for (int j = ft[tid]; j < ft[tid + 1]; ++j) st_vt[p++] = t_lo + j;
     } else if (vv_thread) {
       O.vv_offsets[row0 + vrow] = vv0 + (int)off_vv[vrow];
       const uint32_t* row = bmV + vrow * WV;
-      int p = off_vv[vrow];
-      for (int w = 0; w < wV; ++w) {
-        uint32_t bits = row[w];
-        while (bits) {
-          const int l = w * 32 + __ffs(bits) - 1;
-          bits &= bits - 1;
-          st_vv[p++] = gid[l];
-        }
+      int p = off_vv[vrow], lbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nbits; ++n) {
+        while (bits == 0u) { bits = *row++; lbase += 32; }
+        const int l = lbase + __ffs(bits) - 1;
+        bits &= bits - 1;
+        st_vv[p++] = gid[l];
       }
     }
     __syncthreads();

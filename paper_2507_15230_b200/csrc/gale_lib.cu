@@ -130,10 +130,14 @@ SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
 
 using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::SmemLayout,
                           const gale::OutPtrs);
-KernelFn kernel_for(int D, int NT) {
-  if (D == 4)
-    return NT == 512 ? gale::gale_batch_kernel<4, 512> : (NT == 256 ? gale::gale_batch_kernel<4, 256> : gale::gale_batch_kernel<4, 128>);
-  return NT == 512 ? gale::gale_batch_kernel<3, 512> : (NT == 256 ? gale::gale_batch_kernel<3, 256> : gale::gale_batch_kernel<3, 128>);
+template <int D, bool COUNT>
+KernelFn kernel_for_nt(int NT) {
+  return NT == 512 ? gale::gale_batch_kernel<D, 512, COUNT>
+                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT> : gale::gale_batch_kernel<D, 128, COUNT>);
+}
+KernelFn kernel_for(int D, int NT, bool count) {
+  if (D == 4) return count ? kernel_for_nt<4, true>(NT) : kernel_for_nt<4, false>(NT);
+  return count ? kernel_for_nt<3, true>(NT) : kernel_for_nt<3, false>(NT);
 }
 
 // Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
@@ -343,7 +347,7 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   dm.gid = static_cast<int32_t*>(b_gid.p);
   dm.loc = static_cast<uint2*>(b_loc.p);
   dm.err = static_cast<int32_t*>(b_err.p);
-  KernelFn fn = kernel_for(D, p.NT);
+  KernelFn fn = kernel_for(D, p.NT, true);
   std::vector<long long> part_stats(stats.size());
   for (uint32_t m : parts) {
     const SmemCfg c = cfg_for_mask(full, m, true);
@@ -623,7 +627,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   }
   m->workspace_used = o;
   if (desc->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
-  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT, false), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
   m->plan = std::move(p);
   m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() +
                  (m->plan->analyse_ms);
@@ -719,7 +723,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.tt_base[i] = s.tt_row_begin[b + i];
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    kernel_for(D, p.NT)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
+    kernel_for(D, p.NT, false)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, st));
