@@ -10,19 +10,21 @@
 // Every external simplex has a smaller global id than every internal one (its lowest vertex lies
 // below the tile), so the staged order s = 0..S-1 ascends with the global simplex id.
 //
-// Phases of a block (shared memory of the TT phase is reused by the VT/VV phase):
-//   a1  stage the list (8 B per simplex), the external simplices' global ids and the local->global
-//       vertex table into shared memory with 16-byte cp.async;
-//   a4  TT: every facet (ascending local ids packed in 32 bits) claims or finds its slot in an
-//       open-addressing table of keys by one atomicCAS per probe; the claimer and the finder each
-//       leave their staged index in one half of the slot's pair word, so after a barrier the two
-//       cofaces read each other with no key re-derivation. An external simplex can only meet an
-//       internal one through the facet opposite its lowest vertex, and only if its second vertex is
-//       in the tile;
+// Phases of a block:
+//   a1  stage the list (8 B per simplex), the external simplices' global ids, the local->global
+//       vertex table and the tile's second-vertex index into shared memory with 16-byte cp.async;
+//   a4  TT, one thread per tile vertex p and no atomics: a facet whose lowest vertex is p has all
+//       its cofaces among the simplices whose lowest vertex is p (the contiguous run
+//       first_tet[p]..first_tet[p+1], facets 1..D-1) and the staged simplices whose second vertex
+//       is p (their facet 0; listed per tile vertex by the create-time index, like the paper's
+//       sorted lists bounded by interval arrays). The thread walks these
+//       few records through a private open-addressing table keyed by the facet's other vertices;
+//       the second arrival of a key meets the first and both TT entries are written to a
+//       shared-memory copy of the tile's TT rows;
 //   a5  TT fallback: the facet opposite the lowest vertex a of an internal simplex (a,b,..) with b
-//       outside the tile may have its coface outside the staged set; such facets are compacted
-//       into a queue and resolved one per thread from global memory through the run of simplices
-//       starting with b and the index of simplices whose second vertex is b (DESIGN.md §TT fallback);
+//       outside the tile belongs to no vertex of the tile; such facets are compacted into a queue
+//       and resolved one per thread from global memory through the run of simplices starting with
+//       b and the index of simplices whose second vertex is b (DESIGN.md §TT fallback);
 //   a2  VT: one bit per (row, staged simplex) in a rows x S bitmap (atomicOr); expanding a row
 //       yields its simplices in ascending order with no sort; the simplices whose *lowest* vertex
 //       is v are the contiguous run first_tet[v]..first_tet[v+1] and are appended without bits;
@@ -39,17 +41,17 @@ namespace gale {
 
 constexpr int kMaxBatch = 128;         // clusters per kernel launch (descriptor lives in kernel params)
 constexpr uint32_t kEmpty32 = 0xFFFFFFFFu;
-constexpr uint32_t kNoMate = 0xFFFFu;
 constexpr int kMaxStaged = 65534;      // staged simplices per tile (16-bit staged indices)
-constexpr int kMaxCap = 65535;         // facet-table slots (16-bit slot numbers)
-constexpr int kMaxLocal4 = 1024;       // tetrahedra: 10-bit local ids (30-bit facet key)
-constexpr int kMaxLocal3 = 65534;      // triangles: 16-bit local ids
+constexpr int kMaxLocal4 = 1024;       // tetrahedra: 10-bit local ids (20-bit facet key + 12-bit record)
+constexpr int kMaxLocal3 = 65534;      // triangles: 16-bit local ids (16-bit facet key + 16-bit record)
+constexpr int kMaxGroup4 = 4095;       // facet records of one vertex (tetrahedra / triangles)
+constexpr int kMaxGroup3 = 65534;
 constexpr int kMaxNnz16 = 65535;       // VT / VV entries of one tile (16-bit packed scan)
 
 enum { REL_VT = 1, REL_VV = 2, REL_TT = 4, MODE_COUNT = 8 };
 enum { ERR_TT_TABLE_FULL = 2, ERR_SIZE_MISMATCH = 4 };
 
-// Per-tile record built by gale_mesh_create (80 bytes, 16-byte aligned).
+// Per-tile record built by gale_mesh_create (96 bytes, 16-byte aligned).
 struct TileDesc {
   int32_t v_lo, nrows;        // vertices [v_lo, v_lo+nrows)
   int32_t t_lo, s_int;        // internal simplices [t_lo, t_lo+s_int)
@@ -58,12 +60,14 @@ struct TileDesc {
   int32_t row_rel, tt_rel;    // first row / first TT row of the tile inside its cluster
   int32_t vt_rel, vv_rel;     // first VT / VV entry of the tile inside its cluster
   int32_t vt_nnz, vv_nnz;     // entries of the tile (fixed at create; the kernel re-derives them)
-  int32_t pad0;
+  int32_t n_opp;              // staged simplices whose second vertex is in the tile
   long long stg_off;          // first staged simplex of the tile in DeviceMesh::loc (even)
   long long tex_off;          // first entry in DeviceMesh::tex (multiple of 4)
   long long gid_off;          // first entry in DeviceMesh::gid (multiple of 4)
+  long long opp_off;          // first entry in DeviceMesh::opp (multiple of 8)
+  long long pad0;
 };
-static_assert(sizeof(TileDesc) == 80, "TileDesc layout");
+static_assert(sizeof(TileDesc) == 96, "TileDesc layout");
 
 // Device-resident index built by gale_mesh_create (all pointers DEVICE).
 struct DeviceMesh {
@@ -75,6 +79,8 @@ struct DeviceMesh {
   const uint2* loc;                   // staged simplices in tile-local ids, 4 x uint16 each
   const int32_t* tex;                 // per-tile ascending global ids of external simplices (T_ex)
   const int32_t* gid;                 // per-tile global vertex id of every local id (ascending)
+  const uint16_t* opp;                // per tile: [tv_pad] start of row r, then the staged indices of the
+                                      // simplices whose second vertex is row r, ascending, rows in order
   const int32_t* cluster_tile_begin;  // [nC+1]
   int32_t* err;                       // sticky device error flags (host-mapped)
 };
@@ -86,8 +92,9 @@ struct SmemCfg {
   int smax;      // staged simplices (even)
   int sext;      // external simplices (multiple of 4)
   int nloc;      // local vertex ids (multiple of 4)
-  int sint;      // internal simplices (even): slot words + fallback queue
-  int cap;       // facet table slots, 0 without TT
+  int sint;      // internal simplices (even): TT row copy + fallback queue, 0 without TT
+  int nopp;      // second-vertex index entries incl. the row starts (multiple of 8), 0 without TT
+  int hs;        // table slots per tile vertex (power of two), 0 without TT
   int WT;        // VT bitmap words per row (odd), 0 without VT
   int WV;        // VV bitmap words per row (odd), 0 without VV
   int vt_max;    // VT entries staged for write-out, 0 without VT or in count mode
@@ -95,39 +102,41 @@ struct SmemCfg {
 };
 
 // Byte offsets of the shared-memory regions, computed on the host (make_layout) and passed as a
-// kernel parameter. [keys, pair, slots] and [bmT, bmV, stage_vt, stage_vv] share one union.
+// kernel parameter. The TT tables / TT row copy and the VT/VV staging share one union (the tables
+// are dead before the rows are expanded).
 struct SmemLayout {
-  int tets, texid, gid, ft, off_vt, off_vv, fbq, scan, uni;
-  int keys, pair, slots;            // TT phase
-  int bmT, bmV, st_vt, st_vv;       // VT/VV phase
-  int uni_tt_end, bm_end, total;
+  int tets, texid, gid, opp, ft, off_vt, off_vv, fbq, scan, bmT, bmV, bm_end;
+  int tbl, ttrow, tt_end;           // TT phase
+  int st_vt, st_vv;                 // write-out staging
+  int total;
 };
 
 __host__ __device__ inline int align16(int x) { return (x + 15) & ~15; }
+__host__ __device__ inline int opp_rows_pad(int tv) { return (tv + 1 + 7) & ~7; }
 
+template <int D>
 __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   SmemLayout L;
   int o = 0;
   L.tets = o;   o = align16(o + c.smax * 8);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
+  L.opp = o;    o = align16(o + c.nopp * 2);
   L.ft = o;     o = align16(o + (c.tv + 1) * 4);
   L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
   L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
-  L.fbq = o;    o = align16(o + (c.cap ? c.sint * 2 : 0));
+  L.fbq = o;    o = align16(o + c.sint * 2);
   L.scan = o;   o = align16(o + 48 * 4);
-  L.uni = o;
-  L.keys = o;   o = align16(o + c.cap * 4);
-  L.pair = o;   o = align16(o + c.cap * 4);
-  L.slots = o;  o = align16(o + (c.cap ? c.sint * 8 : 0));
-  L.uni_tt_end = o;
-  o = L.uni;
   L.bmT = o;    o = align16(o + c.tv * c.WT * 4);
   L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
   L.bm_end = o;
+  L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
+  L.ttrow = o;  o = align16(o + c.sint * D * 4);
+  L.tt_end = o;
+  o = L.tbl;
   L.st_vt = o;  o = align16(o + c.vt_max * 4);
   L.st_vv = o;  o = align16(o + c.vv_max * 4);
-  L.total = o > L.uni_tt_end ? o : L.uni_tt_end;
+  L.total = o > L.tt_end ? o : L.tt_end;
   return L;
 }
 
@@ -152,7 +161,7 @@ struct OutPtrs {
   int32_t* vv_offsets;
   int32_t* vv_indices;
   int32_t* tt_indices;
-  long long* stats;                  // count mode: [nTiles][4] = VT nnz, VV nnz, distinct facets, probes
+  long long* stats;                  // count mode: [nTiles][4] = VT nnz, VV nnz, 0, 0
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -167,54 +176,6 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 __device__ __forceinline__ void unpack_local(const uint2 q, int (&l)[4]) {
   l[0] = q.x & 0xFFFF; l[1] = q.x >> 16; l[2] = q.y & 0xFFFF; l[3] = q.y >> 16;
-}
-
-// Key of the facet opposite local vertex K: the remaining local ids (ascending) packed in 32 bits
-// (tetrahedra: 3 x 10 bits, triangles: 2 x 16 bits). Never equals kEmpty32.
-template <int D, int K>
-__device__ __forceinline__ uint32_t facet_key(const int (&l)[4]) {
-  if constexpr (D == 4) {
-    const int a = K == 0 ? l[1] : l[0];
-    const int b = K <= 1 ? l[2] : l[1];
-    const int c = K <= 2 ? l[3] : l[2];
-    return (uint32_t)a | ((uint32_t)b << 10) | ((uint32_t)c << 20);
-  } else {
-    const int a = K == 0 ? l[1] : l[0];
-    const int b = K <= 1 ? l[2] : l[1];
-    return (uint32_t)a | ((uint32_t)b << 16);
-  }
-}
-__device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t cap) {
-  uint32_t h = key * 0x9E3779B1u;
-  h ^= h >> 15;
-  h *= 0x85EBCA77u;
-  return __umulhi(h, cap);
-}
-
-// a4: claim or find the slot of facet `key` for staged simplex `s`. The first arrival (claimer)
-// leaves s in the low half of the slot's pair word, the second (finder) in the high half; a facet
-// has at most two cofaces (C4). Returns the slot. COUNT (sizing run): `stat` accumulates claims
-// (low 16 bits) and probes (high bits).
-template <bool COUNT>
-__device__ __forceinline__ uint32_t tt_insert(uint32_t* keys, uint16_t* pair16, uint32_t cap, uint32_t key, int s,
-                                              uint32_t& stat, int32_t* err) {
-  uint32_t slot = hash_slot(key, cap);
-  for (uint32_t probe = 0; probe < cap; ++probe) {
-    const uint32_t prev = atomicCAS(&keys[slot], kEmpty32, key);
-    if (COUNT) stat += 0x10000u;
-    if (prev == kEmpty32) {
-      pair16[2 * slot] = (uint16_t)s;
-      if (COUNT) stat += 1u;
-      return slot;
-    }
-    if (prev == key) {
-      pair16[2 * slot + 1] = (uint16_t)s;
-      return slot;
-    }
-    slot = slot + 1 == cap ? 0u : slot + 1;
-  }
-  raise_err(err, ERR_TT_TABLE_FULL);
-  return 0u;
 }
 
 template <int D>
@@ -287,10 +248,82 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* s
   return base + inc - x;
 }
 
+
 // ------------------------------------------------------------------------------------------------
-// The batch kernel: VT + VV + TT for every tile of the requested clusters (or, with MODE_COUNT,
-// the exact output sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer
-// likewise sizes its relation arrays before launch). NT >= 2 * rows per tile.
+// a4 helpers. A facet record of vertex p's group is numbered j: first the facets 1..D-1 of the
+// simplices of the run of p (j = (D-1) * q + k-1 for the q-th simplex of the run), then facet 0 of
+// the simplices whose second vertex is p, in the order of the tile's second-vertex index.
+template <int D>
+struct FacetBits {  // table word = key | (j << kKeyBits); the key holds the facet's vertices other than p
+  static constexpr int kKeyBits = D == 4 ? 20 : 16;
+  static constexpr uint32_t kKeyMask = (1u << kKeyBits) - 1u;
+};
+
+struct GroupCtx {
+  uint32_t* tbl;           // this vertex's table, hs slots
+  uint32_t hmask;
+  int hshift;
+  int32_t* ttrow;          // shared-memory copy of the tile's TT rows, D entries per internal simplex
+  const int32_t* texid;
+  const uint16_t* opp_idx; // second-vertex records of p
+  int run0;                // first internal simplex (index in the tile) of the run of p
+  int nrun;                // (D-1) * simplices in the run
+  int s_ext, t_lo;
+};
+
+__device__ __forceinline__ int global_simplex(const GroupCtx& g, int s) {
+  return s < g.s_ext ? g.texid[s] : g.t_lo + (s - g.s_ext);
+}
+
+// Place record j = facet k of staged simplex s with key `key`: claim an empty slot, or meet the
+// record that holds the same key (the other coface) and write both TT entries.
+template <int D>
+__device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int j, int s, int k, int32_t* err) {
+  using FB = FacetBits<D>;
+  uint32_t h = (key * 0x9E3779B1u) >> g.hshift;
+  for (uint32_t probe = 0; probe <= g.hmask; ++probe) {
+    const uint32_t cur = g.tbl[h];
+    if (cur == kEmpty32) {
+      g.tbl[h] = key | ((uint32_t)j << FB::kKeyBits);
+      return;
+    }
+    if ((cur & FB::kKeyMask) == key) {
+      const int j2 = (int)(cur >> FB::kKeyBits);
+      int s2, k2;
+      if (j2 < g.nrun) {
+        const int q = j2 / (D - 1);
+        s2 = g.s_ext + g.run0 + q;
+        k2 = 1 + j2 - q * (D - 1);
+      } else {
+        s2 = g.opp_idx[j2 - g.nrun];
+        k2 = 0;
+      }
+      if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = global_simplex(g, s2);
+      if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = global_simplex(g, s);
+      return;
+    }
+    h = (h + 1) & g.hmask;
+  }
+  raise_err(err, ERR_TT_TABLE_FULL);
+}
+
+// Key of the facet of a simplex with lowest vertex p that omits local vertex K (1 <= K < D): the
+// facet's vertices other than p, ascending. For K = 0 (simplex (x, p, ..)): the vertices after p.
+template <int D, int K>
+__device__ __forceinline__ uint32_t group_key(const int (&l)[4]) {
+  if constexpr (D == 4) {
+    const int a = K <= 1 ? l[2] : l[1];
+    const int b = (K == 0 || K == 1 || K == 2) ? l[3] : l[2];
+    return (uint32_t)a | ((uint32_t)b << 10);
+  } else {
+    return (uint32_t)(K <= 1 ? l[2] : l[1]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The batch kernel: VT + VV + TT for every tile of the requested clusters (or, COUNT, the exact
+// VT / VV sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer likewise
+// sizes its relation arrays before launch). NT >= 2 * rows per tile.
 template <int D, int NT, bool COUNT>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2)))
 gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
@@ -298,12 +331,12 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t mask = P.mask;
-  constexpr bool count_only = COUNT;  // the host sets MODE_COUNT in the mask for this instantiation
-  const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0, do_tt = (mask & REL_TT) != 0;
+  const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0;
+  const bool do_tt = !COUNT && (mask & REL_TT) != 0;
 
   // ---- block -> (cluster slot, tile) ----------------------------------------------------------
   int slot = 0, tile;
-  if (count_only) {
+  if (COUNT) {
     tile = P.tile_base + (int)blockIdx.x;
   } else {
     if (blockIdx.x == 0 && tid == 0) {  // terminal offsets (also covers batches without rows)
@@ -333,16 +366,16 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   uint2* tets = reinterpret_cast<uint2*>(smem + L.tets);
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
+  uint16_t* opp = reinterpret_cast<uint16_t*>(smem + L.opp);
   int32_t* ft = reinterpret_cast<int32_t*>(smem + L.ft);
   int32_t* off_vt = reinterpret_cast<int32_t*>(smem + L.off_vt);
   int32_t* off_vv = reinterpret_cast<int32_t*>(smem + L.off_vv);
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
-  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scan, [36] queue length, [37] claims, [38] probes
-  uint32_t* keys = reinterpret_cast<uint32_t*>(smem + L.keys);
-  uint32_t* pair = reinterpret_cast<uint32_t*>(smem + L.pair);
-  uint2* slots = reinterpret_cast<uint2*>(smem + L.slots);
+  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scan, [36] queue length, [37] chunk counter
   uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
   uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
+  uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
+  int32_t* ttrow = reinterpret_cast<int32_t*>(smem + L.ttrow);
   int32_t* st_vt = reinterpret_cast<int32_t*>(smem + L.st_vt);
   int32_t* st_vv = reinterpret_cast<int32_t*>(smem + L.st_vv);
 
@@ -350,6 +383,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   const int vt0 = P.vt_base[slot] + td.vt_rel;
   const int vv0 = P.vv_base[slot] + td.vv_rel;
   const int tt0 = P.tt_base[slot] + td.tt_rel;
+  const int opp_rows = opp_rows_pad(nrows);
 
   // ---- a1: stage + clear ----------------------------------------------------------------------
   {
@@ -362,176 +396,136 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
     int4* gdst = reinterpret_cast<int4*>(gid);
     for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
+    if (do_tt) {
+      const int4* osrc = reinterpret_cast<const int4*>(M.opp + td.opp_off);
+      int4* odst = reinterpret_cast<int4*>(opp);
+      for (int i = tid; i < (opp_rows + td.n_opp + 7) >> 3; i += NT) cp_async16(odst + i, osrc + i);
+    }
   }
   for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + v_lo + i) - t_lo;
-  if (do_tt) {  // keys = empty, pair = (no claimer, no finder): both all-ones, contiguous
-    int4* z = reinterpret_cast<int4*>(keys);
-    const int n16 = (L.slots - L.keys) >> 4;
-    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
-  } else {
+  {
     int4* z = reinterpret_cast<int4*>(smem + L.bmT);
     const int n16 = (L.bm_end - L.bmT) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
   }
-  if (tid < 3) scan[36 + tid] = 0u;
+  if (do_tt) {  // tables empty, TT rows -1: both all-ones, contiguous
+    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
+    const int n16 = (L.tt_end - L.tbl) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
+  }
+  if (tid < 2) scan[36 + tid] = 0u;
   cp_async_wait_all();
   __syncthreads();
 
-  if (do_tt) {
-    // ---- a4: every facet claims or finds its table slot --------------------------------------
-    uint16_t* pair16 = reinterpret_cast<uint16_t*>(pair);
-    const uint32_t cap = (uint32_t)C.cap;
-    uint32_t stat = 0u;
-    {
-      // A thread walks the facets of its internal simplices i = tid, tid + NT, ... in ONE flat probe
-      // loop: a lane whose facet settles goes on to its next facet while others still probe.
-      int i = tid, k = 0;
-      uint32_t kq[4] = {0u, 0u, 0u, 0u};  // keys of the facets of simplex i not yet placed; kq[0] is current
-      uint32_t sl_lo = 0u, sl_hi = 0u;    // the D slots of simplex i, 16 bits each, shifted in from the top
-      if (i < s_int) {
-        int l[4];
-        unpack_local(tets[s_ext + i], l);
-        kq[0] = facet_key<D, 0>(l); kq[1] = facet_key<D, 1>(l); kq[2] = facet_key<D, 2>(l);
-        if constexpr (D == 4) kq[3] = facet_key<D, 3>(l);
-      }
-      uint32_t slot = hash_slot(kq[0], cap), tries = 0u;
-      while (i < s_int) {
-        const uint32_t prev = atomicCAS(&keys[slot], kEmpty32, kq[0]);
-        if (COUNT) stat += 0x10000u;
-        if (prev == kEmpty32 || prev == kq[0]) {
-          pair16[2 * slot + (prev != kEmpty32 ? 1 : 0)] = (uint16_t)(s_ext + i);
-          if (COUNT) stat += prev == kEmpty32 ? 1u : 0u;
-          sl_lo = __funnelshift_r(sl_lo, sl_hi, 16);
-          sl_hi = (sl_hi >> 16) | (slot << 16);
-          if (++k == D) {
-            if constexpr (D == 3) { sl_lo = __funnelshift_r(sl_lo, sl_hi, 16); sl_hi >>= 16; }
-            slots[i] = make_uint2(sl_lo, sl_hi);
-            i += NT;
-            k = 0;
-            if (i < s_int) {
-              int l[4];
-              unpack_local(tets[s_ext + i], l);
-              kq[0] = facet_key<D, 0>(l); kq[1] = facet_key<D, 1>(l); kq[2] = facet_key<D, 2>(l);
-              if constexpr (D == 4) kq[3] = facet_key<D, 3>(l);
-            }
-          } else {
-            kq[0] = kq[1]; kq[1] = kq[2]; kq[2] = kq[3];
-          }
-          slot = hash_slot(kq[0], cap);
-          tries = 0u;
-        } else {
-          slot = slot + 1 == cap ? 0u : slot + 1;
-          if (++tries > cap) { raise_err(M.err, ERR_TT_TABLE_FULL); break; }
-        }
-      }
-    }
-    for (int e = tid; e < s_ext; e += NT) {
+  // ---- a4: thread p matches the facets whose lowest vertex is tile vertex p -------------------
+  if (do_tt && tid < nrows) {
+    GroupCtx g;
+    const int hs = C.hs;
+    g.tbl = tbl + tid * (hs + 1);
+    g.hmask = (uint32_t)hs - 1u;
+    g.hshift = 32 - (31 - __clz(hs));
+    g.ttrow = ttrow;
+    g.texid = texid;
+    const int r0 = ft[tid], r1 = ft[tid + 1];
+    const int o0 = opp[tid], o1 = opp[tid + 1];
+    g.opp_idx = opp + opp_rows + o0;
+    g.run0 = r0;
+    g.nrun = (r1 - r0) * (D - 1);
+    g.s_ext = s_ext;
+    g.t_lo = t_lo;
+    int j = 0;
+    for (int i = r0; i < r1; ++i) {
       int l[4];
-      unpack_local(tets[e], l);
-      if ((unsigned)(l[1] - nlo) < (unsigned)nrows) tt_insert<COUNT>(keys, pair16, cap, facet_key<D, 0>(l), e, stat, M.err);
+      unpack_local(tets[s_ext + i], l);
+      group_place<D>(g, group_key<D, 1>(l), j, s_ext + i, 1, M.err);
+      group_place<D>(g, group_key<D, 2>(l), j + 1, s_ext + i, 2, M.err);
+      if constexpr (D == 4) group_place<D>(g, group_key<D, 3>(l), j + 2, s_ext + i, 3, M.err);
+      j += D - 1;
     }
-    if (count_only) {
-      atomicAdd(&scan[37], stat & 0xFFFFu);
-      atomicAdd(&scan[38], stat >> 16);
-    }
-    __syncthreads();
-
-    if (!count_only) {
-      // ---- TT rows of the internal simplices; unresolved outer facets go to the queue ----------
-      for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
-        const int i = base + lane;
-        bool need_fb = false;
-        if (i < s_int) {
-          const int s = s_ext + i;
-          int l[4];
-          unpack_local(tets[s], l);
-          const uint2 sl = slots[i];
-          const uint32_t sk[4] = {sl.x & 0xFFFFu, sl.x >> 16, sl.y & 0xFFFFu, sl.y >> 16};
-          int nb[4];
-#pragma unroll
-          for (int k = 0; k < D; ++k) {
-            const uint32_t pw = pair[sk[k]];
-            const uint32_t plo = pw & 0xFFFFu, phi = pw >> 16;
-            const uint32_t mate = plo == (uint32_t)s ? phi : plo;
-            nb[k] = mate == kNoMate ? -1 : ((int)mate < s_ext ? texid[mate] : t_lo + ((int)mate - s_ext));
-            if (k == 0) need_fb = mate == kNoMate && (l[1] - nlo) >= nrows;
-          }
-          if constexpr (D == 4) {
-            reinterpret_cast<int4*>(O.tt_indices)[tt0 + i] = make_int4(nb[0], nb[1], nb[2], nb[3]);
-          } else {
-            int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
-            o[0] = nb[0]; o[1] = nb[1]; o[2] = nb[2];
-          }
-        }
-        const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
-        if (fbm) {
-          const int leader = __ffs(fbm) - 1;
-          uint32_t pos = 0u;
-          if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
-          pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
-          if (need_fb) fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
-        }
-      }
-    }
-    __syncthreads();  // table is dead from here on; the bitmaps take its place
-
-    {
-      int4* z = reinterpret_cast<int4*>(smem + L.bmT);
-      const int n16 = (L.bm_end - L.bmT) >> 4;
-      for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
-    }
-    if (!count_only) {
-      // ---- a5: one queued facet per thread, resolved from global memory ------------------------
-      const int nq = (int)scan[36];
-      for (int q = tid; q < nq; q += NT) {
-        const int i = fbq[q];
-        int l[4];
-        unpack_local(tets[s_ext + i], l);
-        const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
-        const int r = tt_fallback<D>(M, b, c, d, t_lo + i);
-        if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barrier
-      }
-    }
-    __syncthreads();
-  }
-
-  uint32_t tot = 0u;
-  if (do_vt || do_vv) {
-    // ---- a2/a3: one bit per incidence / per adjacent pair ---------------------------------------
-    for (int s = tid; s < S; s += NT) {
+    for (int o = o0; o < o1; ++o, ++j) {
+      const int s = opp[opp_rows + o];
       int l[4];
       unpack_local(tets[s], l);
-      bool in[D];
+      group_place<D>(g, group_key<D, 0>(l), j, s, 0, M.err);
+    }
+  }
+
+  // ---- a2/a3: one bit per incidence / per adjacent pair; warps take chunks of 32 simplices -----
+  if (do_vt || do_vv) {
+    const int nchunks = (S + 31) >> 5;
+    for (;;) {
+      uint32_t c = 0u;
+      if (lane == 0) c = atomicAdd(&scan[37], 1u);
+      c = __shfl_sync(0xFFFFFFFFu, c, 0);
+      if ((int)c >= nchunks) break;
+      const int s = (int)c * 32 + lane;
+      if (s < S) {
+        int l[4];
+        unpack_local(tets[s], l);
+        bool in[D];
 #pragma unroll
-      for (int k = 0; k < D; ++k) in[k] = (unsigned)(l[k] - nlo) < (unsigned)nrows;
-      if (do_vt) {
-        const uint32_t bit = 1u << (s & 31);
-        uint32_t* col = bmT + (s >> 5);
+        for (int k = 0; k < D; ++k) in[k] = (unsigned)(l[k] - nlo) < (unsigned)nrows;
+        if (do_vt) {
+          const uint32_t bit = 1u << lane;
+          uint32_t* col = bmT + c;
 #pragma unroll
-        for (int k = 1; k < D; ++k)
-          if (in[k]) atomicOr(col + (l[k] - nlo) * WT, bit);
-      }
-      if (do_vv) {
-        uint32_t w[D], b[D];
+          for (int k = 1; k < D; ++k)
+            if (in[k]) atomicOr(col + (l[k] - nlo) * WT, bit);
+        }
+        if (do_vv) {
+          uint32_t w[D], b[D];
 #pragma unroll
-        for (int k = 0; k < D; ++k) { w[k] = (uint32_t)l[k] >> 5; b[k] = 1u << (l[k] & 31); }
+          for (int k = 0; k < D; ++k) { w[k] = (uint32_t)l[k] >> 5; b[k] = 1u << (l[k] & 31); }
 #pragma unroll
-        for (int k = 0; k < D; ++k) {
-          if (!in[k]) continue;
-          uint32_t* row = bmV + (l[k] - nlo) * WV;
+          for (int k = 0; k < D; ++k) {
+            if (!in[k]) continue;
+            uint32_t* row = bmV + (l[k] - nlo) * WV;
 #pragma unroll
-          for (int j = 0; j < D; ++j)
-            if (j != k) atomicOr(row + w[j], b[j]);
+            for (int j = 0; j < D; ++j)
+              if (j != k) atomicOr(row + w[j], b[j]);
+          }
         }
       }
     }
-    __syncthreads();
+  }
+  __syncthreads();
 
+  if (do_tt) {
+    // ---- TT rows to global; facets no tile vertex owns go to the queue --------------------------
+    for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
+      const int i = base + lane;
+      bool need_fb = false;
+      if (i < s_int) {
+        int first;
+        if constexpr (D == 4) {
+          const int4 v = reinterpret_cast<const int4*>(ttrow)[i];
+          reinterpret_cast<int4*>(O.tt_indices)[tt0 + i] = v;
+          first = v.x;
+        } else {
+          int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
+          first = ttrow[i * 3];
+          o[0] = first; o[1] = ttrow[i * 3 + 1]; o[2] = ttrow[i * 3 + 2];
+        }
+        need_fb = first < 0 && (int)(tets[s_ext + i].x >> 16) - nlo >= nrows;
+      }
+      const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
+      if (fbm) {
+        const int leader = __ffs(fbm) - 1;
+        uint32_t pos = 0u;
+        if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
+        pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
+        if (need_fb) fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
+      }
+    }
+  }
+
+  if (do_vt || do_vv) {
     // ---- row degrees -> offsets: threads [0, rows) own the VT rows, [NT/2, NT/2+rows) the VV rows
     const bool vt_thread = do_vt && tid < nrows;
     const int vrow = tid - NT / 2;
     const bool vv_thread = do_vv && vrow >= 0 && vrow < nrows;
     const int wT = (S + 31) >> 5, wV = (td.nloc + 31) >> 5;
+    uint32_t tot = 0u;
     int nbits = 0;  // set bits of this thread's row
     {
       uint32_t deg = 0u;
@@ -546,17 +540,17 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         for (int w = 0; w < wV; ++w) nbits += __popc(row[w]);
         deg = (uint32_t)nbits << 16;
       }
-      const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);
-      if (vt_thread) off_vt[tid] = (int)(ex & 0xFFFFu);
+      const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // (also orders the TT row copy
+      if (vt_thread) off_vt[tid] = (int)(ex & 0xFFFFu);               //  before the staging reuse)
       if (vv_thread) off_vv[vrow] = (int)(ex >> 16);
     }
     const int n_vt = (int)(tot & 0xFFFFu), n_vv = (int)(tot >> 16);
-    if (count_only) {
+    if (COUNT) {
       if (tid == 0) {
         O.stats[(long long)tile * 4 + 0] = n_vt;
         O.stats[(long long)tile * 4 + 1] = n_vv;
-        O.stats[(long long)tile * 4 + 2] = scan[37];
-        O.stats[(long long)tile * 4 + 3] = scan[38];
+        O.stats[(long long)tile * 4 + 2] = 0;
+        O.stats[(long long)tile * 4 + 3] = 0;
       }
       return;
     }
@@ -597,11 +591,21 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       for (int i = tid; i < n_vt; i += NT) O.vt_indices[vt0 + i] = st_vt[i];
     if (do_vv)
       for (int i = tid; i < n_vv; i += NT) O.vv_indices[vv0 + i] = st_vv[i];
-  } else if (count_only && tid == 0) {
-    O.stats[(long long)tile * 4 + 0] = 0;
-    O.stats[(long long)tile * 4 + 1] = 0;
-    O.stats[(long long)tile * 4 + 2] = scan[37];
-    O.stats[(long long)tile * 4 + 3] = scan[38];
+  } else {
+    __syncthreads();  // queue complete
+  }
+
+  if (do_tt) {
+    // ---- a5: one queued facet per thread, resolved from global memory (no barrier follows) ------
+    const int nq = (int)scan[36];
+    for (int q = tid; q < nq; q += NT) {
+      const int i = fbq[q];
+      int l[4];
+      unpack_local(tets[s_ext + i], l);
+      const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
+      const int r = tt_fallback<D>(M, b, c, d, t_lo + i);
+      if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barriers
+    }
   }
 }
 

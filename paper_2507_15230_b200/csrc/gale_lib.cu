@@ -53,6 +53,7 @@ struct Plan {
   int tv = 0, nTiles = 0, NT = 0;
   std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
   std::vector<uint16_t> loc;            // 4 per staged simplex
+  std::vector<uint16_t> opp;            // per tile: row starts, then staged indices by second vertex
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
   int smem_bytes = 0;
@@ -66,7 +67,7 @@ struct Plan {
   size_t index_bytes() const {
     return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
            up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16);
+           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16) + up(opp.size() * 2 + 16);
   }
 };
 
@@ -122,10 +123,14 @@ inline int threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : 1
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
   SmemCfg c = full;
   if (!(mask & gale::REL_VV)) { c.WV = 0; c.vv_max = 0; }
-  if (!(mask & gale::REL_TT)) c.cap = 0;
+  if (!(mask & gale::REL_TT) || count_mode) { c.hs = 0; c.nopp = 0; c.sint = 0; }
   if (!(mask & gale::REL_VT)) { c.WT = 0; c.vt_max = 0; }
   if (count_mode) { c.vt_max = 0; c.vv_max = 0; }
   return c;
+}
+
+inline gale::SmemLayout layout_for(int D, const SmemCfg& c) {
+  return D == 4 ? gale::make_layout<4>(c) : gale::make_layout<3>(c);
 }
 
 using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::SmemLayout,
@@ -205,7 +210,7 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       d.stg_off = stg;
       d.tex_off = texo;
       const long long S = (long long)d.s_int + d.s_ext;
-      if (S > gale::kMaxStaged || (long long)D * d.s_int + d.s_ext + 32 > gale::kMaxCap) return false;
+      if (S > gale::kMaxStaged) return false;
       stg += pad_to(S, 2);
       texo += pad_to(d.s_ext, 4);
     }
@@ -216,13 +221,17 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   // halo + local encoding, tiles split over host threads
   const int nth = std::max(1, std::min<int>(32, std::min<int>(int(std::thread::hardware_concurrency()), nTiles / 64 + 1)));
   std::vector<std::vector<int32_t>> gid_part(nth);
+  std::vector<std::vector<uint16_t>> opp_part(nth);
+  std::vector<int> group_max(nth, 0);
+  const int max_group = D == 4 ? gale::kMaxGroup4 : gale::kMaxGroup3;
   std::vector<int> tile_lo(nth + 1);
   for (int w = 0; w <= nth; ++w) tile_lo[w] = int((long long)nTiles * w / nth);
   std::atomic<bool> ok{true};
   auto work = [&](int w) {
     std::vector<uint16_t> map(size_t(p.nV), uint16_t(0xFFFF));
     std::vector<int32_t>& hp = gid_part[w];
-    std::vector<int32_t> h;
+    std::vector<uint16_t>& op = opp_part[w];
+    std::vector<int32_t> h, cnt;
     for (int i = tile_lo[w]; i < tile_lo[w + 1] && ok.load(std::memory_order_relaxed); ++i) {
       TileDesc& d = p.tiles[i];
       const int v_lo = d.v_lo, v_hi = d.v_lo + d.nrows;
@@ -254,6 +263,29 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
           out[s * 4 + k] = k >= D ? uint16_t(0xFFFF)
                                   : (r[k] >= v_lo && r[k] < v_hi) ? uint16_t(nlo + (r[k] - v_lo)) : map[r[k]];
       }
+      // second-vertex index of the tile: row r lists the staged simplices whose second vertex is r
+      {
+        const int rp = gale::opp_rows_pad(d.nrows);
+        cnt.assign(size_t(d.nrows) + 1, 0);
+        for (int s = 0; s < S; ++s) {
+          const int r = int(out[s * 4 + 1]) - nlo;
+          if (r >= 0 && r < d.nrows) ++cnt[r + 1];
+        }
+        for (int r = 0; r < d.nrows; ++r) {
+          const int group = (D - 1) * (p.first_tet[v_lo + r + 1] - p.first_tet[v_lo + r]) + cnt[r + 1];
+          group_max[w] = std::max(group_max[w], group);
+          cnt[r + 1] += cnt[r];
+        }
+        d.n_opp = cnt[d.nrows];
+        d.opp_off = (long long)op.size();  // relative; rebased below
+        const size_t base = op.size();
+        op.resize(base + size_t(rp) + size_t(pad_to(d.n_opp, 8)), 0);
+        for (int r = 0; r <= d.nrows; ++r) op[base + r] = uint16_t(cnt[r]);
+        for (int s = 0; s < S; ++s) {
+          const int r = int(out[s * 4 + 1]) - nlo;
+          if (r >= 0 && r < d.nrows) op[base + rp + size_t(cnt[r]++)] = uint16_t(s);
+        }
+      }
       hp.insert(hp.end(), h.begin(), h.begin() + nlo);  // local id -> global id, ascending
       for (int v = v_lo; v < v_hi; ++v) hp.push_back(v);
       hp.insert(hp.end(), h.begin() + nlo, h.end());
@@ -280,9 +312,25 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     hoff += (long long)gid_part[w].size();
     std::vector<int32_t>().swap(gid_part[w]);
   }
+  long long ooff = 0;
+  int gmax = 1;
+  for (int w = 0; w < nth; ++w) {
+    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].opp_off += ooff;
+    ooff += (long long)opp_part[w].size();
+    gmax = std::max(gmax, group_max[w]);
+  }
+  if (gmax > max_group) return false;
+  p.opp.assign(size_t(ooff) + 8, 0);
+  ooff = 0;
+  for (int w = 0; w < nth; ++w) {
+    std::copy(opp_part[w].begin(), opp_part[w].end(), p.opp.begin() + ooff);
+    ooff += (long long)opp_part[w].size();
+    std::vector<uint16_t>().swap(opp_part[w]);
+  }
   // shared-memory capacities known so far
-  long long smax = 2, sext = 4, sint = 2, nloc = 4;
+  long long smax = 2, sext = 4, sint = 2, nloc = 4, nopp = 8;
   for (const TileDesc& d : p.tiles) {
+    nopp = std::max(nopp, (long long)gale::opp_rows_pad(d.nrows) + pad_to(d.n_opp, 8));
     smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 2));
     sext = std::max(sext, pad_to(d.s_ext, 4));
     sint = std::max(sint, pad_to(d.s_int, 2));
@@ -294,6 +342,9 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   p.cfg.sext = int(sext);
   p.cfg.nloc = int(nloc);
   p.cfg.sint = int(sint);
+  p.cfg.nopp = int(nopp);
+  p.cfg.hs = 8;
+  while (p.cfg.hs < gmax + gmax / 4 + 1) p.cfg.hs *= 2;  // a group never fills its table
   p.cfg.WT = int((smax + 31) / 32) | 1;
   p.cfg.WV = int((nloc + 31) / 32) | 1;
   return true;
@@ -313,24 +364,16 @@ struct DevBuf {  // temporary device memory of the analysis
   }
 };
 
-// Sizing run (count mode of the batch kernel) over all tiles: exact VT / VV entry counts and the
-// number of distinct facets per tile. Returns GALE_ERR_WORKSPACE-like codes via rc; `fits` tells
-// whether the count-mode shared memory fits at this tile size.
+// Sizing run (count mode of the batch kernel) over all tiles: exact VT / VV entry counts per tile.
+// `fits` tells whether the count-mode shared memory fits at this tile size.
 int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long long>& stats, bool& fits) {
   const int D = p.dim + 1;
   fits = true;
   stats.assign(size_t(p.nTiles) * 4, 0);
   if (p.nTiles == 0) return GALE_OK;
-  long long rec_max = 1;
-  for (const TileDesc& d : p.tiles) rec_max = std::max(rec_max, (long long)D * d.s_int + d.s_ext);
-  SmemCfg full = p.cfg;
-  full.cap = int(rec_max + 32);  // distinct facets <= facet records
-  // one launch for all three relations if the shared memory allows, else VT|VV and TT apart
-  std::vector<uint32_t> parts;
-  if (gale::make_layout(cfg_for_mask(full, 7, true)).total <= kSmemLimit) parts = {7u};
-  else parts = {3u, 4u};
-  for (uint32_t m : parts)
-    if (gale::make_layout(cfg_for_mask(full, m, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
+  const SmemCfg full = p.cfg;
+  const std::vector<uint32_t> parts = {3u};
+  if (layout_for(D, cfg_for_mask(full, 3, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
 
   DevBuf b_ft, b_tiles, b_tex, b_gid, b_loc, b_stats, b_err;
   int rc;
@@ -351,7 +394,7 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   std::vector<long long> part_stats(stats.size());
   for (uint32_t m : parts) {
     const SmemCfg c = cfg_for_mask(full, m, true);
-    const gale::SmemLayout lay = gale::make_layout(c);
+    const gale::SmemLayout lay = layout_for(D, c);
     const int smem = lay.total;
     GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     gale::BatchParams P{};
@@ -365,7 +408,6 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
     for (int i = 0; i < p.nTiles; ++i) {
       if (m & 1) stats[i * 4 + 0] = part_stats[i * 4 + 0];
       if (m & 2) stats[i * 4 + 1] = part_stats[i * 4 + 1];
-      if (m & 4) { stats[i * 4 + 2] = part_stats[i * 4 + 2]; stats[i * 4 + 3] = part_stats[i * 4 + 3]; }
     }
   }
   int err = 0;
@@ -426,18 +468,15 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
       if (rc != GALE_OK) return rc;
     }
     if (fits) {
-      long long vt_max = 1, vv_max = 1, faces_max = 1;
+      long long vt_max = 1, vv_max = 1;
       for (int i = 0; i < p->nTiles; ++i) {
         vt_max = std::max(vt_max, stats[i * 4 + 0]);
         vv_max = std::max(vv_max, stats[i * 4 + 1]);
-        faces_max = std::max(faces_max, stats[i * 4 + 2]);
       }
       p->cfg.vt_max = int(pad_to(vt_max, 8));
       p->cfg.vv_max = int(pad_to(vv_max, 8));
-      p->cfg.cap = int(std::min<long long>(pad_to(faces_max * 2 + 32, 4), gale::kMaxCap & ~3));   // load factor <= 1/2
-      p->smem_bytes = gale::make_layout(p->cfg).total;
-      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit &&
-             faces_max + 32 <= p->cfg.cap;
+      p->smem_bytes = layout_for(D, p->cfg).total;
+      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
     }
     if (fits) break;
     if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
@@ -600,6 +639,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
   m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
   m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
+  m->dm.opp = static_cast<uint16_t*>(put(p->opp.data(), p->opp.size() * 2, 16));
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
   GALE_CUDA(cudaStreamSynchronize(st));
@@ -607,6 +647,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   std::vector<int32_t>().swap(p->tex);
   std::vector<int32_t>().swap(p->gid);
   std::vector<uint16_t>().swap(p->loc);
+  std::vector<uint16_t>().swap(p->opp);
   std::vector<int32_t>().swap(p->opp_first);
 
   GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
@@ -705,7 +746,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
 
   const SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
-  const gale::SmemLayout lay = gale::make_layout(cfg);
+  const gale::SmemLayout lay = layout_for(D, cfg);
   const int smem = lay.total;
   GALE_CUDA(cudaEventRecord(s.ev_start, st));
   for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
