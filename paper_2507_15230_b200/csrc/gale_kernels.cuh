@@ -10,28 +10,31 @@
 // Every external simplex has a smaller global id than every internal one (its lowest vertex lies
 // below the tile), so the staged order s = 0..S-1 ascends with the global simplex id.
 //
-// Phases of a block:
-//   a1  stage the list (8 B per simplex), the external simplices' global ids, the local->global
-//       vertex table and the tile's second-vertex index into shared memory with 16-byte cp.async;
-//   a4  TT, one thread per tile vertex p and no atomics: a facet whose lowest vertex is p has all
-//       its cofaces among the simplices whose lowest vertex is p (the contiguous run
-//       first_tet[p]..first_tet[p+1], facets 1..D-1) and the staged simplices whose second vertex
-//       is p (their facet 0; listed per tile vertex by the create-time index, like the paper's
-//       sorted lists bounded by interval arrays). The thread walks these
-//       few records through a private open-addressing table keyed by the facet's other vertices;
-//       the second arrival of a key meets the first and both TT entries are written to a
-//       shared-memory copy of the tile's TT rows;
-//   a5  TT fallback: the facet opposite the lowest vertex a of an internal simplex (a,b,..) with b
-//       outside the tile belongs to no vertex of the tile; such facets are compacted into a queue
-//       and resolved one per thread from global memory through the run of simplices starting with
-//       b and the index of simplices whose second vertex is b (DESIGN.md §TT fallback);
-//   a2  VT: one bit per (row, staged simplex) in a rows x S bitmap (atomicOr); expanding a row
-//       yields its simplices in ascending order with no sort; the simplices whose *lowest* vertex
-//       is v are the contiguous run first_tet[v]..first_tet[v+1] and are appended without bits;
-//   a3  VV: one bit per (row, local neighbour) in a rows x nloc bitmap (atomicOr: "no duplicates",
-//       PAPER.md:228); local ids ascend with global ids, so a row expands sorted;
-//   a6  rows are expanded into shared-memory staging (ids translated back to global) and written
-//       out with coalesced stores.
+// A block has NT = 2 * TV threads: two threads per tile vertex p, an "A" thread (tid = p) and a
+// "B" thread (tid = TV + p), so that lanes of a warp are consecutive vertices (their bitmap rows
+// and tables fall into distinct shared-memory banks). Phases:
+//   P0  stage the list (8 B per simplex), the external simplices' global ids and the local->global
+//       vertex table into shared memory with 16-byte cp.async; clear the bitmaps and tables;
+//   P1  VT incidence bits, one thread per staged simplex: bit (row v, column s) for every tile
+//       vertex v of s other than its lowest vertex (the simplices whose *lowest* vertex is v are
+//       the contiguous run first_tet[v]..first_tet[v+1], and need no bits);
+//   P2  row degrees (popc) -> exclusive scan -> VT offsets;
+//   P3  A(p): walks the set bits of row p in ascending order = VT(p) without its run, already
+//             sorted; per simplex: emit the VT entry, OR the simplex's vertices into VV row p
+//             (the thread owns the row: "no duplicates", without contention), and
+//             flag the entry when p is the simplex's second vertex;
+//       B(p): walks the run of p: VT entries, VV bits, and the TT facet records 1..D-1 of every
+//             simplex of the run into p's private open-addressing table;
+//   P4  A(p): the flagged entries are the simplices (x, p, ..): their facet 0 has lowest vertex p
+//             and joins p's table. A facet whose lowest vertex is p has all its cofaces among
+//             run(p) and those simplices, so the second arrival of a key meets the first and both
+//             TT entries are written (no atomics, no global traffic);
+//       B(p): VV row p -> degree -> scan -> expansion (sorted because local ids ascend);
+//   P5  TT rows, VT and VV indices are translated to global ids and written with coalesced
+//       stores; the facet opposite the lowest vertex a of an internal simplex (a, b, ..) with b
+//       outside the tile belongs to no vertex of the tile: such facets are queued and resolved
+//       one per thread from global memory through the run of simplices starting with b and the
+//       index of simplices whose second vertex is b (DESIGN.md §TT fallback).
 // All arithmetic is integer index work; no floating point.
 #pragma once
 #include <cuda_runtime.h>
@@ -41,17 +44,17 @@ namespace gale {
 
 constexpr int kMaxBatch = 128;         // clusters per kernel launch (descriptor lives in kernel params)
 constexpr uint32_t kEmpty32 = 0xFFFFFFFFu;
-constexpr int kMaxStaged = 65534;      // staged simplices per tile (16-bit staged indices)
-constexpr int kMaxLocal4 = 1024;       // tetrahedra: 10-bit local ids (20-bit facet key + 12-bit record)
-constexpr int kMaxLocal3 = 65534;      // triangles: 16-bit local ids (16-bit facet key + 16-bit record)
-constexpr int kMaxGroup4 = 4095;       // facet records of one vertex (tetrahedra / triangles)
-constexpr int kMaxGroup3 = 65534;
-constexpr int kMaxNnz16 = 65535;       // VT / VV entries of one tile (16-bit packed scan)
+constexpr int kMaxStaged4 = 4094;      // tetrahedra: 12-bit staged index in a table word
+constexpr int kMaxStaged3 = 16382;     // triangles: 14-bit staged index
+constexpr int kMaxLocal4 = 512;        // tetrahedra: 9-bit local ids (18-bit facet key)
+constexpr int kMaxLocal3 = 65534;      // triangles: 16-bit local ids
+constexpr int kMaxNnz16 = 65535;       // VT / VV entries of one tile (16-bit packed scans)
+constexpr int kMaxTileVertices = 256;
 
 enum { REL_VT = 1, REL_VV = 2, REL_TT = 4, MODE_COUNT = 8 };
 enum { ERR_TT_TABLE_FULL = 2, ERR_SIZE_MISMATCH = 4 };
 
-// Per-tile record built by gale_mesh_create (96 bytes, 16-byte aligned).
+// Per-tile record built by gale_mesh_create (80 bytes, 16-byte aligned).
 struct TileDesc {
   int32_t v_lo, nrows;        // vertices [v_lo, v_lo+nrows)
   int32_t t_lo, s_int;        // internal simplices [t_lo, t_lo+s_int)
@@ -60,14 +63,12 @@ struct TileDesc {
   int32_t row_rel, tt_rel;    // first row / first TT row of the tile inside its cluster
   int32_t vt_rel, vv_rel;     // first VT / VV entry of the tile inside its cluster
   int32_t vt_nnz, vv_nnz;     // entries of the tile (fixed at create; the kernel re-derives them)
-  int32_t n_opp;              // staged simplices whose second vertex is in the tile
+  int32_t pad0;
   long long stg_off;          // first staged simplex of the tile in DeviceMesh::loc (even)
   long long tex_off;          // first entry in DeviceMesh::tex (multiple of 4)
   long long gid_off;          // first entry in DeviceMesh::gid (multiple of 4)
-  long long opp_off;          // first entry in DeviceMesh::opp (multiple of 8)
-  long long pad0;
 };
-static_assert(sizeof(TileDesc) == 96, "TileDesc layout");
+static_assert(sizeof(TileDesc) == 80, "TileDesc layout");
 
 // Device-resident index built by gale_mesh_create (all pointers DEVICE).
 struct DeviceMesh {
@@ -79,8 +80,6 @@ struct DeviceMesh {
   const uint2* loc;                   // staged simplices in tile-local ids, 4 x uint16 each
   const int32_t* tex;                 // per-tile ascending global ids of external simplices (T_ex)
   const int32_t* gid;                 // per-tile global vertex id of every local id (ascending)
-  const uint16_t* opp;                // per tile: [tv_pad] start of row r, then the staged indices of the
-                                      // simplices whose second vertex is row r, ascending, rows in order
   const int32_t* cluster_tile_begin;  // [nC+1]
   int32_t* err;                       // sticky device error flags (host-mapped)
 };
@@ -92,27 +91,24 @@ struct SmemCfg {
   int smax;      // staged simplices (even)
   int sext;      // external simplices (multiple of 4)
   int nloc;      // local vertex ids (multiple of 4)
-  int sint;      // internal simplices (even): TT row copy + fallback queue, 0 without TT
-  int nopp;      // second-vertex index entries incl. the row starts (multiple of 8), 0 without TT
+  int sint;      // internal simplices (even): TT rows + fallback queue, 0 without TT
   int hs;        // table slots per tile vertex (power of two), 0 without TT
-  int WT;        // VT bitmap words per row (odd), 0 without VT
+  int WT;        // VT bitmap words per row (odd)
   int WV;        // VV bitmap words per row (odd), 0 without VV
-  int vt_max;    // VT entries staged for write-out, 0 without VT or in count mode
-  int vv_max;    // VV entries staged for write-out
+  int vt_max;    // VT entries staged for write-out (16-bit)
+  int vv_max;    // VV entries staged for write-out (16-bit), 0 without VV or in count mode
 };
 
 // Byte offsets of the shared-memory regions, computed on the host (make_layout) and passed as a
-// kernel parameter. The TT tables / TT row copy and the VT/VV staging share one union (the tables
-// are dead before the rows are expanded).
+// kernel parameter.
 struct SmemLayout {
-  int tets, texid, gid, opp, ft, off_vt, off_vv, fbq, scan, bmT, bmV, bm_end;
-  int tbl, ttrow, tt_end;           // TT phase
-  int st_vt, st_vv;                 // write-out staging
+  int tets, texid, gid, ft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
+  int tbl, ttrow, tt_end;
+  int st_vt, st_vv;
   int total;
 };
 
 __host__ __device__ inline int align16(int x) { return (x + 15) & ~15; }
-__host__ __device__ inline int opp_rows_pad(int tv) { return (tv + 1 + 7) & ~7; }
 
 template <int D>
 __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
@@ -121,22 +117,21 @@ __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   L.tets = o;   o = align16(o + c.smax * 8);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
-  L.opp = o;    o = align16(o + c.nopp * 2);
   L.ft = o;     o = align16(o + (c.tv + 1) * 4);
   L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
   L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
+  L.cnt = o;    o = align16(o + c.tv * 4);
   L.fbq = o;    o = align16(o + c.sint * 2);
   L.scan = o;   o = align16(o + 48 * 4);
   L.bmT = o;    o = align16(o + c.tv * c.WT * 4);
   L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
   L.bm_end = o;
   L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
-  L.ttrow = o;  o = align16(o + c.sint * D * 4);
+  L.ttrow = o;  o = align16(o + c.sint * D * 2);
   L.tt_end = o;
-  o = L.tbl;
-  L.st_vt = o;  o = align16(o + c.vt_max * 4);
-  L.st_vv = o;  o = align16(o + c.vv_max * 4);
-  L.total = o > L.tt_end ? o : L.tt_end;
+  L.st_vt = o;  o = align16(o + c.vt_max * 2);
+  L.st_vv = o;  o = align16(o + c.vv_max * 2);
+  L.total = o;
   return L;
 }
 
@@ -174,54 +169,68 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
+// Barrier among the `count` threads that name the same id (ids 1..15; 0 is __syncthreads).
+__device__ __forceinline__ void named_barrier(int id, int count) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory");
+}
+
 __device__ __forceinline__ void unpack_local(const uint2 q, int (&l)[4]) {
   l[0] = q.x & 0xFFFF; l[1] = q.x >> 16; l[2] = q.y & 0xFFFF; l[3] = q.y >> 16;
 }
 
-template <int D>
-__device__ __forceinline__ void load_simplex_global(const int32_t* T, int t, int (&v)[4]) {
-  if constexpr (D == 4) {
-    const int4 q = __ldg(reinterpret_cast<const int4*>(T) + t);
-    v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
-  } else {
-    v[0] = __ldg(T + (long long)t * 3); v[1] = __ldg(T + (long long)t * 3 + 1); v[2] = __ldg(T + (long long)t * 3 + 2);
-    v[3] = -1;
-  }
-}
+// 1 << (l mod 32)
+__device__ __forceinline__ uint32_t bit_of(int l) { return 1u << (l & 31); }
 
 // a5, one request per thread: coface != self of the facet (b, c[, d]) (ascending global ids) whose
 // vertices all lie outside the tile. Both cofaces of a facet with lowest vertex b have b as
-// lowest or second-lowest vertex: candidates are the run of simplices starting with b (sorted, so
-// the scan stops once the second vertex exceeds c) and the simplices whose second vertex is b
-// (those are (x, b, c, d) exactly).
+// lowest or second-lowest vertex: candidates are the run of simplices starting with b and the
+// simplices whose second vertex is b (those are (x, b, c, d) exactly). Candidates are fetched four
+// at a time without early exit so that their loads overlap.
 template <int D>
 __device__ __forceinline__ int tt_fallback(const DeviceMesh& M, int b, int c, int d, int self) {
   const int f0 = __ldg(M.first_tet + b), f1 = __ldg(M.first_tet + b + 1);
   const int o0 = __ldg(M.opp_first + b), o1 = __ldg(M.opp_first + b + 1);
-  for (int t = f0; t < f1; ++t) {
-    int v[4];
-    load_simplex_global<D>(M.T, t, v);
-    if (v[1] > c) break;
-    bool hit;
-    if constexpr (D == 4) hit = (v[1] == c && (v[2] == d || v[3] == d)) || (v[2] == c && v[3] == d);
-    else hit = v[1] == c || v[2] == c;
-    if (hit) return t;
+  int found = -1;
+  if constexpr (D == 4) {
+    const int4* T4 = reinterpret_cast<const int4*>(M.T);
+    for (int t = f0; t < f1; t += 4) {
+      int4 q[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) q[u] = __ldg(T4 + min(t + u, f1 - 1));
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const bool hit = (q[u].y == c && (q[u].z == d || q[u].w == d)) || (q[u].z == c && q[u].w == d);
+        if (hit) found = min(t + u, f1 - 1);
+      }
+    }
+    if (found >= 0) return found;
+    for (int j = o0; j < o1; j += 4) {
+      int t[4];
+      int4 q[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) t[u] = __ldg(M.opp_perm + min(j + u, o1 - 1));
+#pragma unroll
+      for (int u = 0; u < 4; ++u) q[u] = __ldg(T4 + t[u]);
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (t[u] != self && q[u].z == c && q[u].w == d) found = t[u];
+    }
+  } else {
+    for (int t = f0; t < f1; ++t) {
+      const int v1 = __ldg(M.T + (long long)t * 3 + 1), v2 = __ldg(M.T + (long long)t * 3 + 2);
+      if (v1 == c || v2 == c) found = t;
+    }
+    if (found >= 0) return found;
+    for (int j = o0; j < o1; ++j) {
+      const int t = __ldg(M.opp_perm + j);
+      if (t != self && __ldg(M.T + (long long)t * 3 + 2) == c) found = t;
+    }
   }
-  for (int j = o0; j < o1; ++j) {
-    const int t = __ldg(M.opp_perm + j);
-    if (t == self) continue;
-    int v[4];
-    load_simplex_global<D>(M.T, t, v);
-    bool hit;
-    if constexpr (D == 4) hit = v[2] == c && v[3] == d;
-    else hit = v[2] == c;
-    if (hit) return t;
-  }
-  return -1;
+  return found;
 }
 
 // Block-wide exclusive scan of one value per thread. Returns the exclusive prefix; *total gets
-// the block sum. scratch: 33 ints of shared memory.
+// the block sum. scratch: 33 ints of shared memory. Ends with all threads past the last barrier.
 template <int NT>
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* scratch, uint32_t* total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -248,58 +257,41 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* s
   return base + inc - x;
 }
 
-
 // ------------------------------------------------------------------------------------------------
-// a4 helpers. A facet record of vertex p's group is numbered j: first the facets 1..D-1 of the
-// simplices of the run of p (j = (D-1) * q + k-1 for the q-th simplex of the run), then facet 0 of
-// the simplices whose second vertex is p, in the order of the tile's second-vertex index.
+// TT tables. A table word of vertex p's group = key | s << kKeyBits | k << 30: the facet's
+// vertices other than p (local ids, ascending), the staged simplex s it belongs to, and the local
+// vertex k it is opposite to.
 template <int D>
-struct FacetBits {  // table word = key | (j << kKeyBits); the key holds the facet's vertices other than p
-  static constexpr int kKeyBits = D == 4 ? 20 : 16;
+struct FacetBits {
+  static constexpr int kKeyBits = D == 4 ? 18 : 16;
   static constexpr uint32_t kKeyMask = (1u << kKeyBits) - 1u;
+  static constexpr uint32_t kIdxMask = (1u << (30 - kKeyBits)) - 1u;
 };
 
 struct GroupCtx {
-  uint32_t* tbl;           // this vertex's table, hs slots
+  uint32_t* tbl;       // this vertex's table, hs slots
   uint32_t hmask;
   int hshift;
-  int32_t* ttrow;          // shared-memory copy of the tile's TT rows, D entries per internal simplex
-  const int32_t* texid;
-  const uint16_t* opp_idx; // second-vertex records of p
-  int run0;                // first internal simplex (index in the tile) of the run of p
-  int nrun;                // (D-1) * simplices in the run
-  int s_ext, t_lo;
+  uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
+  int s_ext;
 };
 
-__device__ __forceinline__ int global_simplex(const GroupCtx& g, int s) {
-  return s < g.s_ext ? g.texid[s] : g.t_lo + (s - g.s_ext);
-}
-
-// Place record j = facet k of staged simplex s with key `key`: claim an empty slot, or meet the
-// record that holds the same key (the other coface) and write both TT entries.
+// Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
+// holds the same key (the other coface) and write both TT entries.
 template <int D>
-__device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int j, int s, int k, int32_t* err) {
+__device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
   using FB = FacetBits<D>;
   uint32_t h = (key * 0x9E3779B1u) >> g.hshift;
   for (uint32_t probe = 0; probe <= g.hmask; ++probe) {
     const uint32_t cur = g.tbl[h];
     if (cur == kEmpty32) {
-      g.tbl[h] = key | ((uint32_t)j << FB::kKeyBits);
+      g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
       return;
     }
     if ((cur & FB::kKeyMask) == key) {
-      const int j2 = (int)(cur >> FB::kKeyBits);
-      int s2, k2;
-      if (j2 < g.nrun) {
-        const int q = j2 / (D - 1);
-        s2 = g.s_ext + g.run0 + q;
-        k2 = 1 + j2 - q * (D - 1);
-      } else {
-        s2 = g.opp_idx[j2 - g.nrun];
-        k2 = 0;
-      }
-      if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = global_simplex(g, s2);
-      if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = global_simplex(g, s);
+      const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
+      if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2;
+      if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s;
       return;
     }
     h = (h + 1) & g.hmask;
@@ -307,32 +299,65 @@ __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int
   raise_err(err, ERR_TT_TABLE_FULL);
 }
 
-// Key of the facet of a simplex with lowest vertex p that omits local vertex K (1 <= K < D): the
-// facet's vertices other than p, ascending. For K = 0 (simplex (x, p, ..)): the vertices after p.
+// Key of the facet opposite local vertex K: the facet's vertices other than its lowest one.
 template <int D, int K>
 __device__ __forceinline__ uint32_t group_key(const int (&l)[4]) {
   if constexpr (D == 4) {
     const int a = K <= 1 ? l[2] : l[1];
-    const int b = (K == 0 || K == 1 || K == 2) ? l[3] : l[2];
-    return (uint32_t)a | ((uint32_t)b << 10);
+    const int b = K == 3 ? l[2] : l[3];
+    return (uint32_t)a | ((uint32_t)b << 9);
   } else {
     return (uint32_t)(K <= 1 ? l[2] : l[1]);
+  }
+}
+
+// Exclusive scan over the B half of the block (threads [NT/2, NT)), one value per thread, with a
+// named barrier so that the A half is not held up. Returns the exclusive prefix; *total = sum.
+template <int NT>
+__device__ __forceinline__ uint32_t half_exclusive_scan(uint32_t x, uint32_t* scratch, uint32_t* total) {
+  constexpr int TV = NT / 2;
+  const int lane = threadIdx.x & 31, warp = (threadIdx.x - TV) >> 5;
+  uint32_t inc = x;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+    if (lane >= d) inc += y;
+  }
+  if constexpr (TV <= 32) {
+    *total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+    return inc - x;
+  } else {
+    constexpr int NW = TV / 32;
+    if (lane == 31) scratch[warp] = inc;
+    named_barrier(1, TV);
+    uint32_t base = 0u, tot = 0u;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const uint32_t v = scratch[w];
+      if (w < warp) base += v;
+      tot += v;
+    }
+    named_barrier(1, TV);  // scratch may be reused
+    *total = tot;
+    return base + inc - x;
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 // The batch kernel: VT + VV + TT for every tile of the requested clusters (or, COUNT, the exact
 // VT / VV sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer likewise
-// sizes its relation arrays before launch). NT >= 2 * rows per tile.
+// sizes its relation arrays before launch). NT = 2 * (rows per tile capacity).
 template <int D, int NT, bool COUNT>
-__global__ void __launch_bounds__(NT, (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2)))
+__global__ void __launch_bounds__(NT, (NT <= 64 ? 16 : (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2))))
 gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
                   const SmemLayout L, const OutPtrs O) {
   extern __shared__ __align__(16) unsigned char smem[];
+  constexpr int TV = NT / 2;
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t mask = P.mask;
   const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0;
   const bool do_tt = !COUNT && (mask & REL_TT) != 0;
+  const bool entries = !COUNT && (do_vt || do_tt);  // VT entries are staged (TT reads their flags)
 
   // ---- block -> (cluster slot, tile) ----------------------------------------------------------
   int slot = 0, tile;
@@ -366,40 +391,36 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   uint2* tets = reinterpret_cast<uint2*>(smem + L.tets);
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
-  uint16_t* opp = reinterpret_cast<uint16_t*>(smem + L.opp);
   int32_t* ft = reinterpret_cast<int32_t*>(smem + L.ft);
-  int32_t* off_vt = reinterpret_cast<int32_t*>(smem + L.off_vt);
-  int32_t* off_vv = reinterpret_cast<int32_t*>(smem + L.off_vv);
+  uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
-  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scan, [36] queue length, [37] chunk counter
+  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [36] queue length, [38] n_vv
   uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
   uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
   uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
-  int32_t* ttrow = reinterpret_cast<int32_t*>(smem + L.ttrow);
-  int32_t* st_vt = reinterpret_cast<int32_t*>(smem + L.st_vt);
-  int32_t* st_vv = reinterpret_cast<int32_t*>(smem + L.st_vv);
+  uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);
+  uint16_t* st_vt = reinterpret_cast<uint16_t*>(smem + L.st_vt);
+  uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
 
   const int row0 = P.row_base[slot] + td.row_rel;
   const int vt0 = P.vt_base[slot] + td.vt_rel;
   const int vv0 = P.vv_base[slot] + td.vv_rel;
   const int tt0 = P.tt_base[slot] + td.tt_rel;
-  const int opp_rows = opp_rows_pad(nrows);
 
-  // ---- a1: stage + clear ----------------------------------------------------------------------
+  // ---- P0: stage + clear ----------------------------------------------------------------------
   {
     const int4* src = reinterpret_cast<const int4*>(M.loc + td.stg_off);
     int4* dst = reinterpret_cast<int4*>(tets);
     for (int i = tid; i < (S + 1) >> 1; i += NT) cp_async16(dst + i, src + i);
-    const int4* tsrc = reinterpret_cast<const int4*>(M.tex + td.tex_off);
-    int4* tdst = reinterpret_cast<int4*>(texid);
-    for (int i = tid; i < (s_ext + 3) >> 2; i += NT) cp_async16(tdst + i, tsrc + i);
-    const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
-    int4* gdst = reinterpret_cast<int4*>(gid);
-    for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
-    if (do_tt) {
-      const int4* osrc = reinterpret_cast<const int4*>(M.opp + td.opp_off);
-      int4* odst = reinterpret_cast<int4*>(opp);
-      for (int i = tid; i < (opp_rows + td.n_opp + 7) >> 3; i += NT) cp_async16(odst + i, osrc + i);
+    if (!COUNT) {
+      const int4* tsrc = reinterpret_cast<const int4*>(M.tex + td.tex_off);
+      int4* tdst = reinterpret_cast<int4*>(texid);
+      for (int i = tid; i < (s_ext + 3) >> 2; i += NT) cp_async16(tdst + i, tsrc + i);
+      if (do_vv || do_tt) {
+        const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
+        int4* gdst = reinterpret_cast<int4*>(gid);
+        for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
+      }
     }
   }
   for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + v_lo + i) - t_lo;
@@ -408,105 +429,195 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     const int n16 = (L.bm_end - L.bmT) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
   }
-  if (do_tt) {  // tables empty, TT rows -1: both all-ones, contiguous
+  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
     int4* z = reinterpret_cast<int4*>(smem + L.tbl);
     const int n16 = (L.tt_end - L.tbl) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
   }
-  if (tid < 2) scan[36 + tid] = 0u;
+  if (tid == 0) { scan[36] = 0u; scan[38] = 0u; }
   cp_async_wait_all();
   __syncthreads();
 
-  // ---- a4: thread p matches the facets whose lowest vertex is tile vertex p -------------------
-  if (do_tt && tid < nrows) {
-    GroupCtx g;
-    const int hs = C.hs;
-    g.tbl = tbl + tid * (hs + 1);
-    g.hmask = (uint32_t)hs - 1u;
-    g.hshift = 32 - (31 - __clz(hs));
-    g.ttrow = ttrow;
-    g.texid = texid;
-    const int r0 = ft[tid], r1 = ft[tid + 1];
-    const int o0 = opp[tid], o1 = opp[tid + 1];
-    g.opp_idx = opp + opp_rows + o0;
-    g.run0 = r0;
-    g.nrun = (r1 - r0) * (D - 1);
-    g.s_ext = s_ext;
-    g.t_lo = t_lo;
-    int j = 0;
-    for (int i = r0; i < r1; ++i) {
-      int l[4];
-      unpack_local(tets[s_ext + i], l);
-      group_place<D>(g, group_key<D, 1>(l), j, s_ext + i, 1, M.err);
-      group_place<D>(g, group_key<D, 2>(l), j + 1, s_ext + i, 2, M.err);
-      if constexpr (D == 4) group_place<D>(g, group_key<D, 3>(l), j + 2, s_ext + i, 3, M.err);
-      j += D - 1;
-    }
-    for (int o = o0; o < o1; ++o, ++j) {
-      const int s = opp[opp_rows + o];
-      int l[4];
-      unpack_local(tets[s], l);
-      group_place<D>(g, group_key<D, 0>(l), j, s, 0, M.err);
+  // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
+  for (int s = tid; s < S; s += NT) {
+    int l[4];
+    unpack_local(tets[s], l);
+    uint32_t* col = bmT + (s >> 5);
+    const uint32_t bit = bit_of(s);
+#pragma unroll
+    for (int k = 1; k < D; ++k) {
+      const int r = l[k] - nlo;
+      if ((unsigned)r < (unsigned)nrows) atomicOr(col + r * WT, bit);
     }
   }
+  __syncthreads();
 
-  // ---- a2/a3: one bit per incidence / per adjacent pair; warps take chunks of 32 simplices -----
-  if (do_vt || do_vv) {
-    const int nchunks = (S + 31) >> 5;
-    for (;;) {
-      uint32_t c = 0u;
-      if (lane == 0) c = atomicAdd(&scan[37], 1u);
-      c = __shfl_sync(0xFFFFFFFFu, c, 0);
-      if ((int)c >= nchunks) break;
-      const int s = (int)c * 32 + lane;
-      if (s < S) {
+  // ---- P2: row degrees -> VT offsets ----------------------------------------------------------
+  const bool isB = tid >= TV;
+  const int p = isB ? tid - TV : tid;
+  const bool live = p < nrows;
+  const int ploc = nlo + p;
+  const int wT = (S + 31) >> 5;
+  if (live) {
+    const int half = (wT + 1) >> 1;
+    const uint32_t* row = bmT + p * WT;
+    int c = 0;
+    const int w0 = isB ? half : 0, w1 = isB ? wT : half;
+#pragma unroll 4
+    for (int w = w0; w < w1; ++w) c += __popc(row[w]);
+    cnt[(isB ? C.tv : 0) + p] = (uint16_t)c;
+  }
+  __syncthreads();
+  int nb = 0, off = 0, n_vt;
+  {
+    uint32_t deg = 0u, tot;
+    if (live) {
+      nb = (int)cnt[p] + (int)cnt[C.tv + p];
+      deg = (uint32_t)(nb + ft[p + 1] - ft[p]);
+    }
+    const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // A and B halves carry the same values
+    n_vt = (int)(tot >> 1);
+    off = (int)ex - (isB ? n_vt : 0);
+  }
+  if (!COUNT && do_vt && live && !isB) O.vt_offsets[row0 + p] = vt0 + off;
+
+  // ---- P3: A walks the bits of row p, B walks the run of p ------------------------------------
+  if (live) {
+    uint32_t* vvrow = bmV + p * WV;
+    if (!isB) {
+      const uint32_t* row = bmT + p * WT;
+      int pos = off, sbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nb; ++n) {
+        while (bits == 0u) { bits = *row++; sbase += 32; }
+        const int s = sbase + __ffs(bits) - 1;
+        bits &= bits - 1;
         int l[4];
         unpack_local(tets[s], l);
-        bool in[D];
-#pragma unroll
-        for (int k = 0; k < D; ++k) in[k] = (unsigned)(l[k] - nlo) < (unsigned)nrows;
-        if (do_vt) {
-          const uint32_t bit = 1u << lane;
-          uint32_t* col = bmT + c;
-#pragma unroll
-          for (int k = 1; k < D; ++k)
-            if (in[k]) atomicOr(col + (l[k] - nlo) * WT, bit);
-        }
+        if (entries) st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
         if (do_vv) {
-          uint32_t w[D], b[D];
 #pragma unroll
-          for (int k = 0; k < D; ++k) { w[k] = (uint32_t)l[k] >> 5; b[k] = 1u << (l[k] & 31); }
+          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));  // self bit cleared in P4
+        }
+      }
+    } else {
+      GroupCtx g;
+      if (do_tt) {
+        const int hs = C.hs;
+        g.tbl = tbl + p * (hs + 1);
+        g.hmask = (uint32_t)hs - 1u;
+        g.hshift = 32 - (31 - __clz(hs));
+        g.ttrow = ttrow;
+        g.s_ext = s_ext;
+      }
+      int pos = off + nb;
+      const int r1 = ft[p + 1];
+      for (int i = ft[p]; i < r1; ++i) {
+        const int s = s_ext + i;
+        int l[4];
+        unpack_local(tets[s], l);
+        if (entries) st_vt[pos++] = (uint16_t)s;
+        if (do_vv) {
 #pragma unroll
-          for (int k = 0; k < D; ++k) {
-            if (!in[k]) continue;
-            uint32_t* row = bmV + (l[k] - nlo) * WV;
-#pragma unroll
-            for (int j = 0; j < D; ++j)
-              if (j != k) atomicOr(row + w[j], b[j]);
-          }
+          for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));
+        }
+        if (do_tt) {
+          group_place<D>(g, group_key<D, 1>(l), s, 1, M.err);
+          group_place<D>(g, group_key<D, 2>(l), s, 2, M.err);
+          if constexpr (D == 4) group_place<D>(g, group_key<D, 3>(l), s, 3, M.err);
         }
       }
     }
   }
   __syncthreads();
 
+  // ---- P4: A joins the facets 0 of the simplices (x, p, ..); B expands VV row p ----------------
+  int n_vv = 0;
+  if (!isB) {
+    if (do_tt && live) {
+      GroupCtx g;
+      const int hs = C.hs;
+      g.tbl = tbl + p * (hs + 1);
+      g.hmask = (uint32_t)hs - 1u;
+      g.hshift = 32 - (31 - __clz(hs));
+      g.ttrow = ttrow;
+      g.s_ext = s_ext;
+      int i = off;
+      const int end = off + nb;
+      for (;;) {
+        uint32_t e = 0u;
+        while (i < end && !((e = st_vt[i]) & 0x8000u)) ++i;
+        if (i >= end) break;
+        ++i;
+        const int s = (int)(e & 0x7FFFu);
+        int l[4];
+        unpack_local(tets[s], l);
+        group_place<D>(g, group_key<D, 0>(l), s, 0, M.err);
+      }
+    }
+  } else if (do_vv) {
+    const int wV = (td.nloc + 31) >> 5;
+    uint32_t* row = bmV + p * WV;
+    int nbv = 0;
+    if (live) {
+      row[ploc >> 5] &= ~bit_of(ploc);  // a vertex is not its own neighbour
+#pragma unroll 4
+      for (int w = 0; w < wV; ++w) nbv += __popc(row[w]);
+    }
+    uint32_t tot;
+    const int offv = (int)half_exclusive_scan<NT>((uint32_t)nbv, scan, &tot);
+    if (tid == TV) scan[38] = tot;
+    if (live && !COUNT) {
+      O.vv_offsets[row0 + p] = vv0 + offv;
+      int pos = offv, lbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nbv; ++n) {
+        while (bits == 0u) { bits = *row++; lbase += 32; }
+        st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
+        bits &= bits - 1;
+      }
+    }
+  }
+  __syncthreads();
+  n_vv = (int)scan[38];
+
+  if (COUNT) {
+    if (tid == 0) {
+      O.stats[(long long)tile * 4 + 0] = n_vt;
+      O.stats[(long long)tile * 4 + 1] = n_vv;
+      O.stats[(long long)tile * 4 + 2] = 0;
+      O.stats[(long long)tile * 4 + 3] = 0;
+    }
+    return;
+  }
+  if (tid == 0 && ((do_vt && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
+    raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
+
+  // ---- P5: translate to global ids, coalesced write-out ----------------------------------------
   if (do_tt) {
-    // ---- TT rows to global; facets no tile vertex owns go to the queue --------------------------
+    // facets no tile vertex owns go to the queue
     for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
       const int i = base + lane;
       bool need_fb = false;
       if (i < s_int) {
-        int first;
+        uint32_t e[D];
         if constexpr (D == 4) {
-          const int4 v = reinterpret_cast<const int4*>(ttrow)[i];
-          reinterpret_cast<int4*>(O.tt_indices)[tt0 + i] = v;
-          first = v.x;
+          const uint2 q = reinterpret_cast<const uint2*>(ttrow)[i];
+          e[0] = q.x & 0xFFFFu; e[1] = q.x >> 16; e[2] = q.y & 0xFFFFu; e[3] = q.y >> 16;
+        } else {
+          e[0] = ttrow[i * 3]; e[1] = ttrow[i * 3 + 1]; e[2] = ttrow[i * 3 + 2];
+        }
+        int r[D];
+#pragma unroll
+        for (int k = 0; k < D; ++k)
+          r[k] = e[k] == 0xFFFFu ? -1 : ((int)e[k] < s_ext ? texid[e[k]] : t_lo + ((int)e[k] - s_ext));
+        if constexpr (D == 4) {
+          reinterpret_cast<int4*>(O.tt_indices)[tt0 + i] = make_int4(r[0], r[1], r[2], r[3]);
         } else {
           int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
-          first = ttrow[i * 3];
-          o[0] = first; o[1] = ttrow[i * 3 + 1]; o[2] = ttrow[i * 3 + 2];
+          o[0] = r[0]; o[1] = r[1]; o[2] = r[2];
         }
-        need_fb = first < 0 && (int)(tets[s_ext + i].x >> 16) - nlo >= nrows;
+        need_fb = r[0] < 0 && (int)(tets[s_ext + i].x >> 16) - nlo >= nrows;
       }
       const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
       if (fbm) {
@@ -518,93 +629,26 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       }
     }
   }
-
-  if (do_vt || do_vv) {
-    // ---- row degrees -> offsets: threads [0, rows) own the VT rows, [NT/2, NT/2+rows) the VV rows
-    const bool vt_thread = do_vt && tid < nrows;
-    const int vrow = tid - NT / 2;
-    const bool vv_thread = do_vv && vrow >= 0 && vrow < nrows;
-    const int wT = (S + 31) >> 5, wV = (td.nloc + 31) >> 5;
-    uint32_t tot = 0u;
-    int nbits = 0;  // set bits of this thread's row
-    {
-      uint32_t deg = 0u;
-      if (vt_thread) {
-        const uint32_t* row = bmT + tid * WT;
-#pragma unroll 4
-        for (int w = 0; w < wT; ++w) nbits += __popc(row[w]);
-        deg = (uint32_t)(nbits + ft[tid + 1] - ft[tid]);
-      } else if (vv_thread) {
-        const uint32_t* row = bmV + vrow * WV;
-#pragma unroll 4
-        for (int w = 0; w < wV; ++w) nbits += __popc(row[w]);
-        deg = (uint32_t)nbits << 16;
-      }
-      const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // (also orders the TT row copy
-      if (vt_thread) off_vt[tid] = (int)(ex & 0xFFFFu);               //  before the staging reuse)
-      if (vv_thread) off_vv[vrow] = (int)(ex >> 16);
+  if (do_vt)
+    for (int i = tid; i < n_vt; i += NT) {
+      const int s = (int)(st_vt[i] & 0x7FFFu);
+      O.vt_indices[vt0 + i] = s < s_ext ? texid[s] : t_lo + (s - s_ext);
     }
-    const int n_vt = (int)(tot & 0xFFFFu), n_vv = (int)(tot >> 16);
-    if (COUNT) {
-      if (tid == 0) {
-        O.stats[(long long)tile * 4 + 0] = n_vt;
-        O.stats[(long long)tile * 4 + 1] = n_vv;
-        O.stats[(long long)tile * 4 + 2] = 0;
-        O.stats[(long long)tile * 4 + 3] = 0;
-      }
-      return;
-    }
-    if (tid == 0 && ((do_vt && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
-      raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
-
-    // ---- expand the rows into the staging areas, ids translated back to global ------------------
-    // One loop iteration per set bit (not per word): lanes of a warp run in step however their
-    // bits are spread over the words of their rows.
-    if (vt_thread) {
-      O.vt_offsets[row0 + tid] = vt0 + (int)off_vt[tid];
-      const uint32_t* row = bmT + tid * WT;
-      int p = off_vt[tid], sbase = -32;
-      uint32_t bits = 0u;
-      for (int n = 0; n < nbits; ++n) {
-        while (bits == 0u) { bits = *row++; sbase += 32; }
-        const int s = sbase + __ffs(bits) - 1;
-        bits &= bits - 1;
-        st_vt[p++] = s < s_ext ? texid[s] : t_lo + (s - s_ext);
-      }
-      for (int j = ft[tid]; j < ft[tid + 1]; ++j) st_vt[p++] = t_lo + j;
-    } else if (vv_thread) {
-      O.vv_offsets[row0 + vrow] = vv0 + (int)off_vv[vrow];
-      const uint32_t* row = bmV + vrow * WV;
-      int p = off_vv[vrow], lbase = -32;
-      uint32_t bits = 0u;
-      for (int n = 0; n < nbits; ++n) {
-        while (bits == 0u) { bits = *row++; lbase += 32; }
-        const int l = lbase + __ffs(bits) - 1;
-        bits &= bits - 1;
-        st_vv[p++] = gid[l];
-      }
-    }
-    __syncthreads();
-
-    // ---- a6: coalesced write-out ----------------------------------------------------------------
-    if (do_vt)
-      for (int i = tid; i < n_vt; i += NT) O.vt_indices[vt0 + i] = st_vt[i];
-    if (do_vv)
-      for (int i = tid; i < n_vv; i += NT) O.vv_indices[vv0 + i] = st_vv[i];
-  } else {
-    __syncthreads();  // queue complete
-  }
+  if (do_vv)
+    for (int i = tid; i < n_vv; i += NT) O.vv_indices[vv0 + i] = gid[st_vv[i]];
 
   if (do_tt) {
-    // ---- a5: one queued facet per thread, resolved from global memory (no barrier follows) ------
+    __syncthreads();  // queue complete, TT rows stored
+    // ---- a5: one queued facet per thread, resolved from global memory -------------------------
     const int nq = (int)scan[36];
     for (int q = tid; q < nq; q += NT) {
       const int i = fbq[q];
       int l[4];
       unpack_local(tets[s_ext + i], l);
+      const int t = t_lo + i;
       const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
-      const int r = tt_fallback<D>(M, b, c, d, t_lo + i);
-      if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barriers
+      const int r = tt_fallback<D>(M, b, c, d, t);
+      if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barrier
     }
   }
 }

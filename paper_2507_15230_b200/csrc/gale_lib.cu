@@ -53,7 +53,6 @@ struct Plan {
   int tv = 0, nTiles = 0, NT = 0;
   std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
   std::vector<uint16_t> loc;            // 4 per staged simplex
-  std::vector<uint16_t> opp;            // per tile: row starts, then staged indices by second vertex
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
   int smem_bytes = 0;
@@ -67,7 +66,7 @@ struct Plan {
   size_t index_bytes() const {
     return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
            up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16) + up(opp.size() * 2 + 16);
+           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16);
   }
 };
 
@@ -117,14 +116,14 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-inline int threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : 128); }  // NT >= 2 * tv
+inline int threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : (tv > 32 ? 128 : 64)); }  // NT >= 2 * tv
 
 // Kernel capacities for one launch: regions the relation mask does not need are dropped.
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
   SmemCfg c = full;
   if (!(mask & gale::REL_VV)) { c.WV = 0; c.vv_max = 0; }
-  if (!(mask & gale::REL_TT) || count_mode) { c.hs = 0; c.nopp = 0; c.sint = 0; }
-  if (!(mask & gale::REL_VT)) { c.WT = 0; c.vt_max = 0; }
+  if (!(mask & gale::REL_TT) || count_mode) { c.hs = 0; c.sint = 0; }
+  if (!(mask & (gale::REL_VT | gale::REL_TT))) c.vt_max = 0;  // TT reads the staged VT entries' flags
   if (count_mode) { c.vt_max = 0; c.vv_max = 0; }
   return c;
 }
@@ -138,7 +137,8 @@ using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemC
 template <int D, bool COUNT>
 KernelFn kernel_for_nt(int NT) {
   return NT == 512 ? gale::gale_batch_kernel<D, 512, COUNT>
-                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT> : gale::gale_batch_kernel<D, 128, COUNT>);
+                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT>
+                                : (NT == 128 ? gale::gale_batch_kernel<D, 128, COUNT> : gale::gale_batch_kernel<D, 64, COUNT>));
 }
 KernelFn kernel_for(int D, int NT, bool count) {
   if (D == 4) return count ? kernel_for_nt<4, true>(NT) : kernel_for_nt<4, false>(NT);
@@ -210,7 +210,7 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       d.stg_off = stg;
       d.tex_off = texo;
       const long long S = (long long)d.s_int + d.s_ext;
-      if (S > gale::kMaxStaged) return false;
+      if (S > (D == 4 ? gale::kMaxStaged4 : gale::kMaxStaged3)) return false;
       stg += pad_to(S, 2);
       texo += pad_to(d.s_ext, 4);
     }
@@ -221,17 +221,13 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   // halo + local encoding, tiles split over host threads
   const int nth = std::max(1, std::min<int>(32, std::min<int>(int(std::thread::hardware_concurrency()), nTiles / 64 + 1)));
   std::vector<std::vector<int32_t>> gid_part(nth);
-  std::vector<std::vector<uint16_t>> opp_part(nth);
-  std::vector<int> group_max(nth, 0);
-  const int max_group = D == 4 ? gale::kMaxGroup4 : gale::kMaxGroup3;
   std::vector<int> tile_lo(nth + 1);
   for (int w = 0; w <= nth; ++w) tile_lo[w] = int((long long)nTiles * w / nth);
   std::atomic<bool> ok{true};
   auto work = [&](int w) {
     std::vector<uint16_t> map(size_t(p.nV), uint16_t(0xFFFF));
     std::vector<int32_t>& hp = gid_part[w];
-    std::vector<uint16_t>& op = opp_part[w];
-    std::vector<int32_t> h, cnt;
+    std::vector<int32_t> h;
     for (int i = tile_lo[w]; i < tile_lo[w + 1] && ok.load(std::memory_order_relaxed); ++i) {
       TileDesc& d = p.tiles[i];
       const int v_lo = d.v_lo, v_hi = d.v_lo + d.nrows;
@@ -263,29 +259,6 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
           out[s * 4 + k] = k >= D ? uint16_t(0xFFFF)
                                   : (r[k] >= v_lo && r[k] < v_hi) ? uint16_t(nlo + (r[k] - v_lo)) : map[r[k]];
       }
-      // second-vertex index of the tile: row r lists the staged simplices whose second vertex is r
-      {
-        const int rp = gale::opp_rows_pad(d.nrows);
-        cnt.assign(size_t(d.nrows) + 1, 0);
-        for (int s = 0; s < S; ++s) {
-          const int r = int(out[s * 4 + 1]) - nlo;
-          if (r >= 0 && r < d.nrows) ++cnt[r + 1];
-        }
-        for (int r = 0; r < d.nrows; ++r) {
-          const int group = (D - 1) * (p.first_tet[v_lo + r + 1] - p.first_tet[v_lo + r]) + cnt[r + 1];
-          group_max[w] = std::max(group_max[w], group);
-          cnt[r + 1] += cnt[r];
-        }
-        d.n_opp = cnt[d.nrows];
-        d.opp_off = (long long)op.size();  // relative; rebased below
-        const size_t base = op.size();
-        op.resize(base + size_t(rp) + size_t(pad_to(d.n_opp, 8)), 0);
-        for (int r = 0; r <= d.nrows; ++r) op[base + r] = uint16_t(cnt[r]);
-        for (int s = 0; s < S; ++s) {
-          const int r = int(out[s * 4 + 1]) - nlo;
-          if (r >= 0 && r < d.nrows) op[base + rp + size_t(cnt[r]++)] = uint16_t(s);
-        }
-      }
       hp.insert(hp.end(), h.begin(), h.begin() + nlo);  // local id -> global id, ascending
       for (int v = v_lo; v < v_hi; ++v) hp.push_back(v);
       hp.insert(hp.end(), h.begin() + nlo, h.end());
@@ -312,25 +285,14 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     hoff += (long long)gid_part[w].size();
     std::vector<int32_t>().swap(gid_part[w]);
   }
-  long long ooff = 0;
+  // largest facet group of a tile vertex: D-1 facets per simplex of its run + facet 0 of every
+  // simplex whose second vertex it is
   int gmax = 1;
-  for (int w = 0; w < nth; ++w) {
-    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].opp_off += ooff;
-    ooff += (long long)opp_part[w].size();
-    gmax = std::max(gmax, group_max[w]);
-  }
-  if (gmax > max_group) return false;
-  p.opp.assign(size_t(ooff) + 8, 0);
-  ooff = 0;
-  for (int w = 0; w < nth; ++w) {
-    std::copy(opp_part[w].begin(), opp_part[w].end(), p.opp.begin() + ooff);
-    ooff += (long long)opp_part[w].size();
-    std::vector<uint16_t>().swap(opp_part[w]);
-  }
+  for (int v = 0; v < p.nV; ++v)
+    gmax = std::max(gmax, (D - 1) * (p.first_tet[v + 1] - p.first_tet[v]) + (p.opp_first[v + 1] - p.opp_first[v]));
   // shared-memory capacities known so far
-  long long smax = 2, sext = 4, sint = 2, nloc = 4, nopp = 8;
+  long long smax = 2, sext = 4, sint = 2, nloc = 4;
   for (const TileDesc& d : p.tiles) {
-    nopp = std::max(nopp, (long long)gale::opp_rows_pad(d.nrows) + pad_to(d.n_opp, 8));
     smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 2));
     sext = std::max(sext, pad_to(d.s_ext, 4));
     sint = std::max(sint, pad_to(d.s_int, 2));
@@ -342,7 +304,6 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   p.cfg.sext = int(sext);
   p.cfg.nloc = int(nloc);
   p.cfg.sint = int(sint);
-  p.cfg.nopp = int(nopp);
   p.cfg.hs = 8;
   while (p.cfg.hs < gmax + gmax / 4 + 1) p.cfg.hs *= 2;  // a group never fills its table
   p.cfg.WT = int((smax + 31) / 32) | 1;
@@ -457,7 +418,7 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   p->cl_t_lo.resize(p->nC + 1);
   for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
 
-  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, 256) : (d.dim == 3 ? 128 : 256);
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 64 : 128);
   std::vector<long long> stats;
   for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
@@ -639,7 +600,6 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
   m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
   m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
-  m->dm.opp = static_cast<uint16_t*>(put(p->opp.data(), p->opp.size() * 2, 16));
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
   GALE_CUDA(cudaStreamSynchronize(st));
@@ -647,7 +607,6 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   std::vector<int32_t>().swap(p->tex);
   std::vector<int32_t>().swap(p->gid);
   std::vector<uint16_t>().swap(p->loc);
-  std::vector<uint16_t>().swap(p->opp);
   std::vector<int32_t>().swap(p->opp_first);
 
   GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
