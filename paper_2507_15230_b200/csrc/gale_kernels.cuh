@@ -92,7 +92,7 @@ struct SmemCfg {
   int sext;      // external simplices (multiple of 4)
   int nloc;      // local vertex ids (multiple of 4)
   int sint;      // internal simplices (even): TT rows + fallback queue, 0 without TT
-  int hs;        // table slots per tile vertex (power of two), 0 without TT
+  int hs;        // table slots per tile vertex (even, so that the row stride hs+1 is odd), 0 without TT
   int WT;        // VT bitmap words per row (odd)
   int WV;        // VV bitmap words per row (odd), 0 without VV
   int vt_max;    // VT entries staged for write-out (16-bit)
@@ -121,16 +121,23 @@ __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
   L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
   L.cnt = o;    o = align16(o + c.tv * 4);
-  L.fbq = o;    o = align16(o + c.sint * 2);
   L.scan = o;   o = align16(o + 48 * 4);
-  L.bmT = o;    o = align16(o + c.tv * c.WT * 4);
+  // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
+  // fallback queue (written in P5)
+  L.bmT = o;
+  {
+    const int bm = align16(c.tv * c.WT * 4);
+    L.st_vv = o;
+    L.fbq = o + align16(c.vv_max * 2);
+    const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
+    o += bm > reuse ? bm : reuse;
+  }
   L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
   L.bm_end = o;
   L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
   L.ttrow = o;  o = align16(o + c.sint * D * 2);
   L.tt_end = o;
   L.st_vt = o;  o = align16(o + c.vt_max * 2);
-  L.st_vv = o;  o = align16(o + c.vv_max * 2);
   L.total = o;
   return L;
 }
@@ -142,6 +149,7 @@ struct BatchParams {
   int tile_base;                     // count mode: first tile of the launch
   int total_rows;                    // VT/VV rows of the whole batch
   int total_vt_nnz, total_vv_nnz;    // terminal offsets
+  int uniform_tiles;                 // > 0: every cluster of the batch has this many tiles (slot = block / it)
   int tile_prefix[kMaxBatch + 1];    // tiles of the batch before cluster slot i  (block -> cluster slot)
   int cluster[kMaxBatch];            // cluster id of slot i
   int row_base[kMaxBatch];           // first VT/VV row of slot i in the batch
@@ -270,8 +278,7 @@ struct FacetBits {
 
 struct GroupCtx {
   uint32_t* tbl;       // this vertex's table, hs slots
-  uint32_t hmask;
-  int hshift;
+  uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
   uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
   int s_ext;
 };
@@ -281,22 +288,21 @@ struct GroupCtx {
 template <int D>
 __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
   using FB = FacetBits<D>;
-  uint32_t h = (key * 0x9E3779B1u) >> g.hshift;
-  for (uint32_t probe = 0; probe <= g.hmask; ++probe) {
-    const uint32_t cur = g.tbl[h];
-    if (cur == kEmpty32) {
-      g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
-      return;
-    }
-    if ((cur & FB::kKeyMask) == key) {
-      const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
-      if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2;
-      if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s;
-      return;
-    }
-    h = (h + 1) & g.hmask;
+  uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
+  uint32_t cur = g.tbl[h];
+  uint32_t probe = 0;
+  while (cur != kEmpty32 && (cur & FB::kKeyMask) != key) {  // probe loop kept minimal: lanes diverge here
+    h = h + 1 == g.hs ? 0u : h + 1;
+    cur = g.tbl[h];
+    if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
   }
-  raise_err(err, ERR_TT_TABLE_FULL);
+  if (cur == kEmpty32) {
+    g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
+  } else {
+    const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
+    if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2;
+    if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s;
+  }
 }
 
 // Key of the facet opposite local vertex K: the facet's vertices other than its lowest one.
@@ -369,12 +375,16 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       if (do_vv) { O.vv_offsets[0] = 0; O.vv_offsets[P.total_rows] = P.total_vv_nnz; }
     }
     if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
-    int lo = 0, hi = P.n_clusters;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+    if (P.uniform_tiles > 0) {
+      slot = (int)blockIdx.x / P.uniform_tiles;
+    } else {
+      int lo = 0, hi = P.n_clusters;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+      }
+      slot = lo;
     }
-    slot = lo;
     tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
   }
   TileDesc td;
@@ -505,8 +515,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       if (do_tt) {
         const int hs = C.hs;
         g.tbl = tbl + p * (hs + 1);
-        g.hmask = (uint32_t)hs - 1u;
-        g.hshift = 32 - (31 - __clz(hs));
+        g.hs = (uint32_t)hs;
         g.ttrow = ttrow;
         g.s_ext = s_ext;
       }
@@ -538,8 +547,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       GroupCtx g;
       const int hs = C.hs;
       g.tbl = tbl + p * (hs + 1);
-      g.hmask = (uint32_t)hs - 1u;
-      g.hshift = 32 - (31 - __clz(hs));
+      g.hs = (uint32_t)hs;
       g.ttrow = ttrow;
       g.s_ext = s_ext;
       int i = off;

@@ -304,8 +304,9 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   p.cfg.sext = int(sext);
   p.cfg.nloc = int(nloc);
   p.cfg.sint = int(sint);
-  p.cfg.hs = 8;
-  while (p.cfg.hs < gmax + gmax / 4 + 1) p.cfg.hs *= 2;  // a group never fills its table
+  // one slot per record: distinct facets <= records, so a group cannot overflow its table, and since
+  // every interior facet is recorded twice the usual load is about one half
+  p.cfg.hs = std::max(8, (gmax + 1) & ~1);
   p.cfg.WT = int((smax + 31) / 32) | 1;
   p.cfg.WV = int((nloc + 31) / 32) | 1;
   return true;
@@ -721,6 +722,12 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.vt_base[i] = int(vtb[b + i]);
       P.vv_base[i] = int(vvb[b + i]);
       P.tt_base[i] = s.tt_row_begin[b + i];
+    }
+    {  // all clusters with the same tile count: the kernel divides instead of searching tile_prefix
+      const int per = nb > 0 ? P.tile_prefix[1] : 0;
+      bool uniform = per > 0;
+      for (int i = 0; i < nb && uniform; ++i) uniform = P.tile_prefix[i + 1] - P.tile_prefix[i] == per;
+      P.uniform_tiles = uniform ? per : 0;
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
     kernel_for(D, p.NT, false)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
