@@ -52,6 +52,7 @@ struct Plan {
   // index (host copies)
   int tv = 0, nTiles = 0, NT = 0;
   std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
+  std::vector<int2> hft;                // parallel to gid: (first_tet[g], first_tet[g+1])
   std::vector<uint16_t> loc;            // 4 per staged simplex
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
@@ -66,7 +67,7 @@ struct Plan {
   size_t index_bytes() const {
     return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
            up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(gid.size() * 4 + 16) + up(loc.size() * 2 + 16);
+           up(gid.size() * 4 + 16) + up(hft.size() * sizeof(int2) + 16) + up(loc.size() * 2 + 16);
   }
 };
 
@@ -285,6 +286,11 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     hoff += (long long)gid_part[w].size();
     std::vector<int32_t>().swap(gid_part[w]);
   }
+  p.hft.resize(p.gid.size());
+  for (size_t i = 0; i < p.gid.size(); ++i) {
+    const int g = std::min(std::max(p.gid[i], 0), std::max(p.nV - 1, 0));
+    p.hft[i] = p.nV > 0 ? make_int2(p.first_tet[g], p.first_tet[g + 1]) : make_int2(0, 0);
+  }
   // largest facet group of a tile vertex: D-1 facets per simplex of its run + facet 0 of every
   // simplex whose second vertex it is
   int gmax = 1;
@@ -337,10 +343,10 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   const std::vector<uint32_t> parts = {3u};
   if (layout_for(D, cfg_for_mask(full, 3, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
 
-  DevBuf b_ft, b_tiles, b_tex, b_gid, b_loc, b_stats, b_err;
+  DevBuf b_ft, b_tiles, b_tex, b_gid, b_hft, b_loc, b_stats, b_err;
   int rc;
   if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
-      (rc = b_gid.upload(p.gid, st)) || (rc = b_loc.upload(p.loc, st)) ||
+      (rc = b_gid.upload(p.gid, st)) || (rc = b_hft.upload(p.hft, st)) || (rc = b_loc.upload(p.loc, st)) ||
       (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
     return rc;
   GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
@@ -350,6 +356,7 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   dm.tiles = static_cast<TileDesc*>(b_tiles.p);
   dm.tex = static_cast<int32_t*>(b_tex.p);
   dm.gid = static_cast<int32_t*>(b_gid.p);
+  dm.hft = static_cast<int2*>(b_hft.p);
   dm.loc = static_cast<uint2*>(b_loc.p);
   dm.err = static_cast<int32_t*>(b_err.p);
   KernelFn fn = kernel_for(D, p.NT, true);
@@ -600,6 +607,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.tiles = static_cast<TileDesc*>(put(p->tiles.data(), p->tiles.size() * sizeof(TileDesc), 16));
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
   m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
+  m->dm.hft = static_cast<int2*>(put(p->hft.data(), p->hft.size() * sizeof(int2), 16));
   m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
@@ -607,6 +615,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   std::vector<int32_t>().swap(p->opp_perm);
   std::vector<int32_t>().swap(p->tex);
   std::vector<int32_t>().swap(p->gid);
+  std::vector<int2>().swap(p->hft);
   std::vector<uint16_t>().swap(p->loc);
   std::vector<int32_t>().swap(p->opp_first);
 
