@@ -64,7 +64,7 @@ struct TileDesc {
   int32_t vt_rel, vv_rel;     // first VT / VV entry of the tile inside its cluster
   int32_t vt_nnz, vv_nnz;     // entries of the tile (fixed at create; the kernel re-derives them)
   int32_t pad0;
-  long long stg_off;          // first staged simplex of the tile in DeviceMesh::loc (even)
+  long long stg_off;          // first staged simplex of the tile in DeviceMesh::loc (multiple of 4)
   long long tex_off;          // first entry in DeviceMesh::tex (multiple of 4)
   long long gid_off;          // first entry in DeviceMesh::gid (multiple of 4)
 };
@@ -77,7 +77,8 @@ struct DeviceMesh {
   const int32_t* opp_first;           // [nV+1] first position in opp_perm whose second vertex is >= v
   const int32_t* opp_perm;            // [nT]   simplex ids grouped by second vertex
   const TileDesc* tiles;              // [nTiles]
-  const uint2* loc;                   // staged simplices in tile-local ids, 4 x uint16 each
+  const void* loc;                    // staged simplices in tile-local ids: 4 x uint16 each, or 4 x uint8
+                                      //   when no tile of the mesh has more than 255 local vertices (SmemCfg::lb)
   const int32_t* tex;                 // per-tile ascending global ids of external simplices (T_ex)
   const int32_t* gid;                 // per-tile global vertex id of every local id (ascending)
   const int2* hft;                    // per-tile, parallel to gid: (first_tet[g], first_tet[g+1]) — the
@@ -90,7 +91,8 @@ struct DeviceMesh {
 // the launch's relation mask does not need the region.
 struct SmemCfg {
   int tv;        // rows (vertices) per tile, <= NT/2
-  int smax;      // staged simplices (even)
+  int smax;      // staged simplices (multiple of 4)
+  int lb;        // bytes per local vertex id in the staged list: 1 or 2
   int sext;      // external simplices (multiple of 4)
   int nloc;      // local vertex ids (multiple of 4)
   int sint;      // internal simplices (even): TT rows + fallback queue, 0 without TT
@@ -116,7 +118,7 @@ template <int D>
 __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   SmemLayout L;
   int o = 0;
-  L.tets = o;   o = align16(o + c.smax * 8);
+  L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
   L.hft = o;    o = align16(o + c.nloc * 8);
@@ -184,8 +186,16 @@ __device__ __forceinline__ void named_barrier(int id, int count) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory");
 }
 
-__device__ __forceinline__ void unpack_local(const uint2 q, int (&l)[4]) {
-  l[0] = q.x & 0xFFFF; l[1] = q.x >> 16; l[2] = q.y & 0xFFFF; l[3] = q.y >> 16;
+// Local vertex ids of staged simplex s (LB bytes each).
+template <int LB>
+__device__ __forceinline__ void load_local(const unsigned char* tets, int s, int (&l)[4]) {
+  if constexpr (LB == 2) {
+    const uint2 q = reinterpret_cast<const uint2*>(tets)[s];
+    l[0] = q.x & 0xFFFF; l[1] = q.x >> 16; l[2] = q.y & 0xFFFF; l[3] = q.y >> 16;
+  } else {
+    const uint32_t q = reinterpret_cast<const uint32_t*>(tets)[s];
+    l[0] = q & 0xFF; l[1] = (q >> 8) & 0xFF; l[2] = (q >> 16) & 0xFF; l[3] = q >> 24;
+  }
 }
 
 // 1 << (l mod 32)
@@ -355,7 +365,7 @@ __device__ __forceinline__ uint32_t half_exclusive_scan(uint32_t x, uint32_t* sc
 // The batch kernel: VT + VV + TT for every tile of the requested clusters (or, COUNT, the exact
 // VT / VV sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer likewise
 // sizes its relation arrays before launch). NT = 2 * (rows per tile capacity).
-template <int D, int NT, bool COUNT>
+template <int D, int NT, bool COUNT, int LB>
 __global__ void __launch_bounds__(NT, (NT <= 64 ? 16 : (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2))))
 gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
                   const SmemLayout L, const OutPtrs O) {
@@ -400,7 +410,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   const int S = s_int + s_ext;
   const int WT = C.WT, WV = C.WV;
 
-  uint2* tets = reinterpret_cast<uint2*>(smem + L.tets);
+  unsigned char* tets = smem + L.tets;
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
   const int2* hft = reinterpret_cast<const int2*>(smem + L.hft);
@@ -421,9 +431,9 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
 
   // ---- P0: stage + clear ----------------------------------------------------------------------
   {
-    const int4* src = reinterpret_cast<const int4*>(M.loc + td.stg_off);
+    const int4* src = reinterpret_cast<const int4*>(static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB));
     int4* dst = reinterpret_cast<int4*>(tets);
-    for (int i = tid; i < (S + 1) >> 1; i += NT) cp_async16(dst + i, src + i);
+    for (int i = tid; i < (S * 4 * LB + 15) >> 4; i += NT) cp_async16(dst + i, src + i);
     {
       const int4* hsrc = reinterpret_cast<const int4*>(M.hft + td.gid_off);
       int4* hdst = reinterpret_cast<int4*>(smem + L.hft);
@@ -457,7 +467,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
   for (int s = tid; s < S; s += NT) {
     int l[4];
-    unpack_local(tets[s], l);
+    load_local<LB>(tets, s, l);
     uint32_t* col = bmT + (s >> 5);
     const uint32_t bit = bit_of(s);
 #pragma unroll
@@ -519,7 +529,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         const int s = sbase + __ffs(bits) - 1;
         bits &= bits - 1;
         int l[4];
-        unpack_local(tets[s], l);
+        load_local<LB>(tets, s, l);
         if (entries) st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
         if (do_vv) {
 #pragma unroll
@@ -541,7 +551,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       for (int i = run.x - t_lo; i < r1; ++i) {
         const int s = s_ext + i;
         int l[4];
-        unpack_local(tets[s], l);
+        load_local<LB>(tets, s, l);
         if (entries) st_vt[pos++] = (uint16_t)s;
         if (do_vv) {
 #pragma unroll
@@ -576,7 +586,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         ++i;
         const int s = (int)(e & 0x7FFFu);
         int l[4];
-        unpack_local(tets[s], l);
+        load_local<LB>(tets, s, l);
         group_place<D>(g, group_key<D, 0>(l), s, 0, M.err);
       }
     }
@@ -642,7 +652,11 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
           int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
           o[0] = r[0]; o[1] = r[1]; o[2] = r[2];
         }
-        need_fb = r[0] < 0 && (int)(tets[s_ext + i].x >> 16) - nlo >= nrows;
+        if (r[0] < 0) {
+          int l[4];
+          load_local<LB>(tets, s_ext + i, l);
+          need_fb = l[1] - nlo >= nrows;
+        }
       }
       const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
       if (fbm) {
@@ -669,7 +683,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     for (int q = tid; q < nq; q += NT) {
       const int i = fbq[q];
       int l[4];
-      unpack_local(tets[s_ext + i], l);
+      load_local<LB>(tets, s_ext + i, l);
       const int t = t_lo + i;
       const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
       const int2 run = hft[l[1]];

@@ -53,7 +53,9 @@ struct Plan {
   int tv = 0, nTiles = 0, NT = 0;
   std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
   std::vector<int2> hft;                // parallel to gid: (first_tet[g], first_tet[g+1])
-  std::vector<uint16_t> loc;            // 4 per staged simplex
+  std::vector<uint16_t> loc;            // 4 per staged simplex (build); compacted into loc8 when lb == 1
+  std::vector<uint8_t> loc8;
+  long long staged_padded = 0;          // staged simplices incl. per-tile padding
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
   int smem_bytes = 0;
@@ -67,7 +69,7 @@ struct Plan {
   size_t index_bytes() const {
     return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
            up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(gid.size() * 4 + 16) + up(hft.size() * sizeof(int2) + 16) + up(loc.size() * 2 + 16);
+           up(gid.size() * 4 + 16) + up(hft.size() * sizeof(int2) + 16) + up(size_t(staged_padded) * 4 * cfg.lb + 64);
   }
 };
 
@@ -135,15 +137,17 @@ inline gale::SmemLayout layout_for(int D, const SmemCfg& c) {
 
 using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::SmemLayout,
                           const gale::OutPtrs);
-template <int D, bool COUNT>
+template <int D, bool COUNT, int LB>
 KernelFn kernel_for_nt(int NT) {
-  return NT == 512 ? gale::gale_batch_kernel<D, 512, COUNT>
-                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT>
-                                : (NT == 128 ? gale::gale_batch_kernel<D, 128, COUNT> : gale::gale_batch_kernel<D, 64, COUNT>));
+  return NT == 512 ? gale::gale_batch_kernel<D, 512, COUNT, LB>
+                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT, LB>
+                                : (NT == 128 ? gale::gale_batch_kernel<D, 128, COUNT, LB> : gale::gale_batch_kernel<D, 64, COUNT, LB>));
 }
-KernelFn kernel_for(int D, int NT, bool count) {
-  if (D == 4) return count ? kernel_for_nt<4, true>(NT) : kernel_for_nt<4, false>(NT);
-  return count ? kernel_for_nt<3, true>(NT) : kernel_for_nt<3, false>(NT);
+template <int D, bool COUNT>
+KernelFn kernel_for_lb(int NT, int lb) { return lb == 1 ? kernel_for_nt<D, COUNT, 1>(NT) : kernel_for_nt<D, COUNT, 2>(NT); }
+KernelFn kernel_for(int D, int NT, bool count, int lb) {
+  if (D == 4) return count ? kernel_for_lb<4, true>(NT, lb) : kernel_for_lb<4, false>(NT, lb);
+  return count ? kernel_for_lb<3, true>(NT, lb) : kernel_for_lb<3, false>(NT, lb);
 }
 
 // Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
@@ -212,10 +216,12 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       d.tex_off = texo;
       const long long S = (long long)d.s_int + d.s_ext;
       if (S > (D == 4 ? gale::kMaxStaged4 : gale::kMaxStaged3)) return false;
-      stg += pad_to(S, 2);
+      stg += pad_to(S, 4);
       texo += pad_to(d.s_ext, 4);
     }
-  p.loc.assign(size_t(stg) * 4 + 8, 0);
+  p.staged_padded = stg;
+  p.loc.assign(size_t(stg) * 4 + 16, 0);
+  p.loc8.clear();
   p.tex.assign(size_t(texo) + 4, 0);
   for (int i = 0; i < nTiles; ++i)
     std::copy(raw.begin() + raw_off[i], raw.begin() + raw_off[i + 1], p.tex.begin() + p.tiles[i].tex_off);
@@ -297,9 +303,9 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   for (int v = 0; v < p.nV; ++v)
     gmax = std::max(gmax, (D - 1) * (p.first_tet[v + 1] - p.first_tet[v]) + (p.opp_first[v + 1] - p.opp_first[v]));
   // shared-memory capacities known so far
-  long long smax = 2, sext = 4, sint = 2, nloc = 4;
+  long long smax = 4, sext = 4, sint = 2, nloc = 4;
   for (const TileDesc& d : p.tiles) {
-    smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 2));
+    smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 4));
     sext = std::max(sext, pad_to(d.s_ext, 4));
     sint = std::max(sint, pad_to(d.s_int, 2));
     nloc = std::max(nloc, pad_to(d.nloc, 4));
@@ -309,10 +315,18 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
   p.cfg.smax = int(smax);
   p.cfg.sext = int(sext);
   p.cfg.nloc = int(nloc);
+  // 8-bit local ids when every tile has at most 255 local vertices: half the staged bytes (HBM and
+  // shared memory). 0xFF only pads the unused 4th entry of a triangle.
+  p.cfg.lb = nloc <= 255 ? 1 : 2;
+  if (p.cfg.lb == 1) {
+    p.loc8.resize(p.loc.size());
+    for (size_t i = 0; i < p.loc.size(); ++i) p.loc8[i] = uint8_t(p.loc[i]);
+    std::vector<uint16_t>().swap(p.loc);
+  }
   p.cfg.sint = int(sint);
-  // one slot per record: distinct facets <= records, so a group cannot overflow its table, and since
-  // every interior facet is recorded twice the usual load is about one half
-  p.cfg.hs = std::max(8, (gmax + 1) & ~1);
+  // distinct facets <= records, so a group cannot overflow its table; every interior facet is recorded
+  // twice, so the usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
+  p.cfg.hs = std::max(8, (gmax + gmax / 3 + 1) & ~1);  // load <= 3/4 even if no facet of a group is shared
   p.cfg.WT = int((smax + 31) / 32) | 1;
   p.cfg.WV = int((nloc + 31) / 32) | 1;
   return true;
@@ -346,7 +360,7 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   DevBuf b_ft, b_tiles, b_tex, b_gid, b_hft, b_loc, b_stats, b_err;
   int rc;
   if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
-      (rc = b_gid.upload(p.gid, st)) || (rc = b_hft.upload(p.hft, st)) || (rc = b_loc.upload(p.loc, st)) ||
+      (rc = b_gid.upload(p.gid, st)) || (rc = b_hft.upload(p.hft, st)) || (rc = (p.cfg.lb == 1 ? b_loc.upload(p.loc8, st) : b_loc.upload(p.loc, st))) ||
       (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
     return rc;
   GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
@@ -357,9 +371,9 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   dm.tex = static_cast<int32_t*>(b_tex.p);
   dm.gid = static_cast<int32_t*>(b_gid.p);
   dm.hft = static_cast<int2*>(b_hft.p);
-  dm.loc = static_cast<uint2*>(b_loc.p);
+  dm.loc = b_loc.p;
   dm.err = static_cast<int32_t*>(b_err.p);
-  KernelFn fn = kernel_for(D, p.NT, true);
+  KernelFn fn = kernel_for(D, p.NT, true, p.cfg.lb);
   std::vector<long long> part_stats(stats.size());
   for (uint32_t m : parts) {
     const SmemCfg c = cfg_for_mask(full, m, true);
@@ -608,7 +622,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
   m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
   m->dm.hft = static_cast<int2*>(put(p->hft.data(), p->hft.size() * sizeof(int2), 16));
-  m->dm.loc = static_cast<uint2*>(put(p->loc.data(), p->loc.size() * 2, 16));
+  m->dm.loc = p->cfg.lb == 1 ? put(p->loc8.data(), p->loc8.size(), 64) : put(p->loc.data(), p->loc.size() * 2, 64);
   GALE_CUDA(cudaGetLastError());
   // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
   GALE_CUDA(cudaStreamSynchronize(st));
@@ -617,6 +631,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   std::vector<int32_t>().swap(p->gid);
   std::vector<int2>().swap(p->hft);
   std::vector<uint16_t>().swap(p->loc);
+  std::vector<uint8_t>().swap(p->loc8);
   std::vector<int32_t>().swap(p->opp_first);
 
   GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
@@ -637,7 +652,7 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   }
   m->workspace_used = o;
   if (desc->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
-  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT, false), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT, false, p->cfg.lb), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
   m->plan = std::move(p);
   m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() +
                  (m->plan->analyse_ms);
@@ -739,7 +754,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.uniform_tiles = uniform ? per : 0;
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    kernel_for(D, p.NT, false)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
+    kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, st>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, st));
