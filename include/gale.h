@@ -116,6 +116,9 @@ typedef struct {
   size_t slot_bytes;             /* bytes of one result slot                                         */
   size_t workspace_used;
   double create_ms;
+  int32_t local_id_bytes;        /* width of the tile-local vertex ids in the staged lists: 1 when every
+                                    tile has at most 255 local vertices (tile + halo), else 2           */
+  int32_t block_threads;         /* threads per block of the batch kernel                            */
 } gale_mesh_info_t;
 
 /* Upper bound of the device workspace gale_mesh_create needs for this descriptor

@@ -46,7 +46,8 @@ class gale_mesh_info_t(ctypes.Structure):
     _fields_ = [("tile_vertices", ctypes.c_int32), ("num_tiles", ctypes.c_int32),
                 ("num_external_refs", ctypes.c_int64), ("vt_nnz", ctypes.c_int64), ("vv_nnz", ctypes.c_int64),
                 ("smem_bytes", ctypes.c_int32), ("max_staged", ctypes.c_int32),
-                ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double)]
+                ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double),
+                ("local_id_bytes", ctypes.c_int32), ("block_threads", ctypes.c_int32)]
 
 
 EXPORTS = ["gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",

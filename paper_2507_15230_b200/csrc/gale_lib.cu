@@ -673,6 +673,8 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   out->slot_bytes = m->cap.total;
   out->workspace_used = m->workspace_used;
   out->create_ms = m->create_ms;
+  out->local_id_bytes = p.cfg.lb;
+  out->block_threads = p.NT;
   return GALE_OK;
 }
 

@@ -72,6 +72,26 @@ def test_parity_tile_sizes(tv):
     _compare(got, ref, f"2d tv={tv}")
 
 
+def test_both_local_id_widths():
+    """The staged lists use 8-bit tile-local vertex ids when every tile has at most 255 local vertices
+    and 16-bit ids otherwise; both encodings must be exercised and both must be bit-exact."""
+    m = meshgen.make_mesh(3, 20, clustering="octree", capacity=2000, permute=True, drop_frac=0.05, seed=21)
+    assert int(np.diff(m.cluster_offsets).max()) >= 256
+    got, ref, info = _run_all(m, 4, tile_vertices=16)
+    assert info.local_id_bytes == 1
+    _compare(got, ref, "8-bit local ids")
+    got, ref, info = _run_all(m, 4, tile_vertices=256)
+    # tets keep 9-bit local ids in the facet key (<= 512 per tile), so create may halve the requested tile;
+    # 128 rows plus their halo still exceed 255 local ids
+    assert info.tile_vertices in (128, 256) and info.local_id_bytes == 2
+    _compare(got, ref, "16-bit local ids")
+    m2 = meshgen.make_mesh(2, 120, clustering="octree", capacity=3000, seed=22)
+    for tv, lb in ((32, 1), (256, 2)):
+        got, ref, info = _run_all(m2, 3, tile_vertices=tv)
+        assert info.local_id_bytes == lb
+        _compare(got, ref, f"2d local id bytes {lb}")
+
+
 @pytest.mark.parametrize("mask", [1, 2, 4, 3, 5, 6])
 def test_relation_masks(mask):
     gale = _gale()

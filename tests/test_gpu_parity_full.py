@@ -1,0 +1,107 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (batches of 64
+clusters, default tile size, device ring): configs 2-5 (config 1 is the small case of test_gpu_parity.py).
+
+Two kinds of check per config:
+  * sampled outputs — clusters taken from the first, a middle and the last batch are compared element by
+    element, bit-exactly, with the CPU oracle (its restricted evaluation, which tests/test_oracle_pins.py
+    pins to the global definitions);
+  * properties that hold at any size, over one complete pass of every cluster — the closed forms of an
+    n^dim Kuhn/Freudenthal grid (tests/golden/kuhn_closed_forms.txt: 3-D E = 3n^2 m + 3n m^2 + m^3,
+    boundary facets 12 m^2; 2-D E = 2nm + m^2, boundary edges 4m; m = n-1):
+        sum |VT| = (dim+1) T,   sum |VV| = 2 E,   #(-1 in TT) = boundary facets,
+    plus CSR well-formedness of every batch (offsets start at 0, are non-decreasing and end at nnz;
+    indices in range; every TT entry is -1 or a valid simplex id other than its own row).
+Permutation (config 3), coordinate warp (config 4) and clustering change the numbering only, so the
+closed forms apply to all four.
+"""
+import numpy as np
+import pytest
+
+import meshgen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+BATCH = 64                       # bench.py --batch default
+GRID_N = {2: 4096, 3: 128, 4: 192, 5: 256}   # BASELINE.json configs[1..4]
+
+
+def _closed_forms(dim, n):
+    m = n - 1
+    if dim == 3:
+        return dict(T=6 * m ** 3, E=3 * n * n * m + 3 * n * m * m + m ** 3, boundary=12 * m * m)
+    return dict(T=2 * m * m, E=2 * n * m + m * m, boundary=4 * m)
+
+
+def _compare(got, ref, what):
+    assert len(got) == len(ref)
+    for g, r in zip(got, ref):
+        c = r["cluster"]
+        assert g["cluster"] == c
+        for k in ("vt", "vv"):
+            assert np.array_equal(g[k][0], r[k][0]), f"{what} {k} offsets, cluster {c}"
+            assert np.array_equal(g[k][1], r[k][1]), f"{what} {k} indices, cluster {c}"
+        assert g["tt"].shape == r["tt"].shape, f"{what} tt shape, cluster {c}"
+        assert np.array_equal(g["tt"], r["tt"]), f"{what} tt, cluster {c}"
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_in_bench_configuration(cfg):
+    import torch
+    import paper_2507_15230_b200 as gale
+
+    m = meshgen.make_config(cfg)
+    D = m.dim + 1
+    cf = _closed_forms(m.dim, GRID_N[cfg])
+    nT, nV, nC = m.num_simplices, m.num_vertices, m.num_clusters
+    assert nT == cf["T"] and nV == GRID_N[cfg] ** m.dim
+
+    gm = gale.GaleMesh(m.dim, nV, m.simplices, m.cluster_offsets, max_batch_clusters=BATCH, queue_depth=0,
+                       device_ring=4, tile_vertices=0, flags=0)          # exactly bench.py's handle
+    assert gm.info.vt_nnz == D * nT                                      # sizes fixed at create
+    assert gm.info.vv_nnz == 2 * cf["E"]
+
+    batches = [np.arange(b, min(nC, b + BATCH), dtype=np.int32) for b in range(0, nC, BATCH)]
+    sampled_batches = sorted({0, len(batches) // 2, len(batches) - 1})
+    rng = np.random.default_rng(1000 + cfg)
+    kept = []                                                            # host copies of sampled clusters
+    tot = dict(vt=0, vv=0, minus1=0, rows=0, tt_rows=0)
+    first_tet = np.searchsorted(m.simplices[:, 0], m.cluster_offsets)    # I_T per cluster (host, for row ids)
+
+    for bi, ids in enumerate(batches):
+        assert gm.compute(ids) == gale.OK
+        st, v = gm.pop(-1)
+        assert st == gale.OK and v.on_device == 1 and v.n_clusters == len(ids)
+        a = gm.view_arrays(v)                                            # torch views of the device slot
+        for k in ("vt", "vv"):
+            off, idx = a[k + "_offsets"], a[k + "_indices"]
+            assert int(off[0]) == 0 and int(off[-1]) == idx.numel()
+            assert bool((off[1:] >= off[:-1]).all()), f"{k} offsets not monotone, batch {bi}"
+            if idx.numel():
+                assert int(idx.min()) >= 0 and int(idx.max()) < (nT if k == "vt" else nV)
+            tot[k] += idx.numel()
+        tt = a["tt_indices"].view(-1, D)
+        t_begin = int(first_tet[ids[0]])
+        assert tt.shape[0] == int(first_tet[ids[-1] + 1]) - t_begin      # contiguous cluster ids: one tet range
+        own = torch.arange(t_begin, t_begin + tt.shape[0], device=tt.device, dtype=tt.dtype).unsqueeze(1)
+        assert bool(((tt >= -1) & (tt < nT) & (tt != own)).all()), f"tt entry out of range, batch {bi}"
+        tot["minus1"] += int((tt == -1).sum())
+        tot["rows"] += a["vt_offsets"].numel() - 1
+        tot["tt_rows"] += tt.shape[0]
+        if bi in sampled_batches:
+            host = {k: (x.cpu().numpy() if hasattr(x, "cpu") else x) for k, x in a.items()}
+            pick = sorted({0, len(ids) - 1, *rng.integers(0, len(ids), size=2).tolist()})
+            per = gale.split_batch(host, D)
+            kept += [per[i] for i in pick]
+        gm.release(v)
+
+    assert tot["rows"] == nV and tot["tt_rows"] == nT                    # every row exactly once
+    assert tot["vt"] == D * nT, "sum |VT| = (dim+1) T"
+    assert tot["vv"] == 2 * cf["E"], "sum |VV| = 2 E (closed form)"
+    assert tot["minus1"] == cf["boundary"], "#(-1 in TT) = boundary facets (closed form)"
+    info = gm.info
+    gm.destroy()
+
+    sel = [k["cluster"] for k in kept]
+    ref = oracle.cluster_results(m.dim, nV, m.simplices, m.cluster_offsets, sel, restricted=True)
+    _compare(kept, ref, f"config {cfg} full size (tile {info.tile_vertices}, {info.local_id_bytes}-byte local ids)")
