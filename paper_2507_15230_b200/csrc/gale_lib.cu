@@ -440,7 +440,7 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   p->cl_t_lo.resize(p->nC + 1);
   for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
 
-  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 128);  // measured optimum on config 5 (profiles/r1_v5_ncu_summary.md)
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 64);  // measured optima on configs 5 and 2 (profiles/r1_v5_ncu_summary.md)
   std::vector<long long> stats;
   for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
