@@ -83,6 +83,23 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(x: float, dist=None, device="cuda") -> float:
+    """Timing rule of the bench contract: a multi-rank number is the MAX over ranks (the slowest replica).
+    `dist` is torch.distributed when WORLD_SIZE > 1, else None."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, units_per_rank: int, ms_per_step: float) -> float:
+    """`value` of the JSON line: units processed by ALL ranks (independent replicas: the path has no
+    exchange step) divided by the max-over-ranks time of a step."""
+    return world * units_per_rank / (ms_per_step * 1e-3)
+
+
 def make_workload(args):
     t0 = time.time()
     mesh = meshgen.make_config(args.config, n=args.n)
@@ -232,12 +249,9 @@ def main():
     w1 = time.time()
     clocks = sampler.stop(w0, w1)
     ms = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist)
     ms_per_step = ms / args.steps
-    value = world * mesh.num_simplices / (ms_per_step * 1e-3)
+    value = whole_job_value(world, mesh.num_simplices, ms_per_step)
 
     # roofline of the dominant kernel (gale_batch_kernel): algorithmic bytes per launch / avg launch time
     rows = mesh.num_vertices
@@ -302,11 +316,8 @@ def main():
             e2e_pass()
         barrier()
         dt = (time.perf_counter() - t0) / e2e_steps
-        if dist:
-            t = torch.tensor([dt], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * mesh.num_simplices / dt, "unit": "tets/s", "h2d_bytes_per_step": int(h2d),
+        dt = max_over_ranks(dt, dist)
+        e2e = {"value": whole_job_value(world, mesh.num_simplices, dt * 1e3), "unit": "tets/s", "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": dt * 1e3, "steps": e2e_steps,
                "what": "H2D of the simplex array from pinned memory + streamed pass, queue_depth=3, "
                        "D2H of every CSR batch to pinned slots, pop+read+release on the host"}

@@ -442,6 +442,7 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
 
   int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 64);  // measured optima on configs 5 and 2 (profiles/r1_v5_ncu_summary.md)
   std::vector<long long> stats;
+  bool shrunk = false;
   for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
     const bool last = tv == 1;
@@ -460,6 +461,12 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
       p->cfg.vv_max = int(pad_to(vv_max, 8));
       p->smem_bytes = layout_for(D, p->cfg).total;
       fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
+    }
+    // automatic tile size: tiles whose vertices are scattered in the mesh (graded meshes, config 4) need
+    // large per-block capacities and leave few resident blocks; half the tile measured +25 % there
+    if (fits && d.tile_vertices == 0 && !shrunk && tv >= 32 && D == 4 && p->smem_bytes > 20 * 1024) {
+      shrunk = true;
+      continue;
     }
     if (fits) break;
     if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
