@@ -72,7 +72,10 @@ typedef struct {
   int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4);
                                        a popped view stays valid until device_ring-1 later batches
                                        have been submitted                                            */
-  int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = default)           */
+  int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = automatic: 32 for
+                                       tets, 64 for triangles, halved once when a tile would need more
+                                       than 20 KB of shared memory; create may reduce any request that
+                                       exceeds a kernel limit — gale_mesh_info reports the value used) */
   void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
                                        must outlive the handle                                       */
   size_t workspace_bytes;

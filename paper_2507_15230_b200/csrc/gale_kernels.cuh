@@ -4,7 +4,8 @@
 // (a tile plays the role of the paper's <=100-vertex segment; a cluster is the
 // request unit). gale_mesh_create stores, per tile, the simplices incident to it
 // (internal ones = rows I_T of T; external ones = the tile's T_ex list)
-// re-encoded in *tile-local* 16-bit vertex ids that ascend with the global id:
+// re-encoded in *tile-local* vertex ids (8-bit when no tile of the mesh has more than 255 local
+// vertices, template argument LB = 1, else 16-bit) that ascend with the global id:
 //     [lower halo 0..nlo) [tile vertices nlo..nlo+nrows) [upper halo ..nloc)
 // ("halo" = vertices outside the tile that share a simplex with it), external simplices first.
 // Every external simplex has a smaller global id than every internal one (its lowest vertex lies
@@ -13,11 +14,14 @@
 // A block has NT = 2 * TV threads: two threads per tile vertex p, an "A" thread (tid = p) and a
 // "B" thread (tid = TV + p), so that lanes of a warp are consecutive vertices (their bitmap rows
 // and tables fall into distinct shared-memory banks). Phases:
-//   P0  stage the list (8 B per simplex), the external simplices' global ids and the local->global
-//       vertex table into shared memory with 16-byte cp.async; clear the bitmaps and tables;
+//   P0  stage the list (4*LB bytes per simplex), the external simplices' global ids, the
+//       local->global vertex table gid and, parallel to it, hft = (first_tet[g], first_tet[g+1]) of
+//       every local vertex (the interval array I_T, restricted to the tile and its
+//       halo) into shared memory with 16-byte cp.async; clear the bitmaps and tables;
 //   P1  VT incidence bits, one thread per staged simplex: bit (row v, column s) for every tile
 //       vertex v of s other than its lowest vertex (the simplices whose *lowest* vertex is v are
-//       the contiguous run first_tet[v]..first_tet[v+1], and need no bits);
+//       the contiguous run hft[v], and need no bits); for an internal simplex whose
+//       second vertex b lies outside the tile, an L2 prefetch of the rows of T that P5 will read;
 //   P2  row degrees (popc) -> exclusive scan -> VT offsets;
 //   P3  A(p): walks the set bits of row p in ascending order = VT(p) without its run, already
 //             sorted; per simplex: emit the VT entry, OR the simplex's vertices into VV row p
@@ -33,8 +37,9 @@
 //   P5  TT rows, VT and VV indices are translated to global ids and written with coalesced
 //       stores; the facet opposite the lowest vertex a of an internal simplex (a, b, ..) with b
 //       outside the tile belongs to no vertex of the tile: such facets are queued and resolved
-//       one per thread from global memory through the run of simplices starting with b and the
-//       index of simplices whose second vertex is b (DESIGN.md §TT fallback).
+//       one per thread from global memory: first the run of simplices starting with b (its bounds
+//       come from hft: one round trip; measured > 99 % of the cofaces are found there), else the
+//       index of simplices whose second vertex is b.
 // All arithmetic is integer index work; no floating point.
 #pragma once
 #include <cuda_runtime.h>
