@@ -70,10 +70,11 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
         return _lib
     if build_if_missing:
         build_library()
-    if not os.path.exists(LIB):
-        raise RuntimeError(f"{LIB} not built (no fallback path exists); run "
+    path = os.environ.get("GALE_LIBRARY", LIB)   # another build of the same sources, e.g. libgale_checked.so
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} not built (no fallback path exists); run "
                            "`python -c 'import __graft_entry__ as g; g.build()'`")
-    lib = ctypes.CDLL(LIB)
+    lib = ctypes.CDLL(path)
     vp = ctypes.c_void_p
     lib.gale_mesh_workspace_bytes.restype = ctypes.c_int32
     lib.gale_mesh_workspace_bytes.argtypes = [ctypes.POINTER(gale_mesh_desc_t), ctypes.POINTER(ctypes.c_size_t)]

@@ -57,7 +57,7 @@ constexpr int kMaxNnz16 = 65535;       // VT / VV entries of one tile (16-bit pa
 constexpr int kMaxTileVertices = 256;
 
 enum { REL_VT = 1, REL_VV = 2, REL_TT = 4, MODE_COUNT = 8 };
-enum { ERR_TT_TABLE_FULL = 2, ERR_SIZE_MISMATCH = 4 };
+enum { ERR_TT_TABLE_FULL = 2, ERR_SIZE_MISMATCH = 4, ERR_BOUNDS = 8 };
 
 // Per-tile record built by gale_mesh_create (80 bytes, 16-byte aligned).
 struct TileDesc {
@@ -175,6 +175,20 @@ struct OutPtrs {
   int32_t* tt_indices;
   long long* stats;                  // count mode: [nTiles][4] = VT nnz, VV nnz, 0, 0
 };
+
+// Bounds-checked build (-DGALE_CHECK_BOUNDS=1, libgale_checked.so; tests/test_gpu_bounds.py): every tile
+// is checked against the launch's shared-memory capacities and every computed staging index before it
+// is written; a violation raises ERR_BOUNDS through the device error word and skips the write.
+// compute-sanitizer is not available on the build pool, this is its stand-in. Off by default: no code.
+__device__ __forceinline__ void raise_err(int32_t* err, int code);
+#ifndef GALE_CHECK_BOUNDS
+#define GALE_CHECK_BOUNDS 0
+#endif
+#if GALE_CHECK_BOUNDS
+#define GALE_IN_BOUNDS(err, cond) ((cond) ? true : (raise_err((err), ERR_BOUNDS), false))
+#else
+#define GALE_IN_BOUNDS(err, cond) true
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // Guard codes go to a host-mapped word (plain store: no PCIe atomics needed; any code is fatal).
@@ -298,6 +312,7 @@ struct GroupCtx {
   uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
   uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
   int s_ext;
+  int s_all;           // staged simplices of the tile (bounds-checked build)
 };
 
 // Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
@@ -313,10 +328,12 @@ __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int
     cur = g.tbl[h];
     if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
   }
+  if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
   if (cur == kEmpty32) {
     g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
   } else {
     const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
+    if (!GALE_IN_BOUNDS(err, s < g.s_all && s2 < g.s_all && k2 < D)) return;
     if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2;
     if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s;
   }
@@ -411,9 +428,23 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
 #pragma unroll
     for (int i = 0; i < (int)(sizeof(TileDesc) / 16); ++i) dst[i] = __ldg(src + i);
   }
-  const int v_lo = td.v_lo, nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
+  const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
   const int S = s_int + s_ext;
   const int WT = C.WT, WV = C.WV;
+#if GALE_CHECK_BOUNDS
+  {
+    bool ok = nrows >= 0 && nrows <= C.tv && NT >= 2 * C.tv && S >= 0 && S <= C.smax && s_ext <= C.sext &&
+              td.nloc <= C.nloc && nlo >= 0 && nlo + nrows <= td.nloc && ((S + 31) >> 5) <= WT;
+    if (mask & REL_VV) ok = ok && ((td.nloc + 31) >> 5) <= WV;
+    if (!COUNT && (mask & REL_TT)) ok = ok && s_int <= C.sint && C.hs >= 2;
+    if (!COUNT && (mask & (REL_VT | REL_TT))) ok = ok && td.vt_nnz <= C.vt_max;
+    if (!COUNT && (mask & REL_VV)) ok = ok && td.vv_nnz <= C.vv_max;
+    if (!ok) {  // block-uniform: leave before anything is staged
+      if (tid == 0) raise_err(M.err, ERR_BOUNDS);
+      return;
+    }
+  }
+#endif
 
   unsigned char* tets = smem + L.tets;
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
@@ -473,6 +504,11 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   for (int s = tid; s < S; s += NT) {
     int l[4];
     load_local<LB>(tets, s, l);
+#if GALE_CHECK_BOUNDS
+    for (int k = 0; k < D; ++k)
+      if (!GALE_IN_BOUNDS(M.err, l[k] >= 0 && l[k] < td.nloc)) l[k] = nlo;  // keep later indexing inside the row
+    if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
+#endif
     uint32_t* col = bmT + (s >> 5);
     const uint32_t bit = bit_of(s);
 #pragma unroll
@@ -535,7 +571,8 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         bits &= bits - 1;
         int l[4];
         load_local<LB>(tets, s, l);
-        if (entries) st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
+        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= 0 && s < S))
+          st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
         if (do_vv) {
 #pragma unroll
           for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));  // self bit cleared in P4
@@ -548,7 +585,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         g.tbl = tbl + p * (hs + 1);
         g.hs = (uint32_t)hs;
         g.ttrow = ttrow;
-        g.s_ext = s_ext;
+        g.s_ext = s_ext; g.s_all = S;
       }
       int pos = off + nb;
       const int2 run = hft[ploc];
@@ -557,7 +594,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         const int s = s_ext + i;
         int l[4];
         load_local<LB>(tets, s, l);
-        if (entries) st_vt[pos++] = (uint16_t)s;
+        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= s_ext && s < S)) st_vt[pos++] = (uint16_t)s;
         if (do_vv) {
 #pragma unroll
           for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));
@@ -581,7 +618,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       g.tbl = tbl + p * (hs + 1);
       g.hs = (uint32_t)hs;
       g.ttrow = ttrow;
-      g.s_ext = s_ext;
+      g.s_ext = s_ext; g.s_all = S;
       int i = off;
       const int end = off + nb;
       for (;;) {
@@ -613,7 +650,8 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       uint32_t bits = 0u;
       for (int n = 0; n < nbv; ++n) {
         while (bits == 0u) { bits = *row++; lbase += 32; }
-        st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
+        if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vv_max && lbase + __ffs(bits) - 1 < td.nloc))
+          st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
         bits &= bits - 1;
       }
     }
@@ -669,7 +707,8 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         uint32_t pos = 0u;
         if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
         pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
-        if (need_fb) fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
+        if (need_fb && GALE_IN_BOUNDS(M.err, (int)(pos + __popc(fbm & ((1u << lane) - 1u))) < C.sint))
+          fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
       }
     }
   }

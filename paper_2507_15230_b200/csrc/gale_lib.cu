@@ -10,6 +10,7 @@
 #include <atomic>
 #include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <mutex>
@@ -738,8 +739,13 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   O.vv_indices = reinterpret_cast<int32_t*>(s.dev + s.used.vv_idx);
   O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
 
-  const SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
+  SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
   const gale::SmemLayout lay = layout_for(D, cfg);
+#if GALE_CHECK_BOUNDS
+  // negative control of the bounds-checked build: understate one capacity (the layout keeps its real
+  // size) so that the kernel's checks must fire
+  if (std::getenv("GALE_CHECK_SELFTEST") && cfg.vt_max > 8) cfg.vt_max -= 8;
+#endif
   const int smem = lay.total;
   GALE_CUDA(cudaEventRecord(s.ev_start, st));
   for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
