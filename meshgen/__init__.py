@@ -180,6 +180,48 @@ def make_config(i: int, n: int | None = None, keep_fields: bool = False, **overr
     return mesh
 
 
+def from_simplices(dim: int, coords, simplices, *, capacity: int = 512, name: str = "user") -> Mesh:
+    """Arbitrary simplicial mesh (vertex coordinates + simplices in any numbering) -> PR-octree clustering
+    of the vertices -> renumbering so that clusters are contiguous id ranges -> canonical form (each simplex
+    ascending, simplices in lexicographic order; DESIGN.md §2 reading 2). Input plumbing only.
+    meta["vertex_rank"][old vertex] = new id; meta["simplex_perm"][new simplex] = old simplex index."""
+    lib = _load()
+    D = dim + 1
+    coords = np.ascontiguousarray(coords, dtype=np.float32)
+    simplices = np.ascontiguousarray(simplices, dtype=np.int32)
+    nV = int(coords.shape[0])
+    assert coords.shape == (nV, dim) and simplices.ndim == 2 and simplices.shape[1] == D
+    order = np.empty(nV, np.int32)
+    offsets = np.empty(nV + 1, np.int32)
+    nC = int(lib.mg_octree_clusters(dim, nV, _p(coords, ctypes.c_float), capacity,
+                                    _p(order, ctypes.c_int32), _p(offsets, ctypes.c_int32)))
+    offsets = np.ascontiguousarray(offsets[:nC + 1])
+    rank = np.empty(nV, np.int32)
+    rank[order] = np.arange(nV, dtype=np.int32)
+    T = np.sort(rank[simplices], axis=1)
+    perm = np.lexsort(T.T[::-1]).astype(np.int64)          # rows in lexicographic order
+    T = np.ascontiguousarray(T[perm], dtype=np.int32)
+    meta = dict(name=name, clustering="octree", capacity=capacity, vertex_rank=rank, simplex_perm=perm)
+    return Mesh(dim, nV, T, offsets, np.ascontiguousarray(coords[order]), None, meta)
+
+
+def make_delaunay(dim: int, npoints: int, *, seed: int = 1, capacity: int = 512) -> Mesh:
+    """Delaunay triangulation (scipy / Qhull) of seeded uniform random points in the unit cube: an
+    irregular test mesh (vertex degrees vary widely, unlike a Kuhn grid) with the topology of a ball.
+    meta["qhull_neighbors"] is Qhull's own simplex-adjacency array in the ORIGINAL numbering
+    (neighbors[i][k] = simplex opposite vertex k of simplex i, -1 on the hull), kept so that tests can
+    pin TT against an implementation that shares nothing with this repository."""
+    from scipy.spatial import Delaunay
+
+    pts = np.random.default_rng(seed).random((npoints, dim))
+    tri = Delaunay(pts)
+    m = from_simplices(dim, pts.astype(np.float32), tri.simplices, capacity=capacity,
+                       name=f"delaunay{dim}d_{npoints}_seed{seed}")
+    m.meta["qhull_simplices"] = np.asarray(tri.simplices, dtype=np.int64)
+    m.meta["qhull_neighbors"] = np.asarray(tri.neighbors, dtype=np.int64)
+    return m
+
+
 def toy_two_tets() -> Mesh:
     """PAPER.md:60-64 (Fig. 1): two tetrahedra sharing a triangle, one cluster."""
     T = np.array([[0, 1, 2, 3], [1, 2, 3, 4]], np.int32)

@@ -26,6 +26,9 @@ CASES = [
     ("holes3d tv=1", lambda: meshgen.make_mesh(3, 14, clustering="octree", capacity=300, permute=True, drop_frac=0.1, seed=13), 9, 1, 7),
     ("holes3d tv=256 (16-bit ids)", lambda: meshgen.make_mesh(3, 20, clustering="octree", capacity=2000, permute=True, drop_frac=0.05, seed=21), 4, 256, 7),
     ("tri2d tv=256 (16-bit ids)", lambda: meshgen.make_mesh(2, 120, clustering="octree", capacity=3000, seed=22), 3, 256, 7),
+    ("delaunay3d", lambda: meshgen.make_delaunay(3, 4000, seed=41, capacity=500), 6, 0, 7),
+    ("delaunay3d tv=5", lambda: meshgen.make_delaunay(3, 1500, seed=42, capacity=300), 6, 5, 7),
+    ("delaunay2d", lambda: meshgen.make_delaunay(2, 8000, seed=43, capacity=900), 6, 0, 7),
     ("holes2d", lambda: meshgen.make_mesh(2, 150, clustering="octree", capacity=900, warp=True, drop_frac=0.2, seed=6), 16, 0, 7),
 ]
 

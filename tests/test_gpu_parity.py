@@ -50,6 +50,9 @@ SMALL = [
     ("cfg5@48", lambda: meshgen.make_config(5, n=48), 64),
     ("holes3d", lambda: meshgen.make_mesh(3, 24, clustering="octree", capacity=700, permute=True, drop_frac=0.15, seed=5), 16),
     ("holes2d", lambda: meshgen.make_mesh(2, 150, clustering="octree", capacity=900, warp=True, drop_frac=0.2, seed=6), 16),
+    # irregular meshes (Delaunay of random points: |VT| up to ~60 against a mean of 26)
+    ("delaunay3d", lambda: meshgen.make_delaunay(3, 6000, seed=31, capacity=600), 8),
+    ("delaunay2d", lambda: meshgen.make_delaunay(2, 20000, seed=32, capacity=1500), 8),
 ]
 
 
@@ -58,6 +61,13 @@ def test_parity_small(name, make, batch):
     m = make()
     got, ref, _ = _run_all(m, batch)
     _compare(got, ref, name)
+
+
+@pytest.mark.parametrize("tv", [3, 16, 64])
+def test_parity_irregular_mesh_tile_sizes(tv):
+    m = meshgen.make_delaunay(3, 2500, seed=33, capacity=400)
+    got, ref, _ = _run_all(m, 5, tile_vertices=tv, flags=3)          # VALIDATE | VALIDATE_MANIFOLD
+    _compare(got, ref, f"delaunay3d tv={tv}")
 
 
 @pytest.mark.parametrize("tv", [1, 7, 32, 100, 256])
