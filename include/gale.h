@@ -105,7 +105,8 @@ typedef struct {
   const int32_t *vv_indices;     /* [vv_nnz]                                                         */
   int64_t tt_rows;
   const int32_t *tt_indices;     /* [tt_rows*(dim+1)] or NULL                                        */
-  float kernel_ms;               /* CUDA-event time of this batch's kernel                           */
+  float kernel_ms;               /* CUDA-event time of this batch's kernel, start to end; it includes
+                                    the time the GPU was shared with an overlapping neighbour batch  */
   int32_t slot;                  /* internal: pass the view back unchanged to gale_queue_release     */
 } gale_batch_view_t;
 
@@ -137,8 +138,14 @@ int32_t gale_mesh_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_m
 int32_t gale_mesh_info(const gale_mesh_t *mesh, gale_mesh_info_t *out);
 
 /* Producer side: enqueue the relation kernels for the clusters
- * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) on cuda_stream and,
- * when queue_depth > 0, the D2H copy into a pinned slot on the library's side stream.
+ * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) and, when
+ * queue_depth > 0, the D2H copy into a pinned slot on the library's side stream.
+ * Stream semantics: the kernels run on library-owned streams (consecutive batches alternate between
+ * two of them so that the draining tail of one launch overlaps the next), ORDERED AFTER everything
+ * already enqueued on cuda_stream at the time of the call — e.g. an upload of the simplices. Work the
+ * caller enqueues on cuda_stream afterwards is NOT ordered after the batch: completion is observed
+ * through gale_queue_pop only, and the simplices / workspace must not be modified or freed before the
+ * batches using them have been popped (gale_destroy drains them).
  * Asynchronous w.r.t. the host. Returns GALE_ERR_WOULD_BLOCK when all slots are un-released. */
 int32_t gale_cluster_batch_compute(gale_mesh_t *mesh, uint32_t relation_mask, const int32_t *h_cluster_ids,
                                    int32_t n_clusters, void *cuda_stream);
