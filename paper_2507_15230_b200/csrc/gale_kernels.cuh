@@ -181,6 +181,18 @@ struct OutPtrs {
 // is written; a violation raises ERR_BOUNDS through the device error word and skips the write.
 // compute-sanitizer is not available on the build pool, this is its stand-in. Off by default: no code.
 __device__ __forceinline__ void raise_err(int32_t* err, int code);
+// Output stores: the CSR arrays are written once and never read by the kernels, so the stores are marked
+// evict-first (st.global.cs) and leave L2 to the data the fall-back look-ups re-read. Measured +0.7 %
+// (24.18 / 24.19 vs 24.36 / 24.36 G tets/s, alternating runs); -DGALE_STREAM_OUT=0 restores plain stores.
+#ifndef GALE_STREAM_OUT
+#define GALE_STREAM_OUT 1
+#endif
+#if GALE_STREAM_OUT
+#define GALE_ST(ptr, val) __stcs((ptr), (val))
+#else
+#define GALE_ST(ptr, val) (*(ptr) = (val))
+#endif
+
 #ifndef GALE_CHECK_BOUNDS
 #define GALE_CHECK_BOUNDS 0
 #endif
@@ -690,7 +702,7 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         for (int k = 0; k < D; ++k)
           r[k] = e[k] == 0xFFFFu ? -1 : ((int)e[k] < s_ext ? texid[e[k]] : t_lo + ((int)e[k] - s_ext));
         if constexpr (D == 4) {
-          reinterpret_cast<int4*>(O.tt_indices)[tt0 + i] = make_int4(r[0], r[1], r[2], r[3]);
+          GALE_ST(reinterpret_cast<int4*>(O.tt_indices) + tt0 + i, make_int4(r[0], r[1], r[2], r[3]));
         } else {
           int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
           o[0] = r[0]; o[1] = r[1]; o[2] = r[2];
@@ -715,10 +727,10 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   if (do_vt)
     for (int i = tid; i < n_vt; i += NT) {
       const int s = (int)(st_vt[i] & 0x7FFFu);
-      O.vt_indices[vt0 + i] = s < s_ext ? texid[s] : t_lo + (s - s_ext);
+      GALE_ST(O.vt_indices + vt0 + i, s < s_ext ? texid[s] : t_lo + (s - s_ext));
     }
   if (do_vv)
-    for (int i = tid; i < n_vv; i += NT) O.vv_indices[vv0 + i] = gid[st_vv[i]];
+    for (int i = tid; i < n_vv; i += NT) GALE_ST(O.vv_indices + vv0 + i, gid[st_vv[i]]);
 
   if (do_tt) {
     __syncthreads();  // queue complete, TT rows stored
