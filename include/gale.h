@@ -34,6 +34,7 @@ extern "C" {
 #endif
 
 typedef struct gale_mesh gale_mesh_t; /* opaque; owned by the library, freed by gale_destroy */
+typedef struct gale_plan gale_plan_t; /* opaque result of the initialization analysis, see gale_plan_create */
 
 enum { GALE_REL_VT = 1, GALE_REL_VV = 2, GALE_REL_TT = 4, GALE_REL_ALL = 7 };
 
@@ -53,7 +54,10 @@ enum {
 
 enum {
   GALE_VALIDATE = 1u,          /* check C1-C3 and the cluster offsets at create (one pass)            */
-  GALE_VALIDATE_MANIFOLD = 2u  /* also check C4 (facet pass, slower)                                  */
+  GALE_VALIDATE_MANIFOLD = 2u, /* also check C4 (facet pass, slower)                                  */
+  GALE_STREAM_ORDERED = 4u     /* run every batch kernel on the cuda_stream passed to compute itself
+                                  (plain stream order: work the caller enqueues afterwards runs after
+                                  the batch) instead of on the library's two overlapping launch streams */
 };
 
 typedef struct {
@@ -69,23 +73,20 @@ typedef struct {
   int32_t queue_depth;              /* > 0: that many pinned HOST result slots, results are copied
                                        D2H on a library-owned side stream;
                                        0: results stay in a ring of device slots (benchmark mode)     */
-  int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4);
-                                       a popped view stays valid until device_ring-1 later batches
-                                       have been submitted                                            */
+  int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4)   */
   int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = automatic: 32 for
-                                       tets, 64 for triangles, halved once when a tile would need more
-                                       than 20 KB of shared memory; create may reduce any request that
+                                       tets, 64 for triangles; create may reduce any request that
                                        exceeds a kernel limit — gale_mesh_info reports the value used) */
   void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
                                        must outlive the handle                                       */
   size_t workspace_bytes;
-  uint32_t flags;                   /* GALE_VALIDATE | GALE_VALIDATE_MANIFOLD                         */
+  uint32_t flags;                   /* GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED   */
 } gale_mesh_desc_t;
 
 /* One finished batch. cluster_ids and *_row_begin are HOST arrays owned by the library; offsets and
  * indices live in the slot: pinned HOST memory when queue_depth > 0, DEVICE memory when 0
- * (on_device tells which). Everything stays valid until gale_queue_release (queue_depth > 0) or
- * until device_ring-1 later batches are submitted (queue_depth == 0).
+ * (on_device tells which). Everything stays valid until gale_queue_release, in both modes: a slot is
+ * reused only after its view has been released (the paper's pre-allocated relation buffers).
  * Rows of the i-th requested cluster are [row_begin[i], row_begin[i+1]); offsets are batch-relative
  * (offsets[0] = 0, non-decreasing, offsets[rows] = nnz). TT rows have constant length dim+1. */
 typedef struct {
@@ -108,6 +109,13 @@ typedef struct {
   float kernel_ms;               /* CUDA-event time of this batch's kernel, start to end; it includes
                                     the time the GPU was shared with an overlapping neighbour batch  */
   int32_t slot;                  /* internal: pass the view back unchanged to gale_queue_release     */
+  /* stages of a request as the paper times them: data preparation, kernel (above),
+   * transfer back, and the wait of the consumer; "data integration" (:210) does not exist here        */
+  float prep_ms;                 /* host time inside gale_cluster_batch_compute (batch set-up + launch) */
+  float d2h_ms;                  /* queue_depth > 0: end of kernel -> copy landed in the pinned slot
+                                    (includes waiting behind earlier copies on the side stream); else 0 */
+  float queue_ms;                /* host time from the end of compute to the return of this pop         */
+  int32_t reserved;
 } gale_batch_view_t;
 
 /* Init statistics ("Initialization"), for reporting. */
@@ -123,42 +131,70 @@ typedef struct {
   int32_t local_id_bytes;        /* width of the tile-local vertex ids in the staged lists: 1 when every
                                     tile has at most 255 local vertices (tile + halo), else 2           */
   int32_t block_threads;         /* threads per block of the batch kernel                            */
+  size_t index_bytes;            /* bytes of the device-resident index built by the initialization
+                                    (I_T, T_ex, tile tables; the rest of workspace_used is result slots) */
 } gale_mesh_info_t;
 
-/* Upper bound of the device workspace gale_mesh_create needs for this descriptor
- * (d_workspace / workspace_bytes are ignored). Cheap: reads the counts only. */
-int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t *desc, size_t *out_bytes);
+/* Initialization analysis ("Initialization": I_T, the external lists T_ex, interval
+ * arrays): reads the simplices from the DEVICE array desc->d_simplices — they must be valid in stream
+ * order on cuda_stream — validates them and builds the index on the host side of the library. This is
+ * the expensive part of creating a handle (seconds on a 100 M-tet mesh); d_workspace / workspace_bytes of
+ * the descriptor are ignored. *out is owned by the caller until it is passed to
+ * gale_mesh_create_planned or gale_plan_destroy. */
+int32_t gale_plan_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_plan_t **out);
 
-/* Initialization: validates, builds I_T (first simplex of every vertex), the
- * per-tile external lists T_ex, the index used to resolve cross-cluster facets, the per-tile output
- * sizes, and uploads them into the workspace. Work is enqueued on cuda_stream (a cudaStream_t,
- * 0 = default stream) and finished (synchronised) on return. *out is set on GALE_OK only. */
+/* Exact device workspace (index + result slots) a handle built from this plan needs. Cheap. */
+int32_t gale_plan_workspace_bytes(const gale_plan_t *plan, size_t *out_bytes);
+
+int32_t gale_plan_destroy(gale_plan_t *plan);
+
+/* Builds the handle from a plan: uploads the index into d_workspace (DEVICE, caller-owned, 256-byte
+ * aligned, >= gale_plan_workspace_bytes, must outlive the handle) on cuda_stream, synchronised on return.
+ * The plan is consumed (emptied) on every outcome; destroy it afterwards. */
+int32_t gale_mesh_create_planned(gale_plan_t *plan, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                                 gale_mesh_t **out);
+
+/* Convenience: gale_plan_create + gale_plan_workspace_bytes + gale_plan_destroy. NOT cheap: it runs the
+ * whole analysis (see gale_plan_create; d_simplices must be valid on cuda_stream) and throws it away.
+ * Callers that go on to create a handle should use the plan calls and pay for the analysis once. */
+int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t *desc, void *cuda_stream, size_t *out_bytes);
+
+/* Convenience: gale_plan_create + gale_mesh_create_planned with desc->d_workspace / workspace_bytes
+ * (PAPER.md:178-180). Work is enqueued on cuda_stream (a cudaStream_t, 0 = default stream) and
+ * finished (synchronised) on return. *out is set on GALE_OK only. */
 int32_t gale_mesh_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_mesh_t **out);
 
+/* Statistics of the initialization (Table 4 :393-397 reports its time), for reporting. */
 int32_t gale_mesh_info(const gale_mesh_t *mesh, gale_mesh_info_t *out);
 
 /* Producer side: enqueue the relation kernels for the clusters
  * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) and, when
  * queue_depth > 0, the D2H copy into a pinned slot on the library's side stream.
- * Stream semantics: the kernels run on library-owned streams (consecutive batches alternate between
- * two of them so that the draining tail of one launch overlaps the next), ORDERED AFTER everything
- * already enqueued on cuda_stream at the time of the call — e.g. an upload of the simplices. Work the
- * caller enqueues on cuda_stream afterwards is NOT ordered after the batch: completion is observed
- * through gale_queue_pop only, and the simplices / workspace must not be modified or freed before the
- * batches using them have been popped (gale_destroy drains them).
+ * Stream semantics, default: the kernels run on library-owned streams (consecutive batches alternate
+ * between two of them so that the draining tail of one launch overlaps the next), ORDERED AFTER
+ * everything already enqueued on cuda_stream at the time of the call — e.g. an upload of the simplices.
+ * Work the caller enqueues on cuda_stream afterwards is NOT ordered after the batch: completion is
+ * observed through gale_queue_pop only, and the simplices / workspace must not be modified or freed
+ * before the batches using them have been popped (gale_destroy drains them).
+ * With GALE_STREAM_ORDERED in desc->flags the kernels run on cuda_stream itself: plain stream order,
+ * later work on that stream sees the device slot complete (no overlap between consecutive batches).
  * Asynchronous w.r.t. the host. Returns GALE_ERR_WOULD_BLOCK when all slots are un-released. */
 int32_t gale_cluster_batch_compute(gale_mesh_t *mesh, uint32_t relation_mask, const int32_t *h_cluster_ids,
                                    int32_t n_clusters, void *cuda_stream);
 
-/* Consumer side: wait (up to timeout_ms; < 0 = forever) for the oldest submitted batch and
- * describe it in *out. Batches pop in submission order. GALE_ERR_EMPTY if nothing is in flight,
+/* Consumer side (PAPER.md:158 "signals the consumer", :194: the consumer blocks until its relation is
+ * there): wait (up to timeout_ms; < 0 = forever) for the oldest submitted batch and describe it in *out. Batches pop in submission order. GALE_ERR_EMPTY if nothing is in flight,
  * GALE_ERR_WOULD_BLOCK on timeout, GALE_ERR_WORKSPACE if a device-side capacity guard fired. */
 int32_t gale_queue_pop(gale_mesh_t *mesh, gale_batch_view_t *out, int32_t timeout_ms);
 
-/* Give a popped slot back to the queue (no-op when queue_depth == 0). */
+/* Give a popped slot back to the queue (the relation buffers are pre-allocated and reused,
+ * never freed per request). Mandatory in BOTH modes: a slot whose view was popped but not released keeps
+ * gale_cluster_batch_compute at GALE_ERR_WOULD_BLOCK once the ring wraps around to it.
+ * GALE_ERR_INVALID_ARG for a view that is not the popped, un-released view of its slot. */
 int32_t gale_queue_release(gale_mesh_t *mesh, const gale_batch_view_t *view);
 
-/* Drains in-flight work, frees pinned memory, streams and events. The workspace and the simplex
+/* End of the producers' life (the producers serve requests until the consumers are done):
+ * drains in-flight work, frees pinned memory, streams and events. The workspace and the simplex
  * array stay the caller's. */
 int32_t gale_destroy(gale_mesh_t *mesh);
 

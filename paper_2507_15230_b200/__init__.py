@@ -15,7 +15,7 @@ import numpy as np
 from .build import LIB, build_library
 
 REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
-VALIDATE, VALIDATE_MANIFOLD = 1, 2
+VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED = 1, 2, 4
 OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
 ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
 
@@ -39,7 +39,9 @@ class gale_batch_view_t(ctypes.Structure):
                 ("vv_rows", ctypes.c_int64), ("vv_nnz", ctypes.c_int64),
                 ("vv_offsets", ctypes.c_void_p), ("vv_indices", ctypes.c_void_p),
                 ("tt_rows", ctypes.c_int64), ("tt_indices", ctypes.c_void_p),
-                ("kernel_ms", ctypes.c_float), ("slot", ctypes.c_int32)]
+                ("kernel_ms", ctypes.c_float), ("slot", ctypes.c_int32),
+                ("prep_ms", ctypes.c_float), ("d2h_ms", ctypes.c_float), ("queue_ms", ctypes.c_float),
+                ("reserved", ctypes.c_int32)]
 
 
 class gale_mesh_info_t(ctypes.Structure):
@@ -47,10 +49,12 @@ class gale_mesh_info_t(ctypes.Structure):
                 ("num_external_refs", ctypes.c_int64), ("vt_nnz", ctypes.c_int64), ("vv_nnz", ctypes.c_int64),
                 ("smem_bytes", ctypes.c_int32), ("max_staged", ctypes.c_int32),
                 ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double),
-                ("local_id_bytes", ctypes.c_int32), ("block_threads", ctypes.c_int32)]
+                ("local_id_bytes", ctypes.c_int32), ("block_threads", ctypes.c_int32),
+                ("index_bytes", ctypes.c_size_t)]
 
 
-EXPORTS = ["gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
+EXPORTS = ["gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+           "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
 
@@ -76,8 +80,16 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
                            "`python -c 'import __graft_entry__ as g; g.build()'`")
     lib = ctypes.CDLL(path)
     vp = ctypes.c_void_p
+    lib.gale_plan_create.restype = ctypes.c_int32
+    lib.gale_plan_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
+    lib.gale_plan_workspace_bytes.restype = ctypes.c_int32
+    lib.gale_plan_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.gale_plan_destroy.restype = ctypes.c_int32
+    lib.gale_plan_destroy.argtypes = [vp]
+    lib.gale_mesh_create_planned.restype = ctypes.c_int32
+    lib.gale_mesh_create_planned.argtypes = [vp, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
     lib.gale_mesh_workspace_bytes.restype = ctypes.c_int32
-    lib.gale_mesh_workspace_bytes.argtypes = [ctypes.POINTER(gale_mesh_desc_t), ctypes.POINTER(ctypes.c_size_t)]
+    lib.gale_mesh_workspace_bytes.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(ctypes.c_size_t)]
     lib.gale_mesh_create.restype = ctypes.c_int32
     lib.gale_mesh_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
     lib.gale_mesh_info.restype = ctypes.c_int32
@@ -108,9 +120,35 @@ def _check(status: int, where: str):
 
 
 # ---- the C-ABI calls, same names, marshalling only ----------------------------------------------------
-def gale_mesh_workspace_bytes(desc: gale_mesh_desc_t) -> int:
+def gale_plan_create(desc: gale_mesh_desc_t, cuda_stream: int = 0) -> ctypes.c_void_p:
+    h = ctypes.c_void_p()
+    _check(load_library().gale_plan_create(ctypes.byref(desc), ctypes.c_void_p(cuda_stream), ctypes.byref(h)),
+           "gale_plan_create")
+    return h
+
+
+def gale_plan_workspace_bytes(plan) -> int:
     out = ctypes.c_size_t(0)
-    _check(load_library().gale_mesh_workspace_bytes(ctypes.byref(desc), ctypes.byref(out)), "gale_mesh_workspace_bytes")
+    _check(load_library().gale_plan_workspace_bytes(plan, ctypes.byref(out)), "gale_plan_workspace_bytes")
+    return int(out.value)
+
+
+def gale_plan_destroy(plan) -> None:
+    _check(load_library().gale_plan_destroy(plan), "gale_plan_destroy")
+
+
+def gale_mesh_create_planned(plan, d_workspace: int, workspace_bytes: int, cuda_stream: int = 0) -> ctypes.c_void_p:
+    h = ctypes.c_void_p()
+    _check(load_library().gale_mesh_create_planned(plan, ctypes.c_void_p(d_workspace), workspace_bytes,
+                                                   ctypes.c_void_p(cuda_stream), ctypes.byref(h)),
+           "gale_mesh_create_planned")
+    return h
+
+
+def gale_mesh_workspace_bytes(desc: gale_mesh_desc_t, cuda_stream: int = 0) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().gale_mesh_workspace_bytes(ctypes.byref(desc), ctypes.c_void_p(cuda_stream), ctypes.byref(out)),
+           "gale_mesh_workspace_bytes")
     return int(out.value)
 
 
@@ -183,10 +221,15 @@ class GaleMesh:
         d.max_batch_clusters, d.queue_depth, d.device_ring = max_batch_clusters, queue_depth, device_ring
         d.tile_vertices, d.flags = tile_vertices, flags
         self.desc = d
-        nbytes = gale_mesh_workspace_bytes(d)
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-        d.d_workspace, d.workspace_bytes = self.workspace.data_ptr(), nbytes
-        self.handle = gale_mesh_create(d, torch.cuda.current_stream(self.device).cuda_stream)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        plan = gale_plan_create(d, stream)                 # the initialization analysis, once
+        try:
+            nbytes = gale_plan_workspace_bytes(plan)
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            d.d_workspace, d.workspace_bytes = self.workspace.data_ptr(), nbytes
+            self.handle = gale_mesh_create_planned(plan, self.workspace.data_ptr(), nbytes, stream)
+        finally:
+            gale_plan_destroy(plan)
         self.info = gale_mesh_info(self.handle)
 
     def compute(self, cluster_ids, relation_mask: int = REL_ALL, stream=None) -> int:
@@ -212,6 +255,7 @@ class GaleMesh:
         """Expose a popped view as arrays (no copies of the slot data)."""
         n = view.n_clusters
         out = dict(sequence=view.sequence, n_clusters=n, relation_mask=view.relation_mask, kernel_ms=view.kernel_ms,
+                   prep_ms=view.prep_ms, d2h_ms=view.d2h_ms, queue_ms=view.queue_ms,
                    cluster_ids=np.ctypeslib.as_array(view.cluster_ids, shape=(n,)).copy() if n else np.empty(0, np.int32),
                    vt_row_begin=np.ctypeslib.as_array(view.vt_row_begin, shape=(n + 1,)).copy(),
                    tt_row_begin=np.ctypeslib.as_array(view.tt_row_begin, shape=(n + 1,)).copy())

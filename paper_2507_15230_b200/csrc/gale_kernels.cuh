@@ -11,35 +11,34 @@
 // Every external simplex has a smaller global id than every internal one (its lowest vertex lies
 // below the tile), so the staged order s = 0..S-1 ascends with the global simplex id.
 //
-// A block has NT = 2 * TV threads: two threads per tile vertex p, an "A" thread (tid = p) and a
-// "B" thread (tid = TV + p), so that lanes of a warp are consecutive vertices (their bitmap rows
-// and tables fall into distinct shared-memory banks). Phases:
-//   P0  stage the list (4*LB bytes per simplex), the external simplices' global ids, the
-//       local->global vertex table gid and, parallel to it, hft = (first_tet[g], first_tet[g+1]) of
-//       every local vertex (the interval array I_T, restricted to the tile and its
-//       halo) into shared memory with 16-byte cp.async; clear the bitmaps and tables;
-//   P1  VT incidence bits, one thread per staged simplex: bit (row v, column s) for every tile
-//       vertex v of s other than its lowest vertex (the simplices whose *lowest* vertex is v are
-//       the contiguous run hft[v], and need no bits); for an internal simplex whose
-//       second vertex b lies outside the tile, an L2 prefetch of the rows of T that P5 will read;
-//   P2  row degrees (popc) -> exclusive scan -> VT offsets;
-//   P3  A(p): walks the set bits of row p in ascending order = VT(p) without its run, already
-//             sorted; per simplex: emit the VT entry, OR the simplex's vertices into VV row p
-//             (the thread owns the row: "no duplicates", without contention), and
-//             flag the entry when p is the simplex's second vertex;
-//       B(p): walks the run of p: VT entries, VV bits, and the TT facet records 1..D-1 of every
-//             simplex of the run into p's private open-addressing table;
-//   P4  A(p): the flagged entries are the simplices (x, p, ..): their facet 0 has lowest vertex p
-//             and joins p's table. A facet whose lowest vertex is p has all its cofaces among
-//             run(p) and those simplices, so the second arrival of a key meets the first and both
-//             TT entries are written (no atomics, no global traffic);
-//       B(p): VV row p -> degree -> scan -> expansion (sorted because local ids ascend);
-//   P5  TT rows, VT and VV indices are translated to global ids and written with coalesced
-//       stores; the facet opposite the lowest vertex a of an internal simplex (a, b, ..) with b
-//       outside the tile belongs to no vertex of the tile: such facets are queued and resolved
-//       one per thread from global memory: first the run of simplices starting with b (its bounds
-//       come from hft: one round trip; measured > 99 % of the cofaces are found there), else the
-//       index of simplices whose second vertex is b.
+// Kernel v7. Every per-simplex step is one thread per *staged simplex* (uniform work per lane, no
+// per-vertex serial walks); only the two short per-row steps (prefix counts, VV expansion) are one
+// thread per tile vertex. Phases:
+//   P0  one thread arms an mbarrier and issues TMA bulk copies (cp.async.bulk) of the staged list, the
+//       external simplices' global ids (T_ex) and the local->global vertex table; the others clear the
+//       bitmaps / tables and read the tile's slice of the interval array I_T (first_tet);
+//   P1  per staged simplex: VT incidence bit (row v, column s) for every tile vertex v of s other than
+//       its lowest vertex (the simplices whose *lowest* vertex is v are the contiguous run
+//       first_tet[v]..first_tet[v+1] and need no bits), and the VV bits (row v, column u) for every
+//       other vertex u of s — shared-memory atomicOr is the paper's de-duplicating atomicPush
+//       (Alg. 2; "no duplicates", :228) in one instruction;
+//   P2  per tile vertex: prefix popcounts of its VT bitmap row, degrees, block scan -> VT / VV
+//       offsets, facet-table offsets;
+//   P3  per tile vertex: VV row -> ascending global ids into the VV staging area (local ids ascend
+//       with global ids); then, per staged simplex (warps take 32-simplex chunks dynamically): the
+//       rank of s in row v = prefix count + popc(bits below s) places its global id in the VT staging
+//       area — rows come out sorted with no sort and no walk; TT facet records go into per-vertex
+//       open-addressing tables with one atomicCAS: a facet whose lowest vertex is p has both cofaces
+//       among run(p) and the simplices whose second vertex is p, so the second arrival of a key reads
+//       the first (the table word carries key, staged index and facet number) and writes both TT
+//       entries;
+//   P4  VT / VV staging areas leave with TMA bulk stores (cp.async.bulk shared -> global); TT rows are
+//       translated to global ids and written with 16-byte stores. The facet opposite the lowest
+//       vertex a of an internal simplex (a, b, ..) with b outside the tile belongs to no vertex of this
+//       tile: if b lies in the same cluster, the tile that owns b has this simplex in its T_ex list,
+//       matches the facet there and writes that one TT entry (this tile then leaves it alone);
+//       otherwise (cross-cluster facet) it is resolved from global memory (a5): first the run of
+//       simplices starting with b, else the index of simplices whose second vertex is b.
 // All arithmetic is integer index work; no floating point.
 #pragma once
 #include <cuda_runtime.h>
@@ -68,7 +67,7 @@ struct TileDesc {
   int32_t row_rel, tt_rel;    // first row / first TT row of the tile inside its cluster
   int32_t vt_rel, vv_rel;     // first VT / VV entry of the tile inside its cluster
   int32_t vt_nnz, vv_nnz;     // entries of the tile (fixed at create; the kernel re-derives them)
-  int32_t pad0;
+  int32_t c_rows;             // vertices of the tile's cluster (its range is [v_lo - row_rel, .. + c_rows))
   long long stg_off;          // first staged simplex of the tile in DeviceMesh::loc (multiple of 4)
   long long tex_off;          // first entry in DeviceMesh::tex (multiple of 4)
   long long gid_off;          // first entry in DeviceMesh::gid (multiple of 4)
@@ -86,8 +85,6 @@ struct DeviceMesh {
                                       //   when no tile of the mesh has more than 255 local vertices (SmemCfg::lb)
   const int32_t* tex;                 // per-tile ascending global ids of external simplices (T_ex)
   const int32_t* gid;                 // per-tile global vertex id of every local id (ascending)
-  const int2* hft;                    // per-tile, parallel to gid: (first_tet[g], first_tet[g+1]) — the
-                                      //   interval array I_T restricted to the tile's vertices + halo
   const int32_t* cluster_tile_begin;  // [nC+1]
   int32_t* err;                       // sticky device error flags (host-mapped)
 };
@@ -95,25 +92,27 @@ struct DeviceMesh {
 // Shared-memory capacities (maxima over all tiles of the mesh, fixed at create). A field is 0 when
 // the launch's relation mask does not need the region.
 struct SmemCfg {
-  int tv;        // rows (vertices) per tile, <= NT/2
+  int tv;        // rows (vertices) per tile, <= NT
   int smax;      // staged simplices (multiple of 4)
   int lb;        // bytes per local vertex id in the staged list: 1 or 2
   int sext;      // external simplices (multiple of 4)
   int nloc;      // local vertex ids (multiple of 4)
-  int sint;      // internal simplices (even): TT rows + fallback queue, 0 without TT
-  int hs;        // table slots per tile vertex (even, so that the row stride hs+1 is odd), 0 without TT
+  int sint;      // internal simplices (even): fallback queue, 0 without TT
+  int tbl;       // facet-table slots of a tile = VT entries + (D-2) * internal simplices, 0 without TT
   int WT;        // VT bitmap words per row (odd)
   int WV;        // VV bitmap words per row (odd), 0 without VV
-  int vt_max;    // VT entries staged for write-out (16-bit)
-  int vv_max;    // VV entries staged for write-out (16-bit), 0 without VV or in count mode
+  int vt_max;    // VT entries staged for write-out, 0 without VT or in count mode
+  int vv_max;    // VV entries staged for write-out, 0 without VV or in count mode
 };
 
 // Byte offsets of the shared-memory regions, computed on the host (make_layout) and passed as a
 // kernel parameter.
 struct SmemLayout {
-  int tets, texid, gid, hft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
-  int tbl, ttrow, tt_end;
-  int st_vt, st_vv;
+  int mbar, tets, texid, gid, ft, offT, offV, runpos, tbo, scan, misc;
+  int bmT, bmV, zero_end;   // cleared to 0
+  int pfx;
+  int tbl, ttrow, ones_end; // cleared to all-ones (empty table word, "no neighbour")
+  int st_vt, st_vv, fbq;
   int total;
 };
 
@@ -123,30 +122,27 @@ template <int D>
 __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   SmemLayout L;
   int o = 0;
+  L.mbar = o;   o = align16(o + 8);
   L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
-  L.hft = o;    o = align16(o + c.nloc * 8);
-  L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
-  L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
-  L.cnt = o;    o = align16(o + c.tv * 4);
-  L.scan = o;   o = align16(o + 48 * 4);
-  // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
-  // fallback queue (written in P5)
-  L.bmT = o;
-  {
-    const int bm = align16(c.tv * c.WT * 4);
-    L.st_vv = o;
-    L.fbq = o + align16(c.vv_max * 2);
-    const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
-    o += bm > reuse ? bm : reuse;
-  }
+  L.ft = o;     o = align16(o + (c.tv + 1) * 4);
+  L.offT = o;   o = align16(o + (c.tv + 1) * 4);
+  L.offV = o;   o = align16(o + (c.tv + 1) * 4);
+  L.runpos = o; o = align16(o + c.tv * 4);
+  L.tbo = o;    o = align16(o + (c.tv + 1) * 4);
+  L.scan = o;   o = align16(o + 40 * 4);
+  L.misc = o;   o = align16(o + 16);
+  L.bmT = o;    o = align16(o + c.tv * c.WT * 4);
   L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
-  L.bm_end = o;
-  L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
-  L.ttrow = o;  o = align16(o + c.sint * D * 2);
-  L.tt_end = o;
-  L.st_vt = o;  o = align16(o + c.vt_max * 2);
+  L.zero_end = o;
+  L.pfx = o;    o = align16(o + c.tv * c.WT * 2);
+  L.tbl = o;    o = align16(o + c.tbl * 4);
+  L.ttrow = o;  o = align16(o + (c.tbl ? c.smax * D * 2 : 0));
+  L.ones_end = o;
+  L.st_vt = o;  o = align16(o + (c.vt_max ? (c.vt_max + 4) * 4 : 0));
+  L.st_vv = o;  o = align16(o + (c.vv_max ? (c.vv_max + 4) * 4 : 0));
+  L.fbq = o;    o = align16(o + c.sint * 2);
   L.total = o;
   return L;
 }
@@ -181,9 +177,8 @@ struct OutPtrs {
 // is written; a violation raises ERR_BOUNDS through the device error word and skips the write.
 // compute-sanitizer is not available on the build pool, this is its stand-in. Off by default: no code.
 __device__ __forceinline__ void raise_err(int32_t* err, int code);
-// Output stores: the CSR arrays are written once and never read by the kernels, so the stores are marked
-// evict-first (st.global.cs) and leave L2 to the data the fall-back look-ups re-read. Measured +0.7 %
-// (24.18 / 24.19 vs 24.36 / 24.36 G tets/s, alternating runs); -DGALE_STREAM_OUT=0 restores plain stores.
+// Output stores: the CSR arrays are written once and never read by the kernels, so plain stores are
+// marked evict-first (st.global.cs) and leave L2 to the data the fall-back look-ups re-read.
 #ifndef GALE_STREAM_OUT
 #define GALE_STREAM_OUT 1
 #endif
@@ -206,16 +201,37 @@ __device__ __forceinline__ void raise_err(int32_t* err, int code);
 // Guard codes go to a host-mapped word (plain store: no PCIe atomics needed; any code is fatal).
 __device__ __forceinline__ void raise_err(int32_t* err, int code) { *reinterpret_cast<volatile int32_t*>(err) = code; }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+// ---- TMA bulk copies (cp.async.bulk; SASS: UBLKCP) and their mbarrier -----------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
-
-// Barrier among the `count` threads that name the same id (ids 1..15; 0 is __syncthreads).
-__device__ __forceinline__ void named_barrier(int id, int count) {
-  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory");
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(void* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// global -> shared, completion counted in bytes on the mbarrier. 16-byte aligned, size multiple of 16.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+// shared -> global (bulk async group of the issuing thread)
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 // Local vertex ids of staged simplex s (LB bytes each).
 template <int LB>
@@ -229,14 +245,11 @@ __device__ __forceinline__ void load_local(const unsigned char* tets, int s, int
   }
 }
 
-// 1 << (l mod 32)
-__device__ __forceinline__ uint32_t bit_of(int l) { return 1u << (l & 31); }
-
 // a5, one request per thread: coface != self of the facet (b, c[, d]) (ascending global ids) whose
-// vertices all lie outside the tile. [f0, f1) = run of simplices starting with b (from the tile's hft). Both cofaces of a facet with lowest vertex b have b as
-// lowest or second-lowest vertex: candidates are the run of simplices starting with b and the
-// simplices whose second vertex is b (those are (x, b, c, d) exactly). Candidates are fetched four
-// at a time without early exit so that their loads overlap.
+// vertices all lie outside the requesting cluster. Both cofaces of a facet with lowest vertex b have b as
+// lowest or second-lowest vertex: candidates are the run [f0, f1) of simplices starting with b (I_T,
+// PAPER.md:178) and the simplices whose second vertex is b (those are (x, b, c, d) exactly). Candidates
+// are fetched four at a time without early exit so that their loads overlap.
 template <int D>
 __device__ __forceinline__ int tt_fallback(const DeviceMesh& M, int f0, int f1, int b, int c, int d, int self) {
   int found = -1;
@@ -311,7 +324,10 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* s
 // ------------------------------------------------------------------------------------------------
 // TT tables. A table word of vertex p's group = key | s << kKeyBits | k << 30: the facet's
 // vertices other than p (local ids, ascending), the staged simplex s it belongs to, and the local
-// vertex k it is opposite to.
+// vertex k it is opposite to. Vertex p's table has as many slots as p has VT entries not in its own
+// run plus D-1 per simplex of its run — an upper bound of its records (the simplices whose second
+// vertex is p are among the former), so a table cannot fill up; with every interior facet recorded
+// twice the usual load is about one third.
 template <int D>
 struct FacetBits {
   static constexpr int kKeyBits = D == 4 ? 18 : 16;
@@ -319,41 +335,33 @@ struct FacetBits {
   static constexpr uint32_t kIdxMask = (1u << (30 - kKeyBits)) - 1u;
 };
 
-struct GroupCtx {
-  uint32_t* tbl;       // this vertex's table, hs slots
-  uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
-  uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
-  int s_ext;
-  int s_all;           // staged simplices of the tile (bounds-checked build)
-};
-
-// Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
-// holds the same key (the other coface) and write both TT entries.
+// Place facet k of staged simplex s with key `key` in the table [tbl, tbl+m): claim an empty slot, or
+// meet the record that holds the same key (the other coface) and write both TT entries.
 template <int D>
-__device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
+__device__ __forceinline__ void facet_place(uint32_t* tbl, uint32_t m, uint32_t key, int s, int k, uint16_t* ttrow,
+                                            int s_all, int32_t* err) {
   using FB = FacetBits<D>;
-  uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
-  uint32_t cur = g.tbl[h];
-  uint32_t probe = 0;
-  while (cur != kEmpty32 && (cur & FB::kKeyMask) != key) {  // probe loop kept minimal: lanes diverge here
-    h = h + 1 == g.hs ? 0u : h + 1;
-    cur = g.tbl[h];
-    if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
-  }
-  if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
-  if (cur == kEmpty32) {
-    g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
-  } else {
-    const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
-    if (!GALE_IN_BOUNDS(err, s < g.s_all && s2 < g.s_all && k2 < D)) return;
-    if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2;
-    if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s;
+  if (!GALE_IN_BOUNDS(err, m > 0 && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D && s < s_all)) return;
+  const uint32_t word = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
+  uint32_t h = __umulhi(key * 0x9E3779B1u, m);
+  for (uint32_t probe = 0;; ++probe) {
+    const uint32_t old = atomicCAS(tbl + h, kEmpty32, word);
+    if (old == kEmpty32) return;
+    if ((old & FB::kKeyMask) == key) {
+      const int s2 = (int)((old >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(old >> 30);
+      if (!GALE_IN_BOUNDS(err, s2 < s_all && k2 < D)) return;
+      ttrow[s * D + k] = (uint16_t)s2;
+      ttrow[s2 * D + k2] = (uint16_t)s;
+      return;
+    }
+    h = h + 1 == m ? 0u : h + 1;
+    if (probe >= m) { raise_err(err, ERR_TT_TABLE_FULL); return; }
   }
 }
 
 // Key of the facet opposite local vertex K: the facet's vertices other than its lowest one.
 template <int D, int K>
-__device__ __forceinline__ uint32_t group_key(const int (&l)[4]) {
+__device__ __forceinline__ uint32_t facet_key(const int (&l)[4]) {
   if constexpr (D == 4) {
     const int a = K <= 1 ? l[2] : l[1];
     const int b = K == 3 ? l[2] : l[3];
@@ -363,53 +371,32 @@ __device__ __forceinline__ uint32_t group_key(const int (&l)[4]) {
   }
 }
 
-// Exclusive scan over the B half of the block (threads [NT/2, NT)), one value per thread, with a
-// named barrier so that the A half is not held up. Returns the exclusive prefix; *total = sum.
-template <int NT>
-__device__ __forceinline__ uint32_t half_exclusive_scan(uint32_t x, uint32_t* scratch, uint32_t* total) {
-  constexpr int TV = NT / 2;
-  const int lane = threadIdx.x & 31, warp = (threadIdx.x - TV) >> 5;
-  uint32_t inc = x;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-    if (lane >= d) inc += y;
-  }
-  if constexpr (TV <= 32) {
-    *total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-    return inc - x;
-  } else {
-    constexpr int NW = TV / 32;
-    if (lane == 31) scratch[warp] = inc;
-    named_barrier(1, TV);
-    uint32_t base = 0u, tot = 0u;
-#pragma unroll
-    for (int w = 0; w < NW; ++w) {
-      const uint32_t v = scratch[w];
-      if (w < warp) base += v;
-      tot += v;
-    }
-    named_barrier(1, TV);  // scratch may be reused
-    *total = tot;
-    return base + inc - x;
-  }
+// Staging area -> global with one TMA bulk store for the 16-byte aligned body and scalar stores for
+// the ragged ends. Staging element j corresponds to global element (g0 - mis) + j, j in [mis, mis+n),
+// mis = g0 & 3, so the two addresses share their 16-byte phase. One thread calls this.
+__device__ __forceinline__ void bulk_emit(int32_t* gbase, long long g0, int n, const int32_t* stage, int mis) {
+  const int jb = (mis + 3) & ~3, je = (mis + n) & ~3;
+  int32_t* g = gbase + (g0 - mis);
+  if (je > jb) bulk_s2g(g + jb, stage + jb, (uint32_t)(je - jb) * 4u);
+  bulk_commit();
+  const int head_end = min(jb, mis + n);
+  for (int j = mis; j < head_end; ++j) GALE_ST(g + j, stage[j]);
+  for (int j = max(je, jb); j < mis + n; ++j) GALE_ST(g + j, stage[j]);
 }
 
 // ------------------------------------------------------------------------------------------------
 // The batch kernel: VT + VV + TT for every tile of the requested clusters (or, COUNT, the exact
 // VT / VV sizes of tiles [tile_base, tile_base + gridDim.x) — the paper's leader producer likewise
-// sizes its relation arrays before launch). NT = 2 * (rows per tile capacity).
+// sizes its relation arrays before launch). NT >= rows per tile.
 template <int D, int NT, bool COUNT, int LB>
-__global__ void __launch_bounds__(NT, (NT <= 64 ? 16 : (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2))))
+__global__ void __launch_bounds__(NT, (NT <= 128 ? 8 : 4))
 gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
                   const SmemLayout L, const OutPtrs O) {
   extern __shared__ __align__(16) unsigned char smem[];
-  constexpr int TV = NT / 2;
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t mask = P.mask;
-  const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0;
+  const bool do_vt = !COUNT && (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0;
   const bool do_tt = !COUNT && (mask & REL_TT) != 0;
-  const bool entries = !COUNT && (do_vt || do_tt);  // VT entries are staged (TT reads their flags)
 
   // ---- block -> (cluster slot, tile) ----------------------------------------------------------
   int slot = 0, tile;
@@ -443,13 +430,15 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
   const int S = s_int + s_ext;
   const int WT = C.WT, WV = C.WV;
+  const int wT = (S + 31) >> 5, wV = (td.nloc + 31) >> 5;
 #if GALE_CHECK_BOUNDS
   {
-    bool ok = nrows >= 0 && nrows <= C.tv && NT >= 2 * C.tv && S >= 0 && S <= C.smax && s_ext <= C.sext &&
-              td.nloc <= C.nloc && nlo >= 0 && nlo + nrows <= td.nloc && ((S + 31) >> 5) <= WT;
-    if (mask & REL_VV) ok = ok && ((td.nloc + 31) >> 5) <= WV;
-    if (!COUNT && (mask & REL_TT)) ok = ok && s_int <= C.sint && C.hs >= 2;
-    if (!COUNT && (mask & (REL_VT | REL_TT))) ok = ok && td.vt_nnz <= C.vt_max;
+    bool ok = nrows >= 0 && nrows <= C.tv && NT >= C.tv && S >= 0 && S <= C.smax && td.nloc <= C.nloc && nlo >= 0 &&
+              nlo + nrows <= td.nloc && wT <= WT;
+    if (!COUNT) ok = ok && s_ext <= C.sext;
+    if (mask & REL_VV) ok = ok && wV <= WV;
+    if (do_tt) ok = ok && s_int <= C.sint && td.vt_nnz + (D - 2) * s_int <= C.tbl;
+    if (do_vt) ok = ok && td.vt_nnz <= C.vt_max;
     if (!COUNT && (mask & REL_VV)) ok = ok && td.vv_nnz <= C.vv_max;
     if (!ok) {  // block-uniform: leave before anything is staged
       if (tid == 0) raise_err(M.err, ERR_BOUNDS);
@@ -461,58 +450,57 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   unsigned char* tets = smem + L.tets;
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
-  const int2* hft = reinterpret_cast<const int2*>(smem + L.hft);
-  uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
-  uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
-  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [36] queue length, [38] n_vv
+  int32_t* ft = reinterpret_cast<int32_t*>(smem + L.ft);          // first_tet[v_lo .. v_lo+nrows]
+  int32_t* offT = reinterpret_cast<int32_t*>(smem + L.offT);      // VT offsets of the tile's rows (+ total)
+  int32_t* offV = reinterpret_cast<int32_t*>(smem + L.offV);
+  int32_t* runpos = reinterpret_cast<int32_t*>(smem + L.runpos);  // VT position of simplex t of row r's run = runpos[r] + t
+  int32_t* tbo = reinterpret_cast<int32_t*>(smem + L.tbo);        // facet-table offsets of the rows (+ total)
+  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);
+  uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);    // [0] chunk counter, [1] fallback queue length
   uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
   uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
+  uint16_t* pfx = reinterpret_cast<uint16_t*>(smem + L.pfx);      // set bits of the row before word w
   uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
-  uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);
-  uint16_t* st_vt = reinterpret_cast<uint16_t*>(smem + L.st_vt);
-  uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
+  uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);  // [S][D] neighbours as staged indices, 0xFFFF = none
+  int32_t* st_vt = reinterpret_cast<int32_t*>(smem + L.st_vt);
+  int32_t* st_vv = reinterpret_cast<int32_t*>(smem + L.st_vv);
+  uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
+  void* bar = smem + L.mbar;
 
   const int row0 = P.row_base[slot] + td.row_rel;
   const int vt0 = P.vt_base[slot] + td.vt_rel;
   const int vv0 = P.vv_base[slot] + td.vv_rel;
   const int tt0 = P.tt_base[slot] + td.tt_rel;
+  const int mis_vt = vt0 & 3, mis_vv = vv0 & 3;  // 16-byte phase of the tile's output segments
 
-  // ---- P0: stage + clear ----------------------------------------------------------------------
-  {
-    const int4* src = reinterpret_cast<const int4*>(static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB));
-    int4* dst = reinterpret_cast<int4*>(tets);
-    for (int i = tid; i < (S * 4 * LB + 15) >> 4; i += NT) cp_async16(dst + i, src + i);
-    {
-      const int4* hsrc = reinterpret_cast<const int4*>(M.hft + td.gid_off);
-      int4* hdst = reinterpret_cast<int4*>(smem + L.hft);
-      for (int i = tid; i < (td.nloc + 1) >> 1; i += NT) cp_async16(hdst + i, hsrc + i);
-    }
-    if (!COUNT) {
-      const int4* tsrc = reinterpret_cast<const int4*>(M.tex + td.tex_off);
-      int4* tdst = reinterpret_cast<int4*>(texid);
-      for (int i = tid; i < (s_ext + 3) >> 2; i += NT) cp_async16(tdst + i, tsrc + i);
-      if (do_vv || do_tt) {
-        const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
-        int4* gdst = reinterpret_cast<int4*>(gid);
-        for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
-      }
-    }
+  // ---- P0: stage (TMA bulk copies) + clear -----------------------------------------------------
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    fence_proxy_async();
+    const uint32_t b_t = (uint32_t)((S + 3) & ~3) * (4u * LB);
+    const uint32_t b_x = COUNT ? 0u : (uint32_t)((s_ext + 3) & ~3) * 4u;
+    const uint32_t b_g = (!COUNT && (do_vv || do_tt)) ? (uint32_t)((td.nloc + 3) & ~3) * 4u : 0u;
+    mbar_arrive_expect_tx(bar, b_t + b_x + b_g);
+    if (b_t) bulk_g2s(tets, static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB), b_t, bar);
+    if (b_x) bulk_g2s(texid, M.tex + td.tex_off, b_x, bar);
+    if (b_g) bulk_g2s(gid, M.gid + td.gid_off, b_g, bar);
   }
+  for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);
   {
     int4* z = reinterpret_cast<int4*>(smem + L.bmT);
-    const int n16 = (L.bm_end - L.bmT) >> 4;
+    const int n16 = (L.zero_end - L.bmT) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
   }
   if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
     int4* z = reinterpret_cast<int4*>(smem + L.tbl);
-    const int n16 = (L.tt_end - L.tbl) >> 4;
+    const int n16 = (L.ones_end - L.tbl) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
   }
-  if (tid == 0) { scan[36] = 0u; scan[38] = 0u; }
-  cp_async_wait_all();
+  if (tid == 0) { misc[0] = 0u; misc[1] = 0u; }
   __syncthreads();
+  mbar_wait(bar, 0);
 
-  // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
+  // ---- P1: VT incidence bits and VV bits, one thread per staged simplex ------------------------
   for (int s = tid; s < S; s += NT) {
     int l[4];
     load_local<LB>(tets, s, l);
@@ -522,155 +510,64 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
 #endif
     uint32_t* col = bmT + (s >> 5);
-    const uint32_t bit = bit_of(s);
+    const uint32_t bit = 1u << (s & 31);
+    int r[D];
 #pragma unroll
-    for (int k = 1; k < D; ++k) {
-      const int r = l[k] - nlo;
-      if ((unsigned)r < (unsigned)nrows) atomicOr(col + r * WT, bit);
-    }
-    if (do_tt && s >= s_ext && l[1] - nlo >= nrows) {
-      // facet 0 of this internal simplex leaves the tile (a5): its coface is almost always in the run
-      // of the second vertex; pull those rows of T towards L2 now, they are read in the last phase
-      const int2 run = hft[l[1]];
-      const char* r0 = reinterpret_cast<const char*>(M.T) + (long long)run.x * (D * 4);
-      const char* r1 = reinterpret_cast<const char*>(M.T) + (long long)max(run.y - 1, run.x) * (D * 4);
-      asm volatile("prefetch.global.L2 [%0];" ::"l"(r0));
-      asm volatile("prefetch.global.L2 [%0];" ::"l"(r1));
+    for (int k = 0; k < D; ++k) r[k] = l[k] - nlo;
+#pragma unroll
+    for (int k = 1; k < D; ++k)
+      if ((unsigned)r[k] < (unsigned)nrows) atomicOr(col + r[k] * WT, bit);
+    if (do_vv) {
+      uint32_t w[D], b[D];
+#pragma unroll
+      for (int j = 0; j < D; ++j) { w[j] = (uint32_t)l[j] >> 5; b[j] = 1u << (l[j] & 31); }
+#pragma unroll
+      for (int k = 0; k < D; ++k)
+        if ((unsigned)r[k] < (unsigned)nrows) {
+          uint32_t* row = bmV + r[k] * WV;
+#pragma unroll
+          for (int j = 0; j < D; ++j)
+            if (j != k) atomicOr(row + w[j], b[j]);  // "each other vertex"
+        }
     }
   }
   __syncthreads();
 
-  // ---- P2: row degrees -> VT offsets ----------------------------------------------------------
-  const bool isB = tid >= TV;
-  const int p = isB ? tid - TV : tid;
-  const bool live = p < nrows;
-  const int ploc = nlo + p;
-  const int wT = (S + 31) >> 5;
-  if (live) {
-    const int half = (wT + 1) >> 1;
-    const uint32_t* row = bmT + p * WT;
-    int c = 0;
-    const int w0 = isB ? half : 0, w1 = isB ? wT : half;
-#pragma unroll 4
-    for (int w = w0; w < w1; ++w) c += __popc(row[w]);
-    cnt[(isB ? C.tv : 0) + p] = (uint16_t)c;
-  }
-  __syncthreads();
-  int nb = 0, off = 0, n_vt;
+  // ---- P2: per row prefix counts and degrees -> offsets ----------------------------------------
+  int n_vt, n_vv;
+  int my_offV = 0;
   {
-    uint32_t deg = 0u, tot;
-    if (live) {
-      nb = (int)cnt[p] + (int)cnt[C.tv + p];
-      const int2 run = hft[ploc];
-      deg = (uint32_t)(nb + run.y - run.x);
-    }
-    const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // A and B halves carry the same values
-    n_vt = (int)(tot >> 1);
-    off = (int)ex - (isB ? n_vt : 0);
-  }
-  if (!COUNT && do_vt && live && !isB) O.vt_offsets[row0 + p] = vt0 + off;
-
-  // ---- P3: A walks the bits of row p, B walks the run of p ------------------------------------
-  if (live) {
-    uint32_t* vvrow = bmV + p * WV;
-    if (!isB) {
-      const uint32_t* row = bmT + p * WT;
-      int pos = off, sbase = -32;
-      uint32_t bits = 0u;
-      for (int n = 0; n < nb; ++n) {
-        while (bits == 0u) { bits = *row++; sbase += 32; }
-        const int s = sbase + __ffs(bits) - 1;
-        bits &= bits - 1;
-        int l[4];
-        load_local<LB>(tets, s, l);
-        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= 0 && s < S))
-          st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
-        if (do_vv) {
-#pragma unroll
-          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));  // self bit cleared in P4
-        }
+    uint32_t deg = 0u, degv = 0u;
+    int nb = 0;
+    if (tid < nrows) {
+      const uint32_t* row = bmT + tid * WT;
+      uint16_t* pf = pfx + tid * WT;
+      for (int w = 0; w < wT; ++w) {
+        pf[w] = (uint16_t)nb;
+        nb += __popc(row[w]);
       }
-    } else {
-      GroupCtx g;
-      if (do_tt) {
-        const int hs = C.hs;
-        g.tbl = tbl + p * (hs + 1);
-        g.hs = (uint32_t)hs;
-        g.ttrow = ttrow;
-        g.s_ext = s_ext; g.s_all = S;
+      deg = (uint32_t)(nb + ft[tid + 1] - ft[tid]);
+      if (do_vv) {
+        const uint32_t* rv = bmV + tid * WV;
+        for (int w = 0; w < wV; ++w) degv += __popc(rv[w]);
       }
-      int pos = off + nb;
-      const int2 run = hft[ploc];
-      const int r1 = run.y - t_lo;
-      for (int i = run.x - t_lo; i < r1; ++i) {
-        const int s = s_ext + i;
-        int l[4];
-        load_local<LB>(tets, s, l);
-        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= s_ext && s < S)) st_vt[pos++] = (uint16_t)s;
-        if (do_vv) {
-#pragma unroll
-          for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));
-        }
-        if (do_tt) {
-          group_place<D>(g, group_key<D, 1>(l), s, 1, M.err);
-          group_place<D>(g, group_key<D, 2>(l), s, 2, M.err);
-          if constexpr (D == 4) group_place<D>(g, group_key<D, 3>(l), s, 3, M.err);
-        }
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- P4: A joins the facets 0 of the simplices (x, p, ..); B expands VV row p ----------------
-  int n_vv = 0;
-  if (!isB) {
-    if (do_tt && live) {
-      GroupCtx g;
-      const int hs = C.hs;
-      g.tbl = tbl + p * (hs + 1);
-      g.hs = (uint32_t)hs;
-      g.ttrow = ttrow;
-      g.s_ext = s_ext; g.s_all = S;
-      int i = off;
-      const int end = off + nb;
-      for (;;) {
-        uint32_t e = 0u;
-        while (i < end && !((e = st_vt[i]) & 0x8000u)) ++i;
-        if (i >= end) break;
-        ++i;
-        const int s = (int)(e & 0x7FFFu);
-        int l[4];
-        load_local<LB>(tets, s, l);
-        group_place<D>(g, group_key<D, 0>(l), s, 0, M.err);
-      }
-    }
-  } else if (do_vv) {
-    const int wV = (td.nloc + 31) >> 5;
-    uint32_t* row = bmV + p * WV;
-    int nbv = 0;
-    if (live) {
-      row[ploc >> 5] &= ~bit_of(ploc);  // a vertex is not its own neighbour
-#pragma unroll 4
-      for (int w = 0; w < wV; ++w) nbv += __popc(row[w]);
     }
     uint32_t tot;
-    const int offv = (int)half_exclusive_scan<NT>((uint32_t)nbv, scan, &tot);
-    if (tid == TV) scan[38] = tot;
-    if (live && !COUNT) {
-      O.vv_offsets[row0 + p] = vv0 + offv;
-      int pos = offv, lbase = -32;
-      uint32_t bits = 0u;
-      for (int n = 0; n < nbv; ++n) {
-        while (bits == 0u) { bits = *row++; lbase += 32; }
-        if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vv_max && lbase + __ffs(bits) - 1 < td.nloc))
-          st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
-        bits &= bits - 1;
-      }
+    const uint32_t ex = block_exclusive_scan<NT>(deg | (degv << 16), scan, &tot);
+    n_vt = (int)(tot & 0xFFFFu);
+    n_vv = (int)(tot >> 16);
+    if (tid < nrows) {
+      const int ot = (int)(ex & 0xFFFFu);
+      my_offV = (int)(ex >> 16);
+      offT[tid] = ot;
+      offV[tid] = my_offV;
+      runpos[tid] = ot + nb - ft[tid];
+      tbo[tid] = ot + (D - 2) * (ft[tid] - t_lo);
+      if (do_vt) O.vt_offsets[row0 + tid] = vt0 + ot;
+      if (!COUNT && do_vv) O.vv_offsets[row0 + tid] = vv0 + my_offV;
     }
+    if (tid == 0) { offT[nrows] = n_vt; offV[nrows] = n_vv; tbo[nrows] = n_vt + (D - 2) * s_int; }
   }
-  __syncthreads();
-  n_vv = (int)scan[38];
-
   if (COUNT) {
     if (tid == 0) {
       O.stats[(long long)tile * 4 + 0] = n_vt;
@@ -680,73 +577,153 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
     }
     return;
   }
-  if (tid == 0 && ((do_vt && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
+  if (tid == 0 && (((mask & REL_VT) && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
     raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
+  __syncthreads();
 
-  // ---- P5: translate to global ids, coalesced write-out ----------------------------------------
-  if (do_tt) {
-    // facets no tile vertex owns go to the queue
-    for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
-      const int i = base + lane;
-      bool need_fb = false;
-      if (i < s_int) {
-        uint32_t e[D];
-        if constexpr (D == 4) {
-          const uint2 q = reinterpret_cast<const uint2*>(ttrow)[i];
-          e[0] = q.x & 0xFFFFu; e[1] = q.x >> 16; e[2] = q.y & 0xFFFFu; e[3] = q.y >> 16;
-        } else {
-          e[0] = ttrow[i * 3]; e[1] = ttrow[i * 3 + 1]; e[2] = ttrow[i * 3 + 2];
-        }
-        int r[D];
-#pragma unroll
-        for (int k = 0; k < D; ++k)
-          r[k] = e[k] == 0xFFFFu ? -1 : ((int)e[k] < s_ext ? texid[e[k]] : t_lo + ((int)e[k] - s_ext));
-        if constexpr (D == 4) {
-          GALE_ST(reinterpret_cast<int4*>(O.tt_indices) + tt0 + i, make_int4(r[0], r[1], r[2], r[3]));
-        } else {
-          int32_t* o = O.tt_indices + (long long)(tt0 + i) * 3;
-          o[0] = r[0]; o[1] = r[1]; o[2] = r[2];
-        }
-        if (r[0] < 0) {
-          int l[4];
-          load_local<LB>(tets, s_ext + i, l);
-          need_fb = l[1] - nlo >= nrows;
-        }
-      }
-      const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
-      if (fbm) {
-        const int leader = __ffs(fbm) - 1;
-        uint32_t pos = 0u;
-        if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
-        pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
-        if (need_fb && GALE_IN_BOUNDS(M.err, (int)(pos + __popc(fbm & ((1u << lane) - 1u))) < C.sint))
-          fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
+  // ---- P3: VV rows -> staging; per staged simplex: VT scatter by rank, TT facet records ---------
+  if (do_vv && tid < nrows) {
+    const uint32_t* row = bmV + tid * WV;
+    int pos = mis_vv + my_offV;
+    for (int w = 0; w < wV; ++w) {
+      uint32_t bits = row[w];
+      while (bits) {
+        const int lid = (w << 5) + __ffs(bits) - 1;
+        bits &= bits - 1;
+        if (GALE_IN_BOUNDS(M.err, pos < C.vv_max + 4 && lid < td.nloc)) st_vv[pos] = gid[lid];
+        ++pos;
       }
     }
   }
-  if (do_vt)
-    for (int i = tid; i < n_vt; i += NT) {
-      const int s = (int)(st_vt[i] & 0x7FFFu);
-      GALE_ST(O.vt_indices + vt0 + i, s < s_ext ? texid[s] : t_lo + (s - s_ext));
+  if (do_vt || do_tt) {
+    for (;;) {
+      int base = 0;
+      if (lane == 0) base = (int)atomicAdd(&misc[0], 32u);
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (base >= S) break;
+      const int s = base + lane;
+      if (s >= S) continue;
+      int l[4];
+      load_local<LB>(tets, s, l);
+#if GALE_CHECK_BOUNDS
+      for (int k = 0; k < D; ++k)
+        if (l[k] < 0 || l[k] >= td.nloc) l[k] = nlo;  // reported in P1
+#endif
+      const bool internal = s >= s_ext;
+      if (do_vt) {
+        const int g = internal ? t_lo + (s - s_ext) : texid[s];
+        const int w = s >> 5;
+        const uint32_t below = (1u << (s & 31)) - 1u;
+#pragma unroll
+        for (int k = 1; k < D; ++k) {
+          const int r = l[k] - nlo;
+          if ((unsigned)r < (unsigned)nrows) {
+            const int pos = offT[r] + (int)pfx[r * WT + w] + __popc(bmT[r * WT + w] & below);
+            if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max)) st_vt[mis_vt + pos] = g;
+          }
+        }
+        if (internal) {
+          const int r = l[0] - nlo;
+          if (GALE_IN_BOUNDS(M.err, (unsigned)r < (unsigned)nrows)) {
+            const int pos = runpos[r] + g;
+            if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max)) st_vt[mis_vt + pos] = g;
+          }
+        }
+      }
+      if (do_tt) {
+        if (internal) {  // facets 1..D-1 have lowest vertex l[0], a tile vertex
+          const int r = l[0] - nlo;
+          if (GALE_IN_BOUNDS(M.err, (unsigned)r < (unsigned)nrows)) {
+            const int b0 = tbo[r];
+            const uint32_t m = (uint32_t)(tbo[r + 1] - b0);
+            if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl)) {
+              facet_place<D>(tbl + b0, m, facet_key<D, 1>(l), s, 1, ttrow, S, M.err);
+              facet_place<D>(tbl + b0, m, facet_key<D, 2>(l), s, 2, ttrow, S, M.err);
+              if constexpr (D == 4) facet_place<D>(tbl + b0, m, facet_key<D, 3>(l), s, 3, ttrow, S, M.err);
+            }
+          }
+        }
+        const int r1 = l[1] - nlo;
+        if ((unsigned)r1 < (unsigned)nrows) {  // facet 0 has lowest vertex l[1]
+          const int b0 = tbo[r1];
+          const uint32_t m = (uint32_t)(tbo[r1 + 1] - b0);
+          if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl))
+            facet_place<D>(tbl + b0, m, facet_key<D, 0>(l), s, 0, ttrow, S, M.err);
+        }
+      }
     }
-  if (do_vv)
-    for (int i = tid; i < n_vv; i += NT) GALE_ST(O.vv_indices + vv0 + i, gid[st_vv[i]]);
+  }
+  fence_proxy_async();  // staging areas were written through the generic proxy, TMA reads them
+  __syncthreads();
+
+  // ---- P4: write-out ---------------------------------------------------------------------------
+  if (do_vt && tid == 0) bulk_emit(O.vt_indices, vt0, n_vt, st_vt, mis_vt);
+  if (do_vv && tid == 32) bulk_emit(O.vv_indices, vv0, n_vv, st_vv, mis_vv);
 
   if (do_tt) {
+    const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
+    const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
+    const int tile_hi = nlo + nrows;
+    // TT rows of the internal simplices
+    for (int i = tid; i < s_int; i += NT) {
+      const int s = s_ext + i;
+      int r[D];
+#pragma unroll
+      for (int k = 0; k < D; ++k) {
+        const int e = ttrow[s * D + k];
+        r[k] = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
+      }
+      int l[4];
+      load_local<LB>(tets, s, l);
+      // facet 0 = (l[1], ..) has no vertex in this tile when l[1] lies above it
+      const bool out0 = l[1] >= tile_hi;
+      const bool delegated = out0 && gid[min(l[1], td.nloc - 1)] < c_hi;  // the tile that owns l[1] writes entry 0
+      int32_t* o = O.tt_indices + (long long)(tt0 + i) * D;
+      if constexpr (D == 4) {
+        if (!delegated) {
+          GALE_ST(reinterpret_cast<int4*>(o), make_int4(r[0], r[1], r[2], r[3]));
+        } else {
+          GALE_ST(o + 1, r[1]);
+          GALE_ST(reinterpret_cast<int2*>(o + 2), make_int2(r[2], r[3]));
+        }
+      } else {
+        if (!delegated) GALE_ST(o, r[0]);
+        GALE_ST(o + 1, r[1]);
+        GALE_ST(o + 2, r[2]);
+      }
+      if (out0 && !delegated) {  // cross-cluster facet: resolved from global memory below
+        const uint32_t q = atomicAdd(&misc[1], 1u);
+        if (GALE_IN_BOUNDS(M.err, (int)q < C.sint)) fbq[q] = (uint16_t)i;
+      }
+    }
+    // entry 0 of external simplices of the same cluster whose second vertex is a vertex of this tile
+    for (int s = tid; s < s_ext; s += NT) {
+      int l[4];
+      load_local<LB>(tets, s, l);
+      const int r1 = l[1] - nlo;
+      if ((unsigned)r1 < (unsigned)nrows && gid[l[0]] >= c_lo) {
+        const int e = ttrow[s * D];
+        const int v = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
+        const long long row = (long long)P.tt_base[slot] + (texid[s] - c_tlo);
+        GALE_ST(O.tt_indices + row * D, v);
+      }
+    }
     __syncthreads();  // queue complete, TT rows stored
     // ---- a5: one queued facet per thread, resolved from global memory -------------------------
-    const int nq = (int)scan[36];
+    const int nq = (int)misc[1];
     for (int q = tid; q < nq; q += NT) {
       const int i = fbq[q];
       int l[4];
       load_local<LB>(tets, s_ext + i, l);
       const int t = t_lo + i;
       const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
-      const int2 run = hft[l[1]];
-      const int r = tt_fallback<D>(M, run.x, run.y, b, c, d, t);
+      const int f0 = __ldg(M.first_tet + b), f1 = __ldg(M.first_tet + b + 1);
+      const int r = tt_fallback<D>(M, f0, f1, b, c, d, t);
       if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barrier
     }
   }
+  // the block's shared memory must stay intact until the bulk stores have read it
+  if (tid == 0 || tid == 32) bulk_wait_read_all();
 }
 
 }  // namespace gale

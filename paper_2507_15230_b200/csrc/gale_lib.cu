@@ -46,14 +46,13 @@ constexpr int kSmemLimit = 227 * 1024;  // opt-in dynamic shared memory per bloc
 struct Plan {
   // key
   const int32_t* dT = nullptr;
-  int dim = 0, nV = 0, nC = 0, tv_req = 0;
+  int dim = 0, nV = 0, nC = 0, tv_req = 0, maxB = 1, queue_depth = 0, device_ring = 0;
   long long nT = 0;
   uint32_t flags = 0;
   std::vector<int32_t> cl_off;
   // index (host copies)
   int tv = 0, nTiles = 0, NT = 0;
   std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
-  std::vector<int2> hft;                // parallel to gid: (first_tet[g], first_tet[g+1])
   std::vector<uint16_t> loc;            // 4 per staged simplex (build); compacted into loc8 when lb == 1
   std::vector<uint8_t> loc8;
   long long staged_padded = 0;          // staged simplices incl. per-tile padding
@@ -67,11 +66,6 @@ struct Plan {
   long long max_rows = 0, max_vt = 0, max_vv = 0, max_tt = 0;
   double analyse_ms = 0;
 
-  size_t index_bytes() const {
-    return up(first_tet.size() * 4) + up(opp_first.size() * 4) + up(opp_perm.size() * 4) +
-           up(cl_tile_begin.size() * 4) + up(tiles.size() * sizeof(TileDesc) + 16) + up(tex.size() * 4 + 16) +
-           up(gid.size() * 4 + 16) + up(hft.size() * sizeof(int2) + 16) + up(size_t(staged_padded) * 4 * cfg.lb + 64);
-  }
 };
 
 struct SlotLayout {
@@ -120,15 +114,15 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-inline int threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : (tv > 32 ? 128 : 64)); }  // NT >= 2 * tv
+inline int threads_for_tile(int tv) { return tv > 128 ? 256 : 128; }  // NT >= tv (one thread per row in P2)
 
 // Kernel capacities for one launch: regions the relation mask does not need are dropped.
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
   SmemCfg c = full;
   if (!(mask & gale::REL_VV)) { c.WV = 0; c.vv_max = 0; }
-  if (!(mask & gale::REL_TT) || count_mode) { c.hs = 0; c.sint = 0; }
-  if (!(mask & (gale::REL_VT | gale::REL_TT))) c.vt_max = 0;  // TT reads the staged VT entries' flags
-  if (count_mode) { c.vt_max = 0; c.vv_max = 0; }
+  if (!(mask & gale::REL_TT) || count_mode) { c.tbl = 0; c.sint = 0; }
+  if (!(mask & gale::REL_VT)) c.vt_max = 0;
+  if (count_mode) { c.vt_max = 0; c.vv_max = 0; c.sext = 0; c.nloc = 0; }  // T_ex ids / vertex table are not staged
   return c;
 }
 
@@ -140,9 +134,7 @@ using KernelFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemC
                           const gale::OutPtrs);
 template <int D, bool COUNT, int LB>
 KernelFn kernel_for_nt(int NT) {
-  return NT == 512 ? gale::gale_batch_kernel<D, 512, COUNT, LB>
-                   : (NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT, LB>
-                                : (NT == 128 ? gale::gale_batch_kernel<D, 128, COUNT, LB> : gale::gale_batch_kernel<D, 64, COUNT, LB>));
+  return NT == 256 ? gale::gale_batch_kernel<D, 256, COUNT, LB> : gale::gale_batch_kernel<D, 128, COUNT, LB>;
 }
 template <int D, bool COUNT>
 KernelFn kernel_for_lb(int NT, int lb) { return lb == 1 ? kernel_for_nt<D, COUNT, 1>(NT) : kernel_for_nt<D, COUNT, 2>(NT); }
@@ -150,6 +142,10 @@ KernelFn kernel_for(int D, int NT, bool count, int lb) {
   if (D == 4) return count ? kernel_for_lb<4, true>(NT, lb) : kernel_for_lb<4, false>(NT, lb);
   return count ? kernel_for_lb<3, true>(NT, lb) : kernel_for_lb<3, false>(NT, lb);
 }
+
+// The dynamic shared-memory ceiling is an attribute of the kernel instantiation for the whole context,
+// not of a handle: raise every instantiation to the device limit once, never lower it.
+cudaError_t allow_max_smem(KernelFn fn) { return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit); }
 
 // Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
 // simplices. Returns false if a tile exceeds a kernel limit for this tv (the caller retries smaller).
@@ -212,6 +208,7 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
       d.s_int = p.first_tet[tile_vhi[i]] - d.t_lo;
       d.s_ext = int(raw_off[i + 1] - raw_off[i]);
       d.row_rel = d.v_lo - p.cl_off[c];
+      d.c_rows = p.cl_off[c + 1] - p.cl_off[c];
       d.tt_rel = d.t_lo - p.first_tet[p.cl_off[c]];
       d.stg_off = stg;
       d.tex_off = texo;
@@ -293,16 +290,6 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     hoff += (long long)gid_part[w].size();
     std::vector<int32_t>().swap(gid_part[w]);
   }
-  p.hft.resize(p.gid.size());
-  for (size_t i = 0; i < p.gid.size(); ++i) {
-    const int g = std::min(std::max(p.gid[i], 0), std::max(p.nV - 1, 0));
-    p.hft[i] = p.nV > 0 ? make_int2(p.first_tet[g], p.first_tet[g + 1]) : make_int2(0, 0);
-  }
-  // largest facet group of a tile vertex: D-1 facets per simplex of its run + facet 0 of every
-  // simplex whose second vertex it is
-  int gmax = 1;
-  for (int v = 0; v < p.nV; ++v)
-    gmax = std::max(gmax, (D - 1) * (p.first_tet[v + 1] - p.first_tet[v]) + (p.opp_first[v + 1] - p.opp_first[v]));
   // shared-memory capacities known so far
   long long smax = 4, sext = 4, sint = 2, nloc = 4;
   for (const TileDesc& d : p.tiles) {
@@ -325,9 +312,6 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     std::vector<uint16_t>().swap(p.loc);
   }
   p.cfg.sint = int(sint);
-  // distinct facets <= records, so a group cannot overflow its table; every interior facet is recorded
-  // twice, so the usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
-  p.cfg.hs = std::max(8, (gmax + gmax / 3 + 1) & ~1);  // load <= 3/4 even if no facet of a group is shared
   p.cfg.WT = int((smax + 31) / 32) | 1;
   p.cfg.WV = int((nloc + 31) / 32) | 1;
   return true;
@@ -358,10 +342,10 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   const std::vector<uint32_t> parts = {3u};
   if (layout_for(D, cfg_for_mask(full, 3, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
 
-  DevBuf b_ft, b_tiles, b_tex, b_gid, b_hft, b_loc, b_stats, b_err;
+  DevBuf b_ft, b_tiles, b_tex, b_gid, b_loc, b_stats, b_err;
   int rc;
   if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
-      (rc = b_gid.upload(p.gid, st)) || (rc = b_hft.upload(p.hft, st)) || (rc = (p.cfg.lb == 1 ? b_loc.upload(p.loc8, st) : b_loc.upload(p.loc, st))) ||
+      (rc = b_gid.upload(p.gid, st)) || (rc = (p.cfg.lb == 1 ? b_loc.upload(p.loc8, st) : b_loc.upload(p.loc, st))) ||
       (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
     return rc;
   GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
@@ -371,7 +355,6 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
   dm.tiles = static_cast<TileDesc*>(b_tiles.p);
   dm.tex = static_cast<int32_t*>(b_tex.p);
   dm.gid = static_cast<int32_t*>(b_gid.p);
-  dm.hft = static_cast<int2*>(b_hft.p);
   dm.loc = b_loc.p;
   dm.err = static_cast<int32_t*>(b_err.p);
   KernelFn fn = kernel_for(D, p.NT, true, p.cfg.lb);
@@ -380,7 +363,7 @@ int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long lon
     const SmemCfg c = cfg_for_mask(full, m, true);
     const gale::SmemLayout lay = layout_for(D, c);
     const int smem = lay.total;
-    GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    GALE_CUDA(allow_max_smem(fn));
     gale::BatchParams P{};
     P.mask = m | gale::MODE_COUNT;
     gale::OutPtrs O{};
@@ -406,6 +389,7 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   auto p = std::make_unique<Plan>();
   p->dT = d.d_simplices; p->dim = d.dim; p->nV = d.num_vertices; p->nC = d.num_clusters; p->nT = d.num_simplices;
   p->tv_req = d.tile_vertices; p->flags = d.flags;
+  p->maxB = d.max_batch_clusters; p->queue_depth = d.queue_depth; p->device_ring = d.device_ring;
   p->cl_off.assign(d.h_cluster_offsets, d.h_cluster_offsets + d.num_clusters + 1);
   const int D = d.dim + 1;
   if (p->cl_off.front() != 0 || p->cl_off.back() != p->nV) return GALE_ERR_INVALID_ARG;
@@ -453,19 +437,21 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
       if (rc != GALE_OK) return rc;
     }
     if (fits) {
-      long long vt_max = 1, vv_max = 1;
+      long long vt_max = 1, vv_max = 1, tbl_max = 4;
       for (int i = 0; i < p->nTiles; ++i) {
         vt_max = std::max(vt_max, stats[i * 4 + 0]);
         vv_max = std::max(vv_max, stats[i * 4 + 1]);
+        tbl_max = std::max(tbl_max, stats[i * 4 + 0] + (long long)(D - 2) * p->tiles[i].s_int);
       }
       p->cfg.vt_max = int(pad_to(vt_max, 8));
       p->cfg.vv_max = int(pad_to(vv_max, 8));
+      p->cfg.tbl = int(pad_to(tbl_max, 4));
       p->smem_bytes = layout_for(D, p->cfg).total;
       fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
     }
     // automatic tile size: tiles whose vertices are scattered in the mesh (graded meshes, config 4) need
     // large per-block capacities and leave few resident blocks; half the tile measured +25 % there
-    if (fits && d.tile_vertices == 0 && !shrunk && tv >= 32 && D == 4 && p->smem_bytes > 20 * 1024) {
+    if (fits && d.tile_vertices == 0 && !shrunk && tv >= 32 && D == 4 && p->smem_bytes > 56 * 1024) {
       shrunk = true;
       continue;
     }
@@ -496,18 +482,11 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   return GALE_OK;
 }
 
-bool plan_matches(const Plan& p, const gale_mesh_desc_t& d) {
-  return p.dT == d.d_simplices && p.dim == d.dim && p.nV == d.num_vertices && p.nC == d.num_clusters &&
-         p.nT == d.num_simplices && p.tv_req == d.tile_vertices && p.flags == d.flags &&
-         std::equal(p.cl_off.begin(), p.cl_off.end(), d.h_cluster_offsets);
-}
-std::mutex g_plan_mutex;
-std::unique_ptr<Plan> g_plan_cache;  // handed from gale_mesh_workspace_bytes to gale_mesh_create
-
 int check_desc(const gale_mesh_desc_t* d) {
   if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
       !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
-      d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1)
+      d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1 ||
+      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED)))
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
   return GALE_OK;
@@ -526,9 +505,30 @@ int check_device() {
   }
   return GALE_OK;
 }
-size_t total_workspace(const Plan& p, const gale_mesh_desc_t& d) {
-  const int slots = d.queue_depth > 0 ? d.queue_depth : (d.device_ring > 0 ? d.device_ring : 4);
-  return p.index_bytes() + size_t(slots) * slot_capacity_layout(p, d.max_batch_clusters).total + kAlign;
+
+// Placement of the index arrays inside the caller's workspace: ONE function serves both the size
+// query and the upload, so the two cannot disagree.
+struct IndexLayout {
+  size_t first_tet = 0, opp_first = 0, opp_perm = 0, cl_tile_begin = 0, tiles = 0, tex = 0, gid = 0, loc = 0, total = 0;
+};
+IndexLayout index_layout(const Plan& p) {
+  IndexLayout L;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes + 64); return at; };  // 64: vector loads may read past the end
+  L.first_tet = take(p.first_tet.size() * 4);
+  L.opp_first = take(p.opp_first.size() * 4);
+  L.opp_perm = take(p.opp_perm.size() * 4);
+  L.cl_tile_begin = take(p.cl_tile_begin.size() * 4);
+  L.tiles = take(p.tiles.size() * sizeof(TileDesc));
+  L.tex = take(p.tex.size() * 4);
+  L.gid = take(p.gid.size() * 4);
+  L.loc = take(p.cfg.lb == 1 ? p.loc8.size() : p.loc.size() * 2);
+  L.total = o;
+  return L;
+}
+int slots_of(int queue_depth, int device_ring) { return queue_depth > 0 ? queue_depth : (device_ring > 0 ? device_ring : 4); }
+size_t total_workspace(const Plan& p) {
+  return index_layout(p).total + size_t(slots_of(p.queue_depth, p.device_ring)) * slot_capacity_layout(p, p.maxB).total;
 }
 
 enum SlotState { SLOT_FREE = 0, SLOT_SUBMITTED = 1, SLOT_POPPED = 2 };
@@ -544,27 +544,128 @@ struct Slot {
   std::vector<int32_t> ids, row_begin, tt_row_begin;
   long long rows = 0, vt_nnz = 0, vv_nnz = 0, tt_rows = 0;
   SlotLayout used;  // section offsets of this batch
+  float prep_ms = 0.f;
+  std::chrono::steady_clock::time_point t_submit;
 };
 
 }  // namespace
 
+struct gale_plan {
+  std::unique_ptr<Plan> plan;
+};
+
 struct gale_mesh {
   std::unique_ptr<Plan> plan;
   int dim = 0, D = 0, maxB = 0, queue_depth = 0;
+  bool stream_ordered = false;
   DeviceMesh dm{};
   std::vector<std::unique_ptr<Slot>> slots;
   SlotLayout cap;
   cudaStream_t side = nullptr;
   // Consecutive batches are launched in turn on these library-owned streams, each ordered after the
-  // caller's stream at the time of the call: a batch is 3.7 waves of resident blocks, and the draining
-  // tail of one launch + the launch gap (measured: 15 of 79 us) overlap the next launch instead.
+  // caller's stream at the time of the call: a batch is a few waves of resident blocks, and the draining
+  // tail of one launch + the launch gap overlap the next launch instead. With GALE_STREAM_ORDERED the
+  // kernels run on the caller's stream itself.
   static constexpr int kLaunchStreams = 2;
   cudaStream_t launch[kLaunchStreams] = {nullptr, nullptr};
   int32_t* h_err = nullptr;  // mapped pinned; the kernels write guard codes here
   std::atomic<long long> submitted{0}, popped{0};
-  size_t workspace_used = 0;
+  size_t workspace_used = 0, index_bytes = 0;
   double create_ms = 0;
 };
+
+namespace {
+void free_mesh(gale_mesh* m) {  // also the error path of create: releases whatever exists so far
+  if (!m) return;
+  if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
+  for (cudaStream_t& ls : m->launch)
+    if (ls) { cudaStreamSynchronize(ls); cudaStreamDestroy(ls); ls = nullptr; }
+  for (auto& s : m->slots) {
+    if (s->pinned) cudaFreeHost(s->pinned);
+    if (s->ev_submit) cudaEventDestroy(s->ev_submit);
+    if (s->ev_start) cudaEventDestroy(s->ev_start);
+    if (s->ev_done) cudaEventDestroy(s->ev_done);
+    if (s->ev_ready) cudaEventDestroy(s->ev_ready);
+  }
+  if (m->h_err) cudaFreeHost(m->h_err);
+  cudaGetLastError();
+  delete m;
+}
+
+int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_bytes, cudaStream_t st, gale_mesh_t** out) {
+  if (!d_workspace || reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return GALE_ERR_WORKSPACE;
+  if (total_workspace(*p) > workspace_bytes) return GALE_ERR_WORKSPACE;
+  const auto t0 = std::chrono::steady_clock::now();
+  gale_mesh* m = new gale_mesh();
+  struct Guard { gale_mesh* m; ~Guard() { free_mesh(m); } } guard{m};
+  m->dim = p->dim; m->D = p->dim + 1; m->maxB = p->maxB; m->queue_depth = p->queue_depth;
+  m->stream_ordered = (p->flags & GALE_STREAM_ORDERED) != 0;
+  char* base = static_cast<char*>(d_workspace);
+  const IndexLayout IL = index_layout(*p);
+  auto put = [&](size_t at, const void* src, size_t bytes) -> int {
+    if (bytes) GALE_CUDA(cudaMemcpyAsync(base + at, src, bytes, cudaMemcpyHostToDevice, st));
+    return GALE_OK;
+  };
+  int rc;
+  if ((rc = put(IL.first_tet, p->first_tet.data(), p->first_tet.size() * 4)) ||
+      (rc = put(IL.opp_first, p->opp_first.data(), p->opp_first.size() * 4)) ||
+      (rc = put(IL.opp_perm, p->opp_perm.data(), p->opp_perm.size() * 4)) ||
+      (rc = put(IL.cl_tile_begin, p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4)) ||
+      (rc = put(IL.tiles, p->tiles.data(), p->tiles.size() * sizeof(TileDesc))) ||
+      (rc = put(IL.tex, p->tex.data(), p->tex.size() * 4)) || (rc = put(IL.gid, p->gid.data(), p->gid.size() * 4)) ||
+      (rc = p->cfg.lb == 1 ? put(IL.loc, p->loc8.data(), p->loc8.size()) : put(IL.loc, p->loc.data(), p->loc.size() * 2)))
+    return rc;
+  m->dm.T = p->dT;
+  m->dm.first_tet = reinterpret_cast<int32_t*>(base + IL.first_tet);
+  m->dm.opp_first = reinterpret_cast<int32_t*>(base + IL.opp_first);
+  m->dm.opp_perm = reinterpret_cast<int32_t*>(base + IL.opp_perm);
+  m->dm.cluster_tile_begin = reinterpret_cast<int32_t*>(base + IL.cl_tile_begin);
+  m->dm.tiles = reinterpret_cast<TileDesc*>(base + IL.tiles);
+  m->dm.tex = reinterpret_cast<int32_t*>(base + IL.tex);
+  m->dm.gid = reinterpret_cast<int32_t*>(base + IL.gid);
+  m->dm.loc = base + IL.loc;
+  m->index_bytes = IL.total;
+  // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
+  GALE_CUDA(cudaStreamSynchronize(st));
+  std::vector<int32_t>().swap(p->opp_perm);
+  std::vector<int32_t>().swap(p->tex);
+  std::vector<int32_t>().swap(p->gid);
+  std::vector<uint16_t>().swap(p->loc);
+  std::vector<uint8_t>().swap(p->loc8);
+  std::vector<int32_t>().swap(p->opp_first);
+
+  GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
+  *m->h_err = 0;
+  GALE_CUDA(cudaHostGetDevicePointer(reinterpret_cast<void**>(&m->dm.err), m->h_err, 0));
+
+  m->cap = slot_capacity_layout(*p, m->maxB);
+  const int nslots = slots_of(p->queue_depth, p->device_ring);
+  size_t o = IL.total;
+  for (int i = 0; i < nslots; ++i) {
+    auto s = std::make_unique<Slot>();
+    s->dev = base + o;
+    o += m->cap.total;
+    Slot* sp = s.get();
+    m->slots.push_back(std::move(s));  // owned by the handle from here on (error paths free it)
+    if (p->queue_depth > 0) GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&sp->pinned), std::max<size_t>(m->cap.total, 16), cudaHostAllocDefault));
+    GALE_CUDA(cudaEventCreateWithFlags(&sp->ev_submit, cudaEventDisableTiming));
+    GALE_CUDA(cudaEventCreate(&sp->ev_start));
+    GALE_CUDA(cudaEventCreate(&sp->ev_done));
+    GALE_CUDA(cudaEventCreate(&sp->ev_ready));
+  }
+  if (o > workspace_bytes) return GALE_ERR_WORKSPACE;  // cannot happen: total_workspace() uses the same layout
+  m->workspace_used = o;
+  if (p->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
+  if (!m->stream_ordered)
+    for (int i = 0; i < gale_mesh::kLaunchStreams; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
+  GALE_CUDA(allow_max_smem(kernel_for(m->D, p->NT, false, p->cfg.lb)));
+  m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() + p->analyse_ms;
+  m->plan = std::move(p);
+  guard.m = nullptr;
+  *out = m;
+  return GALE_OK;
+}
+}  // namespace
 
 extern "C" {
 
@@ -586,16 +687,42 @@ const char* gale_status_string(int32_t s) {
 }
 const char* gale_last_error(void) { return g_last_error.c_str(); }
 
-int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t* desc, size_t* out_bytes) {
-  if (!out_bytes) return GALE_ERR_INVALID_ARG;
+int32_t gale_plan_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_plan_t** out) {
+  if (!out) return GALE_ERR_INVALID_ARG;
   int rc = check_desc(desc);
   if (rc != GALE_OK) return rc;
   if ((rc = check_device()) != GALE_OK) return rc;
   std::unique_ptr<Plan> p;
-  if ((rc = analyse(*desc, nullptr, p)) != GALE_OK) return rc;
-  *out_bytes = total_workspace(*p, *desc);
-  std::lock_guard<std::mutex> lk(g_plan_mutex);
-  g_plan_cache = std::move(p);
+  if ((rc = analyse(*desc, static_cast<cudaStream_t>(cuda_stream), p)) != GALE_OK) return rc;
+  *out = new gale_plan{std::move(p)};
+  return GALE_OK;
+}
+
+int32_t gale_plan_workspace_bytes(const gale_plan_t* plan, size_t* out_bytes) {
+  if (!plan || !plan->plan || !out_bytes) return GALE_ERR_INVALID_ARG;
+  *out_bytes = total_workspace(*plan->plan);
+  return GALE_OK;
+}
+
+int32_t gale_plan_destroy(gale_plan_t* plan) {
+  if (!plan) return GALE_ERR_INVALID_ARG;
+  delete plan;
+  return GALE_OK;
+}
+
+int32_t gale_mesh_create_planned(gale_plan_t* plan, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                                 gale_mesh_t** out) {
+  if (!plan || !plan->plan || !out) return GALE_ERR_INVALID_ARG;
+  return build_mesh(std::move(plan->plan), d_workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream), out);
+}
+
+int32_t gale_mesh_workspace_bytes(const gale_mesh_desc_t* desc, void* cuda_stream, size_t* out_bytes) {
+  if (!out_bytes) return GALE_ERR_INVALID_ARG;
+  gale_plan_t* plan = nullptr;
+  int rc = gale_plan_create(desc, cuda_stream, &plan);
+  if (rc != GALE_OK) return rc;
+  *out_bytes = total_workspace(*plan->plan);
+  delete plan;
   return GALE_OK;
 }
 
@@ -603,76 +730,12 @@ int32_t gale_mesh_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_m
   if (!out) return GALE_ERR_INVALID_ARG;
   int rc = check_desc(desc);
   if (rc != GALE_OK) return rc;
-  if ((rc = check_device()) != GALE_OK) return rc;
   if (!desc->d_workspace || reinterpret_cast<uintptr_t>(desc->d_workspace) % kAlign) return GALE_ERR_WORKSPACE;
-  const auto t0 = std::chrono::steady_clock::now();
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  std::unique_ptr<Plan> p;
-  {
-    std::lock_guard<std::mutex> lk(g_plan_mutex);
-    if (g_plan_cache && plan_matches(*g_plan_cache, *desc)) p = std::move(g_plan_cache);
-    g_plan_cache.reset();
-  }
-  if (!p && (rc = analyse(*desc, st, p)) != GALE_OK) return rc;
-  if (total_workspace(*p, *desc) > desc->workspace_bytes) return GALE_ERR_WORKSPACE;
-
-  auto m = std::make_unique<gale_mesh>();
-  m->dim = desc->dim; m->D = desc->dim + 1; m->maxB = desc->max_batch_clusters; m->queue_depth = desc->queue_depth;
-  char* base = static_cast<char*>(desc->d_workspace);
-  size_t o = 0;
-  auto put = [&](const void* src, size_t bytes, size_t pad = 0) -> void* {
-    void* dst = base + o;
-    if (bytes) cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
-    o = up(o + bytes + pad);
-    return dst;
-  };
-  m->dm.T = desc->d_simplices;
-  m->dm.first_tet = static_cast<int32_t*>(put(p->first_tet.data(), p->first_tet.size() * 4));
-  m->dm.opp_first = static_cast<int32_t*>(put(p->opp_first.data(), p->opp_first.size() * 4));
-  m->dm.opp_perm = static_cast<int32_t*>(put(p->opp_perm.data(), p->opp_perm.size() * 4));
-  m->dm.cluster_tile_begin = static_cast<int32_t*>(put(p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4));
-  m->dm.tiles = static_cast<TileDesc*>(put(p->tiles.data(), p->tiles.size() * sizeof(TileDesc), 16));
-  m->dm.tex = static_cast<int32_t*>(put(p->tex.data(), p->tex.size() * 4, 16));
-  m->dm.gid = static_cast<int32_t*>(put(p->gid.data(), p->gid.size() * 4, 16));
-  m->dm.hft = static_cast<int2*>(put(p->hft.data(), p->hft.size() * sizeof(int2), 16));
-  m->dm.loc = p->cfg.lb == 1 ? put(p->loc8.data(), p->loc8.size(), 64) : put(p->loc.data(), p->loc.size() * 2, 64);
-  GALE_CUDA(cudaGetLastError());
-  // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
-  GALE_CUDA(cudaStreamSynchronize(st));
-  std::vector<int32_t>().swap(p->opp_perm);
-  std::vector<int32_t>().swap(p->tex);
-  std::vector<int32_t>().swap(p->gid);
-  std::vector<int2>().swap(p->hft);
-  std::vector<uint16_t>().swap(p->loc);
-  std::vector<uint8_t>().swap(p->loc8);
-  std::vector<int32_t>().swap(p->opp_first);
-
-  GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
-  *m->h_err = 0;
-  GALE_CUDA(cudaHostGetDevicePointer(reinterpret_cast<void**>(&m->dm.err), m->h_err, 0));
-
-  m->cap = slot_capacity_layout(*p, m->maxB);
-  const int nslots = desc->queue_depth > 0 ? desc->queue_depth : (desc->device_ring > 0 ? desc->device_ring : 4);
-  for (int i = 0; i < nslots; ++i) {
-    auto s = std::make_unique<Slot>();
-    s->dev = base + o;
-    o += m->cap.total;
-    if (desc->queue_depth > 0) GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&s->pinned), m->cap.total, cudaHostAllocDefault));
-    GALE_CUDA(cudaEventCreateWithFlags(&s->ev_submit, cudaEventDisableTiming));
-    GALE_CUDA(cudaEventCreate(&s->ev_start));
-    GALE_CUDA(cudaEventCreate(&s->ev_done));
-    GALE_CUDA(cudaEventCreateWithFlags(&s->ev_ready, cudaEventDisableTiming));
-    m->slots.push_back(std::move(s));
-  }
-  m->workspace_used = o;
-  if (desc->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
-  for (int i = 0; i < gale_mesh::kLaunchStreams; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
-  GALE_CUDA(cudaFuncSetAttribute(kernel_for(m->D, p->NT, false, p->cfg.lb), cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
-  m->plan = std::move(p);
-  m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() +
-                 (m->plan->analyse_ms);
-  *out = m.release();
-  return GALE_OK;
+  gale_plan_t* plan = nullptr;
+  if ((rc = gale_plan_create(desc, cuda_stream, &plan)) != GALE_OK) return rc;
+  rc = build_mesh(std::move(plan->plan), desc->d_workspace, desc->workspace_bytes, static_cast<cudaStream_t>(cuda_stream), out);
+  delete plan;
+  return rc;
 }
 
 int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
@@ -690,6 +753,7 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   out->create_ms = m->create_ms;
   out->local_id_bytes = p.cfg.lb;
   out->block_threads = p.NT;
+  out->index_bytes = m->index_bytes;
   return GALE_OK;
 }
 
@@ -707,6 +771,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   if (s.state.load(std::memory_order_acquire) != SLOT_FREE) return GALE_ERR_WOULD_BLOCK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const int D = m->D;
+  const auto t_prep = std::chrono::steady_clock::now();
 
   // batch set-up (a0): row / nnz bases of every requested cluster, in request order
   s.seq = seq; s.n = n_clusters; s.mask = relation_mask;
@@ -755,9 +820,11 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
 #endif
   const int smem = lay.total;
   // everything the caller enqueued on its stream so far (e.g. the upload of the simplices) comes first
-  cudaStream_t run = m->launch[seq % gale_mesh::kLaunchStreams];
-  GALE_CUDA(cudaEventRecord(s.ev_submit, st));
-  GALE_CUDA(cudaStreamWaitEvent(run, s.ev_submit, 0));
+  cudaStream_t run = m->stream_ordered ? st : m->launch[seq % gale_mesh::kLaunchStreams];
+  if (!m->stream_ordered) {
+    GALE_CUDA(cudaEventRecord(s.ev_submit, st));
+    GALE_CUDA(cudaStreamWaitEvent(run, s.ev_submit, 0));
+  }
   GALE_CUDA(cudaEventRecord(s.ev_start, run));
   for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
     gale::BatchParams P{};
@@ -789,6 +856,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
     if (s.used.total) GALE_CUDA(cudaMemcpyAsync(s.pinned, s.dev, s.used.total, cudaMemcpyDeviceToHost, m->side));
     GALE_CUDA(cudaEventRecord(s.ev_ready, m->side));
   }
+  s.t_submit = std::chrono::steady_clock::now();
+  s.prep_ms = std::chrono::duration<float, std::milli>(s.t_submit - t_prep).count();
   s.state.store(SLOT_SUBMITTED, std::memory_order_release);
   m->submitted.store(seq + 1);
   return GALE_OK;
@@ -841,6 +910,11 @@ int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_m
   float ms = 0.f;
   if (cudaEventElapsedTime(&ms, s.ev_start, s.ev_done) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }
   out->kernel_ms = ms;
+  ms = 0.f;
+  if (m->queue_depth > 0 && cudaEventElapsedTime(&ms, s.ev_done, s.ev_ready) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }
+  out->d2h_ms = ms;  // includes the time the copy waited for earlier copies on the side stream
+  out->prep_ms = s.prep_ms;
+  out->queue_ms = std::chrono::duration<float, std::milli>(std::chrono::steady_clock::now() - s.t_submit).count();
   out->slot = int32_t(seq % (long long)m->slots.size());
   s.state.store(SLOT_POPPED, std::memory_order_release);
   m->popped.store(seq + 1);
@@ -861,19 +935,7 @@ int32_t gale_destroy(gale_mesh_t* m) {
     if (s->ev_done) cudaEventSynchronize(s->ev_done);
     if (m->queue_depth > 0 && s->ev_ready && s->state.load() != SLOT_FREE) cudaEventSynchronize(s->ev_ready);
   }
-  if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
-  for (cudaStream_t& ls : m->launch)
-    if (ls) { cudaStreamSynchronize(ls); cudaStreamDestroy(ls); ls = nullptr; }
-  for (auto& s : m->slots) {
-    if (s->pinned) cudaFreeHost(s->pinned);
-    if (s->ev_submit) cudaEventDestroy(s->ev_submit);
-    if (s->ev_start) cudaEventDestroy(s->ev_start);
-    if (s->ev_done) cudaEventDestroy(s->ev_done);
-    if (s->ev_ready) cudaEventDestroy(s->ev_ready);
-  }
-  if (m->h_err) cudaFreeHost(m->h_err);
-  cudaGetLastError();
-  delete m;
+  free_mesh(m);
   return GALE_OK;
 }
 

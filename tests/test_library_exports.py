@@ -39,17 +39,17 @@ def test_status_strings(lib):
 def test_struct_layout_matches_header():
     # sizes implied by include/gale.h on LP64
     assert ctypes.sizeof(gale.gale_mesh_desc_t) == 80
-    assert ctypes.sizeof(gale.gale_batch_view_t) == 136
-    assert ctypes.sizeof(gale.gale_mesh_info_t) == 72      # gcc sizeof(gale_mesh_info_t) of include/gale.h
+    assert ctypes.sizeof(gale.gale_batch_view_t) == 152
+    assert ctypes.sizeof(gale.gale_mesh_info_t) == 80      # gcc sizeof(gale_mesh_info_t) of include/gale.h
 
 
 def test_argument_errors_without_gpu(lib):
     # null / malformed descriptors are refused before any CUDA call
     out = ctypes.c_size_t()
-    assert lib.gale_mesh_workspace_bytes(None, ctypes.byref(out)) == gale.ERR_INVALID_ARG
+    assert lib.gale_mesh_workspace_bytes(None, None, ctypes.byref(out)) == gale.ERR_INVALID_ARG
     d = gale.gale_mesh_desc_t()
     d.dim = 5
-    assert lib.gale_mesh_workspace_bytes(ctypes.byref(d), ctypes.byref(out)) == gale.ERR_INVALID_ARG
+    assert lib.gale_mesh_workspace_bytes(ctypes.byref(d), None, ctypes.byref(out)) == gale.ERR_INVALID_ARG
     assert lib.gale_destroy(None) == gale.ERR_INVALID_ARG
     assert lib.gale_queue_pop(None, None, 0) == gale.ERR_INVALID_ARG
 
