@@ -177,6 +177,8 @@ def main():
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--streams", type=int, default=1,
                     help="CUDA streams the batches are submitted on in turn (consecutive batches overlap)")
+    ap.add_argument("--mask", type=int, default=7, help="relation mask of the device-timed pass (1 VT, 2 VV, 4 TT); "
+                    "the bench line of record uses 7, other values are for per-relation diagnosis")
     ap.add_argument("--impl", default="gale", choices=["gale", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -218,7 +220,7 @@ def main():
         """Submit every batch; pop/release lagging by the ring so the GPU always has work queued."""
         inflight = 0
         for i, ids in enumerate(batches):
-            while g.compute(ids, stream=sub_streams[i % len(sub_streams)]) == gale.ERR_WOULD_BLOCK:
+            while g.compute(ids, args.mask, stream=sub_streams[i % len(sub_streams)]) == gale.ERR_WOULD_BLOCK:
                 st, v = g.pop(-1)
                 if record:
                     kernel_ms.append(v.kernel_ms)

@@ -74,6 +74,14 @@ struct TileDesc {
 };
 static_assert(sizeof(TileDesc) == 80, "TileDesc layout");
 
+// What one warp works out for the block and leaves in shared memory: the tile's record and where its
+// rows / entries go in the batch's output arrays.
+struct BlockCtx {
+  TileDesc td;
+  int32_t row0, vt0, vv0, tt0, tt_slot, tile, pad0, pad1;
+};
+static_assert(sizeof(BlockCtx) == 112, "BlockCtx layout");
+
 // Device-resident index built by gale_mesh_create (all pointers DEVICE).
 struct DeviceMesh {
   const int32_t* T;                   // [nT*D] canonical simplices (caller's array)
@@ -108,10 +116,10 @@ struct SmemCfg {
 // Byte offsets of the shared-memory regions, computed on the host (make_layout) and passed as a
 // kernel parameter.
 struct SmemLayout {
-  int mbar, tets, texid, gid, ft, offT, offV, runpos, tbo, scan, misc;
-  int bmT, bmV, zero_end;   // cleared to 0
+  int mbar, ctx, tets, texid, gid, ft, offT, offV, runpos, tbo, scan, misc;
+  int bmT, bmV, dflag, zero_end;   // cleared to 0
   int pfx;
-  int tbl, ttrow, ones_end; // cleared to all-ones (empty table word, "no neighbour")
+  int tbl, ttres, ones_end; // cleared to all-ones (empty table word, "no neighbour" = -1)
   int st_vt, st_vv, fbq;
   int total;
 };
@@ -123,6 +131,7 @@ __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   SmemLayout L;
   int o = 0;
   L.mbar = o;   o = align16(o + 8);
+  L.ctx = o;    o = align16(o + 112);
   L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
@@ -135,13 +144,21 @@ __host__ __device__ inline SmemLayout make_layout(const SmemCfg& c) {
   L.misc = o;   o = align16(o + 16);
   L.bmT = o;    o = align16(o + c.tv * c.WT * 4);
   L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
+  L.dflag = o;  o = align16(o + (c.tbl ? c.sext : 0));
   L.zero_end = o;
   L.pfx = o;    o = align16(o + c.tv * c.WT * 2);
-  L.tbl = o;    o = align16(o + c.tbl * 4);
-  L.ttrow = o;  o = align16(o + (c.tbl ? c.smax * D * 2 : 0));
+  {
+    // The VT / VV staging areas are written after the facet tables are dead (P3b): with TT they share
+    // the tables' bytes (the region is as large as the larger of the two uses).
+    const int b_vt = align16(c.vt_max ? (c.vt_max + 4) * 4 : 0), b_vv = align16(c.vv_max ? (c.vv_max + 4) * 4 : 0);
+    const int b_tbl = align16(c.tbl * 4);
+    L.tbl = o;
+    L.st_vt = o;
+    L.st_vv = o + b_vt;
+    o += b_tbl > b_vt + b_vv ? b_tbl : b_vt + b_vv;
+  }
+  L.ttres = o;  o = align16(o + (c.tbl ? (c.sext + c.sint * D) * 4 : 0));
   L.ones_end = o;
-  L.st_vt = o;  o = align16(o + (c.vt_max ? (c.vt_max + 4) * 4 : 0));
-  L.st_vv = o;  o = align16(o + (c.vv_max ? (c.vv_max + 4) * 4 : 0));
   L.fbq = o;    o = align16(o + c.sint * 2);
   L.total = o;
   return L;
@@ -232,6 +249,16 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+// atomicOr without return value on a 32-bit shared-window address, predicated instead of branched
+// (SASS: @P ATOMS.OR RZ): lanes whose vertex lies outside the tile skip it without a divergent region.
+__device__ __forceinline__ void red_or_shared_if(bool p, uint32_t saddr, uint32_t v) {
+  asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q red.shared.or.b32 [%1], %2;\n}" ::"r"((uint32_t)p), "r"(saddr), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ void st_shared_if(bool p, uint32_t saddr, int32_t v) {
+  asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.b32 [%1], %2;\n}" ::"r"((uint32_t)p), "r"(saddr), "r"(v) : "memory");
+}
 
 // Local vertex ids of staged simplex s (LB bytes each).
 template <int LB>
@@ -335,27 +362,47 @@ struct FacetBits {
   static constexpr uint32_t kIdxMask = (1u << (30 - kKeyBits)) - 1u;
 };
 
+// Where the TT results of a tile live in shared memory, as GLOBAL simplex ids (-1 = none):
+//   [entry 0 of every external simplex: xpad words][D entries of every internal simplex]
+struct TTRes {
+  int32_t* res;
+  const int32_t* texid;
+  int s_ext, xpad, t_lo;
+  int cap;  // words (bounds-checked build)
+};
+
 // Place facet k of staged simplex s with key `key` in the table [tbl, tbl+m): claim an empty slot, or
 // meet the record that holds the same key (the other coface) and write both TT entries.
 template <int D>
-__device__ __forceinline__ void facet_place(uint32_t* tbl, uint32_t m, uint32_t key, int s, int k, uint16_t* ttrow,
+__device__ __forceinline__ void facet_place(uint32_t* tbl, uint32_t m, uint32_t key, int s, int k, const TTRes& R,
                                             int s_all, int32_t* err) {
   using FB = FacetBits<D>;
   if (!GALE_IN_BOUNDS(err, m > 0 && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D && s < s_all)) return;
   const uint32_t word = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
   uint32_t h = __umulhi(key * 0x9E3779B1u, m);
-  for (uint32_t probe = 0;; ++probe) {
+#if GALE_CHECK_BOUNDS
+  uint32_t probe = 0;
+#endif
+  for (;;) {  // a table has at least as many slots as records: an empty slot or the key is always met
     const uint32_t old = atomicCAS(tbl + h, kEmpty32, word);
     if (old == kEmpty32) return;
     if ((old & FB::kKeyMask) == key) {
       const int s2 = (int)((old >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(old >> 30);
       if (!GALE_IN_BOUNDS(err, s2 < s_all && k2 < D)) return;
-      ttrow[s * D + k] = (uint16_t)s2;
-      ttrow[s2 * D + k2] = (uint16_t)s;
+      // an external simplex only ever records its facet 0
+      const int i1 = s < R.s_ext ? s : R.xpad + (s - R.s_ext) * D + k;
+      const int i2 = s2 < R.s_ext ? s2 : R.xpad + (s2 - R.s_ext) * D + k2;
+      const int g1 = s < R.s_ext ? R.texid[s] : R.t_lo + (s - R.s_ext);
+      const int g2 = s2 < R.s_ext ? R.texid[s2] : R.t_lo + (s2 - R.s_ext);
+      if (!GALE_IN_BOUNDS(err, i1 >= 0 && i1 < R.cap && i2 >= 0 && i2 < R.cap)) return;
+      R.res[i1] = g2;
+      R.res[i2] = g1;
       return;
     }
     h = h + 1 == m ? 0u : h + 1;
-    if (probe >= m) { raise_err(err, ERR_TT_TABLE_FULL); return; }
+#if GALE_CHECK_BOUNDS
+    if (++probe >= m) { raise_err(err, ERR_TT_TABLE_FULL); return; }
+#endif
   }
 }
 
@@ -398,46 +445,85 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   const bool do_vt = !COUNT && (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0;
   const bool do_tt = !COUNT && (mask & REL_TT) != 0;
 
-  // ---- block -> (cluster slot, tile) ----------------------------------------------------------
-  int slot = 0, tile;
-  if (COUNT) {
-    tile = P.tile_base + (int)blockIdx.x;
-  } else {
+  // ---- block -> (cluster slot, tile): worked out by the first warp, shared through BlockCtx ------
+  if (!COUNT) {
     if (blockIdx.x == 0 && tid == 0) {  // terminal offsets (also covers batches without rows)
       if (do_vt) { O.vt_offsets[0] = 0; O.vt_offsets[P.total_rows] = P.total_vt_nnz; }
       if (do_vv) { O.vv_offsets[0] = 0; O.vv_offsets[P.total_rows] = P.total_vv_nnz; }
     }
     if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
-    if (P.uniform_tiles > 0) {
-      slot = (int)blockIdx.x / P.uniform_tiles;
+  }
+  BlockCtx* ctx = reinterpret_cast<BlockCtx*>(smem + L.ctx);
+  void* bar = smem + L.mbar;
+  if (tid < 32) {
+    int slot = 0, tile;
+    if (COUNT) {
+      tile = P.tile_base + (int)blockIdx.x;
     } else {
-      int lo = 0, hi = P.n_clusters;
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+      if (P.uniform_tiles > 0) {
+        slot = (int)blockIdx.x / P.uniform_tiles;
+      } else {
+        int lo = 0, hi = P.n_clusters;
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+        }
+        slot = lo;
       }
-      slot = lo;
+      tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
     }
-    tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
+    if (lane < (int)(sizeof(TileDesc) / 16))
+      reinterpret_cast<int4*>(&ctx->td)[lane] = __ldg(reinterpret_cast<const int4*>(M.tiles + tile) + lane);
+    __syncwarp();
+    if (lane == 0) {
+      const TileDesc& t = ctx->td;
+      ctx->tile = tile;
+      if (!COUNT) {
+        ctx->row0 = P.row_base[slot] + t.row_rel;
+        ctx->vt0 = P.vt_base[slot] + t.vt_rel;
+        ctx->vv0 = P.vv_base[slot] + t.vv_rel;
+        ctx->tt0 = P.tt_base[slot] + t.tt_rel;
+        ctx->tt_slot = P.tt_base[slot];
+      }
+      // P0a: stage the tile's lists with TMA bulk copies; completion is counted on the mbarrier
+      const int S0 = t.s_int + t.s_ext;
+      mbar_init(bar, 1);
+      fence_proxy_async();
+      const uint32_t b_t = (uint32_t)((S0 + 3) & ~3) * (4u * LB);
+      const uint32_t b_x = COUNT ? 0u : (uint32_t)((t.s_ext + 3) & ~3) * 4u;
+      const uint32_t b_g = (!COUNT && (do_vv || do_tt)) ? (uint32_t)((t.nloc + 3) & ~3) * 4u : 0u;
+      mbar_arrive_expect_tx(bar, b_t + b_x + b_g);
+      if (b_t) bulk_g2s(smem + L.tets, static_cast<const unsigned char*>(M.loc) + t.stg_off * (4 * LB), b_t, bar);
+      if (b_x) bulk_g2s(smem + L.texid, M.tex + t.tex_off, b_x, bar);
+      if (b_g) bulk_g2s(smem + L.gid, M.gid + t.gid_off, b_g, bar);
+    }
   }
-  TileDesc td;
+  // P0b: clear (needs nothing of the tile's record)
   {
-    const int4* src = reinterpret_cast<const int4*>(M.tiles + tile);
-    int4* dst = reinterpret_cast<int4*>(&td);
-#pragma unroll
-    for (int i = 0; i < (int)(sizeof(TileDesc) / 16); ++i) dst[i] = __ldg(src + i);
+    int4* z = reinterpret_cast<int4*>(smem + L.bmT);
+    const int n16 = (L.zero_end - L.bmT) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
   }
+  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
+    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
+    const int n16 = (L.ones_end - L.tbl) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
+  }
+  if (tid == 0) { reinterpret_cast<uint32_t*>(smem + L.misc)[0] = 0u; reinterpret_cast<uint32_t*>(smem + L.misc)[1] = 0u; }
+  __syncthreads();
+  const TileDesc& td = ctx->td;
+  const int tile = ctx->tile;
   const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
   const int S = s_int + s_ext;
   const int WT = C.WT, WV = C.WV;
   const int wT = (S + 31) >> 5, wV = (td.nloc + 31) >> 5;
 #if GALE_CHECK_BOUNDS
   {
-    bool ok = nrows >= 0 && nrows <= C.tv && NT >= C.tv && S >= 0 && S <= C.smax && td.nloc <= C.nloc && nlo >= 0 &&
+    bool ok = nrows >= 0 && nrows <= C.tv && NT >= C.tv && S >= 0 && S <= C.smax && nlo >= 0 &&
               nlo + nrows <= td.nloc && wT <= WT;
-    if (!COUNT) ok = ok && s_ext <= C.sext;
+    if (!COUNT) ok = ok && s_ext <= C.sext && td.nloc <= C.nloc;  // count mode stages neither T_ex ids nor the vertex table
     if (mask & REL_VV) ok = ok && wV <= WV;
-    if (do_tt) ok = ok && s_int <= C.sint && td.vt_nnz + (D - 2) * s_int <= C.tbl;
+    if (do_tt) ok = ok && s_int <= C.sint && ((s_ext + 3) & ~3) <= C.sext && td.vt_nnz + (D - 2) * s_int <= C.tbl;
     if (do_vt) ok = ok && td.vt_nnz <= C.vt_max;
     if (!COUNT && (mask & REL_VV)) ok = ok && td.vv_nnz <= C.vv_max;
     if (!ok) {  // block-uniform: leave before anything is staged
@@ -461,74 +547,68 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
   uint16_t* pfx = reinterpret_cast<uint16_t*>(smem + L.pfx);      // set bits of the row before word w
   uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
-  uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);  // [S][D] neighbours as staged indices, 0xFFFF = none
+  unsigned char* dflag = smem + L.dflag;  // external simplex s: this tile writes its TT entry 0 (see P4)
+  TTRes R;                                // TT results as global ids, -1 = none
+  R.res = reinterpret_cast<int32_t*>(smem + L.ttres);
+  R.texid = texid; R.s_ext = s_ext; R.xpad = (s_ext + 3) & ~3; R.t_lo = t_lo;
+  R.cap = C.sext + C.sint * D;
   int32_t* st_vt = reinterpret_cast<int32_t*>(smem + L.st_vt);
   int32_t* st_vv = reinterpret_cast<int32_t*>(smem + L.st_vv);
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
-  void* bar = smem + L.mbar;
 
-  const int row0 = P.row_base[slot] + td.row_rel;
-  const int vt0 = P.vt_base[slot] + td.vt_rel;
-  const int vv0 = P.vv_base[slot] + td.vv_rel;
-  const int tt0 = P.tt_base[slot] + td.tt_rel;
+  const int row0 = ctx->row0, vt0 = ctx->vt0, vv0 = ctx->vv0, tt0 = ctx->tt0;
   const int mis_vt = vt0 & 3, mis_vv = vv0 & 3;  // 16-byte phase of the tile's output segments
-
-  // ---- P0: stage (TMA bulk copies) + clear -----------------------------------------------------
-  if (tid == 0) {
-    mbar_init(bar, 1);
-    fence_proxy_async();
-    const uint32_t b_t = (uint32_t)((S + 3) & ~3) * (4u * LB);
-    const uint32_t b_x = COUNT ? 0u : (uint32_t)((s_ext + 3) & ~3) * 4u;
-    const uint32_t b_g = (!COUNT && (do_vv || do_tt)) ? (uint32_t)((td.nloc + 3) & ~3) * 4u : 0u;
-    mbar_arrive_expect_tx(bar, b_t + b_x + b_g);
-    if (b_t) bulk_g2s(tets, static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB), b_t, bar);
-    if (b_x) bulk_g2s(texid, M.tex + td.tex_off, b_x, bar);
-    if (b_g) bulk_g2s(gid, M.gid + td.gid_off, b_g, bar);
-  }
-  for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);
-  {
-    int4* z = reinterpret_cast<int4*>(smem + L.bmT);
-    const int n16 = (L.zero_end - L.bmT) >> 4;
-    for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
-  }
-  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
-    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
-    const int n16 = (L.ones_end - L.tbl) >> 4;
-    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
-  }
-  if (tid == 0) { misc[0] = 0u; misc[1] = 0u; }
-  __syncthreads();
+  for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);  // read in P2, after a barrier
   mbar_wait(bar, 0);
 
   // ---- P1: VT incidence bits and VV bits, one thread per staged simplex ------------------------
+  const uint32_t aT = smem_u32(bmT), aV = smem_u32(bmV);
+  const uint32_t strideT = (uint32_t)WT * 4u, strideV = (uint32_t)WV * 4u;
+  // Consecutive staged simplices share most of their vertices at the same positions, so neighbouring
+  // lanes would OR into the same bitmap row in the same instruction (shared-memory atomics on one word
+  // serialise: measured 3.1 of 4.0 wavefronts per tet were such conflicts). Each lane therefore visits
+  // its vertices in an order rotated by its lane number (one PRMT on the packed 8-bit ids); the marking
+  // is symmetric in the position, only "k is not the lowest vertex" has to follow the rotation (k0).
+  int rot = 0, k0 = 0;
+  uint32_t rot_sel = 0x3210u;
+  if constexpr (LB == 1) {
+    rot = D == 4 ? (lane & 3) : (lane % 3);
+    k0 = rot == 0 ? 0 : D - rot;  // where the lowest vertex ends up
+    rot_sel = D == 4 ? ((0x32103210u >> (rot * 4)) & 0xFFFFu) : (rot == 0 ? 0x3210u : (rot == 1 ? 0x3021u : 0x3102u));
+  }
   for (int s = tid; s < S; s += NT) {
     int l[4];
-    load_local<LB>(tets, s, l);
+    if constexpr (LB == 1) {
+      const uint32_t q = __byte_perm(reinterpret_cast<const uint32_t*>(tets)[s], 0u, rot_sel);
+      l[0] = q & 0xFF; l[1] = (q >> 8) & 0xFF; l[2] = (q >> 16) & 0xFF; l[3] = q >> 24;
+    } else {
+      load_local<LB>(tets, s, l);
+    }
 #if GALE_CHECK_BOUNDS
     for (int k = 0; k < D; ++k)
       if (!GALE_IN_BOUNDS(M.err, l[k] >= 0 && l[k] < td.nloc)) l[k] = nlo;  // keep later indexing inside the row
-    if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
+    if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[k0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
 #endif
-    uint32_t* col = bmT + (s >> 5);
+    const uint32_t col = aT + (uint32_t)(s >> 5) * 4u;
     const uint32_t bit = 1u << (s & 31);
     int r[D];
 #pragma unroll
     for (int k = 0; k < D; ++k) r[k] = l[k] - nlo;
 #pragma unroll
-    for (int k = 1; k < D; ++k)
-      if ((unsigned)r[k] < (unsigned)nrows) atomicOr(col + r[k] * WT, bit);
+    for (int k = 0; k < D; ++k)
+      red_or_shared_if(k != k0 && (unsigned)r[k] < (unsigned)nrows, col + (uint32_t)r[k] * strideT, bit);
     if (do_vv) {
       uint32_t w[D], b[D];
 #pragma unroll
-      for (int j = 0; j < D; ++j) { w[j] = (uint32_t)l[j] >> 5; b[j] = 1u << (l[j] & 31); }
+      for (int j = 0; j < D; ++j) { w[j] = ((uint32_t)l[j] >> 5) * 4u; b[j] = 1u << (l[j] & 31); }
 #pragma unroll
-      for (int k = 0; k < D; ++k)
-        if ((unsigned)r[k] < (unsigned)nrows) {
-          uint32_t* row = bmV + r[k] * WV;
+      for (int k = 0; k < D; ++k) {
+        const bool in = (unsigned)r[k] < (unsigned)nrows;
+        const uint32_t row = aV + (uint32_t)r[k] * strideV;
 #pragma unroll
-          for (int j = 0; j < D; ++j)
-            if (j != k) atomicOr(row + w[j], b[j]);  // "each other vertex"
-        }
+        for (int j = 0; j < D; ++j)
+          if (j != k) red_or_shared_if(in, row + w[j], b[j]);  // "each other vertex"
+      }
     }
   }
   __syncthreads();
@@ -552,8 +632,22 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         for (int w = 0; w < wV; ++w) degv += __popc(rv[w]);
       }
     }
-    uint32_t tot;
-    const uint32_t ex = block_exclusive_scan<NT>(deg | (degv << 16), scan, &tot);
+    uint32_t tot = 0u, ex = 0u;
+    if (C.tv <= 32) {  // the rows fit one warp: no block-wide scan, no barriers
+      if (tid < 32) {
+        const uint32_t x = deg | (degv << 16);
+        uint32_t inc = x;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+          if (lane >= d) inc += y;
+        }
+        tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        ex = inc - x;
+      }
+    } else {
+      ex = block_exclusive_scan<NT>(deg | (degv << 16), scan, &tot);
+    }
     n_vt = (int)(tot & 0xFFFFu);
     n_vv = (int)(tot >> 16);
     if (tid < nrows) {
@@ -580,8 +674,59 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   if (tid == 0 && (((mask & REL_VT) && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
     raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
   __syncthreads();
+  n_vt = offT[nrows];  // (the scan's totals are only known to the scanning threads)
+  n_vv = offV[nrows];
 
-  // ---- P3: VV rows -> staging; per staged simplex: VT scatter by rank, TT facet records ---------
+  const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
+  const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
+  const int tile_hi = nlo + nrows;
+  // ---- P3a: TT facet records into the per-vertex tables -----------------------------------------
+  if (do_tt) {
+    // facet 0 of every staged simplex whose second vertex is a tile vertex
+    for (int s = tid; s < S; s += NT) {
+      int l[4];
+      load_local<LB>(tets, s, l);
+#if GALE_CHECK_BOUNDS
+      for (int k = 0; k < D; ++k)
+        if (l[k] < 0 || l[k] >= td.nloc) l[k] = nlo;  // reported in P1
+#endif
+      const int r1 = l[1] - nlo;
+      if ((unsigned)r1 < (unsigned)nrows) {  // facet 0 has lowest vertex l[1]
+        const int b0 = tbo[r1];
+        const uint32_t m = (uint32_t)(tbo[r1 + 1] - b0);
+        // an external simplex of this cluster: its own tile cannot see this facet, so this tile writes
+        // entry 0 of its TT row (P4)
+        if (s < s_ext && gid[l[0]] >= c_lo) dflag[s] = 1;
+        if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl))
+          facet_place<D>(tbl + b0, m, facet_key<D, 0>(l), s, 0, R, S, M.err);
+      }
+    }
+    // facets 1..D-1 of the internal simplices: their lowest vertex is l[0], a tile vertex. One thread per
+    // record, every lane busy.
+    const int nrec = (D - 1) * s_int;
+    for (int i = tid; i < nrec; i += NT) {
+      const int q = i / (D - 1);
+      const int k = 1 + (i - q * (D - 1));
+      const int s = s_ext + q;
+      int l[4];
+      load_local<LB>(tets, s, l);
+#if GALE_CHECK_BOUNDS
+      for (int kk = 0; kk < D; ++kk)
+        if (l[kk] < 0 || l[kk] >= td.nloc) l[kk] = nlo;
+#endif
+      const int r = l[0] - nlo;
+      if (!GALE_IN_BOUNDS(M.err, (unsigned)r < (unsigned)nrows)) continue;
+      uint32_t key;
+      if constexpr (D == 4) key = (uint32_t)(k == 1 ? l[2] : l[1]) | ((uint32_t)(k == 3 ? l[2] : l[3]) << 9);
+      else key = (uint32_t)(k == 1 ? l[2] : l[1]);
+      const int b0 = tbo[r];
+      const uint32_t m = (uint32_t)(tbo[r + 1] - b0);
+      if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl)) facet_place<D>(tbl + b0, m, key, s, k, R, S, M.err);
+    }
+    __syncthreads();  // the tables are dead from here on: the VT / VV staging areas reuse their bytes
+  }
+
+  // ---- P3b: VV rows -> staging; per staged simplex: VT scatter by rank ----------------------------
   if (do_vv && tid < nrows) {
     const uint32_t* row = bmV + tid * WV;
     int pos = mis_vv + my_offV;
@@ -595,11 +740,14 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       }
     }
   }
-  if (do_vt || do_tt) {
-    for (;;) {
-      int base = 0;
-      if (lane == 0) base = (int)atomicAdd(&misc[0], 32u);
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+  if (do_vt) {
+    // 32-simplex chunks go to the warps round-robin; the warps that expanded VV rows above sit out the
+    // first round (an expansion is about one chunk's work)
+    const int nexp = do_vv ? (nrows + 31) >> 5 : 0;
+    const uint32_t aSt = smem_u32(st_vt + mis_vt);
+    const int warp = tid >> 5;
+    for (int j = warp < nexp ? warp + NT / 32 : warp;; j += NT / 32) {
+      const int base = (j - nexp) << 5;
       if (base >= S) break;
       const int s = base + lane;
       if (s >= S) continue;
@@ -610,46 +758,22 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         if (l[k] < 0 || l[k] >= td.nloc) l[k] = nlo;  // reported in P1
 #endif
       const bool internal = s >= s_ext;
-      if (do_vt) {
-        const int g = internal ? t_lo + (s - s_ext) : texid[s];
-        const int w = s >> 5;
-        const uint32_t below = (1u << (s & 31)) - 1u;
+      const int g = internal ? t_lo + (s - s_ext) : texid[s];
+      const int w = s >> 5;
+      const uint32_t below = (1u << (s & 31)) - 1u;
 #pragma unroll
-        for (int k = 1; k < D; ++k) {
-          const int r = l[k] - nlo;
-          if ((unsigned)r < (unsigned)nrows) {
-            const int pos = offT[r] + (int)pfx[r * WT + w] + __popc(bmT[r * WT + w] & below);
-            if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max)) st_vt[mis_vt + pos] = g;
-          }
-        }
-        if (internal) {
-          const int r = l[0] - nlo;
-          if (GALE_IN_BOUNDS(M.err, (unsigned)r < (unsigned)nrows)) {
-            const int pos = runpos[r] + g;
-            if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max)) st_vt[mis_vt + pos] = g;
-          }
-        }
+      for (int k = 1; k < D; ++k) {  // branch-free: lanes outside the tile read row 0 and skip the store
+        const int r = l[k] - nlo;
+        const bool in = (unsigned)r < (unsigned)nrows;
+        const int rr = in ? r : 0;
+        const int pos = offT[rr] + (int)pfx[rr * WT + w] + __popc(bmT[rr * WT + w] & below);
+        st_shared_if(in && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max), aSt + (uint32_t)pos * 4u, g);
       }
-      if (do_tt) {
-        if (internal) {  // facets 1..D-1 have lowest vertex l[0], a tile vertex
-          const int r = l[0] - nlo;
-          if (GALE_IN_BOUNDS(M.err, (unsigned)r < (unsigned)nrows)) {
-            const int b0 = tbo[r];
-            const uint32_t m = (uint32_t)(tbo[r + 1] - b0);
-            if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl)) {
-              facet_place<D>(tbl + b0, m, facet_key<D, 1>(l), s, 1, ttrow, S, M.err);
-              facet_place<D>(tbl + b0, m, facet_key<D, 2>(l), s, 2, ttrow, S, M.err);
-              if constexpr (D == 4) facet_place<D>(tbl + b0, m, facet_key<D, 3>(l), s, 3, ttrow, S, M.err);
-            }
-          }
-        }
-        const int r1 = l[1] - nlo;
-        if ((unsigned)r1 < (unsigned)nrows) {  // facet 0 has lowest vertex l[1]
-          const int b0 = tbo[r1];
-          const uint32_t m = (uint32_t)(tbo[r1 + 1] - b0);
-          if (GALE_IN_BOUNDS(M.err, b0 >= 0 && b0 + (int)m <= C.tbl))
-            facet_place<D>(tbl + b0, m, facet_key<D, 0>(l), s, 0, ttrow, S, M.err);
-        }
+      {
+        const int rr = internal ? l[0] - nlo : 0;
+        const int pos = runpos[rr] + g;
+        st_shared_if(internal && GALE_IN_BOUNDS(M.err, (unsigned)rr < (unsigned)nrows && pos >= 0 && pos < C.vt_max),
+                     aSt + (uint32_t)pos * 4u, g);
       }
     }
   }
@@ -661,23 +785,24 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   if (do_vv && tid == 32) bulk_emit(O.vv_indices, vv0, n_vv, st_vv, mis_vv);
 
   if (do_tt) {
-    const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
-    const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
-    const int tile_hi = nlo + nrows;
-    // TT rows of the internal simplices
+    // TT rows of the internal simplices. Entry 0 = -1 means boundary, or a facet (l[1], ..) without a
+    // vertex in this tile (l[1] lies above it): only then the simplex is looked at again.
     for (int i = tid; i < s_int; i += NT) {
-      const int s = s_ext + i;
       int r[D];
+      if constexpr (D == 4) {
+        const int4 v = reinterpret_cast<const int4*>(R.res + R.xpad)[i];
+        r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w;
+      } else {
 #pragma unroll
-      for (int k = 0; k < D; ++k) {
-        const int e = ttrow[s * D + k];
-        r[k] = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
+        for (int k = 0; k < D; ++k) r[k] = R.res[R.xpad + i * D + k];
       }
-      int l[4];
-      load_local<LB>(tets, s, l);
-      // facet 0 = (l[1], ..) has no vertex in this tile when l[1] lies above it
-      const bool out0 = l[1] >= tile_hi;
-      const bool delegated = out0 && gid[min(l[1], td.nloc - 1)] < c_hi;  // the tile that owns l[1] writes entry 0
+      bool out0 = false, delegated = false;
+      if (r[0] < 0) {
+        int l[4];
+        load_local<LB>(tets, s_ext + i, l);
+        out0 = l[1] >= tile_hi;
+        delegated = out0 && gid[min(l[1], td.nloc - 1)] < c_hi;  // the tile that owns l[1] writes entry 0
+      }
       int32_t* o = O.tt_indices + (long long)(tt0 + i) * D;
       if constexpr (D == 4) {
         if (!delegated) {
@@ -696,18 +821,12 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
         if (GALE_IN_BOUNDS(M.err, (int)q < C.sint)) fbq[q] = (uint16_t)i;
       }
     }
-    // entry 0 of external simplices of the same cluster whose second vertex is a vertex of this tile
-    for (int s = tid; s < s_ext; s += NT) {
-      int l[4];
-      load_local<LB>(tets, s, l);
-      const int r1 = l[1] - nlo;
-      if ((unsigned)r1 < (unsigned)nrows && gid[l[0]] >= c_lo) {
-        const int e = ttrow[s * D];
-        const int v = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
-        const long long row = (long long)P.tt_base[slot] + (texid[s] - c_tlo);
-        GALE_ST(O.tt_indices + row * D, v);
+    // entry 0 of the flagged external simplices (same cluster, second vertex in this tile)
+    for (int s = tid; s < s_ext; s += NT)
+      if (dflag[s]) {
+        const long long row = (long long)ctx->tt_slot + (texid[s] - c_tlo);
+        GALE_ST(O.tt_indices + row * D, R.res[s]);
       }
-    }
     __syncthreads();  // queue complete, TT rows stored
     // ---- a5: one queued facet per thread, resolved from global memory -------------------------
     const int nq = (int)misc[1];

@@ -114,7 +114,10 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-inline int threads_for_tile(int tv) { return tv > 128 ? 256 : 128; }  // NT >= tv (one thread per row in P2)
+inline int threads_for_tile(int tv) {  // NT >= tv (one thread per row in P2)
+  if (const char* e = std::getenv("GALE_NT")) { const int v = std::atoi(e); if ((v == 128 || v == 256) && v >= tv) return v; }
+  return tv > 128 ? 256 : 128;
+}
 
 // Kernel capacities for one launch: regions the relation mask does not need are dropped.
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
