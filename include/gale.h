@@ -55,6 +55,10 @@ enum {
 enum {
   GALE_VALIDATE = 1u,          /* check C1-C3 and the cluster offsets at create (one pass)            */
   GALE_VALIDATE_MANIFOLD = 2u, /* also check C4 (facet pass, slower)                                  */
+  GALE_KERNEL_DENSE = 8u,      /* force the dense kernel (one thread per staged simplex)              */
+  GALE_KERNEL_WALK = 16u,      /* force the walk kernel (two threads per tile vertex); UNSUPPORTED if
+                                  its capacity limits do not admit the mesh. Neither flag: create times
+                                  both on a sample batch and keeps the faster (gale_mesh_info tells)   */
   GALE_STREAM_ORDERED = 4u     /* run every batch kernel on the cuda_stream passed to compute itself
                                   (plain stream order: work the caller enqueues afterwards runs after
                                   the batch) instead of on the library's two overlapping launch streams */
@@ -80,7 +84,8 @@ typedef struct {
   void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
                                        must outlive the handle                                       */
   size_t workspace_bytes;
-  uint32_t flags;                   /* GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED   */
+  uint32_t flags;                   /* GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED |
+                                       GALE_KERNEL_DENSE / GALE_KERNEL_WALK                           */
 } gale_mesh_desc_t;
 
 /* One finished batch. cluster_ids and *_row_begin are HOST arrays owned by the library; offsets and
@@ -133,6 +138,9 @@ typedef struct {
   int32_t block_threads;         /* threads per block of the batch kernel                            */
   size_t index_bytes;            /* bytes of the device-resident index built by the initialization
                                     (I_T, T_ex, tile tables; the rest of workspace_used is result slots) */
+  int32_t kernel_variant;        /* 0 = dense kernel, 1 = walk kernel (chosen at create, or forced)     */
+  float tune_dense_ms, tune_walk_ms; /* sample-batch times behind that choice (0 = not timed)           */
+  int32_t reserved;
 } gale_mesh_info_t;
 
 /* Initialization analysis ("Initialization": I_T, the external lists T_ex, interval

@@ -15,7 +15,7 @@ import numpy as np
 from .build import LIB, build_library
 
 REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
-VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED = 1, 2, 4
+VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED, KERNEL_DENSE, KERNEL_WALK = 1, 2, 4, 8, 16
 OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
 ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
 
@@ -50,7 +50,8 @@ class gale_mesh_info_t(ctypes.Structure):
                 ("smem_bytes", ctypes.c_int32), ("max_staged", ctypes.c_int32),
                 ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double),
                 ("local_id_bytes", ctypes.c_int32), ("block_threads", ctypes.c_int32),
-                ("index_bytes", ctypes.c_size_t)]
+                ("index_bytes", ctypes.c_size_t), ("kernel_variant", ctypes.c_int32),
+                ("tune_dense_ms", ctypes.c_float), ("tune_walk_ms", ctypes.c_float), ("reserved", ctypes.c_int32)]
 
 
 EXPORTS = ["gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",

@@ -107,6 +107,7 @@ struct SmemCfg {
   int nloc;      // local vertex ids (multiple of 4)
   int sint;      // internal simplices (even): fallback queue, 0 without TT
   int tbl;       // facet-table slots of a tile = VT entries + (D-2) * internal simplices, 0 without TT
+  int hs;        // walk kernel only: table slots per tile vertex (even), 0 without TT
   int WT;        // VT bitmap words per row (odd)
   int WV;        // VV bitmap words per row (odd), 0 without VV
   int vt_max;    // VT entries staged for write-out, 0 without VT or in count mode

@@ -5,6 +5,7 @@
 // pre-allocated result buffers handed to consumers. Every relation entry is
 // computed by the kernels in gale_kernels.cuh; nothing here computes VT/VV/TT on the CPU.
 #include "gale_kernels.cuh"
+#include "gale_walk.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -59,6 +60,10 @@ struct Plan {
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
   int smem_bytes = 0;
+  // the walk kernel (gale_walk.cuh) on the same tiles: same capacities + per-vertex table size
+  int gmax = 1;                         // largest facet group of a vertex
+  int w_NT = 0, w_smem = 0;
+  bool walk_ok = false;
   long long ext_refs = 0, vt_total = 0, vv_total = 0;
   // per-cluster sizes
   std::vector<long long> cl_vt, cl_vv;  // nnz per cluster
@@ -144,6 +149,30 @@ KernelFn kernel_for_lb(int NT, int lb) { return lb == 1 ? kernel_for_nt<D, COUNT
 KernelFn kernel_for(int D, int NT, bool count, int lb) {
   if (D == 4) return count ? kernel_for_lb<4, true>(NT, lb) : kernel_for_lb<4, false>(NT, lb);
   return count ? kernel_for_lb<3, true>(NT, lb) : kernel_for_lb<3, false>(NT, lb);
+}
+
+using WalkFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::WalkLayout, const gale::OutPtrs);
+template <int D, int LB>
+WalkFn walk_for_nt(int NT) {
+  return NT == 512 ? gale::gale_walk_kernel<D, 512, LB>
+                   : (NT == 256 ? gale::gale_walk_kernel<D, 256, LB>
+                                : (NT == 128 ? gale::gale_walk_kernel<D, 128, LB> : gale::gale_walk_kernel<D, 64, LB>));
+}
+WalkFn walk_kernel_for(int D, int NT, int lb) {
+  if (D == 4) return lb == 1 ? walk_for_nt<4, 1>(NT) : walk_for_nt<4, 2>(NT);
+  return lb == 1 ? walk_for_nt<3, 1>(NT) : walk_for_nt<3, 2>(NT);
+}
+inline int walk_threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : (tv > 32 ? 128 : 64)); }  // NT = 2 * rows
+SmemCfg walk_cfg_for_mask(const SmemCfg& full, uint32_t mask) {
+  SmemCfg c = full;
+  c.tbl = 0;
+  if (!(mask & gale::REL_VV)) { c.WV = 0; c.vv_max = 0; }
+  if (!(mask & gale::REL_TT)) { c.hs = 0; c.sint = 0; }
+  if (!(mask & (gale::REL_VT | gale::REL_TT))) c.vt_max = 0;  // TT reads the staged VT entries' flags
+  return c;
+}
+inline gale::WalkLayout walk_layout_for(int D, const SmemCfg& c) {
+  return D == 4 ? gale::make_walk_layout<4>(c) : gale::make_walk_layout<3>(c);
 }
 
 // The dynamic shared-memory ceiling is an attribute of the kernel instantiation for the whole context,
@@ -293,6 +322,11 @@ bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
     hoff += (long long)gid_part[w].size();
     std::vector<int32_t>().swap(gid_part[w]);
   }
+  // largest facet group of a tile vertex (walk kernel's private tables): D-1 facets per simplex of its
+  // run + facet 0 of every simplex whose second vertex it is
+  p.gmax = 1;
+  for (int v = 0; v < p.nV; ++v)
+    p.gmax = std::max(p.gmax, (D - 1) * (p.first_tet[v + 1] - p.first_tet[v]) + (p.opp_first[v + 1] - p.opp_first[v]));
   // shared-memory capacities known so far
   long long smax = 4, sext = 4, sint = 2, nloc = 4;
   for (const TileDesc& d : p.tiles) {
@@ -461,6 +495,14 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
     if (fits) break;
     if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
   }
+  {  // can the walk kernel run these tiles?
+    // load <= 3/4 even if no facet of a group is shared; every interior facet is recorded twice, so the
+    // usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
+    p->cfg.hs = std::max(8, (p->gmax + p->gmax / 3 + 1) & ~1);
+    p->w_NT = walk_threads_for_tile(p->tv);
+    p->w_smem = walk_layout_for(D, walk_cfg_for_mask(p->cfg, 7)).total;
+    p->walk_ok = p->tv <= 256 && p->w_smem <= kSmemLimit && p->cfg.smax < 32768 && p->cfg.vt_max < 65536;
+  }
   // per-tile output placement inside its cluster, per-cluster sizes
   p->cl_vt.assign(p->nC, 0);
   p->cl_vv.assign(p->nC, 0);
@@ -489,7 +531,8 @@ int check_desc(const gale_mesh_desc_t* d) {
   if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
       !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
       d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1 ||
-      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED)))
+      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) ||
+      (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK))
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
   return GALE_OK;
@@ -561,6 +604,7 @@ struct gale_mesh {
   std::unique_ptr<Plan> plan;
   int dim = 0, D = 0, maxB = 0, queue_depth = 0;
   bool stream_ordered = false;
+  int kernel = 0;  // 0 = dense kernel (gale_kernels.cuh), 1 = walk kernel (gale_walk.cuh)
   DeviceMesh dm{};
   std::vector<std::unique_ptr<Slot>> slots;
   SlotLayout cap;
@@ -575,6 +619,7 @@ struct gale_mesh {
   std::atomic<long long> submitted{0}, popped{0};
   size_t workspace_used = 0, index_bytes = 0;
   double create_ms = 0;
+  float tune_ms[2] = {0.f, 0.f};  // sample-batch time of the dense / walk kernel at create (0 = not timed)
 };
 
 namespace {
@@ -662,8 +707,35 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
   if (!m->stream_ordered)
     for (int i = 0; i < gale_mesh::kLaunchStreams; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
   GALE_CUDA(allow_max_smem(kernel_for(m->D, p->NT, false, p->cfg.lb)));
-  m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() + p->analyse_ms;
+  if (p->walk_ok) GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
+  const uint32_t force = p->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK);
+  const bool may_walk = p->walk_ok;
   m->plan = std::move(p);
+  if (force == GALE_KERNEL_WALK && !may_walk) { g_last_error = "the walk kernel cannot run these tiles (capacity limits)"; return GALE_ERR_UNSUPPORTED; }
+  m->kernel = force == GALE_KERNEL_WALK ? 1 : 0;
+  if (force == 0 && may_walk && m->plan->nC > 0 && m->plan->nT > 0) {
+    // Pick the kernel by measurement: one sample batch (the middle clusters) through each, best of 3
+    // event-timed runs after 1 warm-up. Uniform vertex stars favour the walk kernel, irregular ones the dense.
+    const int nC = m->plan->nC, n = std::min(m->maxB, nC);
+    std::vector<int32_t> ids(static_cast<size_t>(n), 0);
+    for (int i = 0; i < n; ++i) ids[size_t(i)] = (nC - n) / 2 + i;
+    float best[2] = {1e30f, 1e30f};
+    for (int k = 0; k < 2; ++k) {
+      m->kernel = k;
+      for (int rep = 0; rep < 4; ++rep) {
+        int rc2 = gale_cluster_batch_compute(m, GALE_REL_ALL, ids.data(), n, st);
+        gale_batch_view_t v;
+        if (rc2 == GALE_OK) rc2 = gale_queue_pop(m, &v, -1);
+        if (rc2 != GALE_OK) return rc2;
+        if (rep > 0) best[k] = std::min(best[k], v.kernel_ms);
+        if ((rc2 = gale_queue_release(m, &v)) != GALE_OK) return rc2;
+      }
+    }
+    m->kernel = best[1] < best[0] ? 1 : 0;
+    m->tune_ms[0] = best[0]; m->tune_ms[1] = best[1];
+    m->submitted.store(0); m->popped.store(0);  // the sample batches are not the caller's: sequence numbers restart
+  }
+  m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() + m->plan->analyse_ms;
   guard.m = nullptr;
   *out = m;
   return GALE_OK;
@@ -749,14 +821,18 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   out->num_external_refs = p.ext_refs;
   out->vt_nnz = p.vt_total;
   out->vv_nnz = p.vv_total;
-  out->smem_bytes = p.smem_bytes;
+  out->smem_bytes = m->kernel == 1 ? p.w_smem : p.smem_bytes;
   out->max_staged = p.cfg.smax;
   out->slot_bytes = m->cap.total;
   out->workspace_used = m->workspace_used;
   out->create_ms = m->create_ms;
   out->local_id_bytes = p.cfg.lb;
-  out->block_threads = p.NT;
+  out->block_threads = m->kernel == 1 ? p.w_NT : p.NT;
   out->index_bytes = m->index_bytes;
+  out->kernel_variant = m->kernel;
+  out->tune_dense_ms = m->tune_ms[0];
+  out->tune_walk_ms = m->tune_ms[1];
+  out->reserved = 0;
   return GALE_OK;
 }
 
@@ -814,14 +890,16 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   O.vv_indices = reinterpret_cast<int32_t*>(s.dev + s.used.vv_idx);
   O.tt_indices = reinterpret_cast<int32_t*>(s.dev + s.used.tt);
 
-  SmemCfg cfg = cfg_for_mask(p.cfg, relation_mask, false);
+  const bool walk = m->kernel == 1;
+  SmemCfg cfg = walk ? walk_cfg_for_mask(p.cfg, relation_mask) : cfg_for_mask(p.cfg, relation_mask, false);
   const gale::SmemLayout lay = layout_for(D, cfg);
+  const gale::WalkLayout wlay = walk_layout_for(D, cfg);
 #if GALE_CHECK_BOUNDS
   // negative control of the bounds-checked build: understate one capacity (the layout keeps its real
   // size) so that the kernel's checks must fire
   if (std::getenv("GALE_CHECK_SELFTEST") && cfg.vt_max > 8) cfg.vt_max -= 8;
 #endif
-  const int smem = lay.total;
+  const int smem = walk ? wlay.total : lay.total;
   // everything the caller enqueued on its stream so far (e.g. the upload of the simplices) comes first
   cudaStream_t run = m->stream_ordered ? st : m->launch[seq % gale_mesh::kLaunchStreams];
   if (!m->stream_ordered) {
@@ -850,7 +928,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.uniform_tiles = uniform ? per : 0;
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, run>>>(m->dm, P, cfg, lay, O);
+    if (walk) walk_kernel_for(D, p.w_NT, p.cfg.lb)<<<grid, p.w_NT, smem, run>>>(m->dm, P, cfg, wlay, O);
+    else kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, run>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, run));

@@ -1,0 +1,489 @@
+// gale_walk.cuh — the "walk" variant of the batch kernel (same inputs, same outputs as gale_batch_kernel).
+//
+// Two threads per tile vertex p walk p's incidences serially: thread A(p) the set bits of p's VT bitmap
+// row (= VT(p) without its run, already sorted), thread B(p) the run of p. The thread owns its row, so
+// VV bits and TT facet tables need no claiming. This is cheapest when all vertex stars look alike
+// (regular grids: every lane of a warp has the same amount of work); on irregular meshes the lanes of a
+// warp wait for the heaviest vertex and the per-vertex capacities are dictated by it — there the dense
+// kernel (gale_kernels.cuh, one thread per staged simplex) wins. gale_mesh_create times both on a sample
+// batch and keeps the faster one.
+//
+// Phases: P0 stage (16-byte cp.async) + clear; P1 VT incidence bits, one thread per staged simplex;
+// P2 row degrees -> scan -> VT offsets; P3 A(p): walk the bits: VT entries + VV bits + flag "p is the
+// second vertex"; B(p): walk the run: VT entries, VV bits, facet records 1..D-1 into p's private table;
+// P4 A(p): facets 0 of the flagged simplices join p's table (both cofaces of a facet with lowest vertex
+// p have p as lowest or second-lowest vertex, so the second arrival meets the first); B(p): VV row ->
+// degree -> scan -> expansion; P5 translate to global ids, coalesced write-out; facets (l[1], ..) with
+// l[1] outside the tile: same cluster -> written by the tile that owns l[1] (it has the simplex in its
+// T_ex list), else resolved from global memory (a5).
+#pragma once
+#include "gale_kernels.cuh"
+
+namespace gale {
+
+struct WalkLayout {
+  int tets, texid, gid, ft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
+  int tbl, ttrow, ext0, tt_end;
+  int st_vt, st_vv;
+  int total;
+};
+
+// Capacities come in a SmemCfg; `hs` = table slots per tile vertex (even, so the row stride hs+1 is odd).
+template <int D>
+__host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
+  WalkLayout L;
+  int o = 0;
+  L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
+  L.texid = o;  o = align16(o + c.sext * 4);
+  L.gid = o;    o = align16(o + c.nloc * 4);
+  L.ft = o;     o = align16(o + (c.tv + 1) * 4);
+  L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
+  L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
+  L.cnt = o;    o = align16(o + c.tv * 4);
+  L.scan = o;   o = align16(o + 48 * 4);
+  // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
+  // fallback queue (written in P5)
+  L.bmT = o;
+  {
+    const int bm = align16(c.tv * c.WT * 4);
+    L.st_vv = o;
+    L.fbq = o + align16(c.vv_max * 2);
+    const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
+    o += bm > reuse ? bm : reuse;
+  }
+  L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
+  L.bm_end = o;
+  L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
+  L.ttrow = o;  o = align16(o + (c.hs ? c.sint * D * 2 : 0));
+  L.ext0 = o;   o = align16(o + (c.hs ? c.sext * 2 : 0));
+  L.tt_end = o;
+  L.st_vt = o;  o = align16(o + c.vt_max * 2);
+  L.total = o;
+  return L;
+}
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// Barrier among the `count` threads that name the same id (ids 1..15; 0 is __syncthreads).
+__device__ __forceinline__ void named_barrier(int id, int count) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory");
+}
+
+__device__ __forceinline__ uint32_t bit_of(int l) { return 1u << (l & 31); }
+
+struct GroupCtx {
+  uint32_t* tbl;       // this vertex's table, hs slots
+  uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
+  uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
+  uint16_t* ext0;      // entry 0 of the external simplices, same encoding
+  int s_ext;
+  int s_all;           // staged simplices of the tile (bounds-checked build)
+};
+
+// Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
+// holds the same key (the other coface) and write both TT entries. The thread owns the table.
+template <int D>
+__device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
+  using FB = FacetBits<D>;
+  uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
+  uint32_t cur = g.tbl[h];
+  uint32_t probe = 0;
+  while (cur != kEmpty32 && (cur & FB::kKeyMask) != key) {  // probe loop kept minimal: lanes diverge here
+    h = h + 1 == g.hs ? 0u : h + 1;
+    cur = g.tbl[h];
+    if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
+  }
+  if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
+  if (cur == kEmpty32) {
+    g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
+  } else {
+    const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
+    if (!GALE_IN_BOUNDS(err, s < g.s_all && s2 < g.s_all && k2 < D)) return;
+    // an external simplex only ever records its facet 0
+    if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2; else g.ext0[s] = (uint16_t)s2;
+    if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s; else g.ext0[s2] = (uint16_t)s;
+  }
+}
+
+// Exclusive scan over the B half of the block (threads [NT/2, NT)), one value per thread, with a
+// named barrier so that the A half is not held up. Returns the exclusive prefix; *total = sum.
+template <int NT>
+__device__ __forceinline__ uint32_t half_exclusive_scan(uint32_t x, uint32_t* scratch, uint32_t* total) {
+  constexpr int TV = NT / 2;
+  const int lane = threadIdx.x & 31, warp = (threadIdx.x - TV) >> 5;
+  uint32_t inc = x;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+    if (lane >= d) inc += y;
+  }
+  if constexpr (TV <= 32) {
+    *total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+    return inc - x;
+  } else {
+    constexpr int NW = TV / 32;
+    if (lane == 31) scratch[warp] = inc;
+    named_barrier(1, TV);
+    uint32_t base = 0u, tot = 0u;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const uint32_t v = scratch[w];
+      if (w < warp) base += v;
+      tot += v;
+    }
+    named_barrier(1, TV);  // scratch may be reused
+    *total = tot;
+    return base + inc - x;
+  }
+}
+
+// NT = 2 * (rows per tile capacity): thread tid < NT/2 is A(tid), thread NT/2 + p is B(p).
+template <int D, int NT, int LB>
+__global__ void __launch_bounds__(NT, (NT <= 64 ? 16 : (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2))))
+gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
+                 const WalkLayout L, const OutPtrs O) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  constexpr int TV = NT / 2;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const uint32_t mask = P.mask;
+  const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0, do_tt = (mask & REL_TT) != 0;
+  const bool entries = do_vt || do_tt;  // VT entries are staged (TT reads their flags)
+
+  // ---- block -> (cluster slot, tile) ----------------------------------------------------------
+  int slot = 0, tile;
+  if (blockIdx.x == 0 && tid == 0) {  // terminal offsets (also covers batches without rows)
+    if (do_vt) { O.vt_offsets[0] = 0; O.vt_offsets[P.total_rows] = P.total_vt_nnz; }
+    if (do_vv) { O.vv_offsets[0] = 0; O.vv_offsets[P.total_rows] = P.total_vv_nnz; }
+  }
+  if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
+  if (P.uniform_tiles > 0) {
+    slot = (int)blockIdx.x / P.uniform_tiles;
+  } else {
+    int lo = 0, hi = P.n_clusters;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+    }
+    slot = lo;
+  }
+  tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
+  TileDesc td;
+  {
+    const int4* src = reinterpret_cast<const int4*>(M.tiles + tile);
+    int4* dst = reinterpret_cast<int4*>(&td);
+#pragma unroll
+    for (int i = 0; i < (int)(sizeof(TileDesc) / 16); ++i) dst[i] = __ldg(src + i);
+  }
+  const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
+  const int S = s_int + s_ext;
+  const int WT = C.WT, WV = C.WV;
+#if GALE_CHECK_BOUNDS
+  {
+    bool ok = nrows >= 0 && nrows <= C.tv && NT >= 2 * C.tv && S >= 0 && S <= C.smax && s_ext <= C.sext &&
+              td.nloc <= C.nloc && nlo >= 0 && nlo + nrows <= td.nloc && ((S + 31) >> 5) <= WT;
+    if (mask & REL_VV) ok = ok && ((td.nloc + 31) >> 5) <= WV;
+    if (mask & REL_TT) ok = ok && s_int <= C.sint && C.hs >= 2;
+    if (mask & (REL_VT | REL_TT)) ok = ok && td.vt_nnz <= C.vt_max;
+    if (mask & REL_VV) ok = ok && td.vv_nnz <= C.vv_max;
+    if (!ok) {  // block-uniform: leave before anything is staged
+      if (tid == 0) raise_err(M.err, ERR_BOUNDS);
+      return;
+    }
+  }
+#endif
+
+  unsigned char* tets = smem + L.tets;
+  int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
+  int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
+  int32_t* ft = reinterpret_cast<int32_t*>(smem + L.ft);        // first_tet[v_lo .. v_lo+nrows] (I_T)
+  uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
+  uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
+  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [36] queue length, [38] n_vv
+  uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
+  uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
+  uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
+  uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);
+  uint16_t* ext0 = reinterpret_cast<uint16_t*>(smem + L.ext0);
+  uint16_t* st_vt = reinterpret_cast<uint16_t*>(smem + L.st_vt);
+  uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
+
+  const int row0 = P.row_base[slot] + td.row_rel;
+  const int vt0 = P.vt_base[slot] + td.vt_rel;
+  const int vv0 = P.vv_base[slot] + td.vv_rel;
+  const int tt0 = P.tt_base[slot] + td.tt_rel;
+
+  // ---- P0: stage + clear ----------------------------------------------------------------------
+  {
+    const int4* src = reinterpret_cast<const int4*>(static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB));
+    int4* dst = reinterpret_cast<int4*>(tets);
+    for (int i = tid; i < (S * 4 * LB + 15) >> 4; i += NT) cp_async16(dst + i, src + i);
+    const int4* tsrc = reinterpret_cast<const int4*>(M.tex + td.tex_off);
+    int4* tdst = reinterpret_cast<int4*>(texid);
+    for (int i = tid; i < (s_ext + 3) >> 2; i += NT) cp_async16(tdst + i, tsrc + i);
+    if (do_vv || do_tt) {
+      const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
+      int4* gdst = reinterpret_cast<int4*>(gid);
+      for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
+    }
+  }
+  for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);
+  {
+    int4* z = reinterpret_cast<int4*>(smem + L.bmT);
+    const int n16 = (L.bm_end - L.bmT) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
+  }
+  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
+    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
+    const int n16 = (L.tt_end - L.tbl) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
+  }
+  if (tid == 0) { scan[36] = 0u; scan[38] = 0u; }
+  cp_async_wait_all();
+  __syncthreads();
+
+  // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
+  for (int s = tid; s < S; s += NT) {
+    int l[4];
+    load_local<LB>(tets, s, l);
+#if GALE_CHECK_BOUNDS
+    for (int k = 0; k < D; ++k)
+      if (!GALE_IN_BOUNDS(M.err, l[k] >= 0 && l[k] < td.nloc)) l[k] = nlo;  // keep later indexing inside the row
+    if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
+#endif
+    uint32_t* col = bmT + (s >> 5);
+    const uint32_t bit = bit_of(s);
+#pragma unroll
+    for (int k = 1; k < D; ++k) {
+      const int r = l[k] - nlo;
+      if ((unsigned)r < (unsigned)nrows) atomicOr(col + r * WT, bit);
+    }
+  }
+  __syncthreads();
+
+  // ---- P2: row degrees -> VT offsets ----------------------------------------------------------
+  const bool isB = tid >= TV;
+  const int p = isB ? tid - TV : tid;
+  const bool live = p < nrows;
+  const int ploc = nlo + p;
+  const int wT = (S + 31) >> 5;
+  if (live) {
+    const int half = (wT + 1) >> 1;
+    const uint32_t* row = bmT + p * WT;
+    int c = 0;
+    const int w0 = isB ? half : 0, w1 = isB ? wT : half;
+#pragma unroll 4
+    for (int w = w0; w < w1; ++w) c += __popc(row[w]);
+    cnt[(isB ? C.tv : 0) + p] = (uint16_t)c;
+  }
+  __syncthreads();
+  int nb = 0, off = 0, n_vt;
+  int run_lo = 0, run_hi = 0;  // run of p: simplices [run_lo, run_hi) have p as lowest vertex (I_T)
+  {
+    uint32_t deg = 0u, tot;
+    if (live) {
+      nb = (int)cnt[p] + (int)cnt[C.tv + p];
+      run_lo = ft[p]; run_hi = ft[p + 1];
+      deg = (uint32_t)(nb + run_hi - run_lo);
+    }
+    const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // A and B halves carry the same values
+    n_vt = (int)(tot >> 1);
+    off = (int)ex - (isB ? n_vt : 0);
+  }
+  if (do_vt && live && !isB) O.vt_offsets[row0 + p] = vt0 + off;
+
+  // ---- P3: A walks the bits of row p, B walks the run of p ------------------------------------
+  if (live) {
+    uint32_t* vvrow = bmV + p * WV;
+    if (!isB) {
+      const uint32_t* row = bmT + p * WT;
+      int pos = off, sbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nb; ++n) {
+        while (bits == 0u) { bits = *row++; sbase += 32; }
+        const int s = sbase + __ffs(bits) - 1;
+        bits &= bits - 1;
+        int l[4];
+        load_local<LB>(tets, s, l);
+        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= 0 && s < S))
+          st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
+        if (do_vv) {
+#pragma unroll
+          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));  // self bit cleared in P4
+        }
+      }
+    } else {
+      GroupCtx g;
+      if (do_tt) {
+        const int hs = C.hs;
+        g.tbl = tbl + p * (hs + 1);
+        g.hs = (uint32_t)hs;
+        g.ttrow = ttrow; g.ext0 = ext0;
+        g.s_ext = s_ext; g.s_all = S;
+      }
+      int pos = off + nb;
+      const int r1 = run_hi - t_lo;
+      for (int i = run_lo - t_lo; i < r1; ++i) {
+        const int s = s_ext + i;
+        int l[4];
+        load_local<LB>(tets, s, l);
+        if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= s_ext && s < S)) st_vt[pos++] = (uint16_t)s;
+        if (do_vv) {
+#pragma unroll
+          for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));
+        }
+        if (do_tt) {
+          group_place<D>(g, facet_key<D, 1>(l), s, 1, M.err);
+          group_place<D>(g, facet_key<D, 2>(l), s, 2, M.err);
+          if constexpr (D == 4) group_place<D>(g, facet_key<D, 3>(l), s, 3, M.err);
+        }
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- P4: A joins the facets 0 of the simplices (x, p, ..); B expands VV row p ----------------
+  int n_vv = 0;
+  if (!isB) {
+    if (do_tt && live) {
+      GroupCtx g;
+      const int hs = C.hs;
+      g.tbl = tbl + p * (hs + 1);
+      g.hs = (uint32_t)hs;
+      g.ttrow = ttrow; g.ext0 = ext0;
+      g.s_ext = s_ext; g.s_all = S;
+      int i = off;
+      const int end = off + nb;
+      for (;;) {
+        uint32_t e = 0u;
+        while (i < end && !((e = st_vt[i]) & 0x8000u)) ++i;
+        if (i >= end) break;
+        ++i;
+        const int s = (int)(e & 0x7FFFu);
+        int l[4];
+        load_local<LB>(tets, s, l);
+        group_place<D>(g, facet_key<D, 0>(l), s, 0, M.err);
+      }
+    }
+  } else if (do_vv) {
+    const int wV = (td.nloc + 31) >> 5;
+    uint32_t* row = bmV + p * WV;
+    int nbv = 0;
+    if (live) {
+      row[ploc >> 5] &= ~bit_of(ploc);  // a vertex is not its own neighbour
+#pragma unroll 4
+      for (int w = 0; w < wV; ++w) nbv += __popc(row[w]);
+    }
+    uint32_t tot;
+    const int offv = (int)half_exclusive_scan<NT>((uint32_t)nbv, scan, &tot);
+    if (tid == TV) scan[38] = tot;
+    if (live) {
+      O.vv_offsets[row0 + p] = vv0 + offv;
+      int pos = offv, lbase = -32;
+      uint32_t bits = 0u;
+      for (int n = 0; n < nbv; ++n) {
+        while (bits == 0u) { bits = *row++; lbase += 32; }
+        if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vv_max && lbase + __ffs(bits) - 1 < td.nloc))
+          st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
+        bits &= bits - 1;
+      }
+    }
+  }
+  __syncthreads();
+  n_vv = (int)scan[38];
+  if (tid == 0 && ((do_vt && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
+    raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
+
+  // ---- P5: translate to global ids, coalesced write-out ----------------------------------------
+  if (do_tt) {
+    const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
+    const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
+    for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
+      const int i = base + lane;
+      bool need_fb = false;
+      if (i < s_int) {
+        uint32_t e[D];
+        if constexpr (D == 4) {
+          const uint2 q = reinterpret_cast<const uint2*>(ttrow)[i];
+          e[0] = q.x & 0xFFFFu; e[1] = q.x >> 16; e[2] = q.y & 0xFFFFu; e[3] = q.y >> 16;
+        } else {
+          e[0] = ttrow[i * 3]; e[1] = ttrow[i * 3 + 1]; e[2] = ttrow[i * 3 + 2];
+        }
+        int r[D];
+#pragma unroll
+        for (int k = 0; k < D; ++k)
+          r[k] = e[k] == 0xFFFFu ? -1 : ((int)e[k] < s_ext ? texid[e[k]] : t_lo + ((int)e[k] - s_ext));
+        bool delegated = false;
+        if (r[0] < 0) {
+          int l[4];
+          load_local<LB>(tets, s_ext + i, l);
+          // facet 0 = (l[1], ..) has no vertex in this tile when l[1] lies above it: the tile that owns l[1]
+          // writes the entry if it belongs to this cluster, else it is resolved from global memory (a5)
+          const bool out0 = l[1] - nlo >= nrows;
+          delegated = out0 && gid[l[1]] < c_hi;
+          need_fb = out0 && !delegated;
+        }
+        int32_t* o = O.tt_indices + (long long)(tt0 + i) * D;
+        if constexpr (D == 4) {
+          if (!delegated) {
+            GALE_ST(reinterpret_cast<int4*>(o), make_int4(r[0], r[1], r[2], r[3]));
+          } else {
+            GALE_ST(o + 1, r[1]);
+            GALE_ST(reinterpret_cast<int2*>(o + 2), make_int2(r[2], r[3]));
+          }
+        } else {
+          if (!delegated) o[0] = r[0];
+          o[1] = r[1]; o[2] = r[2];
+        }
+      }
+      const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
+      if (fbm) {
+        const int leader = __ffs(fbm) - 1;
+        uint32_t pos = 0u;
+        if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
+        pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
+        if (need_fb && GALE_IN_BOUNDS(M.err, (int)(pos + __popc(fbm & ((1u << lane) - 1u))) < C.sint))
+          fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
+      }
+    }
+    // entry 0 of the external simplices of this cluster whose second vertex is a vertex of this tile
+    for (int s = tid; s < s_ext; s += NT) {
+      int l[4];
+      load_local<LB>(tets, s, l);
+      if ((unsigned)(l[1] - nlo) < (unsigned)nrows && gid[l[0]] >= c_lo) {
+        const int e = ext0[s];
+        const int v = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
+        const long long row = (long long)P.tt_base[slot] + (texid[s] - c_tlo);
+        GALE_ST(O.tt_indices + row * D, v);
+      }
+    }
+  }
+  if (do_vt)
+    for (int i = tid; i < n_vt; i += NT) {
+      const int s = (int)(st_vt[i] & 0x7FFFu);
+      GALE_ST(O.vt_indices + vt0 + i, s < s_ext ? texid[s] : t_lo + (s - s_ext));
+    }
+  if (do_vv)
+    for (int i = tid; i < n_vv; i += NT) GALE_ST(O.vv_indices + vv0 + i, gid[st_vv[i]]);
+
+  if (do_tt) {
+    __syncthreads();  // queue complete, TT rows stored
+    // ---- a5: one queued facet per thread, resolved from global memory -------------------------
+    const int nq = (int)scan[36];
+    for (int q = tid; q < nq; q += NT) {
+      const int i = fbq[q];
+      int l[4];
+      load_local<LB>(tets, s_ext + i, l);
+      const int t = t_lo + i;
+      const int b = gid[l[1]], c = gid[l[2]], d = D == 4 ? gid[l[3]] : 0;
+      const int f0 = __ldg(M.first_tet + b), f1 = __ldg(M.first_tet + b + 1);
+      const int r = tt_fallback<D>(M, f0, f1, b, c, d, t);
+      if (r >= 0) O.tt_indices[(long long)(tt0 + i) * D] = r;  // ordered after the row store by the barrier
+    }
+  }
+}
+
+}  // namespace gale

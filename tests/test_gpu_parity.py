@@ -56,30 +56,51 @@ SMALL = [
 ]
 
 
+KERNELS = {"auto": 0, "dense": 8, "walk": 16}       # GALE_KERNEL_DENSE / GALE_KERNEL_WALK; auto = timed choice at create
+
+
+def _run_kernel(m, batch, kernel, **kw):
+    """_run_all with a forced kernel variant; skips when the walk kernel's capacity limits refuse the mesh."""
+    gale = _gale()
+    flags = kw.pop("flags", gale.VALIDATE) | KERNELS[kernel]
+    try:
+        got, ref, info = _run_all(m, batch, flags=flags, **kw)
+    except gale.GaleError as e:
+        if kernel == "walk" and e.status == gale.ERR_UNSUPPORTED:
+            pytest.skip("walk kernel does not admit this mesh")
+        raise
+    if kernel != "auto":
+        assert info.kernel_variant == (1 if kernel == "walk" else 0)
+    return got, ref, info
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
 @pytest.mark.parametrize("name,make,batch", SMALL, ids=[s[0] for s in SMALL])
-def test_parity_small(name, make, batch):
+def test_parity_small(name, make, batch, kernel):
     m = make()
-    got, ref, _ = _run_all(m, batch)
-    _compare(got, ref, name)
+    got, ref, _ = _run_kernel(m, batch, kernel)
+    _compare(got, ref, f"{name} [{kernel}]")
 
 
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
 @pytest.mark.parametrize("tv", [3, 16, 64])
-def test_parity_irregular_mesh_tile_sizes(tv):
+def test_parity_irregular_mesh_tile_sizes(tv, kernel):
     m = meshgen.make_delaunay(3, 2500, seed=33, capacity=400)
-    got, ref, _ = _run_all(m, 5, tile_vertices=tv, flags=3)          # VALIDATE | VALIDATE_MANIFOLD
-    _compare(got, ref, f"delaunay3d tv={tv}")
+    got, ref, _ = _run_kernel(m, 5, kernel, tile_vertices=tv, flags=3)          # VALIDATE | VALIDATE_MANIFOLD
+    _compare(got, ref, f"delaunay3d tv={tv} [{kernel}]")
 
 
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
 @pytest.mark.parametrize("tv", [1, 7, 32, 100, 256])
-def test_parity_tile_sizes(tv):
+def test_parity_tile_sizes(tv, kernel):
     """Ragged tiles, one-vertex tiles, and tiles as large as a block."""
     m = meshgen.make_mesh(3, 14, clustering="octree", capacity=300, permute=True, drop_frac=0.1, seed=13)
-    got, ref, info = _run_all(m, 9, tile_vertices=tv)
+    got, ref, info = _run_kernel(m, 9, kernel, tile_vertices=tv)
     assert info.tile_vertices <= max(tv, 1)
-    _compare(got, ref, f"tv={tv}")
+    _compare(got, ref, f"tv={tv} [{kernel}]")
     m2 = meshgen.make_mesh(2, 60, clustering="octree", capacity=500, seed=14)
-    got, ref, _ = _run_all(m2, 4, tile_vertices=tv)
-    _compare(got, ref, f"2d tv={tv}")
+    got, ref, _ = _run_kernel(m2, 4, kernel, tile_vertices=tv)
+    _compare(got, ref, f"2d tv={tv} [{kernel}]")
 
 
 def test_both_local_id_widths():
@@ -102,11 +123,13 @@ def test_both_local_id_widths():
         _compare(got, ref, f"2d local id bytes {lb}")
 
 
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
 @pytest.mark.parametrize("mask", [1, 2, 4, 3, 5, 6])
-def test_relation_masks(mask):
+def test_relation_masks(mask, kernel):
     gale = _gale()
     m = meshgen.make_config(1)
-    gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=8)
+    gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=8,
+                       flags=gale.VALIDATE | KERNELS[kernel])
     host = gm.run_batch([5, 0, 3], mask)
     got = gale.split_batch(host, 4)
     ref = oracle.cluster_results(3, m.num_vertices, m.simplices, m.cluster_offsets, [5, 0, 3], mask=mask)
