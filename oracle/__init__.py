@@ -56,12 +56,20 @@ def _load():
         lib.go_sub_gid.argtypes = [vp]
         lib.go_sub_size.restype = i64
         lib.go_sub_size.argtypes = [vp]
+        lib.go_seconds.restype = None
+        lib.go_seconds.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        lib.go_sub_extract_seconds.restype = ctypes.c_double
+        lib.go_sub_extract_seconds.argtypes = [vp]
         lib.go_sub_free.restype = None
         lib.go_sub_free.argtypes = [vp]
         lib.go_slice_rows.restype = i64
         lib.go_slice_rows.argtypes = [i64p, i32p, i64, i64, i32p, i32p, i32p]
         lib.go_slice_tt.restype = None
         lib.go_slice_tt.argtypes = [i32p, c_int, i64, i64, i32p, i32p]
+        lib.go_internal_range.restype = None
+        lib.go_internal_range.argtypes = [c_int, i64, i32p, i64, i64, i64p]
+        lib.go_external_list.restype = i64
+        lib.go_external_list.argtypes = [c_int, i64, i32p, i64, i64, i32p]
         lib.go_brute_vt.restype = None
         lib.go_brute_vt.argtypes = [c_int, i64, i64, i32p, i64p, i32p]
         lib.go_brute_vv.restype = None
@@ -149,6 +157,16 @@ def _slice_clusters(lib, h, D, offsets, clusters, mask, first_tet, gid, gid_firs
     return res
 
 
+last_timing: dict = {}   # wall seconds of the last cluster_results call: extract (sub-mesh scans), vt, vv, tt, sub_simplices
+
+
+def _timing(lib, h, extract=0.0, sub=0):
+    t = (ctypes.c_double * 3)()
+    lib.go_seconds(h, t)
+    last_timing.clear()
+    last_timing.update(extract=float(extract), vt=t[0], vv=t[1], tt=t[2], sub_simplices=int(sub))
+
+
 def cluster_results(dim: int, num_vertices: int, simplices: np.ndarray, cluster_offsets: np.ndarray,
                     clusters, mask: int = 7, restricted: bool = False) -> list:
     """Oracle output for each cluster id in `clusters`, in that order.
@@ -170,6 +188,7 @@ def cluster_results(dim: int, num_vertices: int, simplices: np.ndarray, cluster_
             if lib.go_status(h) != 0:
                 raise OracleError(f"oracle input contract violated: status {lib.go_status(h)}")
             first = _np(lib.go_first_tet(h), nV + 1, np.int64)
+            _timing(lib, h, 0.0, nT)
             return _slice_clusters(lib, h, D, offsets, clusters, mask, first, None, gfirst)
         finally:
             lib.go_free(h)
@@ -181,9 +200,29 @@ def cluster_results(dim: int, num_vertices: int, simplices: np.ndarray, cluster_
             raise OracleError(f"oracle input contract violated: status {lib.go_status(h)}")
         gid = _np(lib.go_sub_gid(s), int(lib.go_sub_size(s)), np.int32)
         first = _np(lib.go_first_tet(h), nV + 1, np.int64)
+        _timing(lib, h, lib.go_sub_extract_seconds(s), len(gid))
         return _slice_clusters(lib, h, D, offsets, clusters, mask, first, gid, gfirst)
     finally:
         lib.go_sub_free(s)
+
+
+def internal_range(dim: int, simplices: np.ndarray, lo: int, hi: int) -> tuple:
+    """I_T of the segment [lo, hi): (first, last+1) internal simplex."""
+    T = _canon(simplices)
+    out = np.zeros(2, np.int64)
+    _load().go_internal_range(dim, T.shape[0], _i32(T), int(lo), int(hi), _i64(out))
+    return int(out[0]), int(out[1])
+
+
+def external_list(dim: int, simplices: np.ndarray, lo: int, hi: int) -> np.ndarray:
+    """T_ex of the segment [lo, hi): ascending ids of its external simplices."""
+    lib = _load()
+    T = _canon(simplices)
+    n = int(lib.go_external_list(dim, T.shape[0], _i32(T), int(lo), int(hi), None))
+    out = np.empty(n, np.int32)
+    if n:
+        lib.go_external_list(dim, T.shape[0], _i32(T), int(lo), int(hi), _i32(out))
+    return out
 
 
 def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:

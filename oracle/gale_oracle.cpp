@@ -7,7 +7,8 @@
 // call this. It shares no code, header, table or helper with the CUDA path
 // (paper_2507_15230_b200/csrc) and neither includes the other.
 //
-// Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): Fig. 1 toy (PAPER.md:60-64,
+// Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): Fig. 4's stated facts for I_T / T_ex /
+// the edge intervals (tests/golden/fig4_mesh.txt), Fig. 1 toy (PAPER.md:60-64,
 // tests/golden/fig1_toy.txt), brute-force enumeration below (go_brute_*), scipy.sparse transposes /
 // products, Kuhn-grid closed forms, Euler characteristic, TT symmetry, clustering independence.
 // Nothing here is "parity unpinned".
@@ -24,6 +25,7 @@
 //   TT(t)[k] = the t' != t whose vertex set contains T[t] \ {T[t][k]}, else -1  (adjacency, :49)
 #include <algorithm>
 #include <array>
+#include <chrono>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -38,6 +40,7 @@ struct Relations {
   std::vector<int32_t> tt;               // [nT*D]
   std::vector<int64_t> first_tet;        // [nV+1]: first t with T[t][0] >= v   (I_T)
   int status = 0;
+  double seconds[3] = {0, 0, 0};         // wall time of compute_vt / compute_vv / compute_tt (reporting only)
 };
 
 enum { GO_OK = 0, GO_NOT_CANONICAL = -2, GO_NONMANIFOLD = -4 };
@@ -136,9 +139,16 @@ Relations* compute_all(int D, int64_t nV, int64_t nT, const int32_t* T, uint32_t
   R->status = check_canonical(D, nV, nT, T);
   if (R->status != GO_OK) return R;
   compute_first_tet(*R, T);
+  using clk = std::chrono::steady_clock;
+  auto secs = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
+  clk::time_point t0 = clk::now();
   if (mask & 1) compute_vt(*R, T);
+  clk::time_point t1 = clk::now();
   if (mask & 2) compute_vv(*R, T);
+  clk::time_point t2 = clk::now();
   if (mask & 4) R->status = D == 4 ? compute_tt<4>(*R, T) : compute_tt<3>(*R, T);
+  clk::time_point t3 = clk::now();
+  R->seconds[0] = secs(t0, t1); R->seconds[1] = secs(t1, t2); R->seconds[2] = secs(t2, t3);  // timers only: no arithmetic
   return R;
 }
 
@@ -161,6 +171,10 @@ const int32_t* go_vv_indices(void* h) { return static_cast<Relations*>(h)->vv_id
 const int32_t* go_tt(void* h) { return static_cast<Relations*>(h)->tt.data(); }
 const int64_t* go_first_tet(void* h) { return static_cast<Relations*>(h)->first_tet.data(); }
 int64_t go_vv_nnz(void* h) { return int64_t(static_cast<Relations*>(h)->vv_idx.size()); }
+// Wall time the three relation routines took inside go_compute_* (for bench.py's cpu_baseline split).
+void go_seconds(void* h, double* out3) {
+  for (int i = 0; i < 3; ++i) out3[i] = static_cast<Relations*>(h)->seconds[i];
+}
 
 // ---- restriction to a set of clusters (for meshes too large for the global pass) -----------------
 // Exactness: let W = vertices of the selected clusters plus every vertex of their internal
@@ -175,12 +189,14 @@ struct SubMesh {
   Relations* R = nullptr;
   std::vector<int32_t> gid;  // sub-mesh simplex -> global simplex id
   std::vector<int32_t> Tsub;
+  double extract_seconds = 0;  // the two whole-mesh scans that build the sub-mesh (reporting only)
 };
 
 void* go_compute_restricted(int dim, int64_t nV, int64_t nT, const int32_t* T, int32_t nC,
                             const int32_t* offsets, int32_t nSel, const int32_t* sel, uint32_t mask) {
   const int D = dim + 1;
   (void)nC;
+  const auto t_begin = std::chrono::steady_clock::now();
   std::vector<uint8_t> inW(nV, 0);
   for (int32_t i = 0; i < nSel; ++i)
     for (int32_t v = offsets[sel[i]]; v < offsets[sel[i] + 1]; ++v) inW[v] = 1;
@@ -197,12 +213,14 @@ void* go_compute_restricted(int dim, int64_t nV, int64_t nT, const int32_t* T, i
       S->Tsub.insert(S->Tsub.end(), T + t * D, T + t * D + D);
     }
   }
+  S->extract_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
   S->R = compute_all(D, nV, int64_t(S->gid.size()), S->Tsub.data(), mask);
   return S;
 }
 void* go_sub_relations(void* s) { return static_cast<SubMesh*>(s)->R; }
 const int32_t* go_sub_gid(void* s) { return static_cast<SubMesh*>(s)->gid.data(); }
 int64_t go_sub_size(void* s) { return int64_t(static_cast<SubMesh*>(s)->gid.size()); }
+double go_sub_extract_seconds(void* s) { return static_cast<SubMesh*>(s)->extract_seconds; }
 void go_sub_free(void* s) {
   SubMesh* S = static_cast<SubMesh*>(s);
   delete S->R;
@@ -224,6 +242,40 @@ int64_t go_slice_rows(const int64_t* off, const int32_t* idx, int64_t lo, int64_
 // TT rows of simplices [t_lo, t_hi) (ids of the handle's own mesh); entries renamed through map.
 void go_slice_tt(const int32_t* tt, int D, int64_t t_lo, int64_t t_hi, const int32_t* map, int32_t* out) {
   for (int64_t i = t_lo * D; i < t_hi * D; ++i) out[i - t_lo * D] = (tt[i] < 0 || !map) ? tt[i] : map[tt[i]];
+}
+
+// ---- initialization data of a segment -----------------------------------------
+// Plain scans over all simplices; a segment is the vertex range [lo, hi).
+// I_T: the internal simplices of the segment, {t : lo <= T[t][0] < hi} ("internal ... iff the vertex with
+// the lowest index also belongs to S_i", :172), are a contiguous id range by C2; out2 = {first, last+1}
+// (first = last+1 = number of simplices with a lower lowest vertex when there is none).
+void go_internal_range(int dim, int64_t nT, const int32_t* T, int64_t lo, int64_t hi, int64_t* out2) {
+  const int D = dim + 1;
+  int64_t below = 0, inside = 0;
+  for (int64_t t = 0; t < nT; ++t) {
+    if (T[t * D] < lo) ++below;
+    else if (T[t * D] < hi) ++inside;
+  }
+  out2[0] = below;
+  out2[1] = below + inside;
+}
+// T_ex: the external simplices of the segment, ascending: simplices with a vertex in [lo, hi) whose
+// lowest vertex is not in it ("external to all other intersecting segments", :172; "T_ex encodes the list
+// of external tetrahedra for each segment", :178). out may be null (count only). Returns the count.
+int64_t go_external_list(int dim, int64_t nT, const int32_t* T, int64_t lo, int64_t hi, int32_t* out) {
+  const int D = dim + 1;
+  int64_t n = 0;
+  for (int64_t t = 0; t < nT; ++t) {
+    const int32_t* r = T + t * D;
+    if (r[0] >= lo && r[0] < hi) continue;  // internal
+    bool touches = false;
+    for (int k = 1; k < D; ++k) touches |= (r[k] >= lo && r[k] < hi);
+    if (touches) {
+      if (out) out[n] = int32_t(t);
+      ++n;
+    }
+  }
+  return n;
 }
 
 // ---- brute-force enumeration (tiny meshes; pins the routines above) ------------------------------

@@ -255,3 +255,55 @@ def test_rejects_bad_input():
     T = np.array([[0, 1, 2], [0, 1, 3], [0, 1, 4]], np.int32)
     with pytest.raises(oracle.OracleError):
         oracle.relations_global(2, 5, T)
+
+
+# ---- initialization data: I_T and T_ex -------------------------------------------
+def _fig4(golden_dir):
+    T, S, exp = [], [], {}
+    for line in open(os.path.join(golden_dir, "fig4_mesh.txt")):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] == "T":
+            T.append([int(x) for x in f[1:]])
+        elif f[0] == "S":
+            S.append((int(f[1]), int(f[2])))
+        else:
+            exp[f[0]] = [int(x) for x in f[1:]]
+    return np.array(T, np.int32), S, exp
+
+
+def test_fig4_internal_external_and_edge_intervals(golden_dir):
+    """The paper's own statements about its Fig. 4 example: t1 internal to S1 / external to S2, and the
+    edge interval array I_E = [0, 9, 12] (9 edges with their lowest vertex in S1, 3 in S2)."""
+    T, S, exp = _fig4(golden_dir)
+    ranges = [oracle.internal_range(3, T, lo, hi) for lo, hi in S]
+    assert [ranges[0][0], ranges[0][1], ranges[1][1]] == exp["I_T"] and ranges[1][0] == ranges[0][1]
+    assert ranges[0][0] <= 1 < ranges[0][1]                          # t1 is internal to S1 (PAPER.md:172)
+    assert oracle.external_list(3, T, *S[0]).tolist() == exp["TEX_S1"]
+    tex2 = oracle.external_list(3, T, *S[1]).tolist()
+    assert tex2 == exp["TEX_S2"] and 1 in tex2                       # ... and external to S2
+    # I_E from the VV relation: an edge is internal to the segment of its lower vertex
+    g = oracle.relations_global(3, 6, T, mask=2)
+    per_seg = [sum(int((g["vv_idx"][g["vv_off"][v]:g["vv_off"][v + 1]] > v).sum()) for v in range(lo, hi)) for lo, hi in S]
+    assert [0, per_seg[0], per_seg[0] + per_seg[1]] == exp["I_E"]
+
+
+@pytest.mark.parametrize("dim,n,seed", [(3, 7, 3), (2, 12, 4)])
+def test_internal_external_brute_force(dim, n, seed):
+    """I_T / T_ex against set arithmetic on small meshes with holes: the segments' internal ranges tile
+    [0, nT); internal + external = every simplex touching the segment; no simplex is both."""
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=40, permute=True, drop_frac=0.2, seed=seed)
+    T = m.simplices
+    prev = 0
+    for c in range(m.num_clusters):
+        lo, hi = int(m.cluster_offsets[c]), int(m.cluster_offsets[c + 1])
+        a, b = oracle.internal_range(dim, T, lo, hi)
+        assert a == prev and b >= a
+        prev = b
+        ext = oracle.external_list(dim, T, lo, hi)
+        touching = {t for t in range(len(T)) if any(lo <= v < hi for v in T[t])}
+        internal = {t for t in range(len(T)) if lo <= min(T[t]) < hi}
+        assert set(range(a, b)) == internal
+        assert ext.tolist() == sorted(touching - internal)
+    assert prev == len(T)
