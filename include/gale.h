@@ -175,6 +175,27 @@ int32_t gale_mesh_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_m
 /* Statistics of the initialization (Table 4 :393-397 reports its time), for reporting. */
 int32_t gale_mesh_info(const gale_mesh_t *mesh, gale_mesh_info_t *out);
 
+/* What the initialization built for one tile (the interval array I_T and the external list
+ * T_ex of a segment; a tile is this library's segment). For inspection and tests. The
+ * DEVICE pointers point into the workspace and stay valid as long as the handle. */
+typedef struct {
+  int32_t v_lo, nrows;            /* the tile's vertices [v_lo, v_lo + nrows)                          */
+  int32_t t_lo, num_internal;     /* I_T: its internal simplices [t_lo, t_lo + num_internal)           */
+  int32_t num_external;           /* length of its T_ex list                                           */
+  int32_t num_lower_halo, num_local; /* vertices sharing a simplex with the tile, below it / tile + halo */
+  int32_t cluster;                /* the cluster the tile belongs to                                   */
+  const int32_t *d_external;      /* DEVICE [num_external] ascending simplex ids (T_ex)                */
+  const int32_t *d_local_to_global; /* DEVICE [num_local] ascending vertex ids: halo below, tile, halo above */
+} gale_tile_view_t;
+
+/* tile in [0, gale_mesh_info().num_tiles); tiles are numbered cluster by cluster, ascending v_lo. */
+int32_t gale_mesh_tile(const gale_mesh_t *mesh, int32_t tile, gale_tile_view_t *out);
+
+/* DEVICE pointer to the interval array I_T per vertex, [num_vertices + 1]: entry v = first simplex whose
+ * lowest vertex is >= v, so the internal simplices of any vertex range [lo, hi) are
+ * [I[lo], I[hi]). */
+int32_t gale_mesh_interval_array(const gale_mesh_t *mesh, const int32_t **d_first_simplex);
+
 /* Producer side: enqueue the relation kernels for the clusters
  * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) and, when
  * queue_depth > 0, the D2H copy into a pinned slot on the library's side stream.

@@ -54,7 +54,14 @@ class gale_mesh_info_t(ctypes.Structure):
                 ("tune_dense_ms", ctypes.c_float), ("tune_walk_ms", ctypes.c_float), ("reserved", ctypes.c_int32)]
 
 
-EXPORTS = ["gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+class gale_tile_view_t(ctypes.Structure):
+    _fields_ = [("v_lo", ctypes.c_int32), ("nrows", ctypes.c_int32), ("t_lo", ctypes.c_int32),
+                ("num_internal", ctypes.c_int32), ("num_external", ctypes.c_int32),
+                ("num_lower_halo", ctypes.c_int32), ("num_local", ctypes.c_int32), ("cluster", ctypes.c_int32),
+                ("d_external", ctypes.c_void_p), ("d_local_to_global", ctypes.c_void_p)]
+
+
+EXPORTS = ["gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
            "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
@@ -95,6 +102,10 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
     lib.gale_mesh_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
     lib.gale_mesh_info.restype = ctypes.c_int32
     lib.gale_mesh_info.argtypes = [vp, ctypes.POINTER(gale_mesh_info_t)]
+    lib.gale_mesh_tile.restype = ctypes.c_int32
+    lib.gale_mesh_tile.argtypes = [vp, ctypes.c_int32, ctypes.POINTER(gale_tile_view_t)]
+    lib.gale_mesh_interval_array.restype = ctypes.c_int32
+    lib.gale_mesh_interval_array.argtypes = [vp, ctypes.POINTER(vp)]
     lib.gale_cluster_batch_compute.restype = ctypes.c_int32
     lib.gale_cluster_batch_compute.argtypes = [vp, ctypes.c_uint32, _i32p, ctypes.c_int32, vp]
     lib.gale_queue_pop.restype = ctypes.c_int32
@@ -166,6 +177,19 @@ def gale_mesh_info(handle) -> gale_mesh_info_t:
     return info
 
 
+def gale_mesh_tile(handle, tile: int) -> gale_tile_view_t:
+    v = gale_tile_view_t()
+    _check(load_library().gale_mesh_tile(handle, tile, ctypes.byref(v)), "gale_mesh_tile")
+    return v
+
+
+def gale_mesh_interval_array(handle) -> int:
+    """DEVICE address of I_T per vertex (int32[num_vertices + 1])."""
+    ptr = ctypes.c_void_p()
+    _check(load_library().gale_mesh_interval_array(handle, ctypes.byref(ptr)), "gale_mesh_interval_array")
+    return int(ptr.value)
+
+
 def gale_cluster_batch_compute(handle, relation_mask: int, cluster_ids, cuda_stream: int = 0) -> int:
     """Returns the status (OK or ERR_WOULD_BLOCK); other errors raise."""
     ids = np.ascontiguousarray(cluster_ids, dtype=np.int32)
@@ -232,6 +256,13 @@ class GaleMesh:
         finally:
             gale_plan_destroy(plan)
         self.info = gale_mesh_info(self.handle)
+
+    def device_array(self, ptr: int, n: int):
+        """int32 torch view of n entries of the workspace at DEVICE address ptr (index arrays, slots)."""
+        if not ptr or n == 0:
+            return self.torch.empty(0, dtype=self.torch.int32, device=self.device)
+        off = ptr - self.workspace.data_ptr()
+        return self.workspace[off:off + 4 * n].view(self.torch.int32)
 
     def compute(self, cluster_ids, relation_mask: int = REL_ALL, stream=None) -> int:
         s = (stream or self.torch.cuda.current_stream(self.device)).cuda_stream

@@ -6,6 +6,7 @@
 // computed by the kernels in gale_kernels.cuh; nothing here computes VT/VV/TT on the CPU.
 #include "gale_kernels.cuh"
 #include "gale_walk.cuh"
+#include "gale_init.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -43,7 +44,25 @@ inline size_t up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 inline long long pad_to(long long x, long long a) { return (x + a - 1) / a * a; }
 constexpr int kSmemLimit = 227 * 1024;  // opt-in dynamic shared memory per block on sm_100
 
-// ---- result of the create-time analysis ----------------------------------------------------------
+// Device memory owned by the library for the duration of the initialization.
+struct DevMem {
+  void* p = nullptr;
+  size_t bytes = 0;
+  DevMem() = default;
+  DevMem(const DevMem&) = delete;
+  DevMem& operator=(const DevMem&) = delete;
+  ~DevMem() { release(); }
+  void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+  int alloc(size_t n) {
+    release();
+    bytes = n;
+    GALE_CUDA(cudaMalloc(&p, std::max<size_t>(n, 256)));
+    return GALE_OK;
+  }
+  template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+// ---- result of the initialization analysis -----------------------------------------
 struct Plan {
   // key
   const int32_t* dT = nullptr;
@@ -51,11 +70,12 @@ struct Plan {
   long long nT = 0;
   uint32_t flags = 0;
   std::vector<int32_t> cl_off;
-  // index (host copies)
+  // the index, built on the device (gale_init.cuh); owned here until build_mesh copies it into the
+  // caller's workspace
   int tv = 0, nTiles = 0, NT = 0;
-  std::vector<int32_t> first_tet, opp_first, opp_perm, cl_tile_begin, tex, gid;
-  std::vector<uint16_t> loc;            // 4 per staged simplex (build); compacted into loc8 when lb == 1
-  std::vector<uint8_t> loc8;
+  DevMem d_first_tet, d_opp_first, d_opp_perm, d_tex, d_gid, d_loc;
+  size_t n_tex = 0, n_gid = 0, loc_bytes = 0;   // element counts / bytes of tex, gid, loc incl. padding
+  std::vector<int32_t> cl_tile_begin;
   long long staged_padded = 0;          // staged simplices incl. per-tile padding
   std::vector<TileDesc> tiles;
   SmemCfg cfg{};                        // capacities for the full relation mask
@@ -70,7 +90,6 @@ struct Plan {
   std::vector<int32_t> cl_t_lo;         // [nC+1] first internal simplex of cluster c (I_T)
   long long max_rows = 0, max_vt = 0, max_vv = 0, max_tt = 0;
   double analyse_ms = 0;
-
 };
 
 struct SlotLayout {
@@ -87,18 +106,6 @@ SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
   L.tt = o;     o = up(o + size_t(maxB) * p.max_tt * D * 4);
   L.total = o;
   return L;
-}
-
-int validate_host(const Plan& p, const std::vector<int32_t>& T) {
-  const int D = p.dim + 1;
-  for (long long t = 0; t < p.nT; ++t) {
-    const int32_t* r = T.data() + t * D;
-    if (r[0] < 0 || r[D - 1] >= p.nV) return GALE_ERR_NOT_CANONICAL;
-    for (int k = 1; k < D; ++k)
-      if (r[k] <= r[k - 1]) return GALE_ERR_NOT_CANONICAL;
-    if (t > 0 && !std::lexicographical_compare(r - D, r, r, r + D)) return GALE_ERR_NOT_CANONICAL;
-  }
-  return GALE_OK;
 }
 
 // C4: every facet has at most two cofaces (sorted facet list, like the paper's sorted F list, :178).
@@ -179,245 +186,302 @@ inline gale::WalkLayout walk_layout_for(int D, const SmemCfg& c) {
 // not of a handle: raise every instantiation to the device limit once, never lower it.
 cudaError_t allow_max_smem(KernelFn fn) { return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit); }
 
-// Tiles of `tv` vertices, their T_ex lists, halo lists and the tile-local encoding of their staged
-// simplices. Returns false if a tile exceeds a kernel limit for this tv (the caller retries smaller).
-bool build_tiles(Plan& p, const std::vector<int32_t>& T, int tv) {
-  const int D = p.dim + 1;
+// Host <-> device helpers of the initialization.
+template <class V>
+int upload_vec(DevMem& d, const V& v, cudaStream_t st) {
+  int rc = d.alloc(v.size() * sizeof(typename V::value_type));
+  if (rc != GALE_OK) return rc;
+  if (!v.empty()) GALE_CUDA(cudaMemcpyAsync(d.p, v.data(), v.size() * sizeof(typename V::value_type), cudaMemcpyHostToDevice, st));
+  return GALE_OK;
+}
+template <class T>
+int download_vec(std::vector<T>& v, const void* d, size_t n, cudaStream_t st) {
+  v.resize(n);
+  if (n) GALE_CUDA(cudaMemcpyAsync(v.data(), d, n * sizeof(T), cudaMemcpyDeviceToHost, st));
+  GALE_CUDA(cudaStreamSynchronize(st));
+  return GALE_OK;
+}
+inline int blocks_for(long long n, int threads) { return int(std::max<long long>(1, (n + threads - 1) / threads)); }
+
+constexpr int kRefCap = 16384;  // vertex references (D * staged simplices) a tile may have in the halo pass
+
+// Tiles of `tv` vertices on the device: T_ex lists, halo vertices, the tile-local encoding
+// of the staged simplices. The host sees per-tile scalars only. fits = false: a tile exceeds a kernel
+// limit at this tile size (the caller retries with a smaller one).
+template <int D>
+int build_tiles_device(Plan& p, int tv, cudaStream_t st, bool& fits) {
+  namespace gi = gale::init;
+  fits = true;
   p.tv = tv;
   p.NT = threads_for_tile(tv);
-  std::vector<int32_t> tile_vlo;
+  // tile table (host: one entry per tile)
+  std::vector<int32_t> vlo, nrows, tile_cluster;
   p.cl_tile_begin.assign(p.nC + 1, 0);
   for (int c = 0; c < p.nC; ++c) {
-    p.cl_tile_begin[c] = int(tile_vlo.size());
-    for (int v = p.cl_off[c]; v < p.cl_off[c + 1]; v += tv) tile_vlo.push_back(v);
-  }
-  p.cl_tile_begin[p.nC] = int(tile_vlo.size());
-  p.nTiles = int(tile_vlo.size());
-  tile_vlo.push_back(p.nV);
-  const int nTiles = p.nTiles;
-  std::vector<int32_t> tile_of(p.nV), tile_vhi(nTiles);
-  for (int c = 0; c < p.nC; ++c)
-    for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) {
-      tile_vhi[i] = std::min(tile_vlo[i] + tv, p.cl_off[c + 1]);
-      for (int v = tile_vlo[i]; v < tile_vhi[i]; ++v) tile_of[v] = i;
-    }
-  // T_ex: simplex t is external to every tile it touches other than the tile of its lowest vertex
-  std::vector<long long> raw_off(nTiles + 1, 0);
-  std::vector<int32_t> raw;
-  for (int pass = 0; pass < 2; ++pass) {
-    std::vector<long long> cur;
-    if (pass == 1) {
-      for (int i = 0; i < nTiles; ++i) raw_off[i + 1] += raw_off[i];
-      raw.resize(size_t(raw_off[nTiles]));
-      cur.assign(raw_off.begin(), raw_off.end() - 1);
-    }
-    for (long long t = 0; t < p.nT; ++t) {
-      const int32_t* r = T.data() + t * D;
-      const int t0 = tile_of[r[0]];
-      int seen[3], ns = 0;
-      for (int k = 1; k < D; ++k) {
-        const int tk = tile_of[r[k]];
-        if (tk == t0) continue;
-        bool dup = false;
-        for (int s = 0; s < ns; ++s) dup |= seen[s] == tk;
-        if (dup) continue;
-        seen[ns++] = tk;
-        if (pass == 0) ++raw_off[tk + 1]; else raw[size_t(cur[tk]++)] = int32_t(t);
-      }
+    p.cl_tile_begin[c] = int(vlo.size());
+    for (int v = p.cl_off[c]; v < p.cl_off[c + 1]; v += tv) {
+      vlo.push_back(v);
+      nrows.push_back(std::min(tv, p.cl_off[c + 1] - v));
+      tile_cluster.push_back(c);
     }
   }
-  p.ext_refs = raw_off[nTiles];
-  // descriptors, padded offsets, limits that need no halo
+  const int nTiles = int(vlo.size());
+  p.cl_tile_begin[p.nC] = nTiles;
+  p.nTiles = nTiles;
   p.tiles.assign(nTiles, TileDesc{});
-  long long stg = 0, texo = 0;
-  const int max_local = D == 4 ? gale::kMaxLocal4 : gale::kMaxLocal3;
-  for (int c = 0; c < p.nC; ++c)
-    for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) {
-      TileDesc& d = p.tiles[i];
-      d.v_lo = tile_vlo[i];
-      d.nrows = tile_vhi[i] - tile_vlo[i];
-      d.t_lo = p.first_tet[d.v_lo];
-      d.s_int = p.first_tet[tile_vhi[i]] - d.t_lo;
-      d.s_ext = int(raw_off[i + 1] - raw_off[i]);
-      d.row_rel = d.v_lo - p.cl_off[c];
-      d.c_rows = p.cl_off[c + 1] - p.cl_off[c];
-      d.tt_rel = d.t_lo - p.first_tet[p.cl_off[c]];
-      d.stg_off = stg;
-      d.tex_off = texo;
-      const long long S = (long long)d.s_int + d.s_ext;
-      if (S > (D == 4 ? gale::kMaxStaged4 : gale::kMaxStaged3)) return false;
-      stg += pad_to(S, 4);
-      texo += pad_to(d.s_ext, 4);
-    }
-  p.staged_padded = stg;
-  p.loc.assign(size_t(stg) * 4 + 16, 0);
-  p.loc8.clear();
-  p.tex.assign(size_t(texo) + 4, 0);
-  for (int i = 0; i < nTiles; ++i)
-    std::copy(raw.begin() + raw_off[i], raw.begin() + raw_off[i + 1], p.tex.begin() + p.tiles[i].tex_off);
-  // halo + local encoding, tiles split over host threads
-  const int nth = std::max(1, std::min<int>(32, std::min<int>(int(std::thread::hardware_concurrency()), nTiles / 64 + 1)));
-  std::vector<std::vector<int32_t>> gid_part(nth);
-  std::vector<int> tile_lo(nth + 1);
-  for (int w = 0; w <= nth; ++w) tile_lo[w] = int((long long)nTiles * w / nth);
-  std::atomic<bool> ok{true};
-  auto work = [&](int w) {
-    std::vector<uint16_t> map(size_t(p.nV), uint16_t(0xFFFF));
-    std::vector<int32_t>& hp = gid_part[w];
-    std::vector<int32_t> h;
-    for (int i = tile_lo[w]; i < tile_lo[w + 1] && ok.load(std::memory_order_relaxed); ++i) {
-      TileDesc& d = p.tiles[i];
-      const int v_lo = d.v_lo, v_hi = d.v_lo + d.nrows;
-      const int32_t* ex = p.tex.data() + d.tex_off;
-      auto simplex = [&](int s) { return T.data() + (long long)(s < d.s_ext ? ex[s] : d.t_lo + (s - d.s_ext)) * D; };
-      const int S = d.s_int + d.s_ext;
-      h.clear();
-      for (int s = 0; s < S; ++s) {
-        const int32_t* r = simplex(s);
-        for (int k = 0; k < D; ++k)
-          if ((r[k] < v_lo || r[k] >= v_hi) && map[r[k]] == 0xFFFF) { map[r[k]] = 0xFFFE; h.push_back(r[k]); }
-      }
-      std::sort(h.begin(), h.end());
-      const int nhalo = int(h.size());
-      const int nlo = int(std::lower_bound(h.begin(), h.end(), v_lo) - h.begin());
-      if (nhalo + d.nrows > max_local) {
-        for (int v : h) map[v] = 0xFFFF;
-        ok.store(false);
-        return;
-      }
-      for (int j = 0; j < nhalo; ++j) map[h[j]] = uint16_t(j < nlo ? j : j + d.nrows);
-      d.nlo = nlo;
-      d.nloc = nhalo + d.nrows;
-      d.gid_off = (long long)hp.size();  // relative to this thread's part; rebased below
-      uint16_t* out = p.loc.data() + d.stg_off * 4;
-      for (int s = 0; s < S; ++s) {
-        const int32_t* r = simplex(s);
-        for (int k = 0; k < 4; ++k)
-          out[s * 4 + k] = k >= D ? uint16_t(0xFFFF)
-                                  : (r[k] >= v_lo && r[k] < v_hi) ? uint16_t(nlo + (r[k] - v_lo)) : map[r[k]];
-      }
-      hp.insert(hp.end(), h.begin(), h.begin() + nlo);  // local id -> global id, ascending
-      for (int v = v_lo; v < v_hi; ++v) hp.push_back(v);
-      hp.insert(hp.end(), h.begin() + nlo, h.end());
-      hp.resize(size_t(pad_to((long long)hp.size(), 4)), 0);
-      for (int v : h) map[v] = 0xFFFF;
-    }
-  };
-  {
-    std::vector<std::thread> th;
-    for (int w = 1; w < nth; ++w) th.emplace_back(work, w);
-    work(0);
-    for (auto& t : th) t.join();
-  }
-  if (!ok.load()) return false;
-  long long hoff = 0;
-  for (int w = 0; w < nth; ++w) {
-    for (int i = tile_lo[w]; i < tile_lo[w + 1]; ++i) p.tiles[i].gid_off += hoff;
-    hoff += (long long)gid_part[w].size();
-  }
-  p.gid.assign(size_t(hoff) + 4, 0);
-  hoff = 0;
-  for (int w = 0; w < nth; ++w) {
-    std::copy(gid_part[w].begin(), gid_part[w].end(), p.gid.begin() + hoff);
-    hoff += (long long)gid_part[w].size();
-    std::vector<int32_t>().swap(gid_part[w]);
-  }
-  // largest facet group of a tile vertex (walk kernel's private tables): D-1 facets per simplex of its
-  // run + facet 0 of every simplex whose second vertex it is
-  p.gmax = 1;
-  for (int v = 0; v < p.nV; ++v)
-    p.gmax = std::max(p.gmax, (D - 1) * (p.first_tet[v + 1] - p.first_tet[v]) + (p.opp_first[v + 1] - p.opp_first[v]));
-  // shared-memory capacities known so far
-  long long smax = 4, sext = 4, sint = 2, nloc = 4;
-  for (const TileDesc& d : p.tiles) {
-    smax = std::max(smax, pad_to((long long)d.s_int + d.s_ext, 4));
-    sext = std::max(sext, pad_to(d.s_ext, 4));
-    sint = std::max(sint, pad_to(d.s_int, 2));
-    nloc = std::max(nloc, pad_to(d.nloc, 4));
-  }
+  p.ext_refs = 0; p.staged_padded = 0; p.n_tex = 4; p.n_gid = 4; p.loc_bytes = 64;
   p.cfg = SmemCfg{};
-  p.cfg.tv = tv;
-  p.cfg.smax = int(smax);
-  p.cfg.sext = int(sext);
-  p.cfg.nloc = int(nloc);
-  // 8-bit local ids when every tile has at most 255 local vertices: half the staged bytes (HBM and
-  // shared memory). 0xFF only pads the unused 4th entry of a triangle.
-  p.cfg.lb = nloc <= 255 ? 1 : 2;
-  if (p.cfg.lb == 1) {
-    p.loc8.resize(p.loc.size());
-    for (size_t i = 0; i < p.loc.size(); ++i) p.loc8[i] = uint8_t(p.loc[i]);
-    std::vector<uint16_t>().swap(p.loc);
-  }
-  p.cfg.sint = int(sint);
-  p.cfg.WT = int((smax + 31) / 32) | 1;
-  p.cfg.WV = int((nloc + 31) / 32) | 1;
-  return true;
-}
-
-struct DevBuf {  // temporary device memory of the analysis
-  void* p = nullptr;
-  ~DevBuf() { if (p) cudaFree(p); }
-  int alloc(size_t n) { GALE_CUDA(cudaMalloc(&p, std::max<size_t>(n, 16))); return GALE_OK; }
-  template <class V>
-  int upload(const V& v, cudaStream_t st) {
-    int rc = alloc(v.size() * sizeof(typename V::value_type));
-    if (rc != GALE_OK) return rc;
-    if (!v.empty())
-      GALE_CUDA(cudaMemcpyAsync(p, v.data(), v.size() * sizeof(typename V::value_type), cudaMemcpyHostToDevice, st));
+  p.cfg.tv = tv; p.cfg.smax = 4; p.cfg.sext = 4; p.cfg.sint = 2; p.cfg.nloc = 4; p.cfg.lb = 1;
+  p.cfg.WT = 1; p.cfg.WV = 1;
+  int rc;
+  if (nTiles == 0) {
+    if ((rc = p.d_tex.alloc(16)) || (rc = p.d_gid.alloc(16)) || (rc = p.d_loc.alloc(64))) return rc;
     return GALE_OK;
   }
-};
+  const int TB = 256;
+  DevMem d_vlo, d_nrows, d_tile_of, d_tlo, d_sint, d_cnt, d_scan, d_raw, d_cursor;
+  if ((rc = upload_vec(d_vlo, vlo, st)) || (rc = upload_vec(d_nrows, nrows, st)) ||
+      (rc = d_tile_of.alloc(size_t(std::max(p.nV, 1)) * 4)) || (rc = d_tlo.alloc(size_t(nTiles) * 4)) ||
+      (rc = d_sint.alloc(size_t(nTiles) * 4)) || (rc = d_cnt.alloc(size_t(nTiles + 1) * 4)) ||
+      (rc = d_scan.alloc((size_t(nTiles) / gi::kScanChunk + 2) * 4)))
+    return rc;
+  gi::k_tile_of<<<blocks_for(nTiles, TB), TB, 0, st>>>(d_vlo.as<int32_t>(), d_nrows.as<int32_t>(), nTiles, d_tile_of.as<int32_t>());
+  gi::k_tile_internal<<<blocks_for(nTiles, TB), TB, 0, st>>>(p.d_first_tet.as<int32_t>(), d_vlo.as<int32_t>(), d_nrows.as<int32_t>(),
+                                                             nTiles, d_tlo.as<int32_t>(), d_sint.as<int32_t>());
+  GALE_CUDA(cudaMemsetAsync(d_cnt.p, 0, size_t(nTiles + 1) * 4, st));
+  if (p.nT) gi::k_external<D, true><<<blocks_for(p.nT, TB), TB, 0, st>>>(p.dT, p.nT, d_tile_of.as<int32_t>(), d_cnt.as<int32_t>(), nullptr);
+  GALE_CUDA(gi::exclusive_scan_i32(d_cnt.as<int32_t>(), nTiles + 1, d_scan.as<int32_t>(), st));  // -> raw_off
+  std::vector<int32_t> raw_off, t_lo, s_int;
+  if ((rc = download_vec(raw_off, d_cnt.p, size_t(nTiles) + 1, st)) || (rc = download_vec(t_lo, d_tlo.p, size_t(nTiles), st)) ||
+      (rc = download_vec(s_int, d_sint.p, size_t(nTiles), st)))
+    return rc;
+  p.ext_refs = raw_off[nTiles];
+  // per-tile scalars, padded offsets, limits that need no halo
+  std::vector<int32_t> s_ext(nTiles);
+  std::vector<long long> stg_off(nTiles), tex_off(nTiles);
+  long long stg = 0, texo = 0, smax = 4, sextm = 4, sintm = 2;
+  for (int i = 0; i < nTiles; ++i) {
+    TileDesc& d = p.tiles[i];
+    const int c = tile_cluster[i];
+    d.v_lo = vlo[i]; d.nrows = nrows[i];
+    d.t_lo = t_lo[i]; d.s_int = s_int[i];
+    d.s_ext = s_ext[i] = raw_off[i + 1] - raw_off[i];
+    d.row_rel = d.v_lo - p.cl_off[c];
+    d.c_rows = p.cl_off[c + 1] - p.cl_off[c];
+    d.tt_rel = d.t_lo - p.cl_t_lo[c];
+    d.stg_off = stg_off[i] = stg;
+    d.tex_off = tex_off[i] = texo;
+    const long long S = (long long)d.s_int + d.s_ext;
+    if (S > (D == 4 ? gale::kMaxStaged4 : gale::kMaxStaged3) || S * D > kRefCap) { fits = false; return GALE_OK; }
+    stg += pad_to(S, 4);
+    texo += pad_to(d.s_ext, 4);
+    smax = std::max(smax, pad_to(S, 4));
+    sextm = std::max(sextm, pad_to(d.s_ext, 4));
+    sintm = std::max(sintm, pad_to(d.s_int, 2));
+  }
+  p.staged_padded = stg;
+  p.n_tex = size_t(texo) + 4;
+  // T_ex lists: scatter, then sort each tile's list ascending into its padded place
+  DevMem d_texoff, d_stgoff, d_sext;
+  if ((rc = d_raw.alloc(size_t(std::max<long long>(p.ext_refs, 1)) * 4)) || (rc = d_cursor.alloc(size_t(nTiles + 1) * 4)) ||
+      (rc = p.d_tex.alloc(p.n_tex * 4)) || (rc = upload_vec(d_texoff, tex_off, st)) || (rc = upload_vec(d_stgoff, stg_off, st)) ||
+      (rc = upload_vec(d_sext, s_ext, st)))
+    return rc;
+  GALE_CUDA(cudaMemcpyAsync(d_cursor.p, d_cnt.p, size_t(nTiles + 1) * 4, cudaMemcpyDeviceToDevice, st));
+  if (p.nT) gi::k_external<D, false><<<blocks_for(p.nT, TB), TB, 0, st>>>(p.dT, p.nT, d_tile_of.as<int32_t>(), d_cursor.as<int32_t>(), d_raw.as<int32_t>());
+  {
+    const int smem = gi::pow2_ceil(int(sextm)) * 4;
+    GALE_CUDA(cudaFuncSetAttribute(gi::k_sort_external, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    gi::k_sort_external<<<nTiles, TB, smem, st>>>(d_raw.as<int32_t>(), d_cnt.as<int32_t>(), d_texoff.as<long long>(), p.d_tex.as<int32_t>());
+    GALE_CUDA(cudaGetLastError());
+  }
+  d_raw.release(); d_cursor.release(); d_tile_of.release();
+  // halo of every tile: count, then (offsets known) write gid and loc
+  DevMem d_nlo, d_nhalo, d_gidoff, d_flag;
+  if ((rc = d_nlo.alloc(size_t(nTiles) * 4)) || (rc = d_nhalo.alloc(size_t(nTiles) * 4)) || (rc = d_flag.alloc(4))) return rc;
+  GALE_CUDA(cudaMemsetAsync(d_flag.p, 0, 4, st));
+  gi::TileArrays A{};
+  A.vlo = d_vlo.as<int32_t>(); A.nrows = d_nrows.as<int32_t>(); A.t_lo = d_tlo.as<int32_t>(); A.s_int = d_sint.as<int32_t>();
+  A.s_ext = d_sext.as<int32_t>(); A.tex_off = d_texoff.as<long long>(); A.stg_off = d_stgoff.as<long long>();
+  A.nlo = d_nlo.as<int32_t>(); A.nhalo = d_nhalo.as<int32_t>();
+  const int halo_smem = 2 * gi::pow2_ceil(int(smax) * D) * 4;
+  {
+    auto fn = gi::k_halo<D, 1, false>;
+    GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));  // the kernel has static shared memory too
+    fn<<<nTiles, TB, halo_smem, st>>>(p.dT, p.d_tex.as<int32_t>(), A, kRefCap, nullptr, nullptr, d_flag.as<int>());
+    GALE_CUDA(cudaGetLastError());
+  }
+  std::vector<int32_t> nlo, nhalo;
+  if ((rc = download_vec(nlo, d_nlo.p, size_t(nTiles), st)) || (rc = download_vec(nhalo, d_nhalo.p, size_t(nTiles), st))) return rc;
+  std::vector<long long> gid_off(nTiles);
+  long long gido = 0, nlocm = 4;
+  const int max_local = D == 4 ? gale::kMaxLocal4 : gale::kMaxLocal3;
+  for (int i = 0; i < nTiles; ++i) {
+    TileDesc& d = p.tiles[i];
+    d.nlo = nlo[i];
+    d.nloc = nhalo[i] + d.nrows;
+    if (d.nloc > max_local) { fits = false; return GALE_OK; }
+    d.gid_off = gid_off[i] = gido;
+    gido += pad_to(d.nloc, 4);
+    nlocm = std::max(nlocm, pad_to(d.nloc, 4));
+  }
+  // 8-bit local ids when every tile has at most 255 local vertices: half the staged bytes (HBM and shared
+  // memory). 0xFF only pads the unused 4th entry of a triangle.
+  p.cfg.lb = nlocm <= 255 ? 1 : 2;
+  p.n_gid = size_t(gido) + 4;
+  p.loc_bytes = size_t(stg) * 4 * p.cfg.lb + 64;
+  if ((rc = p.d_gid.alloc(p.n_gid * 4)) || (rc = p.d_loc.alloc(p.loc_bytes)) || (rc = upload_vec(d_gidoff, gid_off, st))) return rc;
+  A.gid_off = d_gidoff.as<long long>();
+  {
+    auto fn = p.cfg.lb == 1 ? gi::k_halo<D, 1, true> : gi::k_halo<D, 2, true>;
+    GALE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));  // the kernel has static shared memory too
+    fn<<<nTiles, TB, halo_smem, st>>>(p.dT, p.d_tex.as<int32_t>(), A, kRefCap, p.d_gid.as<int32_t>(), p.d_loc.p, d_flag.as<int>());
+    GALE_CUDA(cudaGetLastError());
+  }
+  GALE_CUDA(cudaStreamSynchronize(st));
+  p.cfg.smax = int(smax); p.cfg.sext = int(sextm); p.cfg.sint = int(sintm); p.cfg.nloc = int(nlocm);
+  p.cfg.WT = int((smax + 31) / 32) | 1;
+  p.cfg.WV = int((nlocm + 31) / 32) | 1;
+  return GALE_OK;
+}
 
-// Sizing run (count mode of the batch kernel) over all tiles: exact VT / VV entry counts per tile.
+// Sizing run (count mode of the dense kernel) over all tiles: exact VT / VV entry counts per tile.
 // `fits` tells whether the count-mode shared memory fits at this tile size.
-int run_sizing(Plan& p, const int32_t* dT, cudaStream_t st, std::vector<long long>& stats, bool& fits) {
+int run_sizing(Plan& p, cudaStream_t st, std::vector<long long>& stats, bool& fits) {
   const int D = p.dim + 1;
   fits = true;
   stats.assign(size_t(p.nTiles) * 4, 0);
   if (p.nTiles == 0) return GALE_OK;
-  const SmemCfg full = p.cfg;
-  const std::vector<uint32_t> parts = {3u};
-  if (layout_for(D, cfg_for_mask(full, 3, true)).total > kSmemLimit) { fits = false; return GALE_OK; }
-
-  DevBuf b_ft, b_tiles, b_tex, b_gid, b_loc, b_stats, b_err;
+  const SmemCfg c = cfg_for_mask(p.cfg, 3, true);
+  const gale::SmemLayout lay = layout_for(D, c);
+  if (lay.total > kSmemLimit) { fits = false; return GALE_OK; }
+  DevMem b_tiles, b_stats, b_err;
   int rc;
-  if ((rc = b_ft.upload(p.first_tet, st)) || (rc = b_tiles.upload(p.tiles, st)) || (rc = b_tex.upload(p.tex, st)) ||
-      (rc = b_gid.upload(p.gid, st)) || (rc = (p.cfg.lb == 1 ? b_loc.upload(p.loc8, st) : b_loc.upload(p.loc, st))) ||
-      (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4)))
-    return rc;
+  if ((rc = upload_vec(b_tiles, p.tiles, st)) || (rc = b_stats.alloc(stats.size() * 8)) || (rc = b_err.alloc(4))) return rc;
   GALE_CUDA(cudaMemsetAsync(b_err.p, 0, 4, st));
   DeviceMesh dm{};
-  dm.T = dT;
-  dm.first_tet = static_cast<int32_t*>(b_ft.p);
-  dm.tiles = static_cast<TileDesc*>(b_tiles.p);
-  dm.tex = static_cast<int32_t*>(b_tex.p);
-  dm.gid = static_cast<int32_t*>(b_gid.p);
-  dm.loc = b_loc.p;
-  dm.err = static_cast<int32_t*>(b_err.p);
+  dm.T = p.dT;
+  dm.first_tet = p.d_first_tet.as<int32_t>();
+  dm.tiles = b_tiles.as<TileDesc>();
+  dm.tex = p.d_tex.as<int32_t>();
+  dm.gid = p.d_gid.as<int32_t>();
+  dm.loc = p.d_loc.p;
+  dm.err = b_err.as<int32_t>();
   KernelFn fn = kernel_for(D, p.NT, true, p.cfg.lb);
-  std::vector<long long> part_stats(stats.size());
-  for (uint32_t m : parts) {
-    const SmemCfg c = cfg_for_mask(full, m, true);
-    const gale::SmemLayout lay = layout_for(D, c);
-    const int smem = lay.total;
-    GALE_CUDA(allow_max_smem(fn));
-    gale::BatchParams P{};
-    P.mask = m | gale::MODE_COUNT;
-    gale::OutPtrs O{};
-    O.stats = static_cast<long long*>(b_stats.p);
-    fn<<<p.nTiles, p.NT, smem, st>>>(dm, P, c, lay, O);
-    GALE_CUDA(cudaGetLastError());
-    GALE_CUDA(cudaMemcpyAsync(part_stats.data(), b_stats.p, stats.size() * 8, cudaMemcpyDeviceToHost, st));
-    GALE_CUDA(cudaStreamSynchronize(st));
-    for (int i = 0; i < p.nTiles; ++i) {
-      if (m & 1) stats[i * 4 + 0] = part_stats[i * 4 + 0];
-      if (m & 2) stats[i * 4 + 1] = part_stats[i * 4 + 1];
-    }
-  }
+  GALE_CUDA(allow_max_smem(fn));
+  gale::BatchParams P{};
+  P.mask = 3u | gale::MODE_COUNT;
+  gale::OutPtrs O{};
+  O.stats = b_stats.as<long long>();
+  fn<<<p.nTiles, p.NT, lay.total, st>>>(dm, P, c, lay, O);
+  GALE_CUDA(cudaGetLastError());
+  if ((rc = download_vec(stats, b_stats.p, stats.size(), st))) return rc;
   int err = 0;
   GALE_CUDA(cudaMemcpyAsync(&err, b_err.p, 4, cudaMemcpyDeviceToHost, st));
   GALE_CUDA(cudaStreamSynchronize(st));
   if (err) { g_last_error = "device guard fired during sizing: " + std::to_string(err); return GALE_ERR_WORKSPACE; }
+  return GALE_OK;
+}
+
+// The initialization on the device: validation, I_T per vertex, the index of simplices
+// by second vertex, tiles with their T_ex lists and local encodings, exact output sizes.
+template <int D>
+int analyse_device(Plan& p, const gale_mesh_desc_t& d, cudaStream_t st) {
+  namespace gi = gale::init;
+  const int TB = 256;
+  int rc;
+  DevMem d_flags;  // [0] not canonical, [1] gmax
+  if ((rc = d_flags.alloc(8))) return rc;
+  GALE_CUDA(cudaMemsetAsync(d_flags.p, 0, 8, st));
+  if ((d.flags & (GALE_VALIDATE | GALE_VALIDATE_MANIFOLD)) && p.nT)
+    gi::k_validate<D><<<blocks_for(p.nT, TB), TB, 0, st>>>(p.dT, p.nT, p.nV, d_flags.as<int>());
+  {
+    int bad = 0;
+    GALE_CUDA(cudaMemcpyAsync(&bad, d_flags.p, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    if (bad) return GALE_ERR_NOT_CANONICAL;
+  }
+  if (d.flags & GALE_VALIDATE_MANIFOLD) {  // C4, optional: the facet sort runs on the host (slow path, opt-in)
+    std::vector<int32_t> T;
+    if ((rc = download_vec(T, p.dT, size_t(p.nT) * D, st))) return rc;
+    if ((rc = validate_manifold<D>(p, T)) != GALE_OK) return rc;
+  }
+  // I_T per vertex; simplices grouped by second vertex
+  DevMem d_scan, d_cursor;
+  if ((rc = p.d_first_tet.alloc(size_t(p.nV + 2) * 4)) || (rc = p.d_opp_first.alloc(size_t(p.nV + 2) * 4)) ||
+      (rc = p.d_opp_perm.alloc(size_t(std::max<long long>(p.nT, 1)) * 4)) ||
+      (rc = d_scan.alloc((size_t(p.nV + 1) / gi::kScanChunk + 2) * 4)) || (rc = d_cursor.alloc(size_t(p.nV + 2) * 4)))
+    return rc;
+  gi::k_first_tet<D><<<blocks_for(p.nT + 1, TB), TB, 0, st>>>(p.dT, p.nT, p.nV, p.d_first_tet.as<int32_t>());
+  GALE_CUDA(cudaMemsetAsync(p.d_opp_first.p, 0, size_t(p.nV + 2) * 4, st));
+  if (p.nT) gi::k_second_count<D><<<blocks_for(p.nT, TB), TB, 0, st>>>(p.dT, p.nT, p.d_opp_first.as<int32_t>());
+  GALE_CUDA(gi::exclusive_scan_i32(p.d_opp_first.as<int32_t>(), p.nV + 1, d_scan.as<int32_t>(), st));
+  GALE_CUDA(cudaMemcpyAsync(d_cursor.p, p.d_opp_first.p, size_t(p.nV + 1) * 4, cudaMemcpyDeviceToDevice, st));
+  if (p.nT) gi::k_second_fill<D><<<blocks_for(p.nT, TB), TB, 0, st>>>(p.dT, p.nT, d_cursor.as<int32_t>(), p.d_opp_perm.as<int32_t>());
+  if (p.nV) gi::k_gmax<D><<<blocks_for(p.nV, TB), TB, 0, st>>>(p.d_first_tet.as<int32_t>(), p.d_opp_first.as<int32_t>(), p.nV, d_flags.as<int>() + 1);
+  {  // I_T per cluster
+    DevMem d_off, d_out;
+    if ((rc = upload_vec(d_off, p.cl_off, st)) || (rc = d_out.alloc(size_t(p.nC + 1) * 4))) return rc;
+    gi::k_gather<<<blocks_for(p.nC + 1, TB), TB, 0, st>>>(p.d_first_tet.as<int32_t>(), d_off.as<int32_t>(), p.nC + 1, d_out.as<int32_t>());
+    if ((rc = download_vec(p.cl_t_lo, d_out.p, size_t(p.nC) + 1, st))) return rc;
+    int g = 0;
+    GALE_CUDA(cudaMemcpyAsync(&g, d_flags.as<int>() + 1, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    p.gmax = std::max(1, g);
+  }
+  d_cursor.release();
+
+  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 64);  // measured optima on configs 5 and 2
+  std::vector<long long> stats;
+  for (;; tv = (tv + 1) / 2) {
+    if (tv < 1) return GALE_ERR_UNSUPPORTED;
+    const bool last = tv == 1;
+    bool fits = true;
+    if ((rc = build_tiles_device<D>(p, tv, st, fits)) != GALE_OK) return rc;
+    if (fits && (rc = run_sizing(p, st, stats, fits)) != GALE_OK) return rc;
+    if (fits) {
+      long long vt_max = 1, vv_max = 1, tbl_max = 4;
+      for (int i = 0; i < p.nTiles; ++i) {
+        vt_max = std::max(vt_max, stats[i * 4 + 0]);
+        vv_max = std::max(vv_max, stats[i * 4 + 1]);
+        tbl_max = std::max(tbl_max, stats[i * 4 + 0] + (long long)(D - 2) * p.tiles[i].s_int);
+      }
+      p.cfg.vt_max = int(pad_to(vt_max, 8));
+      p.cfg.vv_max = int(pad_to(vv_max, 8));
+      p.cfg.tbl = int(pad_to(tbl_max, 4));
+      p.smem_bytes = layout_for(D, p.cfg).total;
+      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p.smem_bytes <= kSmemLimit;
+    }
+    if (fits) break;
+    if (last) { g_last_error = "a single vertex star exceeds the kernels' shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
+  }
+  {  // can the walk kernel run these tiles?
+    // load <= 3/4 even if no facet of a group is shared; every interior facet is recorded twice, so the
+    // usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
+    p.cfg.hs = std::max(8, (p.gmax + p.gmax / 3 + 1) & ~1);
+    p.w_NT = walk_threads_for_tile(p.tv);
+    p.w_smem = walk_layout_for(D, walk_cfg_for_mask(p.cfg, 7)).total;
+    p.walk_ok = p.tv <= 256 && p.w_smem <= kSmemLimit && p.cfg.smax < 32768 && p.cfg.vt_max < 65536;
+  }
+  // per-tile output placement inside its cluster, per-cluster sizes
+  p.cl_vt.assign(p.nC, 0);
+  p.cl_vv.assign(p.nC, 0);
+  for (int c = 0; c < p.nC; ++c) {
+    long long vt = 0, vv = 0;
+    for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) {
+      TileDesc& t = p.tiles[i];
+      if (vt > INT32_MAX || vv > INT32_MAX) return GALE_ERR_UNSUPPORTED;
+      t.vt_rel = int32_t(vt); t.vv_rel = int32_t(vv);
+      t.vt_nnz = int32_t(stats[i * 4 + 0]); t.vv_nnz = int32_t(stats[i * 4 + 1]);
+      vt += t.vt_nnz; vv += t.vv_nnz;
+    }
+    p.cl_vt[c] = vt; p.cl_vv[c] = vv;
+    p.vt_total += vt; p.vv_total += vv;
+    p.max_rows = std::max<long long>(p.max_rows, p.cl_off[c + 1] - p.cl_off[c]);
+    p.max_vt = std::max(p.max_vt, vt);
+    p.max_vv = std::max(p.max_vv, vv);
+    p.max_tt = std::max<long long>(p.max_tt, p.cl_t_lo[c + 1] - p.cl_t_lo[c]);
+  }
   return GALE_OK;
 }
 
@@ -428,100 +492,11 @@ int analyse(const gale_mesh_desc_t& d, cudaStream_t st, std::unique_ptr<Plan>& o
   p->tv_req = d.tile_vertices; p->flags = d.flags;
   p->maxB = d.max_batch_clusters; p->queue_depth = d.queue_depth; p->device_ring = d.device_ring;
   p->cl_off.assign(d.h_cluster_offsets, d.h_cluster_offsets + d.num_clusters + 1);
-  const int D = d.dim + 1;
   if (p->cl_off.front() != 0 || p->cl_off.back() != p->nV) return GALE_ERR_INVALID_ARG;
   for (int c = 0; c < p->nC; ++c)
     if (p->cl_off[c] > p->cl_off[c + 1]) return GALE_ERR_INVALID_ARG;
-
-  std::vector<int32_t> T(size_t(p->nT) * D);
-  if (p->nT) GALE_CUDA(cudaMemcpy(T.data(), d.d_simplices, T.size() * 4, cudaMemcpyDeviceToHost));
-  if (d.flags & (GALE_VALIDATE | GALE_VALIDATE_MANIFOLD)) {
-    int rc = validate_host(*p, T);
-    if (rc != GALE_OK) return rc;
-  }
-  if (d.flags & GALE_VALIDATE_MANIFOLD) {
-    int rc = D == 4 ? validate_manifold<4>(*p, T) : validate_manifold<3>(*p, T);
-    if (rc != GALE_OK) return rc;
-  }
-  // I_T: first simplex whose lowest vertex is >= v; and the same keyed by the second vertex
-  p->first_tet.assign(p->nV + 1, 0);
-  p->opp_first.assign(p->nV + 1, 0);
-  for (long long t = 0; t < p->nT; ++t) {
-    ++p->first_tet[T[t * D] + 1];
-    ++p->opp_first[T[t * D + 1] + 1];
-  }
-  for (int v = 0; v < p->nV; ++v) {
-    p->first_tet[v + 1] += p->first_tet[v];
-    p->opp_first[v + 1] += p->opp_first[v];
-  }
-  p->opp_perm.resize(size_t(p->nT));
-  {
-    std::vector<int32_t> cur(p->opp_first.begin(), p->opp_first.end() - 1);
-    for (long long t = 0; t < p->nT; ++t) p->opp_perm[cur[T[t * D + 1]]++] = int32_t(t);
-  }
-  p->cl_t_lo.resize(p->nC + 1);
-  for (int c = 0; c <= p->nC; ++c) p->cl_t_lo[c] = p->first_tet[p->cl_off[c]];
-
-  int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 64);  // measured optima on configs 5 and 2 (profiles/r1_v5_ncu_summary.md)
-  std::vector<long long> stats;
-  bool shrunk = false;
-  for (;; tv = (tv + 1) / 2) {
-    if (tv < 1) return GALE_ERR_UNSUPPORTED;
-    const bool last = tv == 1;
-    bool fits = build_tiles(*p, T, tv);
-    if (fits) {
-      int rc = run_sizing(*p, d.d_simplices, st, stats, fits);
-      if (rc != GALE_OK) return rc;
-    }
-    if (fits) {
-      long long vt_max = 1, vv_max = 1, tbl_max = 4;
-      for (int i = 0; i < p->nTiles; ++i) {
-        vt_max = std::max(vt_max, stats[i * 4 + 0]);
-        vv_max = std::max(vv_max, stats[i * 4 + 1]);
-        tbl_max = std::max(tbl_max, stats[i * 4 + 0] + (long long)(D - 2) * p->tiles[i].s_int);
-      }
-      p->cfg.vt_max = int(pad_to(vt_max, 8));
-      p->cfg.vv_max = int(pad_to(vv_max, 8));
-      p->cfg.tbl = int(pad_to(tbl_max, 4));
-      p->smem_bytes = layout_for(D, p->cfg).total;
-      fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p->smem_bytes <= kSmemLimit;
-    }
-    // automatic tile size: tiles whose vertices are scattered in the mesh (graded meshes, config 4) need
-    // large per-block capacities and leave few resident blocks; half the tile measured +25 % there
-    if (fits && d.tile_vertices == 0 && !shrunk && tv >= 32 && D == 4 && p->smem_bytes > 56 * 1024) {
-      shrunk = true;
-      continue;
-    }
-    if (fits) break;
-    if (last) { g_last_error = "a single vertex star exceeds the kernel's shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
-  }
-  {  // can the walk kernel run these tiles?
-    // load <= 3/4 even if no facet of a group is shared; every interior facet is recorded twice, so the
-    // usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
-    p->cfg.hs = std::max(8, (p->gmax + p->gmax / 3 + 1) & ~1);
-    p->w_NT = walk_threads_for_tile(p->tv);
-    p->w_smem = walk_layout_for(D, walk_cfg_for_mask(p->cfg, 7)).total;
-    p->walk_ok = p->tv <= 256 && p->w_smem <= kSmemLimit && p->cfg.smax < 32768 && p->cfg.vt_max < 65536;
-  }
-  // per-tile output placement inside its cluster, per-cluster sizes
-  p->cl_vt.assign(p->nC, 0);
-  p->cl_vv.assign(p->nC, 0);
-  for (int c = 0; c < p->nC; ++c) {
-    long long vt = 0, vv = 0;
-    for (int i = p->cl_tile_begin[c]; i < p->cl_tile_begin[c + 1]; ++i) {
-      TileDesc& t = p->tiles[i];
-      if (vt > INT32_MAX || vv > INT32_MAX) return GALE_ERR_UNSUPPORTED;
-      t.vt_rel = int32_t(vt); t.vv_rel = int32_t(vv);
-      t.vt_nnz = int32_t(stats[i * 4 + 0]); t.vv_nnz = int32_t(stats[i * 4 + 1]);
-      vt += t.vt_nnz; vv += t.vv_nnz;
-    }
-    p->cl_vt[c] = vt; p->cl_vv[c] = vv;
-    p->vt_total += vt; p->vv_total += vv;
-    p->max_rows = std::max<long long>(p->max_rows, p->cl_off[c + 1] - p->cl_off[c]);
-    p->max_vt = std::max(p->max_vt, vt);
-    p->max_vv = std::max(p->max_vv, vv);
-    p->max_tt = std::max<long long>(p->max_tt, p->cl_t_lo[c + 1] - p->cl_t_lo[c]);
-  }
+  const int rc = d.dim == 3 ? analyse_device<4>(*p, d, st) : analyse_device<3>(*p, d, st);
+  if (rc != GALE_OK) return rc;
   p->analyse_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
   out = std::move(p);
   return GALE_OK;
@@ -561,14 +536,14 @@ IndexLayout index_layout(const Plan& p) {
   IndexLayout L;
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes + 64); return at; };  // 64: vector loads may read past the end
-  L.first_tet = take(p.first_tet.size() * 4);
-  L.opp_first = take(p.opp_first.size() * 4);
-  L.opp_perm = take(p.opp_perm.size() * 4);
+  L.first_tet = take(size_t(p.nV + 1) * 4);
+  L.opp_first = take(size_t(p.nV + 1) * 4);
+  L.opp_perm = take(size_t(p.nT) * 4);
   L.cl_tile_begin = take(p.cl_tile_begin.size() * 4);
   L.tiles = take(p.tiles.size() * sizeof(TileDesc));
-  L.tex = take(p.tex.size() * 4);
-  L.gid = take(p.gid.size() * 4);
-  L.loc = take(p.cfg.lb == 1 ? p.loc8.size() : p.loc.size() * 2);
+  L.tex = take(p.n_tex * 4);
+  L.gid = take(p.n_gid * 4);
+  L.loc = take(p.loc_bytes);
   L.total = o;
   return L;
 }
@@ -650,18 +625,19 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
   m->stream_ordered = (p->flags & GALE_STREAM_ORDERED) != 0;
   char* base = static_cast<char*>(d_workspace);
   const IndexLayout IL = index_layout(*p);
-  auto put = [&](size_t at, const void* src, size_t bytes) -> int {
-    if (bytes) GALE_CUDA(cudaMemcpyAsync(base + at, src, bytes, cudaMemcpyHostToDevice, st));
+  auto put = [&](size_t at, const void* src, size_t bytes, cudaMemcpyKind kind) -> int {
+    if (bytes) GALE_CUDA(cudaMemcpyAsync(base + at, src, bytes, kind, st));
     return GALE_OK;
   };
+  const cudaMemcpyKind D2D = cudaMemcpyDeviceToDevice, H2D = cudaMemcpyHostToDevice;
   int rc;
-  if ((rc = put(IL.first_tet, p->first_tet.data(), p->first_tet.size() * 4)) ||
-      (rc = put(IL.opp_first, p->opp_first.data(), p->opp_first.size() * 4)) ||
-      (rc = put(IL.opp_perm, p->opp_perm.data(), p->opp_perm.size() * 4)) ||
-      (rc = put(IL.cl_tile_begin, p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4)) ||
-      (rc = put(IL.tiles, p->tiles.data(), p->tiles.size() * sizeof(TileDesc))) ||
-      (rc = put(IL.tex, p->tex.data(), p->tex.size() * 4)) || (rc = put(IL.gid, p->gid.data(), p->gid.size() * 4)) ||
-      (rc = p->cfg.lb == 1 ? put(IL.loc, p->loc8.data(), p->loc8.size()) : put(IL.loc, p->loc.data(), p->loc.size() * 2)))
+  if ((rc = put(IL.first_tet, p->d_first_tet.p, size_t(p->nV + 1) * 4, D2D)) ||
+      (rc = put(IL.opp_first, p->d_opp_first.p, size_t(p->nV + 1) * 4, D2D)) ||
+      (rc = put(IL.opp_perm, p->d_opp_perm.p, size_t(p->nT) * 4, D2D)) ||
+      (rc = put(IL.cl_tile_begin, p->cl_tile_begin.data(), p->cl_tile_begin.size() * 4, H2D)) ||
+      (rc = put(IL.tiles, p->tiles.data(), p->tiles.size() * sizeof(TileDesc), H2D)) ||
+      (rc = put(IL.tex, p->d_tex.p, p->n_tex * 4, D2D)) || (rc = put(IL.gid, p->d_gid.p, p->n_gid * 4, D2D)) ||
+      (rc = put(IL.loc, p->d_loc.p, p->loc_bytes, D2D)))
     return rc;
   m->dm.T = p->dT;
   m->dm.first_tet = reinterpret_cast<int32_t*>(base + IL.first_tet);
@@ -673,14 +649,10 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
   m->dm.gid = reinterpret_cast<int32_t*>(base + IL.gid);
   m->dm.loc = base + IL.loc;
   m->index_bytes = IL.total;
-  // the index tables can be dropped on the host once uploaded (keep the small per-cluster ones)
+  // the library's own copy of the index is dropped once it sits in the workspace
   GALE_CUDA(cudaStreamSynchronize(st));
-  std::vector<int32_t>().swap(p->opp_perm);
-  std::vector<int32_t>().swap(p->tex);
-  std::vector<int32_t>().swap(p->gid);
-  std::vector<uint16_t>().swap(p->loc);
-  std::vector<uint8_t>().swap(p->loc8);
-  std::vector<int32_t>().swap(p->opp_first);
+  p->d_first_tet.release(); p->d_opp_first.release(); p->d_opp_perm.release();
+  p->d_tex.release(); p->d_gid.release(); p->d_loc.release();
 
   GALE_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&m->h_err), 64, cudaHostAllocMapped));
   *m->h_err = 0;
@@ -833,6 +805,26 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   out->tune_dense_ms = m->tune_ms[0];
   out->tune_walk_ms = m->tune_ms[1];
   out->reserved = 0;
+  return GALE_OK;
+}
+
+int32_t gale_mesh_tile(const gale_mesh_t* m, int32_t tile, gale_tile_view_t* out) {
+  if (!m || !out || tile < 0 || tile >= m->plan->nTiles) return GALE_ERR_INVALID_ARG;
+  const Plan& p = *m->plan;
+  const TileDesc& t = p.tiles[size_t(tile)];
+  out->v_lo = t.v_lo; out->nrows = t.nrows;
+  out->t_lo = t.t_lo; out->num_internal = t.s_int;
+  out->num_external = t.s_ext;
+  out->num_lower_halo = t.nlo; out->num_local = t.nloc;
+  out->cluster = int32_t(std::upper_bound(p.cl_tile_begin.begin(), p.cl_tile_begin.end(), tile) - p.cl_tile_begin.begin()) - 1;
+  out->d_external = m->dm.tex + t.tex_off;
+  out->d_local_to_global = m->dm.gid + t.gid_off;
+  return GALE_OK;
+}
+
+int32_t gale_mesh_interval_array(const gale_mesh_t* m, const int32_t** d_first_simplex) {
+  if (!m || !d_first_simplex) return GALE_ERR_INVALID_ARG;
+  *d_first_simplex = m->dm.first_tet;
   return GALE_OK;
 }
 
