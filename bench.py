@@ -215,6 +215,9 @@ def main():
                     help="kernel variant: auto = gale_mesh_create times both on a sample batch and keeps the faster")
     ap.add_argument("--sustain-s", type=float, default=2.0,
                     help="length of the second, sustained timed region in seconds (0 = skip)")
+    ap.add_argument("--consumer", type=int, default=0,
+                    help="> 0: also run CriticalPoints (VV + VT) over the whole mesh through the pinned queue with "
+                         "this many consumer threads and report the paper's per-stage waiting times (PAPER.md:411)")
     ap.add_argument("--impl", default="gale", choices=["gale", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -413,6 +416,16 @@ def main():
                        "D2H of every CSR batch to pinned slots, pop+read+release on the host"}
         g2.destroy()
 
+    cons = None
+    if args.consumer > 0 and rank == 0:
+        from paper_2507_15230_b200 import consumer as gc
+        mf = mesh if mesh.scalar is not None else meshgen.make_config(args.config, n=args.n, keep_fields=True)
+        r = gc.run_critical_points(mf, mf.scalar, consumers=args.consumer, batch=B, queue_depth=4,
+                                   kernel_flags={"auto": 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[args.kernel])
+        cons = {k: r[k] for k in ("minima", "maxima", "saddles", "regular", "wall_s", "batches", "consumers", "stages_ms", "note", "kernel")}
+        cons["what"] = ("CriticalPoints (PAPER.md:292) on the configs' float32 scalar field: VV + VT of every cluster through "
+                        "the pinned queue, classified by host consumer threads; stage times are sums over all batches")
+
     cpu = None
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         o = oracle_sample(mesh)
@@ -436,6 +449,8 @@ def main():
                                                        "mesh_bytes": int(mesh.simplices.nbytes)}),
                 "clocks": clocks, "sustained": sustained, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu}
+        if cons is not None:
+            line["consumer"] = cons
         print(json.dumps(line))
     if dist:
         dist.destroy_process_group()

@@ -242,3 +242,13 @@ def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:
         raise OracleError(f"non-manifold facet (status {st})")
     return dict(vt_off=vt_off, vt_idx=vt_idx[:vt_off[-1]].copy(), vv_off=vv_off,
                 vv_idx=vv_idx[:vv_off[-1]].copy(), tt=tt)
+
+
+def neighbour_sum(num_vertices: int, vv_off: np.ndarray, vv_idx: np.ndarray, scalar: np.ndarray) -> np.ndarray:
+    """Fig. 1(c) of the paper: for each vertex, the sum of the scalar values of its adjacent
+    vertices, from the oracle's own global VV. Plain loop, float64."""
+    out = np.zeros(num_vertices, np.float64)
+    for v in range(num_vertices):
+        for u in vv_idx[vv_off[v]:vv_off[v + 1]]:
+            out[v] += float(scalar[u])
+    return out

@@ -1,0 +1,110 @@
+"""The scalar-field consumer: Fig. 1's neighbour sum and the critical-point
+classification from VV + VT, on the CPU oracle's relations (no GPU), pinned by what the
+paper prints, closed forms and a naive re-enumeration; then (gpu) through the pinned queue with consumer
+threads and the paper's per-stage waiting-time report."""
+import numpy as np
+import pytest
+
+import meshgen
+import oracle
+from paper_2507_15230_b200 import consumer
+
+
+def _global(m, mask=3):
+    g = oracle.relations_global(m.dim, m.num_vertices, m.simplices, mask=mask)
+    return {k: (v.astype(np.int32) if k.endswith("_off") else v) for k, v in g.items()}
+
+
+def test_fig1_neighbour_sum():
+    """VV(v0) = [v1, v2, v3]; the derived value of v0 is the sum of their scalars."""
+    m = meshgen.toy_two_tets()
+    f = np.array([5.0, 1.0, 2.0, 4.0, 8.0], np.float32)
+    g = _global(m)
+    s = consumer.neighbour_sum(g["vv_off"], g["vv_idx"], f)
+    assert s[0] == f[1] + f[2] + f[3]
+    assert s[4] == f[1] + f[2] + f[3] and s[1] == f[0] + f[2] + f[3] + f[4]
+    assert np.allclose(s, oracle.neighbour_sum(5, g["vv_off"], g["vv_idx"], f))
+
+
+def test_neighbour_sum_closed_form_and_oracle():
+    m = meshgen.make_config(1, keep_fields=True)
+    g = _global(m)
+    ones = np.ones(m.num_vertices, np.float32)
+    deg = consumer.neighbour_sum(g["vv_off"], g["vv_idx"], ones)
+    assert deg.max() == 14 and np.array_equal(deg, np.diff(g["vv_off"]))      # interior Kuhn vertex: 14 neighbours
+    f = m.scalar.astype(np.float32)
+    assert np.allclose(consumer.neighbour_sum(g["vv_off"], g["vv_idx"], f),
+                       oracle.neighbour_sum(m.num_vertices, g["vv_off"], g["vv_idx"], f), rtol=1e-6)
+
+
+def _naive_types(m, g, f):
+    """Independent classification: components of the lower / upper link by flood fill over python sets."""
+    out = np.zeros(m.num_vertices, np.uint8)
+    T = m.simplices
+    for v in range(m.num_vertices):
+        nb = g["vv_idx"][g["vv_off"][v]:g["vv_off"][v + 1]].tolist()
+        low = {u for u in nb if (f[u], u) < (f[v], v)}
+        adj = {u: set() for u in nb}
+        for t in g["vt_idx"][g["vt_off"][v]:g["vt_off"][v + 1]]:
+            others = [int(u) for u in T[t] if u != v]
+            for a in others:
+                for b in others:
+                    if a != b and ((a in low) == (b in low)):
+                        adj[a].add(b)
+        comps = {True: 0, False: 0}
+        seen = set()
+        for u in nb:
+            if u in seen:
+                continue
+            comps[u in low] += 1
+            stack = [u]
+            seen.add(u)
+            while stack:
+                x = stack.pop()
+                for y in adj[x]:
+                    if y not in seen:
+                        seen.add(y)
+                        stack.append(y)
+        lo, up = comps[True], comps[False]
+        out[v] = consumer.MINIMUM if lo == 0 else consumer.MAXIMUM if up == 0 else consumer.REGULAR if (lo, up) == (1, 1) else consumer.SADDLE
+    return out
+
+
+@pytest.mark.parametrize("dim,n", [(3, 6), (2, 9)])
+def test_critical_points_against_naive_enumeration(dim, n):
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=60, permute=True, drop_frac=0.15, seed=11)
+    g = _global(m)
+    f = m.scalar.astype(np.float32)
+    got = consumer.critical_points(0, dim + 1, g["vt_off"], g["vt_idx"], g["vv_off"], g["vv_idx"], m.simplices, f)
+    assert np.array_equal(got, _naive_types(m, g, f))
+    assert (got == consumer.SADDLE).any() and (got == consumer.MINIMUM).any()
+
+
+@pytest.mark.parametrize("dim,n", [(3, 10), (2, 24)])
+def test_linear_function_on_a_convex_grid_has_one_minimum_one_maximum_no_saddle(dim, n):
+    """A linear function restricted to a triangulated convex box is PL with exactly one minimum, one
+    maximum and no saddle (its sub-level sets are convex)."""
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=200, permute=True, seed=12)
+    pos = np.rint(m.coords).astype(np.float64)                      # grid positions (the jitter is +-0.2)
+    f = (pos @ np.array([1.0, np.pi, np.e][:dim])).astype(np.float32)
+    g = _global(m)
+    got = consumer.critical_points(0, dim + 1, g["vt_off"], g["vt_idx"], g["vv_off"], g["vv_idx"], m.simplices, f)
+    hist = np.bincount(got, minlength=4)
+    assert hist[consumer.MINIMUM] == 1 and hist[consumer.MAXIMUM] == 1 and hist[consumer.SADDLE] == 0
+    assert got[np.argmin(f)] == consumer.MINIMUM and got[np.argmax(f)] == consumer.MAXIMUM
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("consumers", [1, 3])
+def test_critical_points_through_the_queue(consumers):
+    m = meshgen.make_config(3, n=32, keep_fields=True)
+    f = m.scalar.astype(np.float32)
+    res = consumer.run_critical_points(m, f, consumers=consumers, batch=4, queue_depth=3)
+    g = _global(m)
+    want = consumer.critical_points(0, m.dim + 1, g["vt_off"], g["vt_idx"], g["vv_off"], g["vv_idx"], m.simplices, f)
+    assert np.array_equal(res["types"], want)
+    assert res["minima"] + res["maxima"] + res["saddles"] + res["regular"] == m.num_vertices
+    st = res["stages_ms"]
+    assert res["batches"] == (m.num_clusters + 3) // 4
+    assert st["kernel_ms"] > 0 and st["d2h_ms"] > 0 and st["consume_ms"] > 0 and st["integrate_ms"] == 0
+    assert all(v >= 0 for v in st.values())
