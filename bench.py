@@ -213,6 +213,8 @@ def main():
                     "the bench line of record uses 7, other values are for per-relation diagnosis")
     ap.add_argument("--kernel", default="auto", choices=["auto", "dense", "walk"],
                     help="kernel variant: auto = gale_mesh_create times both on a sample batch and keeps the faster")
+    ap.add_argument("--stage-from-t", action="store_true",
+                    help="dense kernel: stage T + T_ex and map to local ids in the kernel (A/B of the create-time re-encoding)")
     ap.add_argument("--sustain-s", type=float, default=2.0,
                     help="length of the second, sustained timed region in seconds (0 = skip)")
     ap.add_argument("--consumer", type=int, default=0,
@@ -246,7 +248,8 @@ def main():
     t0 = time.time()
     gm = gale.GaleMesh(mesh.dim, mesh.num_vertices, mesh.simplices, mesh.cluster_offsets, max_batch_clusters=B,
                        queue_depth=0, device_ring=args.ring, tile_vertices=args.tile,
-                       flags={"auto": 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[args.kernel])
+                       flags={"auto": 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[args.kernel] |
+                       (gale.STAGE_FROM_T if args.stage_from_t else 0))
     create_s = time.time() - t0
     info = gm.info
     stream = torch.cuda.current_stream()

@@ -59,6 +59,9 @@ enum {
   GALE_KERNEL_WALK = 16u,      /* force the walk kernel (two threads per tile vertex); UNSUPPORTED if
                                   its capacity limits do not admit the mesh. Neither flag: create times
                                   both on a sample batch and keeps the faster (gale_mesh_info tells)   */
+  GALE_STAGE_FROM_T = 32u,     /* dense kernel only (implies nothing for the walk kernel): stage the rows of T
+                                  and T_ex themselves and derive the tile-local ids in the kernel instead of
+                                  reading the create-time re-encoding; slower, kept for the A/B in DESIGN.md */
   GALE_STREAM_ORDERED = 4u     /* run every batch kernel on the cuda_stream passed to compute itself
                                   (plain stream order: work the caller enqueues afterwards runs after
                                   the batch) instead of on the library's two overlapping launch streams */

@@ -15,7 +15,7 @@ import numpy as np
 from .build import LIB, build_library
 
 REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
-VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED, KERNEL_DENSE, KERNEL_WALK = 1, 2, 4, 8, 16
+VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED, KERNEL_DENSE, KERNEL_WALK, STAGE_FROM_T = 1, 2, 4, 8, 16, 32
 OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
 ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
 

@@ -108,6 +108,7 @@ struct SmemCfg {
   int sint;      // internal simplices (even): fallback queue, 0 without TT
   int tbl;       // facet-table slots of a tile = VT entries + (D-2) * internal simplices, 0 without TT
   int hs;        // walk kernel only: table slots per tile vertex (even), 0 without TT
+  int stage_t;   // dense kernel: 1 = stage from T + T_ex and map global -> local ids in the kernel (A/B)
   int WT;        // VT bitmap words per row (odd)
   int WV;        // VV bitmap words per row (odd), 0 without VV
   int vt_max;    // VT entries staged for write-out, 0 without VT or in count mode
@@ -492,9 +493,9 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
       fence_proxy_async();
       const uint32_t b_t = (uint32_t)((S0 + 3) & ~3) * (4u * LB);
       const uint32_t b_x = COUNT ? 0u : (uint32_t)((t.s_ext + 3) & ~3) * 4u;
-      const uint32_t b_g = (!COUNT && (do_vv || do_tt)) ? (uint32_t)((t.nloc + 3) & ~3) * 4u : 0u;
-      mbar_arrive_expect_tx(bar, b_t + b_x + b_g);
-      if (b_t) bulk_g2s(smem + L.tets, static_cast<const unsigned char*>(M.loc) + t.stg_off * (4 * LB), b_t, bar);
+      const uint32_t b_g = (!COUNT && (do_vv || do_tt || C.stage_t)) ? (uint32_t)((t.nloc + 3) & ~3) * 4u : 0u;
+      mbar_arrive_expect_tx(bar, (C.stage_t ? 0u : b_t) + b_x + b_g);
+      if (b_t && !C.stage_t) bulk_g2s(smem + L.tets, static_cast<const unsigned char*>(M.loc) + t.stg_off * (4 * LB), b_t, bar);
       if (b_x) bulk_g2s(smem + L.texid, M.tex + t.tex_off, b_x, bar);
       if (b_g) bulk_g2s(smem + L.gid, M.gid + t.gid_off, b_g, bar);
     }
@@ -561,6 +562,39 @@ gale_batch_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, con
   const int mis_vt = vt0 & 3, mis_vv = vv0 & 3;  // 16-byte phase of the tile's output segments
   for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);  // read in P2, after a barrier
   mbar_wait(bar, 0);
+  if (!COUNT && C.stage_t) {
+    // A/B of the create-time re-encoding (SURVEY §8 a1 as written): read the rows of T themselves —
+    // internal ones are contiguous, external ones are gathered through T_ex — and map every vertex to
+    // its tile-local id here: tile vertices by subtraction, halo vertices by binary search in the
+    // staged vertex table (sorted: [halo below][tile][halo above]).
+    const int up0 = nlo + nrows, nloc = td.nloc;
+    for (int s = tid; s < S; s += NT) {
+      const long long t = s < s_ext ? texid[s] : t_lo + (s - s_ext);
+      uint32_t l[4] = {LB == 1 ? 0xFFu : 0xFFFFu, LB == 1 ? 0xFFu : 0xFFFFu, LB == 1 ? 0xFFu : 0xFFFFu, LB == 1 ? 0xFFu : 0xFFFFu};
+      int v[D];
+      if constexpr (D == 4) {
+        const int4 q = __ldg(reinterpret_cast<const int4*>(M.T) + t);
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+      } else {
+#pragma unroll
+        for (int k = 0; k < D; ++k) v[k] = __ldg(M.T + t * D + k);
+      }
+#pragma unroll
+      for (int k = 0; k < D; ++k) {
+        const int r = v[k] - td.v_lo;
+        if ((unsigned)r < (unsigned)nrows) { l[k] = (uint32_t)(nlo + r); continue; }
+        int lo = r < 0 ? 0 : up0, hi = r < 0 ? nlo : nloc;
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if (gid[mid] < v[k]) lo = mid + 1; else hi = mid;
+        }
+        l[k] = (uint32_t)lo;
+      }
+      if constexpr (LB == 1) reinterpret_cast<uint32_t*>(tets)[s] = l[0] | (l[1] << 8) | (l[2] << 16) | (l[3] << 24);
+      else reinterpret_cast<uint2*>(tets)[s] = make_uint2(l[0] | (l[1] << 16), l[2] | (l[3] << 16));
+    }
+    __syncthreads();
+  }
 
   // ---- P1: VT incidence bits and VV bits, one thread per staged simplex ------------------------
   const uint32_t aT = smem_u32(bmT), aV = smem_u32(bmV);

@@ -506,7 +506,7 @@ int check_desc(const gale_mesh_desc_t* d) {
   if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
       !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
       d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1 ||
-      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) ||
+      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T)) ||
       (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK))
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
@@ -884,6 +884,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
 
   const bool walk = m->kernel == 1;
   SmemCfg cfg = walk ? walk_cfg_for_mask(p.cfg, relation_mask) : cfg_for_mask(p.cfg, relation_mask, false);
+  cfg.stage_t = (!walk && (p.flags & GALE_STAGE_FROM_T)) ? 1 : 0;
+  if (cfg.stage_t && cfg.nloc == 0) cfg.nloc = p.cfg.nloc;  // the vertex table is needed for the mapping
   const gale::SmemLayout lay = layout_for(D, cfg);
   const gale::WalkLayout wlay = walk_layout_for(D, cfg);
 #if GALE_CHECK_BOUNDS

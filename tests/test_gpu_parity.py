@@ -244,3 +244,14 @@ def test_large_batch_splits_launches():
     assert m.num_clusters > 128
     got, ref, _ = _run_all(m, m.num_clusters)
     _compare(got, ref, "big batch")
+
+
+@pytest.mark.parametrize("name,make,batch", SMALL[:5] + SMALL[7:8], ids=[s[0] for s in SMALL[:5] + SMALL[7:8]])
+def test_parity_staging_from_t(name, make, batch):
+    """Dense kernel with GALE_STAGE_FROM_T: the rows of T and T_ex are staged and mapped to tile-local ids in
+    the kernel (SURVEY §8 a1 as written) instead of reading the create-time re-encoding."""
+    gale = _gale()
+    m = make()
+    got, ref, info = _run_all(m, batch, flags=gale.VALIDATE | gale.KERNEL_DENSE | gale.STAGE_FROM_T)
+    assert info.kernel_variant == 0
+    _compare(got, ref, f"{name} [stage from T]")
