@@ -82,7 +82,8 @@ typedef struct {
                                        0: results stay in a ring of device slots (benchmark mode)     */
   int32_t device_ring;              /* queue_depth == 0 only: number of device slots (0 = default 4)   */
   int32_t tile_vertices;            /* vertices per thread-block tile, <= 256 (0 = automatic: 32 for
-                                       tets, 64 for triangles; create may reduce any request that
+                                       tets — 24 when 32-vertex tiles would need more than 28 KB of shared
+                                       memory per block — and 64 for triangles; create may reduce any request that
                                        exceeds a kernel limit — gale_mesh_info reports the value used) */
   void *d_workspace;                /* DEVICE, caller-owned (e.g. a torch tensor), 256-byte aligned,
                                        must outlive the handle                                       */

@@ -433,6 +433,7 @@ int analyse_device(Plan& p, const gale_mesh_desc_t& d, cudaStream_t st) {
 
   int tv = d.tile_vertices > 0 ? std::min(d.tile_vertices, gale::kMaxTileVertices) : (d.dim == 3 ? 32 : 64);  // measured optima on configs 5 and 2
   std::vector<long long> stats;
+  bool shrunk = false;
   for (;; tv = (tv + 1) / 2) {
     if (tv < 1) return GALE_ERR_UNSUPPORTED;
     const bool last = tv == 1;
@@ -451,6 +452,14 @@ int analyse_device(Plan& p, const gale_mesh_desc_t& d, cudaStream_t st) {
       p.cfg.tbl = int(pad_to(tbl_max, 4));
       p.smem_bytes = layout_for(D, p.cfg).total;
       fits = vt_max <= gale::kMaxNnz16 && vv_max <= gale::kMaxNnz16 && p.smem_bytes <= kSmemLimit;
+    }
+    // automatic tile size: tiles whose vertices are scattered in the mesh (graded or irregular meshes) need
+    // large per-block capacities and leave few resident blocks; 24-vertex tiles measured +10 % on config 4
+    // (8.1 -> 8.9 G tets/s) against 32
+    if (fits && d.tile_vertices == 0 && !shrunk && tv == 32 && D == 4 && p.smem_bytes > 28 * 1024) {
+      shrunk = true;
+      tv = 47;  // the loop step turns it into 24
+      continue;
     }
     if (fits) break;
     if (last) { g_last_error = "a single vertex star exceeds the kernels' shared-memory limits"; return GALE_ERR_UNSUPPORTED; }

@@ -8,7 +8,7 @@
 // kernel (gale_kernels.cuh, one thread per staged simplex) wins. gale_mesh_create times both on a sample
 // batch and keeps the faster one.
 //
-// Phases: P0 stage (16-byte cp.async) + clear; P1 VT incidence bits, one thread per staged simplex;
+// Phases: P0 one warp works out the tile and stages its lists with TMA bulk copies, the others clear; P1 VT incidence bits, one thread per staged simplex;
 // P2 row degrees -> scan -> VT offsets; P3 A(p): walk the bits: VT entries + VV bits + flag "p is the
 // second vertex"; B(p): walk the run: VT entries, VV bits, facet records 1..D-1 into p's private table;
 // P4 A(p): facets 0 of the flagged simplices join p's table (both cofaces of a facet with lowest vertex
@@ -22,7 +22,7 @@
 namespace gale {
 
 struct WalkLayout {
-  int tets, texid, gid, ft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
+  int mbar, ctx, tets, texid, gid, ft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
   int tbl, ttrow, ext0, tt_end;
   int st_vt, st_vv;
   int total;
@@ -33,6 +33,8 @@ template <int D>
 __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   WalkLayout L;
   int o = 0;
+  L.mbar = o;   o = align16(o + 8);
+  L.ctx = o;    o = align16(o + 112);
   L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
@@ -91,11 +93,16 @@ __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int
   using FB = FacetBits<D>;
   uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
   uint32_t cur = g.tbl[h];
+#if GALE_CHECK_BOUNDS
   uint32_t probe = 0;
+#endif
+  // a table has more slots than its group has records, so an empty slot or the key is always met
   while (cur != kEmpty32 && (cur & FB::kKeyMask) != key) {  // probe loop kept minimal: lanes diverge here
     h = h + 1 == g.hs ? 0u : h + 1;
     cur = g.tbl[h];
+#if GALE_CHECK_BOUNDS
     if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
+#endif
   }
   if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
   if (cur == kEmpty32) {
@@ -153,31 +160,64 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0, do_tt = (mask & REL_TT) != 0;
   const bool entries = do_vt || do_tt;  // VT entries are staged (TT reads their flags)
 
-  // ---- block -> (cluster slot, tile) ----------------------------------------------------------
-  int slot = 0, tile;
+  // ---- block -> (cluster slot, tile): worked out by the first warp, shared through BlockCtx; the same
+  // warp issues the TMA bulk copies of the tile's lists (P0a) -------------------------------------
   if (blockIdx.x == 0 && tid == 0) {  // terminal offsets (also covers batches without rows)
     if (do_vt) { O.vt_offsets[0] = 0; O.vt_offsets[P.total_rows] = P.total_vt_nnz; }
     if (do_vv) { O.vv_offsets[0] = 0; O.vv_offsets[P.total_rows] = P.total_vv_nnz; }
   }
   if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
-  if (P.uniform_tiles > 0) {
-    slot = (int)blockIdx.x / P.uniform_tiles;
-  } else {
-    int lo = 0, hi = P.n_clusters;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+  BlockCtx* ctx = reinterpret_cast<BlockCtx*>(smem + L.ctx);
+  void* bar = smem + L.mbar;
+  if (tid < 32) {
+    int slot = 0;
+    if (P.uniform_tiles > 0) {
+      slot = (int)blockIdx.x / P.uniform_tiles;
+    } else {
+      int lo = 0, hi = P.n_clusters;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+      }
+      slot = lo;
     }
-    slot = lo;
+    const int tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
+    if (lane < (int)(sizeof(TileDesc) / 16))
+      reinterpret_cast<int4*>(&ctx->td)[lane] = __ldg(reinterpret_cast<const int4*>(M.tiles + tile) + lane);
+    __syncwarp();
+    if (lane == 0) {
+      const TileDesc& t = ctx->td;
+      ctx->tile = tile;
+      ctx->row0 = P.row_base[slot] + t.row_rel;
+      ctx->vt0 = P.vt_base[slot] + t.vt_rel;
+      ctx->vv0 = P.vv_base[slot] + t.vv_rel;
+      ctx->tt0 = P.tt_base[slot] + t.tt_rel;
+      ctx->tt_slot = P.tt_base[slot];
+      mbar_init(bar, 1);
+      fence_proxy_async();
+      const uint32_t b_t = (uint32_t)((t.s_int + t.s_ext + 3) & ~3) * (4u * LB);
+      const uint32_t b_x = (uint32_t)((t.s_ext + 3) & ~3) * 4u;
+      const uint32_t b_g = (do_vv || do_tt) ? (uint32_t)((t.nloc + 3) & ~3) * 4u : 0u;
+      mbar_arrive_expect_tx(bar, b_t + b_x + b_g);
+      if (b_t) bulk_g2s(smem + L.tets, static_cast<const unsigned char*>(M.loc) + t.stg_off * (4 * LB), b_t, bar);
+      if (b_x) bulk_g2s(smem + L.texid, M.tex + t.tex_off, b_x, bar);
+      if (b_g) bulk_g2s(smem + L.gid, M.gid + t.gid_off, b_g, bar);
+    }
   }
-  tile = __ldg(M.cluster_tile_begin + P.cluster[slot]) + ((int)blockIdx.x - P.tile_prefix[slot]);
-  TileDesc td;
+  // P0b: clear (needs nothing of the tile's record)
   {
-    const int4* src = reinterpret_cast<const int4*>(M.tiles + tile);
-    int4* dst = reinterpret_cast<int4*>(&td);
-#pragma unroll
-    for (int i = 0; i < (int)(sizeof(TileDesc) / 16); ++i) dst[i] = __ldg(src + i);
+    int4* z = reinterpret_cast<int4*>(smem + L.bmT);
+    const int n16 = (L.bm_end - L.bmT) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
   }
+  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
+    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
+    const int n16 = (L.tt_end - L.tbl) >> 4;
+    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
+  }
+  if (tid == 0) { reinterpret_cast<uint32_t*>(smem + L.scan)[36] = 0u; reinterpret_cast<uint32_t*>(smem + L.scan)[38] = 0u; }
+  __syncthreads();
+  const TileDesc& td = ctx->td;
   const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
   const int S = s_int + s_ext;
   const int WT = C.WT, WV = C.WV;
@@ -211,39 +251,10 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   uint16_t* st_vt = reinterpret_cast<uint16_t*>(smem + L.st_vt);
   uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
 
-  const int row0 = P.row_base[slot] + td.row_rel;
-  const int vt0 = P.vt_base[slot] + td.vt_rel;
-  const int vv0 = P.vv_base[slot] + td.vv_rel;
-  const int tt0 = P.tt_base[slot] + td.tt_rel;
-
-  // ---- P0: stage + clear ----------------------------------------------------------------------
-  {
-    const int4* src = reinterpret_cast<const int4*>(static_cast<const unsigned char*>(M.loc) + td.stg_off * (4 * LB));
-    int4* dst = reinterpret_cast<int4*>(tets);
-    for (int i = tid; i < (S * 4 * LB + 15) >> 4; i += NT) cp_async16(dst + i, src + i);
-    const int4* tsrc = reinterpret_cast<const int4*>(M.tex + td.tex_off);
-    int4* tdst = reinterpret_cast<int4*>(texid);
-    for (int i = tid; i < (s_ext + 3) >> 2; i += NT) cp_async16(tdst + i, tsrc + i);
-    if (do_vv || do_tt) {
-      const int4* gsrc = reinterpret_cast<const int4*>(M.gid + td.gid_off);
-      int4* gdst = reinterpret_cast<int4*>(gid);
-      for (int i = tid; i < (td.nloc + 3) >> 2; i += NT) cp_async16(gdst + i, gsrc + i);
-    }
-  }
+  const int row0 = ctx->row0, vt0 = ctx->vt0, vv0 = ctx->vv0, tt0 = ctx->tt0;
   for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);
-  {
-    int4* z = reinterpret_cast<int4*>(smem + L.bmT);
-    const int n16 = (L.bm_end - L.bmT) >> 4;
-    for (int i = tid; i < n16; i += NT) z[i] = make_int4(0, 0, 0, 0);
-  }
-  if (do_tt) {  // tables empty, TT rows "none": both all-ones, contiguous
-    int4* z = reinterpret_cast<int4*>(smem + L.tbl);
-    const int n16 = (L.tt_end - L.tbl) >> 4;
-    for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
-  }
-  if (tid == 0) { scan[36] = 0u; scan[38] = 0u; }
-  cp_async_wait_all();
-  __syncthreads();
+  mbar_wait(bar, 0);
+  __syncthreads();  // ft
 
   // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
   for (int s = tid; s < S; s += NT) {
@@ -456,7 +467,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       if ((unsigned)(l[1] - nlo) < (unsigned)nrows && gid[l[0]] >= c_lo) {
         const int e = ext0[s];
         const int v = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
-        const long long row = (long long)P.tt_base[slot] + (texid[s] - c_tlo);
+        const long long row = (long long)ctx->tt_slot + (texid[s] - c_tlo);
         GALE_ST(O.tt_indices + row * D, v);
       }
     }

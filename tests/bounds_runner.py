@@ -32,9 +32,18 @@ CASES = [
     ("holes2d", lambda: meshgen.make_mesh(2, 150, clustering="octree", capacity=900, warp=True, drop_frac=0.2, seed=6), 16, 0, 7),
 ]
 
-for name, make, batch, tv, mask in CASES:
+RUNS = [(c, k) for c in CASES for k in ("dense", "walk")]
+for (name, make, batch, tv, mask), kernel in RUNS:
     m = make()
-    gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=batch, tile_vertices=tv)
+    name = f"{name} [{kernel}]"
+    try:
+        gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=batch, tile_vertices=tv,
+                           flags=gale.VALIDATE | (gale.KERNEL_WALK if kernel == "walk" else gale.KERNEL_DENSE))
+    except gale.GaleError as e:
+        if kernel == "walk" and e.status == gale.ERR_UNSUPPORTED:
+            print(f"skip {name}: the walk kernel does not admit this mesh")
+            continue
+        raise
     ids = list(range(m.num_clusters))
     got = []
     for b in range(0, len(ids), batch):
