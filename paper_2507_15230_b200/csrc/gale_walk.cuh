@@ -300,9 +300,22 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       run_lo = ft[p]; run_hi = ft[p + 1];
       deg = (uint32_t)(nb + run_hi - run_lo);
     }
-    const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // A and B halves carry the same values
-    n_vt = (int)(tot >> 1);
-    off = (int)ex - (isB ? n_vt : 0);
+    if constexpr (NT == 64) {
+      // one warp per half, both halves carry the same 32 values: each warp scans for itself, no barrier
+      uint32_t inc = deg;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+        if (lane >= d) inc += y;
+      }
+      n_vt = (int)__shfl_sync(0xFFFFFFFFu, inc, 31);
+      off = (int)(inc - deg);
+      (void)tot;
+    } else {
+      const uint32_t ex = block_exclusive_scan<NT>(deg, scan, &tot);  // A and B halves carry the same values
+      n_vt = (int)(tot >> 1);
+      off = (int)ex - (isB ? n_vt : 0);
+    }
   }
   if (do_vt && live && !isB) O.vt_offsets[row0 + p] = vt0 + off;
 
