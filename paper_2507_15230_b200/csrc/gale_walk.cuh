@@ -22,7 +22,7 @@
 namespace gale {
 
 struct WalkLayout {
-  int mbar, ctx, tets, texid, gid, ft, off_vt, off_vv, cnt, fbq, scan, bmT, bmV, bm_end;
+  int mbar, ctx, tets, texid, gid, ft, cnt, fbq, scan, bmT, bmV, bm_end;
   int tbl, ttrow, ext0, tt_end;
   int st_vt, st_vv;
   int total;
@@ -39,8 +39,6 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
   L.ft = o;     o = align16(o + (c.tv + 1) * 4);
-  L.off_vt = o; o = align16(o + (c.tv + 1) * 4);
-  L.off_vv = o; o = align16(o + (c.tv + 1) * 4);
   L.cnt = o;    o = align16(o + c.tv * 4);
   L.scan = o;   o = align16(o + 48 * 4);
   // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
