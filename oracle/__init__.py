@@ -70,6 +70,19 @@ def _load():
         lib.go_internal_range.argtypes = [c_int, i64, i32p, i64, i64, i64p]
         lib.go_external_list.restype = i64
         lib.go_external_list.argtypes = [c_int, i64, i32p, i64, i64, i32p]
+        lib.go_enumerate_sub.restype = vp
+        lib.go_enumerate_sub.argtypes = [c_int, c_int, i64, i64, i32p]
+        lib.go_sub_count.restype = i64
+        lib.go_sub_count.argtypes = [vp]
+        lib.go_sub_list.restype = i32p
+        lib.go_sub_list.argtypes = [vp]
+        for name in ("go_sub_first", "go_sub_v_off"):
+            getattr(lib, name).restype = i64p
+            getattr(lib, name).argtypes = [vp]
+        lib.go_sub_v_idx.restype = i32p
+        lib.go_sub_v_idx.argtypes = [vp]
+        lib.go_sub_release.restype = None
+        lib.go_sub_release.argtypes = [vp]
         lib.go_brute_vt.restype = None
         lib.go_brute_vt.argtypes = [c_int, i64, i64, i32p, i64p, i32p]
         lib.go_brute_vv.restype = None
@@ -223,6 +236,23 @@ def external_list(dim: int, simplices: np.ndarray, lo: int, hi: int) -> np.ndarr
     if n:
         lib.go_external_list(dim, T.shape[0], _i32(T), int(lo), int(hi), _i32(out))
     return out
+
+
+def sub_simplices(dim: int, num_vertices: int, simplices: np.ndarray, k: int) -> dict:
+    """Edges (k = 2) or triangles (k = 3) of the mesh: the sorted list [n, k] (id = row), the
+    interval array `first` per vertex (I_E / I_F), and the coboundary relation VE / VF as CSR over all vertices."""
+    lib = _load()
+    T = _canon(simplices)
+    nV = int(num_vertices)
+    h = lib.go_enumerate_sub(dim, k, nV, T.shape[0], _i32(T))
+    try:
+        n = int(lib.go_sub_count(h))
+        return dict(list=_np(lib.go_sub_list(h), n * k, np.int32).reshape(n, k),
+                    first=_np(lib.go_sub_first(h), nV + 1, np.int64),
+                    v_off=_np(lib.go_sub_v_off(h), nV + 1, np.int64),
+                    v_idx=_np(lib.go_sub_v_idx(h), n * k, np.int32))
+    finally:
+        lib.go_sub_release(h)
 
 
 def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:

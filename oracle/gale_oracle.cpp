@@ -278,6 +278,68 @@ int64_t go_external_list(int dim, int64_t nT, const int32_t* T, int64_t lo, int6
   return n;
 }
 
+// ---- edges, triangles and the coboundary relations VE / VF (Table 1 :53-58) ----------
+// E = every unique combination of two vertices of a simplex, F = of three ("all unique combinations of two
+// vertices (edges) and three vertices (triangles) are stored in sorted indexed lists (E and F) based on
+// vertex indices", :178). Reading: each combination ascending, the list in ascending
+// lexicographic order, the id of an edge / triangle = its position. A sub-simplex is internal to the
+// segment of its lowest vertex (:172), so the interval arrays are I_E[v] / I_F[v] = number of edges /
+// triangles whose lowest vertex is below v. For a 2-D mesh F = T.
+}  // extern "C" (templates below)
+struct SubSimplices {
+  int K = 0;                      // vertices per sub-simplex: 2 (edges) or 3 (triangles)
+  std::vector<int32_t> list;      // [n*K]
+  std::vector<int64_t> first;     // [nV+1] interval array per vertex
+  std::vector<int64_t> v_off;     // [nV+1] VE / VF offsets
+  std::vector<int32_t> v_idx;     // VE / VF indices (ids of the sub-simplices containing v, ascending)
+};
+template <int K>
+static SubSimplices* enumerate_sub(int D, int64_t nV, int64_t nT, const int32_t* T) {
+  using Key = std::array<int32_t, K>;
+  std::vector<Key> all;
+  for (int64_t t = 0; t < nT; ++t) {
+    const int32_t* r = T + t * D;
+    if (K == 2) {
+      for (int i = 0; i < D; ++i)
+        for (int j = i + 1; j < D; ++j) { Key k{}; k[0] = r[i]; k[1] = r[j]; all.push_back(k); }
+    } else {
+      for (int i = 0; i < D; ++i)
+        for (int j = i + 1; j < D; ++j)
+          for (int l = j + 1; l < D; ++l) { Key k{}; k[0] = r[i]; k[1] = r[j]; k[2] = r[l]; all.push_back(k); }
+    }
+  }
+  std::sort(all.begin(), all.end());
+  all.erase(std::unique(all.begin(), all.end()), all.end());
+  SubSimplices* S = new SubSimplices;
+  S->K = K;
+  S->list.resize(all.size() * K);
+  S->first.assign(nV + 1, 0);
+  std::vector<int64_t> deg(nV + 1, 0);
+  for (size_t i = 0; i < all.size(); ++i) {
+    for (int k = 0; k < K; ++k) { S->list[i * K + k] = all[i][k]; ++deg[all[i][k] + 1]; }
+    ++S->first[all[i][0] + 1];
+  }
+  for (int64_t v = 0; v < nV; ++v) { S->first[v + 1] += S->first[v]; deg[v + 1] += deg[v]; }
+  S->v_off = deg;
+  S->v_idx.resize(all.size() * K);
+  std::vector<int64_t> cur(deg.begin(), deg.end() - 1);
+  for (size_t i = 0; i < all.size(); ++i)          // ids ascending => every row ascending
+    for (int k = 0; k < K; ++k) S->v_idx[cur[all[i][k]]++] = int32_t(i);
+  return S;
+}
+extern "C" {
+void* go_enumerate_sub(int dim, int K, int64_t nV, int64_t nT, const int32_t* T) {
+  if (K == 2) return enumerate_sub<2>(dim + 1, nV, nT, T);
+  if (K == 3) return enumerate_sub<3>(dim + 1, nV, nT, T);
+  return nullptr;
+}
+int64_t go_sub_count(void* h) { SubSimplices* S = static_cast<SubSimplices*>(h); return int64_t(S->list.size()) / S->K; }
+const int32_t* go_sub_list(void* h) { return static_cast<SubSimplices*>(h)->list.data(); }
+const int64_t* go_sub_first(void* h) { return static_cast<SubSimplices*>(h)->first.data(); }
+const int64_t* go_sub_v_off(void* h) { return static_cast<SubSimplices*>(h)->v_off.data(); }
+const int32_t* go_sub_v_idx(void* h) { return static_cast<SubSimplices*>(h)->v_idx.data(); }
+void go_sub_release(void* h) { delete static_cast<SubSimplices*>(h); }
+
 // ---- brute-force enumeration (tiny meshes; pins the routines above) ------------------------------
 // Membership scans straight from the definitions; no sorting, no transposition.
 static bool contains(const int32_t* r, int D, int32_t v) {

@@ -307,3 +307,53 @@ def test_internal_external_brute_force(dim, n, seed):
         assert set(range(a, b)) == internal
         assert ext.tolist() == sorted(touching - internal)
     assert prev == len(T)
+
+
+# ---- edges, triangles, VE, VF (Table 1) --------------------------------------------------
+def test_fig4_edge_list_and_interval_array(golden_dir):
+    """The paper's Fig. 4/5 example: 12 edges with I_E = [0, 9, 12]; edge (v0, v3) is e2 and
+    (v3, v4) is e9 (:192). [(v0, v4) = e6 in the paper cannot hold in ANY list sorted by vertex indices that
+    also has (v0, v3) = e2 — the mesh of the figure is not in the text; DESIGN.md §2 reading 18.]"""
+    T, S, exp = _fig4(golden_dir)
+    e = oracle.sub_simplices(3, 6, T, 2)
+    assert len(e["list"]) == 12
+    assert [int(e["first"][S[0][0]]), int(e["first"][S[1][0]]), int(e["first"][6])] == exp["I_E"]
+    assert e["list"][2].tolist() == [0, 3] and e["list"][9].tolist() == [3, 4]
+    f = oracle.sub_simplices(3, 6, T, 3)
+    assert [0, 3, 4] in f["list"].tolist()                          # the triangle f5 of the FE example exists
+
+
+@pytest.mark.parametrize("dim,n", [(3, 6), (2, 9)])
+def test_edges_triangles_closed_forms_and_brute_force(dim, n):
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=60, permute=True, seed=21)
+    T, nV = m.simplices, m.num_vertices
+    cf = meshgen.kuhn_closed_forms(dim, n)
+    e = oracle.sub_simplices(dim, nV, T, 2)
+    f = oracle.sub_simplices(dim, nV, T, 3)
+    assert len(e["list"]) == cf["E"]
+    assert len(f["list"]) == (cf["F"] if dim == 3 else cf["T"])
+    if dim == 2:
+        assert np.array_equal(f["list"], T)                          # in 2-D the triangles are the simplices
+    # brute force with python sets
+    edges = sorted({(int(r[i]), int(r[j])) for r in T for i in range(dim + 1) for j in range(i + 1, dim + 1)})
+    assert e["list"].tolist() == [list(x) for x in edges]
+    tris = sorted({tuple(int(x) for x in np.delete(r, k)) for r in T for k in range(dim + 1)}) if dim == 3 else [tuple(r) for r in T.tolist()]
+    assert f["list"].tolist() == [list(x) for x in tris]
+    g = oracle.relations_global(dim, nV, T, mask=3)
+    for s, name in ((e, "VE"), (f, "VF")):
+        k = s["list"].shape[1]
+        assert s["v_off"][-1] == k * len(s["list"])                  # sum |VE| = 2 E, sum |VF| = 3 F
+        assert (np.diff(s["first"]) >= 0).all() and s["first"][-1] == len(s["list"])
+        assert np.array_equal(np.searchsorted(s["list"][:, 0], np.arange(nV + 1)), s["first"])
+        for v in (0, nV // 2, nV - 1):
+            row = s["v_idx"][s["v_off"][v]:s["v_off"][v + 1]]
+            assert (np.diff(row) > 0).all()
+            assert row.tolist() == [i for i, x in enumerate(s["list"].tolist()) if v in x]
+    assert np.array_equal(np.diff(e["v_off"]), np.diff(g["vv_off"]))  # |VE(v)| = |VV(v)|
+    # VE(v)[i] is the edge (v, VV(v)[i]): edge ids ascend with the neighbour
+    v = nV // 2
+    nb = g["vv_idx"][g["vv_off"][v]:g["vv_off"][v + 1]]
+    ev = e["list"][e["v_idx"][e["v_off"][v]:e["v_off"][v + 1]]]
+    assert np.array_equal(np.where(ev[:, 0] == v, ev[:, 1], ev[:, 0]), nb)
+    if dim == 3:
+        assert np.diff(f["v_off"]).max() == 36                        # interior Kuhn vertex: 36 triangles
