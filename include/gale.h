@@ -36,7 +36,13 @@ extern "C" {
 typedef struct gale_mesh gale_mesh_t; /* opaque; owned by the library, freed by gale_destroy */
 typedef struct gale_plan gale_plan_t; /* opaque result of the initialization analysis, see gale_plan_create */
 
-enum { GALE_REL_VT = 1, GALE_REL_VV = 2, GALE_REL_TT = 4, GALE_REL_ALL = 7 };
+enum {
+  GALE_REL_VT = 1, GALE_REL_VV = 2, GALE_REL_TT = 4,
+  GALE_REL_ALL = 7,  /* the three relations of the hot path                                           */
+  GALE_REL_VE = 8,   /* vertex -> incident edges; needs GALE_WITH_EDGES at create; also delivers VV   */
+  GALE_REL_VF = 16   /* vertex -> incident triangles (tetrahedral meshes); needs GALE_WITH_FACETS; also
+                        delivers VT                                                                  */
+};
 
 enum {
   GALE_OK = 0,
@@ -59,6 +65,10 @@ enum {
   GALE_KERNEL_WALK = 16u,      /* force the walk kernel (two threads per tile vertex); UNSUPPORTED if
                                   its capacity limits do not admit the mesh. Neither flag: create times
                                   both on a sample batch and keeps the faster (gale_mesh_info tells)   */
+  GALE_WITH_EDGES = 64u,       /* initialization also builds the sorted edge list E and its interval array
+                                  I_E (generated "only when the edge or triangle information
+                                  is explicitly needed"); enables GALE_REL_VE                              */
+  GALE_WITH_FACETS = 128u,     /* ... and the sorted triangle list F with I_F; enables GALE_REL_VF (dim = 3)  */
   GALE_STAGE_FROM_T = 32u,     /* dense kernel only (implies nothing for the walk kernel): stage the rows of T
                                   and T_ex themselves and derive the tile-local ids in the kernel instead of
                                   reading the create-time re-encoding; slower, kept for the A/B in DESIGN.md */
@@ -125,6 +135,12 @@ typedef struct {
                                     (includes waiting behind earlier copies on the side stream); else 0 */
   float queue_ms;                /* host time from the end of compute to the return of this pop         */
   int32_t reserved;
+  /* edges / triangles. VE has the rows and offsets of VV: ve_indices[i] is the id of the
+   * edge between the row's vertex and vv_indices[i]. Edge / triangle ids = positions in the sorted lists E / F */
+  const int32_t *ve_indices;     /* [vv_nnz] or NULL                                                   */
+  int64_t vf_nnz;
+  const int32_t *vf_offsets;     /* [vt_rows+1] or NULL                                                */
+  const int32_t *vf_indices;     /* [vf_nnz]                                                           */
 } gale_batch_view_t;
 
 /* Init statistics ("Initialization"), for reporting. */
@@ -142,6 +158,7 @@ typedef struct {
   int32_t block_threads;         /* threads per block of the batch kernel                            */
   size_t index_bytes;            /* bytes of the device-resident index built by the initialization
                                     (I_T, T_ex, tile tables; the rest of workspace_used is result slots) */
+  int64_t num_edges, num_triangles; /* sizes of E / F when built (GALE_WITH_EDGES / GALE_WITH_FACETS), else 0 */
   int32_t kernel_variant;        /* 0 = dense kernel, 1 = walk kernel (chosen at create, or forced)     */
   float tune_dense_ms, tune_walk_ms; /* sample-batch times behind that choice (0 = not timed)           */
   int32_t reserved;
@@ -199,6 +216,14 @@ int32_t gale_mesh_tile(const gale_mesh_t *mesh, int32_t tile, gale_tile_view_t *
  * lowest vertex is >= v, so the internal simplices of any vertex range [lo, hi) are
  * [I[lo], I[hi]). */
 int32_t gale_mesh_interval_array(const gale_mesh_t *mesh, const int32_t **d_first_simplex);
+
+/* The sorted edge list E with its interval array, when built: the edges whose lowest vertex
+ * is a are the ids [d_first[a], d_first[a+1]) and d_upper[id] is their other vertex (ascending). DEVICE
+ * memory owned by the library, valid as long as the handle. GALE_ERR_UNSUPPORTED when not built. */
+int32_t gale_mesh_edges(const gale_mesh_t *mesh, const int32_t **d_first, const int32_t **d_upper, int64_t *num_edges);
+/* Likewise the triangle list F: d_second_third holds two ids per triangle. */
+int32_t gale_mesh_triangles(const gale_mesh_t *mesh, const int32_t **d_first, const int32_t **d_second_third,
+                            int64_t *num_triangles);
 
 /* Producer side: enqueue the relation kernels for the clusters
  * h_cluster_ids[0..n) (HOST array, copied before return; duplicates are legal) and, when

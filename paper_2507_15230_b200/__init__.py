@@ -15,7 +15,9 @@ import numpy as np
 from .build import LIB, build_library
 
 REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
+REL_VE, REL_VF = 8, 16
 VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED, KERNEL_DENSE, KERNEL_WALK, STAGE_FROM_T = 1, 2, 4, 8, 16, 32
+WITH_EDGES, WITH_FACETS = 64, 128
 OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
 ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
 
@@ -41,7 +43,9 @@ class gale_batch_view_t(ctypes.Structure):
                 ("tt_rows", ctypes.c_int64), ("tt_indices", ctypes.c_void_p),
                 ("kernel_ms", ctypes.c_float), ("slot", ctypes.c_int32),
                 ("prep_ms", ctypes.c_float), ("d2h_ms", ctypes.c_float), ("queue_ms", ctypes.c_float),
-                ("reserved", ctypes.c_int32)]
+                ("reserved", ctypes.c_int32),
+                ("ve_indices", ctypes.c_void_p), ("vf_nnz", ctypes.c_int64),
+                ("vf_offsets", ctypes.c_void_p), ("vf_indices", ctypes.c_void_p)]
 
 
 class gale_mesh_info_t(ctypes.Structure):
@@ -50,7 +54,8 @@ class gale_mesh_info_t(ctypes.Structure):
                 ("smem_bytes", ctypes.c_int32), ("max_staged", ctypes.c_int32),
                 ("slot_bytes", ctypes.c_size_t), ("workspace_used", ctypes.c_size_t), ("create_ms", ctypes.c_double),
                 ("local_id_bytes", ctypes.c_int32), ("block_threads", ctypes.c_int32),
-                ("index_bytes", ctypes.c_size_t), ("kernel_variant", ctypes.c_int32),
+                ("index_bytes", ctypes.c_size_t), ("num_edges", ctypes.c_int64), ("num_triangles", ctypes.c_int64),
+                ("kernel_variant", ctypes.c_int32),
                 ("tune_dense_ms", ctypes.c_float), ("tune_walk_ms", ctypes.c_float), ("reserved", ctypes.c_int32)]
 
 
@@ -61,7 +66,7 @@ class gale_tile_view_t(ctypes.Structure):
                 ("d_external", ctypes.c_void_p), ("d_local_to_global", ctypes.c_void_p)]
 
 
-EXPORTS = ["gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+EXPORTS = ["gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
            "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
@@ -102,6 +107,10 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
     lib.gale_mesh_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
     lib.gale_mesh_info.restype = ctypes.c_int32
     lib.gale_mesh_info.argtypes = [vp, ctypes.POINTER(gale_mesh_info_t)]
+    lib.gale_mesh_edges.restype = ctypes.c_int32
+    lib.gale_mesh_edges.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_int64)]
+    lib.gale_mesh_triangles.restype = ctypes.c_int32
+    lib.gale_mesh_triangles.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_int64)]
     lib.gale_mesh_tile.restype = ctypes.c_int32
     lib.gale_mesh_tile.argtypes = [vp, ctypes.c_int32, ctypes.POINTER(gale_tile_view_t)]
     lib.gale_mesh_interval_array.restype = ctypes.c_int32
@@ -175,6 +184,22 @@ def gale_mesh_info(handle) -> gale_mesh_info_t:
     info = gale_mesh_info_t()
     _check(load_library().gale_mesh_info(handle, ctypes.byref(info)), "gale_mesh_info")
     return info
+
+
+def _sub_list(fn, handle, where):
+    first, other, n = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_int64()
+    _check(fn(handle, ctypes.byref(first), ctypes.byref(other), ctypes.byref(n)), where)
+    return int(first.value), int(other.value or 0), int(n.value)
+
+
+def gale_mesh_edges(handle):
+    """(DEVICE address of I_E per vertex, DEVICE address of the edges' upper vertices, number of edges)."""
+    return _sub_list(load_library().gale_mesh_edges, handle, "gale_mesh_edges")
+
+
+def gale_mesh_triangles(handle):
+    """(DEVICE address of I_F per vertex, DEVICE address of (second, third) vertex pairs, number of triangles)."""
+    return _sub_list(load_library().gale_mesh_triangles, handle, "gale_mesh_triangles")
 
 
 def gale_mesh_tile(handle, tile: int) -> gale_tile_view_t:
@@ -299,6 +324,11 @@ class GaleMesh:
             out["vv_indices"] = self._array(view, view.vv_indices, view.vv_nnz)
         if view.relation_mask & REL_TT:
             out["tt_indices"] = self._array(view, view.tt_indices, view.tt_rows * self.D)
+        if view.relation_mask & REL_VE:
+            out["ve_indices"] = self._array(view, view.ve_indices, view.vv_nnz)
+        if view.relation_mask & REL_VF:
+            out["vf_offsets"] = self._array(view, view.vf_offsets, view.vt_rows + 1)
+            out["vf_indices"] = self._array(view, view.vf_indices, view.vf_nnz)
         return out
 
     def run_batch(self, cluster_ids, relation_mask: int = REL_ALL) -> dict:
@@ -340,10 +370,13 @@ def split_batch(host: dict, D: int) -> list:
         r0, r1 = int(host["vt_row_begin"][i]), int(host["vt_row_begin"][i + 1])
         t0, t1 = int(host["tt_row_begin"][i]), int(host["tt_row_begin"][i + 1])
         item = dict(cluster=int(host["cluster_ids"][i]))
-        for k in ("vt", "vv"):
+        for k in ("vt", "vv", "vf"):
             if k + "_offsets" in host:
                 off = host[k + "_offsets"][r0:r1 + 1]
                 item[k] = ((off - off[0]).astype(np.int32), host[k + "_indices"][off[0]:off[-1]])
+        if "ve_indices" in host:                          # VE shares the rows and offsets of VV
+            off = host["vv_offsets"][r0:r1 + 1]
+            item["ve"] = ((off - off[0]).astype(np.int32), host["ve_indices"][off[0]:off[-1]])
         if "tt_indices" in host:
             item["tt"] = host["tt_indices"][t0 * D:t1 * D].reshape(-1, D)
         res.append(item)

@@ -7,6 +7,7 @@
 #include "gale_kernels.cuh"
 #include "gale_walk.cuh"
 #include "gale_init.cuh"
+#include "gale_sub.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -93,7 +94,7 @@ struct Plan {
 };
 
 struct SlotLayout {
-  size_t vt_off = 0, vt_idx = 0, vv_off = 0, vv_idx = 0, tt = 0, total = 0;
+  size_t vt_off = 0, vt_idx = 0, vv_off = 0, vv_idx = 0, tt = 0, ve_idx = 0, vf_off = 0, vf_idx = 0, total = 0;
 };
 SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
   const int D = p.dim + 1;
@@ -104,6 +105,11 @@ SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
   L.vv_off = o; o = up(o + (size_t(maxB) * p.max_rows + 1) * 4);
   L.vv_idx = o; o = up(o + size_t(maxB) * p.max_vv * 4);
   L.tt = o;     o = up(o + size_t(maxB) * p.max_tt * D * 4);
+  if (p.flags & GALE_WITH_EDGES) { L.ve_idx = o; o = up(o + size_t(maxB) * p.max_vv * 4); }
+  if (p.flags & GALE_WITH_FACETS) {  // |VF(v)| <= 3 |VT(v)|: every triangle at v lies in a simplex of its star
+    L.vf_off = o; o = up(o + (size_t(maxB) * p.max_rows + 1) * 4);
+    L.vf_idx = o; o = up(o + size_t(maxB) * p.max_vt * 3 * 4);
+  }
   L.total = o;
   return L;
 }
@@ -515,7 +521,8 @@ int check_desc(const gale_mesh_desc_t* d) {
   if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
       !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
       d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1 ||
-      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T)) ||
+      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T | GALE_WITH_EDGES | GALE_WITH_FACETS)) ||
+      ((d->flags & GALE_WITH_FACETS) && d->dim != 3) ||
       (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK))
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
@@ -572,7 +579,8 @@ struct Slot {
   int n = 0;
   uint32_t mask = 0;
   std::vector<int32_t> ids, row_begin, tt_row_begin;
-  long long rows = 0, vt_nnz = 0, vv_nnz = 0, tt_rows = 0;
+  long long rows = 0, vt_nnz = 0, vv_nnz = 0, tt_rows = 0, vf_nnz = 0;
+  uint32_t eff_mask = 0;  // what the batch kernel computed (VE implies VV, VF implies VT)
   SlotLayout used;  // section offsets of this batch
   float prep_ms = 0.f;
   std::chrono::steady_clock::time_point t_submit;
@@ -603,7 +611,13 @@ struct gale_mesh {
   std::atomic<long long> submitted{0}, popped{0};
   size_t workspace_used = 0, index_bytes = 0;
   double create_ms = 0;
-  float tune_ms[2] = {0.f, 0.f};  // sample-batch time of the dense / walk kernel at create (0 = not timed)
+  float tune_ms[2] = {0.f, 0.f};
+  // edges / triangles (GALE_WITH_EDGES / GALE_WITH_FACETS): library-owned device memory
+  DevMem d_cl_off, d_e_first, d_e_hi, d_f_first, d_f_bc, d_tile_vf_rel;
+  long long nE = 0, nF = 0;
+  int vf_cap = 0;                       // candidate slots per vertex in k_vf (power of two)
+  std::vector<long long> cl_vf;         // VF entries per cluster
+  gale::sub::SubIndex sub{};  // sample-batch time of the dense / walk kernel at create (0 = not timed)
 };
 
 namespace {
@@ -622,6 +636,163 @@ void free_mesh(gale_mesh* m) {  // also the error path of create: releases whate
   if (m->h_err) cudaFreeHost(m->h_err);
   cudaGetLastError();
   delete m;
+}
+
+// Edges / triangles (E, I_E, F, I_F "generated only when the edge or
+// triangle information is explicitly needed"). Built with the handle's own hot path: E from the upper part
+// of the VV rows of every cluster, F from the facet groups of the vertices; the exact VF sizes per tile come
+// from a counting sweep over the VT rows.
+template <class Fn>
+int sweep_batches(gale_mesh* m, uint32_t mask, cudaStream_t st, Fn&& per_batch) {
+  const Plan& p = *m->plan;
+  std::vector<int32_t> ids;
+  for (int c0 = 0; c0 < p.nC; c0 += m->maxB) {
+    const int n = std::min(m->maxB, p.nC - c0);
+    ids.resize(size_t(n));
+    for (int i = 0; i < n; ++i) ids[size_t(i)] = c0 + i;
+    int rc = gale_cluster_batch_compute(m, mask, ids.data(), n, st);
+    gale_batch_view_t v;
+    if (rc == GALE_OK) rc = gale_queue_pop(m, &v, -1);
+    if (rc != GALE_OK) return rc;
+    rc = per_batch(*m->slots[size_t(v.slot)], c0, n);  // the slot's DEVICE copy is complete (pop waited for it)
+    GALE_CUDA(cudaStreamSynchronize(st));
+    const int rc2 = gale_queue_release(m, &v);
+    if (rc != GALE_OK) return rc;
+    if (rc2 != GALE_OK) return rc2;
+  }
+  m->submitted.store(0); m->popped.store(0);  // these batches were the library's own
+  return GALE_OK;
+}
+
+int build_sub_index(gale_mesh* m, cudaStream_t st) {
+  namespace gs = gale::sub;
+  namespace gi = gale::init;
+  const Plan& p = *m->plan;
+  const int TB = 256;
+  int rc;
+  if ((rc = upload_vec(m->d_cl_off, p.cl_off, st))) return rc;
+  m->sub.cl_off = m->d_cl_off.as<int32_t>();
+  DevMem d_scan;
+  if ((rc = d_scan.alloc((size_t(p.nV + 1) / gi::kScanChunk + 2) * 4))) return rc;
+  auto for_chunks = [&](const Slot& s, int n, auto&& fn) {  // <= kMaxBatch clusters per descriptor
+    for (int b = 0; b < n; b += gale::kMaxBatch) {
+      const int nb = std::min(gale::kMaxBatch, n - b);
+      gs::BatchRows B{};
+      B.n_clusters = nb;
+      for (int i = 0; i <= nb; ++i) B.row_base[i] = s.row_begin[size_t(b + i)];
+      for (int i = 0; i < nb; ++i) B.cluster[i] = s.ids[size_t(b + i)];
+      const int rows = B.row_base[nb] - B.row_base[0];
+      if (rows > 0) fn(B, rows);
+    }
+  };
+  if (p.flags & GALE_WITH_EDGES) {
+    if ((rc = m->d_e_first.alloc(size_t(p.nV + 2) * 4))) return rc;
+    GALE_CUDA(cudaMemsetAsync(m->d_e_first.p, 0, size_t(p.nV + 2) * 4, st));
+    int32_t* first = m->d_e_first.as<int32_t>();
+    rc = sweep_batches(m, GALE_REL_VV, st, [&](const Slot& s, int, int n) -> int {
+      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_off);
+      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_idx);
+      for_chunks(s, n, [&](const gs::BatchRows& B, int rows) {
+        gs::k_upper_edges<true><<<blocks_for(rows, TB), TB, 0, st>>>(B, m->sub.cl_off, off, idx, first, nullptr);
+      });
+      GALE_CUDA(cudaGetLastError());
+      return int(GALE_OK);
+    });
+    if (rc != GALE_OK) return rc;
+    GALE_CUDA(gi::exclusive_scan_i32(first, p.nV + 1, d_scan.as<int32_t>(), st));
+    int nE = 0;
+    GALE_CUDA(cudaMemcpyAsync(&nE, first + p.nV, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    m->nE = nE;
+    if ((rc = m->d_e_hi.alloc(size_t(std::max(nE, 1)) * 4 + 64))) return rc;
+    int32_t* hi = m->d_e_hi.as<int32_t>();
+    rc = sweep_batches(m, GALE_REL_VV, st, [&](const Slot& s, int, int n) -> int {
+      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_off);
+      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_idx);
+      for_chunks(s, n, [&](const gs::BatchRows& B, int rows) {
+        gs::k_upper_edges<false><<<blocks_for(rows, TB), TB, 0, st>>>(B, m->sub.cl_off, off, idx, first, hi);
+      });
+      GALE_CUDA(cudaGetLastError());
+      return int(GALE_OK);
+    });
+    if (rc != GALE_OK) return rc;
+    m->sub.e_first = first;
+    m->sub.e_hi = hi;
+  }
+  if (p.flags & GALE_WITH_FACETS) {
+    const int warps = 4, cap = gi::pow2_ceil(std::max(p.gmax, 1));
+    const int smem = warps * cap * 8;
+    if (smem > kSmemLimit - 2048) { g_last_error = "a vertex has too many facets for the triangle enumeration"; return GALE_ERR_UNSUPPORTED; }
+    if ((rc = m->d_f_first.alloc(size_t(p.nV + 2) * 4))) return rc;
+    GALE_CUDA(cudaMemsetAsync(m->d_f_first.p, 0, size_t(p.nV + 2) * 4, st));
+    int32_t* first = m->d_f_first.as<int32_t>();
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_triangles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_triangles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    const int grid = blocks_for(p.nV, warps);
+    if (p.nV) gs::k_triangles<true><<<grid, warps * 32, smem, st>>>(m->dm.T, m->dm.first_tet, m->dm.opp_first, m->dm.opp_perm, p.nV, cap, first, nullptr);
+    GALE_CUDA(cudaGetLastError());
+    GALE_CUDA(gi::exclusive_scan_i32(first, p.nV + 1, d_scan.as<int32_t>(), st));
+    int nF = 0;
+    GALE_CUDA(cudaMemcpyAsync(&nF, first + p.nV, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    m->nF = nF;
+    if ((rc = m->d_f_bc.alloc(size_t(std::max(nF, 1)) * 8 + 64))) return rc;
+    if (p.nV) gs::k_triangles<false><<<grid, warps * 32, smem, st>>>(m->dm.T, m->dm.first_tet, m->dm.opp_first, m->dm.opp_perm, p.nV, cap, first, m->d_f_bc.as<int2>());
+    GALE_CUDA(cudaGetLastError());
+    m->sub.f_first = first;
+    m->sub.f_bc = m->d_f_bc.as<int2>();
+    // sizing of VF: the largest |VT(v)|, then the exact entries per tile
+    DevMem d_max, d_stats;
+    if ((rc = d_max.alloc(4)) || (rc = d_stats.alloc(size_t(std::max(p.nTiles, 1)) * 4))) return rc;
+    GALE_CUDA(cudaMemsetAsync(d_max.p, 0, 4, st));
+    rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int) -> int {
+      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
+      if (s.rows > 0) gs::k_max_row<<<blocks_for(s.rows, TB), TB, 0, st>>>(off, int(s.rows), d_max.as<int>());
+      GALE_CUDA(cudaGetLastError());
+      return int(GALE_OK);
+    });
+    if (rc != GALE_OK) return rc;
+    int maxdeg = 0;
+    GALE_CUDA(cudaMemcpyAsync(&maxdeg, d_max.p, 4, cudaMemcpyDeviceToHost, st));
+    GALE_CUDA(cudaStreamSynchronize(st));
+    m->vf_cap = gi::pow2_ceil(std::max(3 * maxdeg, 32));
+    const int vwarps = 8, vsm = ((p.tv + 4) & ~3) * 4 + vwarps * m->vf_cap * 4;
+    if (vsm > kSmemLimit - 2048) { g_last_error = "a vertex star is too large for the VF kernel"; return GALE_ERR_UNSUPPORTED; }
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int n) -> int {
+      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
+      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_idx);
+      for (int b = 0; b < n; b += gale::kMaxBatch) {
+        const int nb = std::min(gale::kMaxBatch, n - b);
+        gs::VFParams V{};
+        V.n_clusters = nb;
+        for (int i = 0; i < nb; ++i) {
+          const int c = s.ids[size_t(b + i)];
+          V.tile_prefix[i + 1] = V.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
+          V.cluster[i] = c;
+          V.row_base[i] = s.row_begin[size_t(b + i)];
+        }
+        if (V.tile_prefix[nb] > 0)
+          gs::k_vf<true><<<V.tile_prefix[nb], vwarps * 32, vsm, st>>>(m->dm, m->sub, V, m->vf_cap, nullptr, off, idx, nullptr, nullptr, d_stats.as<int32_t>());
+      }
+      GALE_CUDA(cudaGetLastError());
+      return int(GALE_OK);
+    });
+    if (rc != GALE_OK) return rc;
+    std::vector<int32_t> stats, rel(size_t(std::max(p.nTiles, 1)), 0);
+    if ((rc = download_vec(stats, d_stats.p, size_t(p.nTiles), st))) return rc;
+    m->cl_vf.assign(size_t(p.nC), 0);
+    for (int c = 0; c < p.nC; ++c) {
+      long long acc = 0;
+      for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) { rel[size_t(i)] = int32_t(acc); acc += stats[size_t(i)]; }
+      if (acc > 3 * p.cl_vt[size_t(c)] || acc >= (1LL << 31) - 1) return GALE_ERR_UNSUPPORTED;
+      m->cl_vf[size_t(c)] = acc;
+    }
+    if ((rc = upload_vec(m->d_tile_vf_rel, rel, st))) return rc;
+    GALE_CUDA(cudaStreamSynchronize(st));
+  }
+  return GALE_OK;
 }
 
 int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_bytes, cudaStream_t st, gale_mesh_t** out) {
@@ -715,6 +886,10 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
     m->kernel = best[1] < best[0] ? 1 : 0;
     m->tune_ms[0] = best[0]; m->tune_ms[1] = best[1];
     m->submitted.store(0); m->popped.store(0);  // the sample batches are not the caller's: sequence numbers restart
+  }
+  if (m->plan->flags & (GALE_WITH_EDGES | GALE_WITH_FACETS)) {
+    const int rc3 = build_sub_index(m, st);
+    if (rc3 != GALE_OK) return rc3;
   }
   m->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count() + m->plan->analyse_ms;
   guard.m = nullptr;
@@ -810,6 +985,8 @@ int32_t gale_mesh_info(const gale_mesh_t* m, gale_mesh_info_t* out) {
   out->local_id_bytes = p.cfg.lb;
   out->block_threads = m->kernel == 1 ? p.w_NT : p.NT;
   out->index_bytes = m->index_bytes;
+  out->num_edges = m->nE;
+  out->num_triangles = m->nF;
   out->kernel_variant = m->kernel;
   out->tune_dense_ms = m->tune_ms[0];
   out->tune_walk_ms = m->tune_ms[1];
@@ -837,11 +1014,30 @@ int32_t gale_mesh_interval_array(const gale_mesh_t* m, const int32_t** d_first_s
   return GALE_OK;
 }
 
+int32_t gale_mesh_edges(const gale_mesh_t* m, const int32_t** d_first, const int32_t** d_upper, int64_t* num_edges) {
+  if (!m || !d_first || !d_upper || !num_edges) return GALE_ERR_INVALID_ARG;
+  if (!m->sub.e_first) { g_last_error = "the edge list was not built (GALE_WITH_EDGES)"; return GALE_ERR_UNSUPPORTED; }
+  *d_first = m->sub.e_first; *d_upper = m->sub.e_hi; *num_edges = m->nE;
+  return GALE_OK;
+}
+
+int32_t gale_mesh_triangles(const gale_mesh_t* m, const int32_t** d_first, const int32_t** d_second_third, int64_t* num_triangles) {
+  if (!m || !d_first || !d_second_third || !num_triangles) return GALE_ERR_INVALID_ARG;
+  if (!m->sub.f_first) { g_last_error = "the triangle list was not built (GALE_WITH_FACETS)"; return GALE_ERR_UNSUPPORTED; }
+  *d_first = m->sub.f_first; *d_second_third = reinterpret_cast<const int32_t*>(m->sub.f_bc); *num_triangles = m->nF;
+  return GALE_OK;
+}
+
 int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const int32_t* h_cluster_ids,
                                    int32_t n_clusters, void* cuda_stream) {
-  if (!m || (relation_mask & ~uint32_t(GALE_REL_ALL)) || relation_mask == 0 || n_clusters < 0 ||
+  if (!m || (relation_mask & ~uint32_t(GALE_REL_ALL | GALE_REL_VE | GALE_REL_VF)) || relation_mask == 0 || n_clusters < 0 ||
       (n_clusters > 0 && !h_cluster_ids))
     return GALE_ERR_INVALID_ARG;
+  const uint32_t user_mask = relation_mask;
+  if ((user_mask & GALE_REL_VE) && !m->sub.e_first) { g_last_error = "VE needs GALE_WITH_EDGES at create"; return GALE_ERR_UNSUPPORTED; }
+  if ((user_mask & GALE_REL_VF) && !m->sub.f_first) { g_last_error = "VF needs GALE_WITH_FACETS at create"; return GALE_ERR_UNSUPPORTED; }
+  // VE is a map over the VV rows, VF works on the VT rows: the batch kernel computes those too
+  relation_mask = (user_mask & GALE_REL_ALL) | ((user_mask & GALE_REL_VE) ? GALE_REL_VV : 0u) | ((user_mask & GALE_REL_VF) ? GALE_REL_VT : 0u);
   if (n_clusters > m->maxB) return GALE_ERR_BAD_CLUSTER;
   const Plan& p = *m->plan;
   for (int i = 0; i < n_clusters; ++i)
@@ -854,7 +1050,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   const auto t_prep = std::chrono::steady_clock::now();
 
   // batch set-up (a0): row / nnz bases of every requested cluster, in request order
-  s.seq = seq; s.n = n_clusters; s.mask = relation_mask;
+  s.seq = seq; s.n = n_clusters; s.mask = user_mask | relation_mask; s.eff_mask = relation_mask;
   s.ids.assign(h_cluster_ids, h_cluster_ids + n_clusters);
   s.row_begin.assign(n_clusters + 1, 0);
   s.tt_row_begin.assign(n_clusters + 1, 0);
@@ -881,6 +1077,14 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
     s.used.vv_off = o; if (relation_mask & GALE_REL_VV) o = up(o + size_t(s.rows + 1) * 4, 16);
     s.used.vv_idx = o; if (relation_mask & GALE_REL_VV) o = up(o + size_t(s.vv_nnz) * 4, 16);
     s.used.tt = o;     if (relation_mask & GALE_REL_TT) o = up(o + size_t(s.tt_rows) * D * 4, 16);
+    s.used.ve_idx = o; if (user_mask & GALE_REL_VE) o = up(o + size_t(s.vv_nnz) * 4, 16);
+    s.vf_nnz = 0;
+    if (user_mask & GALE_REL_VF) {
+      for (int i = 0; i < n_clusters; ++i) s.vf_nnz += m->cl_vf[size_t(s.ids[i])];
+      if (s.vf_nnz >= (1LL << 31) - 1) return GALE_ERR_INVALID_ARG;
+      s.used.vf_off = o; o = up(o + size_t(s.rows + 1) * 4, 16);
+      s.used.vf_idx = o; o = up(o + size_t(s.vf_nnz) * 4, 16);
+    }
     s.used.total = o;
     if (o > m->cap.total) return GALE_ERR_WORKSPACE;
   }
@@ -934,6 +1138,34 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
     if (walk) walk_kernel_for(D, p.w_NT, p.cfg.lb)<<<grid, p.w_NT, smem, run>>>(m->dm, P, cfg, wlay, O);
     else kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, run>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
+    if (nb > 0 && (user_mask & GALE_REL_VE)) {  // VE: a map over the VV rows just written (gale_sub.cuh)
+      gale::sub::BatchRows B{};
+      B.n_clusters = nb;
+      for (int i = 0; i <= nb; ++i) B.row_base[i] = s.row_begin[b + i];
+      for (int i = 0; i < nb; ++i) B.cluster[i] = s.ids[b + i];
+      const int rows = B.row_base[nb] - B.row_base[0];
+      if (rows > 0)
+        gale::sub::k_ve<<<(rows + 127) / 128, 128, 0, run>>>(B, m->sub, O.vv_offsets, O.vv_indices,
+                                                               reinterpret_cast<int32_t*>(s.dev + s.used.ve_idx));
+      GALE_CUDA(cudaGetLastError());
+    }
+    if (user_mask & GALE_REL_VF) {  // VF from the VT rows just written
+      gale::sub::VFParams V{};
+      V.n_clusters = nb; V.total_rows = int(s.rows); V.total_vf = int(s.vf_nnz);
+      for (int i = 0; i < nb; ++i) {
+        V.tile_prefix[i + 1] = P.tile_prefix[i + 1];
+        V.cluster[i] = P.cluster[i];
+        V.row_base[i] = P.row_base[i];
+      }
+      long long base = 0;
+      for (int i = 0; i < b; ++i) base += m->cl_vf[size_t(s.ids[i])];
+      for (int i = 0; i < nb; ++i) { V.vf_base[i] = int(base); base += m->cl_vf[size_t(s.ids[b + i])]; }
+      const int warps = 8, vsm = ((p.tv + 4) & ~3) * 4 + warps * m->vf_cap * 4;
+      gale::sub::k_vf<false><<<grid, warps * 32, vsm, run>>>(m->dm, m->sub, V, m->vf_cap, m->d_tile_vf_rel.as<int32_t>(), O.vt_offsets,
+                                                           O.vt_indices, reinterpret_cast<int32_t*>(s.dev + s.used.vf_off),
+                                                           reinterpret_cast<int32_t*>(s.dev + s.used.vf_idx), nullptr);
+      GALE_CUDA(cudaGetLastError());
+    }
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, run));
   if (m->queue_depth > 0) {  // a7: D2H into the pinned slot on the side stream
@@ -991,6 +1223,12 @@ int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_m
   if (s.mask & GALE_REL_TT) {
     out->tt_rows = s.tt_rows;
     out->tt_indices = reinterpret_cast<const int32_t*>(b + s.used.tt);
+  }
+  if (s.mask & GALE_REL_VE) out->ve_indices = reinterpret_cast<const int32_t*>(b + s.used.ve_idx);
+  if (s.mask & GALE_REL_VF) {
+    out->vf_nnz = s.vf_nnz;
+    out->vf_offsets = reinterpret_cast<const int32_t*>(b + s.used.vf_off);
+    out->vf_indices = reinterpret_cast<const int32_t*>(b + s.used.vf_idx);
   }
   float ms = 0.f;
   if (cudaEventElapsedTime(&ms, s.ev_start, s.ev_done) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }

@@ -1,0 +1,283 @@
+// gale_sub.cuh — edges and triangles: the sorted lists E and F with their interval
+// arrays I_E / I_F, built at initialization only when asked for (the paper's preconditioning),
+// and the coboundary relations VE and VF of a cluster batch (Table 1 :53-58; DiscreteGradient
+// needs VE, VF, VT, :307).
+//
+// Layout. A sub-simplex is internal to the segment of its lowest vertex, and the lists are
+// sorted by vertex indices, so the edges with lowest vertex a are the contiguous ids
+// [e_first[a], e_first[a+1]) and only their upper vertex is stored (e_hi); likewise the triangles with
+// lowest vertex a are [f_first[a], f_first[a+1]) and (second, third) vertex are stored (f_bc). An id is
+// found by a binary search bounded by the interval array, exactly the paper's look-up (:186-192).
+//
+// VE(v)[i] is the edge between v and VV(v)[i]: edges below v's own block ascend with the lower
+// neighbour, v's own block ascends with the upper neighbour — the order of the sorted VV row. So VE is a
+// map over the VV rows the batch kernel has just written. VF(v) = the distinct triangles of the simplices
+// of VT(v) that contain v, ids ascending: one warp per vertex sorts the candidates in shared memory.
+#pragma once
+#include <cuda_runtime.h>
+#include <limits.h>
+#include <stdint.h>
+
+#include "gale_init.cuh"
+#include "gale_kernels.cuh"
+
+namespace gale {
+namespace sub {
+
+struct SubIndex {               // all DEVICE, owned by the library
+  const int32_t* e_first;       // [nV+1] I_E per vertex
+  const int32_t* e_hi;          // [nE]   upper vertex of every edge
+  const int32_t* f_first;       // [nV+1] I_F per vertex
+  const int2* f_bc;             // [nF]   second and third vertex of every triangle
+  const int32_t* cl_off;        // [nC+1] I_V: first vertex of every cluster
+};
+
+// ---- E from VV rows ----------------------------------------------------------------------------------
+// rows [0, n_rows) of a batch whose vertices are consecutive per cluster; one thread per row.
+// COUNT: deg_hi[v] = number of neighbours above v; else e_hi[e_first[v] + j] = j-th neighbour above v.
+struct BatchRows {
+  int n_clusters;
+  int row_base[kMaxBatch + 1];  // first row of cluster slot i in the batch (+ total)
+  int cluster[kMaxBatch];
+};
+__device__ __forceinline__ int row_vertex(const BatchRows& B, const int32_t* cl_off, int r) {
+  int lo = 0, hi = B.n_clusters;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (B.row_base[mid] <= r) lo = mid; else hi = mid;
+  }
+  return cl_off[B.cluster[lo]] + (r - B.row_base[lo]);
+}
+template <bool COUNT>
+__global__ void k_upper_edges(const __grid_constant__ BatchRows B, const int32_t* __restrict__ cl_off,
+                              const int32_t* __restrict__ vv_off, const int32_t* __restrict__ vv_idx,
+                              int32_t* deg_or_first, int32_t* e_hi) {
+  const int r = B.row_base[0] + blockIdx.x * blockDim.x + threadIdx.x;  // rows of this launch: [row_base[0], row_base[n])
+  if (r >= B.row_base[B.n_clusters]) return;
+  const int v = row_vertex(B, cl_off, r);
+  const int a = vv_off[r], b = vv_off[r + 1];
+  int lo = a, hi = b;  // first entry above v (the row is ascending)
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (vv_idx[mid] < v) lo = mid + 1; else hi = mid;
+  }
+  if (COUNT) {
+    deg_or_first[v] = b - lo;
+  } else {
+    int32_t* out = e_hi + deg_or_first[v];
+    for (int i = lo; i < b; ++i) out[i - lo] = vv_idx[i];
+  }
+}
+
+// ---- F from the facet groups of the vertices ----------------------------------------------------------
+// The triangles with lowest vertex a are the facets (a, x, y) of the simplices of a's run (three each)
+// and the facets opposite the lowest vertex of the simplices whose second vertex is a (one each). One warp
+// per vertex collects them as 64-bit keys (x, y), sorts them in shared memory and drops the duplicates.
+// COUNT: cnt[a] = distinct triangles; else f_bc[f_first[a] + j] = j-th. Dynamic shared memory:
+// (warps per block) * cap * 8 bytes, cap = power of two >= the largest group.
+__device__ __forceinline__ void warp_bitonic64(unsigned long long* a, int n2, int lane) {
+  for (int k = 2; k <= n2; k <<= 1)
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = lane; i < n2; i += 32) {
+        const int p = i ^ j;
+        if (p > i) {
+          const unsigned long long x = a[i], y = a[p];
+          const bool up = (i & k) == 0;
+          if ((x > y) == up) { a[i] = y; a[p] = x; }
+        }
+      }
+      __syncwarp();
+    }
+}
+template <bool COUNT>
+__global__ void k_triangles(const int32_t* __restrict__ T, const int32_t* __restrict__ first_tet,
+                            const int32_t* __restrict__ opp_first, const int32_t* __restrict__ opp_perm, int nV, int cap,
+                            int32_t* cnt_or_first, int2* f_bc) {
+  extern __shared__ unsigned long long shk[];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int a = blockIdx.x * (blockDim.x >> 5) + w;
+  if (a >= nV) return;
+  unsigned long long* keys = shk + (size_t)w * cap;
+  const int r0 = first_tet[a], r1 = first_tet[a + 1], o0 = opp_first[a], o1 = opp_first[a + 1];
+  const int n = 3 * (r1 - r0) + (o1 - o0);
+  const int n2 = init::pow2_ceil(n < 1 ? 1 : n);
+  const int4* T4 = reinterpret_cast<const int4*>(T);
+  auto key = [](int x, int y) { return ((unsigned long long)(unsigned)x << 32) | (unsigned)y; };
+  for (int i = lane; i < n2; i += 32) {
+    unsigned long long k = ~0ull;
+    if (i < 3 * (r1 - r0)) {
+      const int4 q = __ldg(T4 + r0 + i / 3);
+      const int f = i % 3;  // (b,c), (b,d), (c,d)
+      k = f == 0 ? key(q.y, q.z) : (f == 1 ? key(q.y, q.w) : key(q.z, q.w));
+    } else if (i < n) {
+      const int4 q = __ldg(T4 + __ldg(opp_perm + o0 + (i - 3 * (r1 - r0))));
+      k = key(q.z, q.w);
+    }
+    keys[i] = k;
+  }
+  __syncwarp();
+  warp_bitonic64(keys, n2, lane);
+  int base = 0;
+  for (int i0 = 0; i0 < n2; i0 += 32) {  // heads in order
+    const int i = i0 + lane;
+    const bool head = i < n2 && keys[i] != ~0ull && (i == 0 || keys[i] != keys[i - 1]);
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+    if (!COUNT && head) {
+      const unsigned long long k = keys[i];
+      f_bc[cnt_or_first[a] + base + __popc(m & ((1u << lane) - 1u))] = make_int2((int)(k >> 32), (int)(k & 0xFFFFFFFFu));
+    }
+    base += __popc(m);
+  }
+  if (COUNT && lane == 0) cnt_or_first[a] = base;
+}
+
+// ---- VE of a batch: a map over its VV rows -------------------------------------------------------------
+__global__ void k_ve(const __grid_constant__ BatchRows B, const SubIndex X, const int32_t* __restrict__ vv_off,
+                     const int32_t* __restrict__ vv_idx, int32_t* ve_idx) {
+  const int r = B.row_base[0] + blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= B.row_base[B.n_clusters]) return;
+  const int v = row_vertex(B, X.cl_off, r);
+  const int a = vv_off[r], b = vv_off[r + 1];
+  int own = X.e_first[v];
+  for (int i = a; i < b; ++i) {
+    const int u = vv_idx[i];
+    int id;
+    if (u < v) {  // the edge is internal to u's segment: look v up among u's upper neighbours
+      int lo = X.e_first[u], hi = X.e_first[u + 1];
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (X.e_hi[mid] < v) lo = mid + 1; else hi = mid;
+      }
+      id = lo;
+    } else {
+      id = own++;  // v's own block, in the order of its upper neighbours
+    }
+    GALE_ST(ve_idx + i, id);
+  }
+}
+
+// largest row length of a CSR (sizes the candidate buffers of k_vf)
+__global__ void k_max_row(const int32_t* __restrict__ off, int n_rows, int* out) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  int d = r < n_rows ? off[r + 1] - off[r] : 0;
+#pragma unroll
+  for (int k = 16; k > 0; k >>= 1) d = max(d, __shfl_xor_sync(0xFFFFFFFFu, d, k));
+  if ((threadIdx.x & 31) == 0 && d > 0) atomicMax(out, d);
+}
+
+// ---- VF of a batch -------------------------------------------------------------------------------------
+// One block per tile (its rows), one warp per vertex in turn, over the VT rows the batch kernel has just
+// written. Candidates: for every simplex of VT(v) the three triangles that contain v; id of a triangle
+// (a, b, c) = position of (b, c) in a's block of F. COUNT (sizing at create): stats[tile] = entries of the
+// tile, nothing else is written. Dynamic shared memory: ((rows + 4) & ~3) * 4 bytes for the degrees +
+// warps * cap * 4 for the candidates, cap = power of two >= 3 * the largest |VT(v)|.
+struct VFParams {
+  int n_clusters;
+  int total_rows, total_vf;         // terminal offset
+  int tile_prefix[kMaxBatch + 1];
+  int cluster[kMaxBatch];
+  int row_base[kMaxBatch];          // first VT row of slot i in the batch
+  int vf_base[kMaxBatch];           // first VF entry of slot i in the batch
+};
+__device__ __forceinline__ int tri_id(const SubIndex& X, int a, int b, int c) {
+  int lo = X.f_first[a], hi = X.f_first[a + 1];
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    const int2 q = X.f_bc[mid];
+    if (q.x < b || (q.x == b && q.y < c)) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+__device__ __forceinline__ void warp_bitonic32(int32_t* a, int n2, int lane) {
+  for (int k = 2; k <= n2; k <<= 1)
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = lane; i < n2; i += 32) {
+        const int p = i ^ j;
+        if (p > i) {
+          const int x = a[i], y = a[p];
+          const bool up = (i & k) == 0;
+          if ((x > y) == up) { a[i] = y; a[p] = x; }
+        }
+      }
+      __syncwarp();
+    }
+}
+template <bool COUNT>
+__global__ void k_vf(const DeviceMesh M, const SubIndex X, const __grid_constant__ VFParams P, int cap,
+                     const int32_t* __restrict__ tile_vf_rel, const int32_t* __restrict__ vt_off,
+                     const int32_t* __restrict__ vt_idx, int32_t* vf_off, int32_t* vf_idx, int32_t* stats) {
+  extern __shared__ int32_t shv[];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if (!COUNT && blockIdx.x == 0 && threadIdx.x == 0) { vf_off[0] = 0; vf_off[P.total_rows] = P.total_vf; }  // every launch of a batch writes the same two values
+  if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
+  int slot;
+  {
+    int lo = 0, hi = P.n_clusters;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+    }
+    slot = lo;
+  }
+  const int tile = M.cluster_tile_begin[P.cluster[slot]] + ((int)blockIdx.x - P.tile_prefix[slot]);
+  const int nrows = M.tiles[tile].nrows, v_lo = M.tiles[tile].v_lo;
+  const int row0 = P.row_base[slot] + M.tiles[tile].row_rel;
+  int32_t* deg = shv;                         // [nrows + 1]
+  int32_t* cand = shv + ((nrows + 4) & ~3) + (size_t)w * cap;
+  const int4* T4 = reinterpret_cast<const int4*>(M.T);
+  for (int pass = 0; pass < (COUNT ? 1 : 2); ++pass) {
+    // pass 0: degrees; pass 1 (after the scan): the same work again, now written at the rows' offsets
+    for (int r = w; r < nrows; r += nw) {
+      const int v = v_lo + r;
+      const int t0 = vt_off[row0 + r], t1 = vt_off[row0 + r + 1];
+      const int n = min(3 * (t1 - t0), cap);
+      const int n2 = init::pow2_ceil(n < 1 ? 1 : n);
+      for (int i = lane; i < n2; i += 32) {
+        int id = INT_MAX;
+        if (i < n) {
+          const int4 q = __ldg(T4 + vt_idx[t0 + i / 3]);
+          const int s[4] = {q.x, q.y, q.z, q.w};
+          int o[3] = {0, 0, 0}, m = 0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            if (s[k] != v && m < 3) o[m++] = s[k];          // the three other vertices, ascending
+          const int f = i % 3;                              // drop one of them: (v, o1, o2), (v, o0, o2), (v, o0, o1)
+          const int x = f == 0 ? o[1] : o[0], y = f == 2 ? o[1] : o[2];
+          int a = v, b = x, c = y;                          // sort (v, x, y); x < y already
+          if (a > b) { const int tt = a; a = b; b = tt; }
+          if (b > c) { const int tt = b; b = c; c = tt; }
+          id = tri_id(X, a, b, c);
+        }
+        cand[i] = id;
+      }
+      __syncwarp();
+      warp_bitonic32(cand, n2, lane);
+      int base = 0;
+      const int out0 = pass == 1 ? deg[r] : 0;
+      for (int i0 = 0; i0 < n2; i0 += 32) {
+        const int i = i0 + lane;
+        const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
+        const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+        if (pass == 1 && head) GALE_ST(vf_idx + out0 + base + __popc(m & ((1u << lane) - 1u)), cand[i]);
+        base += __popc(m);
+      }
+      __syncwarp();
+      if (pass == 0 && lane == 0) deg[r] = base;
+    }
+    __syncthreads();
+    if (pass == 0) {
+      if (threadIdx.x == 0) {  // a tile has few rows: serial exclusive scan
+        int acc = COUNT ? 0 : P.vf_base[slot] + tile_vf_rel[tile];
+        for (int r = 0; r < nrows; ++r) { const int d = deg[r]; deg[r] = acc; acc += d; }
+        deg[nrows] = acc;
+        if (COUNT) stats[tile] = acc;
+      }
+      __syncthreads();
+      if (!COUNT)
+        for (int r = threadIdx.x; r < nrows; r += blockDim.x) vf_off[row0 + r] = deg[r];
+    }
+  }
+}
+
+}  // namespace sub
+}  // namespace gale

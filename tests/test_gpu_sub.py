@@ -1,0 +1,112 @@
+"""Edges / triangles and the coboundary relations VE / VF (Table 1) through the
+C ABI against the CPU oracle (oracle.sub_simplices: sorted unique combinations, plain definitions), bit-exact:
+the lists E and F with their interval arrays as the initialization builds them on the device, and the VE / VF
+rows of cluster batches."""
+import numpy as np
+import pytest
+
+import meshgen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    ("cfg1", lambda: meshgen.make_config(1), 8, 3),
+    ("cfg3@32", lambda: meshgen.make_config(3, n=32), 5, 3),
+    ("holes3d", lambda: meshgen.make_mesh(3, 20, clustering="octree", capacity=500, permute=True, drop_frac=0.15, seed=5), 7, 3),
+    ("delaunay3d", lambda: meshgen.make_delaunay(3, 4000, seed=31, capacity=500), 4, 3),
+    ("tri2d (VE only)", lambda: meshgen.make_mesh(2, 80, clustering="octree", capacity=700, drop_frac=0.1, seed=6), 5, 2),
+]
+
+
+def _rows(s, lo, hi):
+    off = s["v_off"][lo:hi + 1]
+    return (off - off[0]).astype(np.int32), s["v_idx"][off[0]:off[-1]]
+
+
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
+@pytest.mark.parametrize("name,make,batch,dim", CASES, ids=[c[0] for c in CASES])
+def test_edges_triangles_ve_vf(name, make, batch, dim, kernel):
+    import paper_2507_15230_b200 as gale
+
+    m = make()
+    assert m.dim == dim
+    T, nV = m.simplices, m.num_vertices
+    flags = gale.VALIDATE | gale.WITH_EDGES | (gale.WITH_FACETS if dim == 3 else 0)
+    flags |= gale.KERNEL_WALK if kernel == "walk" else gale.KERNEL_DENSE
+    try:
+        gm = gale.GaleMesh(dim, nV, T, m.cluster_offsets, max_batch_clusters=batch, flags=flags)
+    except gale.GaleError as e:
+        if kernel == "walk" and e.status == gale.ERR_UNSUPPORTED:
+            pytest.skip("walk kernel does not admit this mesh")
+        raise
+    E = oracle.sub_simplices(dim, nV, T, 2)
+    # the edge list and its interval array as built on the device
+    first, upper, nE = gale.gale_mesh_edges(gm.handle)
+    assert nE == len(E["list"]) == gm.info.num_edges
+    e_first = gm_array(gm, first, nV + 1)
+    assert np.array_equal(e_first, E["first"])
+    assert np.array_equal(gm_array(gm, upper, nE), E["list"][:, 1])
+    assert np.array_equal(np.repeat(np.arange(nV), np.diff(e_first)), E["list"][:, 0])
+    mask = gale.REL_VE
+    if dim == 3:
+        F = oracle.sub_simplices(dim, nV, T, 3)
+        ffirst, bc, nF = gale.gale_mesh_triangles(gm.handle)
+        assert nF == len(F["list"]) == gm.info.num_triangles
+        assert np.array_equal(gm_array(gm, ffirst, nV + 1), F["first"])
+        assert np.array_equal(gm_array(gm, bc, 2 * nF).reshape(-1, 2), F["list"][:, 1:])
+        mask |= gale.REL_VF
+    ids = list(range(m.num_clusters))[::-1]                         # any order, several batches
+    ref = oracle.cluster_results(dim, nV, T, m.cluster_offsets, ids, mask=3)
+    k = 0
+    for b in range(0, len(ids), batch):
+        host = gm.run_batch(ids[b:b + batch], mask)
+        assert host["relation_mask"] & gale.REL_VV                  # VE delivers VV too
+        for g in gale.split_batch(host, dim + 1):
+            c = g["cluster"]
+            lo, hi = int(m.cluster_offsets[c]), int(m.cluster_offsets[c + 1])
+            assert np.array_equal(g["vv"][1], ref[k]["vv"][1])
+            off, idx = _rows(E, lo, hi)
+            assert np.array_equal(g["ve"][0], off) and np.array_equal(g["ve"][1], idx), f"{name}: VE of cluster {c}"
+            if dim == 3:
+                off, idx = _rows(F, lo, hi)
+                assert np.array_equal(g["vf"][0], off), f"{name}: VF offsets of cluster {c}"
+                assert np.array_equal(g["vf"][1], idx), f"{name}: VF of cluster {c}"
+                assert np.array_equal(g["vt"][1], ref[k]["vt"][1])  # VF delivers VT too
+            k += 1
+    # all five relations in one call
+    if dim == 3:
+        host = gm.run_batch(ids[:batch], gale.REL_ALL | gale.REL_VE | gale.REL_VF)
+        full = oracle.cluster_results(dim, nV, T, m.cluster_offsets, ids[:batch])
+        for g, r in zip(gale.split_batch(host, dim + 1), full):
+            assert np.array_equal(g["tt"], r["tt"]) and np.array_equal(g["vv"][1], r["vv"][1])
+            lo, hi = int(m.cluster_offsets[g["cluster"]]), int(m.cluster_offsets[g["cluster"] + 1])
+            assert np.array_equal(g["vf"][1], _rows(F, lo, hi)[1]) and np.array_equal(g["ve"][1], _rows(E, lo, hi)[1])
+    gm.destroy()
+
+
+def gm_array(gm, ptr, n):
+    """int32 host copy of n entries at a DEVICE address owned by the library (not inside the caller's workspace)."""
+    from cuda.bindings import runtime as cudart
+
+    out = np.empty(max(n, 1), np.int32)
+    if n:
+        (err,) = cudart.cudaMemcpy(out.ctypes.data, ptr, 4 * n, cudart.cudaMemcpyKind.cudaMemcpyDeviceToHost)
+        assert int(err) == 0, err
+    return out[:n]
+
+
+def test_ve_vf_need_the_lists():
+    import paper_2507_15230_b200 as gale
+
+    m = meshgen.make_config(1)
+    gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=4)
+    for mask in (gale.REL_VE, gale.REL_VF):
+        with pytest.raises(gale.GaleError) as e:
+            gm.compute([0], mask)
+        assert e.value.status == gale.ERR_UNSUPPORTED
+    gm.destroy()
+    tri = meshgen.make_mesh(2, 20, clustering="octree", capacity=100, seed=3)
+    with pytest.raises(gale.GaleError) as e:
+        gale.GaleMesh(2, tri.num_vertices, tri.simplices, tri.cluster_offsets, flags=gale.WITH_FACETS)
+    assert e.value.status == gale.ERR_INVALID_ARG
