@@ -756,8 +756,8 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
     GALE_CUDA(cudaMemcpyAsync(&maxdeg, d_max.p, 4, cudaMemcpyDeviceToHost, st));
     GALE_CUDA(cudaStreamSynchronize(st));
     m->vf_cap = gi::pow2_ceil(std::max(3 * maxdeg, 32));
-    const int vwarps = 8, vsm = ((p.tv + 4) & ~3) * 4 + vwarps * m->vf_cap * 4;
-    if (vsm > kSmemLimit - 2048) { g_last_error = "a vertex star is too large for the VF kernel"; return GALE_ERR_UNSUPPORTED; }
+    const int vwarps = 8, vsm = (2 * ((p.tv + 4) & ~3) + vwarps * m->vf_cap) * 4;   // count mode keeps no results
+    if ((2 * ((p.tv + 4) & ~3) + (vwarps + p.tv) * m->vf_cap) * 4 > kSmemLimit - 2048) { g_last_error = "a vertex star is too large for the VF kernel"; return GALE_ERR_UNSUPPORTED; }
     GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
     GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
     rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int n) -> int {
@@ -1160,7 +1160,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       long long base = 0;
       for (int i = 0; i < b; ++i) base += m->cl_vf[size_t(s.ids[i])];
       for (int i = 0; i < nb; ++i) { V.vf_base[i] = int(base); base += m->cl_vf[size_t(s.ids[b + i])]; }
-      const int warps = 8, vsm = ((p.tv + 4) & ~3) * 4 + warps * m->vf_cap * 4;
+      const int warps = 8, vsm = (2 * ((p.tv + 4) & ~3) + (warps + p.tv) * m->vf_cap) * 4;
       gale::sub::k_vf<false><<<grid, warps * 32, vsm, run>>>(m->dm, m->sub, V, m->vf_cap, m->d_tile_vf_rel.as<int32_t>(), O.vt_offsets,
                                                            O.vt_indices, reinterpret_cast<int32_t*>(s.dev + s.used.vf_off),
                                                            reinterpret_cast<int32_t*>(s.dev + s.used.vf_idx), nullptr);

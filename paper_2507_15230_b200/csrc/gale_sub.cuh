@@ -169,8 +169,9 @@ __global__ void k_max_row(const int32_t* __restrict__ off, int n_rows, int* out)
 // One block per tile (its rows), one warp per vertex in turn, over the VT rows the batch kernel has just
 // written. Candidates: for every simplex of VT(v) the three triangles that contain v; id of a triangle
 // (a, b, c) = position of (b, c) in a's block of F. COUNT (sizing at create): stats[tile] = entries of the
-// tile, nothing else is written. Dynamic shared memory: ((rows + 4) & ~3) * 4 bytes for the degrees +
-// warps * cap * 4 for the candidates, cap = power of two >= 3 * the largest |VT(v)|.
+// tile, nothing else is written. Dynamic shared memory (ints): 2 * ((rows + 4) & ~3) for the degrees +
+// warps * cap for the candidates + rows * cap for the rows' results (not in count mode), cap = power of
+// two >= 3 * the largest |VT(v)|.
 struct VFParams {
   int n_clusters;
   int total_rows, total_vf;         // terminal offset
@@ -222,20 +223,28 @@ __global__ void k_vf(const DeviceMesh M, const SubIndex X, const __grid_constant
   const int tile = M.cluster_tile_begin[P.cluster[slot]] + ((int)blockIdx.x - P.tile_prefix[slot]);
   const int nrows = M.tiles[tile].nrows, v_lo = M.tiles[tile].v_lo;
   const int row0 = P.row_base[slot] + M.tiles[tile].row_rel;
-  int32_t* deg = shv;                         // [nrows + 1]
-  int32_t* cand = shv + ((nrows + 4) & ~3) + (size_t)w * cap;
+  // shared memory: deg[nrows+1] | nlow[nrows] | cand[warps][cap] | keep[nrows][cap] (not in count mode)
+  const int pad = (nrows + 4) & ~3;
+  int32_t* deg = shv;
+  int32_t* nlow = shv + pad;
+  int32_t* cand = shv + 2 * pad + (size_t)w * cap;
+  int32_t* keep = shv + 2 * pad + (size_t)nw * cap;
   const int4* T4 = reinterpret_cast<const int4*>(M.T);
-  for (int pass = 0; pass < (COUNT ? 1 : 2); ++pass) {
-    // pass 0: degrees; pass 1 (after the scan): the same work again, now written at the rows' offsets
-    for (int r = w; r < nrows; r += nw) {
-      const int v = v_lo + r;
-      const int t0 = vt_off[row0 + r], t1 = vt_off[row0 + r + 1];
-      const int n = min(3 * (t1 - t0), cap);
-      const int n2 = init::pow2_ceil(n < 1 ? 1 : n);
-      for (int i = lane; i < n2; i += 32) {
-        int id = INT_MAX;
-        if (i < n) {
-          const int4 q = __ldg(T4 + vt_idx[t0 + i / 3]);
+  // The triangles that have v as their LOWEST vertex are v's own block of F: contiguous ids, no look-up.
+  // The others lie in the blocks of lower vertices (smaller ids): they come from the simplices of VT(v) in
+  // which v is not the lowest vertex — each such triangle is found in at most two of them — and are
+  // looked up, sorted and de-duplicated by the warp.
+  for (int r = w; r < nrows; r += nw) {
+    const int v = v_lo + r;
+    const int t0 = vt_off[row0 + r], t1 = vt_off[row0 + r + 1];
+    const int n = min(3 * (t1 - t0), cap);
+    int nc = 0;  // candidates kept so far (compacted: the sort below is as small as the looked-up part)
+    for (int i0 = 0; i0 < n; i0 += 32) {
+      const int i = i0 + lane;
+      int id = INT_MAX;
+      if (i < n) {
+        const int4 q = __ldg(T4 + vt_idx[t0 + i / 3]);
+        if (q.x != v) {                                      // v is not the lowest vertex of this simplex
           const int s[4] = {q.x, q.y, q.z, q.w};
           int o[3] = {0, 0, 0}, m = 0;
 #pragma unroll
@@ -243,39 +252,46 @@ __global__ void k_vf(const DeviceMesh M, const SubIndex X, const __grid_constant
             if (s[k] != v && m < 3) o[m++] = s[k];          // the three other vertices, ascending
           const int f = i % 3;                              // drop one of them: (v, o1, o2), (v, o0, o2), (v, o0, o1)
           const int x = f == 0 ? o[1] : o[0], y = f == 2 ? o[1] : o[2];
-          int a = v, b = x, c = y;                          // sort (v, x, y); x < y already
-          if (a > b) { const int tt = a; a = b; b = tt; }
-          if (b > c) { const int tt = b; b = c; c = tt; }
-          id = tri_id(X, a, b, c);
+          if (x < v) {                                       // else v is the lowest vertex of the triangle: own block
+            int a = x, b = v, c = y;                         // x < v, x < y: sort (v, y)
+            if (b > c) { const int tt = b; b = c; c = tt; }
+            id = tri_id(X, a, b, c);
+          }
         }
-        cand[i] = id;
       }
-      __syncwarp();
-      warp_bitonic32(cand, n2, lane);
-      int base = 0;
-      const int out0 = pass == 1 ? deg[r] : 0;
-      for (int i0 = 0; i0 < n2; i0 += 32) {
-        const int i = i0 + lane;
-        const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
-        const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
-        if (pass == 1 && head) GALE_ST(vf_idx + out0 + base + __popc(m & ((1u << lane) - 1u)), cand[i]);
-        base += __popc(m);
-      }
-      __syncwarp();
-      if (pass == 0 && lane == 0) deg[r] = base;
+      const unsigned mk = __ballot_sync(0xFFFFFFFFu, id != INT_MAX);
+      if (id != INT_MAX) cand[nc + __popc(mk & ((1u << lane) - 1u))] = id;
+      nc += __popc(mk);
     }
-    __syncthreads();
-    if (pass == 0) {
-      if (threadIdx.x == 0) {  // a tile has few rows: serial exclusive scan
-        int acc = COUNT ? 0 : P.vf_base[slot] + tile_vf_rel[tile];
-        for (int r = 0; r < nrows; ++r) { const int d = deg[r]; deg[r] = acc; acc += d; }
-        deg[nrows] = acc;
-        if (COUNT) stats[tile] = acc;
-      }
-      __syncthreads();
-      if (!COUNT)
-        for (int r = threadIdx.x; r < nrows; r += blockDim.x) vf_off[row0 + r] = deg[r];
+    const int n2 = init::pow2_ceil(nc < 1 ? 1 : nc);
+    for (int i = nc + lane; i < n2; i += 32) cand[i] = INT_MAX;
+    __syncwarp();
+    warp_bitonic32(cand, n2, lane);
+    int base = 0;
+    for (int i0 = 0; i0 < n2; i0 += 32) {
+      const int i = i0 + lane;
+      const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
+      const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+      if (!COUNT && head) keep[(size_t)r * cap + base + __popc(m & ((1u << lane) - 1u))] = cand[i];
+      base += __popc(m);
     }
+    __syncwarp();
+    if (lane == 0) { nlow[r] = base; deg[r] = base + (X.f_first[v + 1] - X.f_first[v]); }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {  // a tile has few rows: serial exclusive scan
+    int acc = COUNT ? 0 : P.vf_base[slot] + tile_vf_rel[tile];
+    for (int r = 0; r < nrows; ++r) { const int d = deg[r]; deg[r] = acc; acc += d; }
+    deg[nrows] = acc;
+    if (COUNT) stats[tile] = acc;
+  }
+  __syncthreads();
+  if (COUNT) return;
+  for (int r = threadIdx.x; r < nrows; r += blockDim.x) vf_off[row0 + r] = deg[r];
+  for (int r = w; r < nrows; r += nw) {  // write-out, one warp per row: the looked-up ids, then the own block
+    const int nl = nlow[r], tot = deg[r + 1] - deg[r], own0 = X.f_first[v_lo + r];
+    int32_t* out = vf_idx + deg[r];
+    for (int i = lane; i < tot; i += 32) GALE_ST(out + i, i < nl ? keep[(size_t)r * cap + i] : own0 + (i - nl));
   }
 }
 
