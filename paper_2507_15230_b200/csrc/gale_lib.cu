@@ -132,10 +132,7 @@ int validate_manifold(const Plan& p, const std::vector<int32_t>& T) {
   return GALE_OK;
 }
 
-inline int threads_for_tile(int tv) {  // NT >= tv (one thread per row in P2)
-  if (const char* e = std::getenv("GALE_NT")) { const int v = std::atoi(e); if ((v == 128 || v == 256) && v >= tv) return v; }
-  return tv > 128 ? 256 : 128;
-}
+inline int threads_for_tile(int tv) { return tv > 128 ? 256 : 128; }  // NT >= tv (one thread per row in P2); 256 threads for 32-vertex tiles measured -25 %
 
 // Kernel capacities for one launch: regions the relation mask does not need are dropped.
 SmemCfg cfg_for_mask(const SmemCfg& full, uint32_t mask, bool count_mode) {
@@ -605,8 +602,9 @@ struct gale_mesh {
   // caller's stream at the time of the call: a batch is a few waves of resident blocks, and the draining
   // tail of one launch + the launch gap overlap the next launch instead. With GALE_STREAM_ORDERED the
   // kernels run on the caller's stream itself.
-  static constexpr int kLaunchStreams = 2;
-  cudaStream_t launch[kLaunchStreams] = {nullptr, nullptr};
+  static constexpr int kMaxLaunchStreams = 2;
+  int n_launch = 2;  // streams in use (3, 4 and 8 measured flat on configs 4 and 5)
+  cudaStream_t launch[kMaxLaunchStreams] = {};
   int32_t* h_err = nullptr;  // mapped pinned; the kernels write guard codes here
   std::atomic<long long> submitted{0}, popped{0};
   size_t workspace_used = 0, index_bytes = 0;
@@ -857,7 +855,7 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
   m->workspace_used = o;
   if (p->queue_depth > 0) GALE_CUDA(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
   if (!m->stream_ordered)
-    for (int i = 0; i < gale_mesh::kLaunchStreams; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
+    for (int i = 0; i < m->n_launch; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
   GALE_CUDA(allow_max_smem(kernel_for(m->D, p->NT, false, p->cfg.lb)));
   if (p->walk_ok) GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
   const uint32_t force = p->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK);
@@ -1108,7 +1106,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
 #endif
   const int smem = walk ? wlay.total : lay.total;
   // everything the caller enqueued on its stream so far (e.g. the upload of the simplices) comes first
-  cudaStream_t run = m->stream_ordered ? st : m->launch[seq % gale_mesh::kLaunchStreams];
+  cudaStream_t run = m->stream_ordered ? st : m->launch[seq % m->n_launch];
   if (!m->stream_ordered) {
     GALE_CUDA(cudaEventRecord(s.ev_submit, st));
     GALE_CUDA(cudaStreamWaitEvent(run, s.ev_submit, 0));
