@@ -162,15 +162,19 @@ KernelFn kernel_for(int D, int NT, bool count, int lb) {
 }
 
 using WalkFn = void (*)(const DeviceMesh, const gale::BatchParams, const SmemCfg, const gale::WalkLayout, const gale::OutPtrs);
-template <int D, int LB>
+template <int D, int LB, bool ALL>
 WalkFn walk_for_nt(int NT) {
-  return NT == 512 ? gale::gale_walk_kernel<D, 512, LB>
-                   : (NT == 256 ? gale::gale_walk_kernel<D, 256, LB>
-                                : (NT == 128 ? gale::gale_walk_kernel<D, 128, LB> : gale::gale_walk_kernel<D, 64, LB>));
+  return NT == 512 ? gale::gale_walk_kernel<D, 512, LB, ALL>
+                   : (NT == 256 ? gale::gale_walk_kernel<D, 256, LB, ALL>
+                                : (NT == 128 ? gale::gale_walk_kernel<D, 128, LB, ALL> : gale::gale_walk_kernel<D, 64, LB, ALL>));
 }
-WalkFn walk_kernel_for(int D, int NT, int lb) {
-  if (D == 4) return lb == 1 ? walk_for_nt<4, 1>(NT) : walk_for_nt<4, 2>(NT);
-  return lb == 1 ? walk_for_nt<3, 1>(NT) : walk_for_nt<3, 2>(NT);
+template <bool ALL>
+WalkFn walk_kernel_for_all(int D, int NT, int lb) {
+  if (D == 4) return lb == 1 ? walk_for_nt<4, 1, ALL>(NT) : walk_for_nt<4, 2, ALL>(NT);
+  return lb == 1 ? walk_for_nt<3, 1, ALL>(NT) : walk_for_nt<3, 2, ALL>(NT);
+}
+WalkFn walk_kernel_for(int D, int NT, int lb, bool all = false) {
+  return all ? walk_kernel_for_all<true>(D, NT, lb) : walk_kernel_for_all<false>(D, NT, lb);
 }
 inline int walk_threads_for_tile(int tv) { return tv > 128 ? 512 : (tv > 64 ? 256 : (tv > 32 ? 128 : 64)); }  // NT = 2 * rows
 SmemCfg walk_cfg_for_mask(const SmemCfg& full, uint32_t mask) {
@@ -857,7 +861,10 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
   if (!m->stream_ordered)
     for (int i = 0; i < m->n_launch; ++i) GALE_CUDA(cudaStreamCreateWithFlags(&m->launch[i], cudaStreamNonBlocking));
   GALE_CUDA(allow_max_smem(kernel_for(m->D, p->NT, false, p->cfg.lb)));
-  if (p->walk_ok) GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
+  if (p->walk_ok) {
+    GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb, false), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
+    GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb, true), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
+  }
   const uint32_t force = p->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK);
   const bool may_walk = p->walk_ok;
   m->plan = std::move(p);
@@ -1133,7 +1140,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       P.uniform_tiles = uniform ? per : 0;
     }
     const int grid = std::max(1, P.tile_prefix[nb]);
-    if (walk) walk_kernel_for(D, p.w_NT, p.cfg.lb)<<<grid, p.w_NT, smem, run>>>(m->dm, P, cfg, wlay, O);
+    if (walk) walk_kernel_for(D, p.w_NT, p.cfg.lb, relation_mask == GALE_REL_ALL)<<<grid, p.w_NT, smem, run>>>(m->dm, P, cfg, wlay, O);
     else kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, run>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
     if (nb > 0 && (user_mask & GALE_REL_VE)) {  // VE: a map over the VV rows just written (gale_sub.cuh)

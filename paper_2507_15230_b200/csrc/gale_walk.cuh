@@ -147,7 +147,8 @@ __device__ __forceinline__ uint32_t half_exclusive_scan(uint32_t x, uint32_t* sc
 }
 
 // NT = 2 * (rows per tile capacity): thread tid < NT/2 is A(tid), thread NT/2 + p is B(p).
-template <int D, int NT, int LB>
+// ALL: the launch computes all three relations (the mask tests fold at compile time).
+template <int D, int NT, int LB, bool ALL>
 __global__ void __launch_bounds__(NT, (NT <= 64 ? 16 : (NT <= 128 ? 8 : (NT <= 256 ? 4 : 2))))
 gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, const SmemCfg C,
                  const WalkLayout L, const OutPtrs O) {
@@ -155,7 +156,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   constexpr int TV = NT / 2;
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t mask = P.mask;
-  const bool do_vt = (mask & REL_VT) != 0, do_vv = (mask & REL_VV) != 0, do_tt = (mask & REL_TT) != 0;
+  const bool do_vt = ALL || (mask & REL_VT) != 0, do_vv = ALL || (mask & REL_VV) != 0, do_tt = ALL || (mask & REL_TT) != 0;
   const bool entries = do_vt || do_tt;  // VT entries are staged (TT reads their flags)
 
   // ---- block -> (cluster slot, tile): worked out by the first warp, shared through BlockCtx; the same
@@ -423,10 +424,9 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   if (do_tt) {
     const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
     const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
-    for (int base = tid - lane; base < s_int; base += NT) {  // warp-uniform trip count
-      const int i = base + lane;
+    for (int i = tid; i < s_int; i += NT) {
       bool need_fb = false;
-      if (i < s_int) {
+      {
         uint32_t e[D];
         if constexpr (D == 4) {
           const uint2 q = reinterpret_cast<const uint2*>(ttrow)[i];
@@ -461,14 +461,9 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
           o[1] = r[1]; o[2] = r[2];
         }
       }
-      const unsigned fbm = __ballot_sync(0xFFFFFFFFu, need_fb);
-      if (fbm) {
-        const int leader = __ffs(fbm) - 1;
-        uint32_t pos = 0u;
-        if (lane == leader) pos = atomicAdd(&scan[36], (uint32_t)__popc(fbm));
-        pos = __shfl_sync(0xFFFFFFFFu, pos, leader);
-        if (need_fb && GALE_IN_BOUNDS(M.err, (int)(pos + __popc(fbm & ((1u << lane) - 1u))) < C.sint))
-          fbq[pos + __popc(fbm & ((1u << lane) - 1u))] = (uint16_t)i;
+      if (need_fb) {  // rare (cross-cluster facets only): a plain atomic per facet
+        const uint32_t pos = atomicAdd(&scan[36], 1u);
+        if (GALE_IN_BOUNDS(M.err, (int)pos < C.sint)) fbq[pos] = (uint16_t)i;
       }
     }
     // entry 0 of the external simplices of this cluster whose second vertex is a vertex of this tile
