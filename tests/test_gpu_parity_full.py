@@ -118,3 +118,55 @@ def test_full_size_in_bench_configuration(cfg):
     assert len(sel) >= (nC if cfg == 3 else nC // 8)
     ref = oracle.cluster_results(m.dim, nV, m.simplices, m.cluster_offsets, sel, restricted=(cfg != 3))
     _compare(kept, ref, f"config {cfg} full size (tile {info.tile_vertices}, {info.local_id_bytes}-byte local ids)")
+
+
+def test_edges_triangles_ve_vf_full_size():
+    """SURVEY §8(f)-2 at full size. Config 3 (12.3 M tets): E, F, I_E, I_F and the VE / VF rows of EVERY cluster
+    against the oracle's sorted unique combinations. Config 5 (99.5 M tets): the numbers of edges and triangles
+    against the Kuhn closed forms (E = 3n^2 m + 3n m^2 + m^3, F = 12 m^3 + 6 m^2), and sum |VE| = 2E,
+    sum |VF| = 3F over a complete pass."""
+    import paper_2507_15230_b200 as gale
+    from test_gpu_sub import gm_array, _rows
+
+    m = meshgen.make_config(3)
+    nV, T = m.num_vertices, m.simplices
+    gm = gale.GaleMesh(3, nV, T, m.cluster_offsets, max_batch_clusters=BATCH, device_ring=2,
+                       flags=gale.WITH_EDGES | gale.WITH_FACETS)
+    E = oracle.sub_simplices(3, nV, T, 2)
+    F = oracle.sub_simplices(3, nV, T, 3)
+    first, upper, nE = gale.gale_mesh_edges(gm.handle)
+    ffirst, bc, nF = gale.gale_mesh_triangles(gm.handle)
+    assert nE == len(E["list"]) and nF == len(F["list"])
+    assert np.array_equal(gm_array(gm, first, nV + 1), E["first"]) and np.array_equal(gm_array(gm, upper, nE), E["list"][:, 1])
+    assert np.array_equal(gm_array(gm, ffirst, nV + 1), F["first"])
+    assert np.array_equal(gm_array(gm, bc, 2 * nF).reshape(-1, 2), F["list"][:, 1:])
+    for b in range(0, m.num_clusters, BATCH):
+        ids = list(range(b, min(m.num_clusters, b + BATCH)))
+        for g in gale.split_batch(gm.run_batch(ids, gale.REL_VE | gale.REL_VF), 4):
+            lo, hi = int(m.cluster_offsets[g["cluster"]]), int(m.cluster_offsets[g["cluster"] + 1])
+            off, idx = _rows(E, lo, hi)
+            assert np.array_equal(g["ve"][0], off) and np.array_equal(g["ve"][1], idx), f"VE cluster {g['cluster']}"
+            off, idx = _rows(F, lo, hi)
+            assert np.array_equal(g["vf"][0], off) and np.array_equal(g["vf"][1], idx), f"VF cluster {g['cluster']}"
+    gm.destroy()
+    del E, F
+
+    m = meshgen.make_config(5)
+    n, mm = GRID_N[5], GRID_N[5] - 1
+    gm = gale.GaleMesh(3, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=BATCH, device_ring=2,
+                       flags=gale.WITH_EDGES | gale.WITH_FACETS)
+    nE_cf, nF_cf = 3 * n * n * mm + 3 * n * mm * mm + mm ** 3, 12 * mm ** 3 + 6 * mm * mm
+    assert gm.info.num_edges == nE_cf and gm.info.num_triangles == nF_cf
+    tot_ve = tot_vf = 0
+    for b in range(0, m.num_clusters, BATCH):
+        ids = np.arange(b, min(m.num_clusters, b + BATCH), dtype=np.int32)
+        assert gm.compute(ids, gale.REL_VE | gale.REL_VF) == gale.OK
+        st, v = gm.pop(-1)
+        a = gm.view_arrays(v)
+        assert int(a["vf_offsets"][-1]) == a["vf_indices"].numel() and bool((a["vf_offsets"][1:] >= a["vf_offsets"][:-1]).all())
+        assert int(a["ve_indices"].max()) < nE_cf and int(a["vf_indices"].max()) < nF_cf and int(a["vf_indices"].min()) >= 0
+        tot_ve += a["ve_indices"].numel()
+        tot_vf += a["vf_indices"].numel()
+        gm.release(v)
+    assert tot_ve == 2 * nE_cf and tot_vf == 3 * nF_cf
+    gm.destroy()
