@@ -83,6 +83,16 @@ def _load():
         lib.go_sub_v_idx.argtypes = [vp]
         lib.go_sub_release.restype = None
         lib.go_sub_release.argtypes = [vp]
+        lib.go_coboundary.restype = vp
+        lib.go_coboundary.argtypes = [c_int, c_int, c_int, i64, i64, i32p]
+        lib.go_cob_rows.restype = i64
+        lib.go_cob_rows.argtypes = [vp]
+        lib.go_cob_off.restype = i64p
+        lib.go_cob_off.argtypes = [vp]
+        lib.go_cob_idx.restype = i32p
+        lib.go_cob_idx.argtypes = [vp]
+        lib.go_cob_release.restype = None
+        lib.go_cob_release.argtypes = [vp]
         lib.go_brute_vt.restype = None
         lib.go_brute_vt.argtypes = [c_int, i64, i64, i32p, i64p, i32p]
         lib.go_brute_vv.restype = None
@@ -253,6 +263,22 @@ def sub_simplices(dim: int, num_vertices: int, simplices: np.ndarray, k: int) ->
                     v_idx=_np(lib.go_sub_v_idx(h), n * k, np.int32))
     finally:
         lib.go_sub_release(h)
+
+
+def coboundary(dim: int, num_vertices: int, simplices: np.ndarray, name: str) -> tuple:
+    """EF, ET or FT (Table 1) over the whole mesh as CSR (int64 offsets, int32 indices): rows = ids of
+    the sorted edge (E..) / triangle (F..) list, entries = ascending ids of the triangles (.F) / simplices (.T)
+    that contain them."""
+    lib = _load()
+    T = _canon(simplices)
+    frm, to = {"EF": (2, 3), "ET": (2, dim + 1), "FT": (3, dim + 1)}[name]
+    h = lib.go_coboundary(dim, frm, to, int(num_vertices), T.shape[0], _i32(T))
+    try:
+        n = int(lib.go_cob_rows(h))
+        off = _np(lib.go_cob_off(h), n + 1, np.int64)
+        return off, _np(lib.go_cob_idx(h), int(off[-1]), np.int32)
+    finally:
+        lib.go_cob_release(h)
 
 
 def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:

@@ -340,6 +340,75 @@ const int64_t* go_sub_v_off(void* h) { return static_cast<SubSimplices*>(h)->v_o
 const int32_t* go_sub_v_idx(void* h) { return static_cast<SubSimplices*>(h)->v_idx.data(); }
 void go_sub_release(void* h) { delete static_cast<SubSimplices*>(h); }
 
+// Coboundary relations between sub-simplices ("the coboundary relation R_{k,p}, k < p, maps a
+// k-simplex to the p-simplices incident in it"; Table 1 :53-58): rows = the sorted list of (from)-vertex
+// sub-simplices (from = 2 edges, 3 triangles), entries = ascending ids of the (to)-vertex simplices that
+// contain them (to = 3: triangles of the sorted list F; to = D: the simplices of T). EF = (2,3), ET = (2,D),
+// FT = (3,D). Plain: for every containing simplex in ascending id order, look each of its sub-simplices up
+// in the sorted row list and append the id.
+}  // extern "C" (templates below)
+struct Cobound {
+  std::vector<int64_t> off;
+  std::vector<int32_t> idx;
+};
+template <int KF>
+static void cobound_fill(Cobound& C, const std::vector<int32_t>& rows, int KT, int64_t nCols, const int32_t* cols) {
+  using Key = std::array<int32_t, KF>;
+  const int64_t nRows = int64_t(rows.size()) / KF;
+  auto row_id = [&](const Key& k) {
+    int64_t lo = 0, hi = nRows;
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) / 2;
+      Key r;
+      for (int i = 0; i < KF; ++i) r[i] = rows[mid * KF + i];
+      if (r < k) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+  };
+  std::vector<std::vector<int32_t>> lists(nRows);
+  std::vector<int> pick(KF);
+  for (int64_t c = 0; c < nCols; ++c) {
+    const int32_t* s = cols + c * KT;
+    // every KF-subset of the KT vertices, positions ascending
+    std::vector<int> p(KF);
+    for (int i = 0; i < KF; ++i) p[i] = i;
+    for (;;) {
+      Key k;
+      for (int i = 0; i < KF; ++i) k[i] = s[p[i]];
+      lists[row_id(k)].push_back(int32_t(c));
+      int i = KF - 1;
+      while (i >= 0 && p[i] == KT - KF + i) --i;
+      if (i < 0) break;
+      ++p[i];
+      for (int j = i + 1; j < KF; ++j) p[j] = p[j - 1] + 1;
+    }
+  }
+  C.off.assign(nRows + 1, 0);
+  for (int64_t r = 0; r < nRows; ++r) {
+    C.off[r + 1] = C.off[r] + int64_t(lists[r].size());
+    C.idx.insert(C.idx.end(), lists[r].begin(), lists[r].end());
+  }
+}
+extern "C" {
+void* go_coboundary(int dim, int from, int to, int64_t nV, int64_t nT, const int32_t* T) {
+  const int D = dim + 1;
+  SubSimplices* R = from == 2 ? enumerate_sub<2>(D, nV, nT, T) : enumerate_sub<3>(D, nV, nT, T);
+  Cobound* C = new Cobound;
+  if (to == D) {
+    if (from == 2) cobound_fill<2>(*C, R->list, D, nT, T); else cobound_fill<3>(*C, R->list, D, nT, T);
+  } else {  // to == 3 < D: the containing simplices are the triangles of F
+    SubSimplices* F = enumerate_sub<3>(D, nV, nT, T);
+    cobound_fill<2>(*C, R->list, 3, int64_t(F->list.size()) / 3, F->list.data());
+    delete F;
+  }
+  delete R;
+  return C;
+}
+int64_t go_cob_rows(void* h) { return int64_t(static_cast<Cobound*>(h)->off.size()) - 1; }
+const int64_t* go_cob_off(void* h) { return static_cast<Cobound*>(h)->off.data(); }
+const int32_t* go_cob_idx(void* h) { return static_cast<Cobound*>(h)->idx.data(); }
+void go_cob_release(void* h) { delete static_cast<Cobound*>(h); }
+
 // ---- brute-force enumeration (tiny meshes; pins the routines above) ------------------------------
 // Membership scans straight from the definitions; no sorting, no transposition.
 static bool contains(const int32_t* r, int D, int32_t v) {

@@ -357,3 +357,30 @@ def test_edges_triangles_closed_forms_and_brute_force(dim, n):
     assert np.array_equal(np.where(ev[:, 0] == v, ev[:, 1], ev[:, 0]), nb)
     if dim == 3:
         assert np.diff(f["v_off"]).max() == 36                        # interior Kuhn vertex: 36 triangles
+
+
+@pytest.mark.parametrize("n", [5, 7])
+def test_ef_et_ft_counts_brute_force_and_tt_consistency(n):
+    """EF / ET / FT (Table 1): closed-form sums, python-set brute force, and FT against TT —
+    a triangle with two cofaces is exactly a pair of face-adjacent simplices."""
+    m = meshgen.make_mesh(3, n, clustering="octree", capacity=80, permute=True, seed=31)
+    T, nV, nT = m.simplices, m.num_vertices, m.num_simplices
+    cf = meshgen.kuhn_closed_forms(3, n)
+    E = oracle.sub_simplices(3, nV, T, 2)["list"]
+    F = oracle.sub_simplices(3, nV, T, 3)["list"]
+    et = oracle.coboundary(3, nV, T, "ET")
+    ft = oracle.coboundary(3, nV, T, "FT")
+    ef = oracle.coboundary(3, nV, T, "EF")
+    assert et[0][-1] == 6 * nT and ft[0][-1] == 4 * nT and ef[0][-1] == 3 * len(F)       # incidences counted from the other side
+    assert len(et[0]) - 1 == len(E) and len(ft[0]) - 1 == len(F) == len(ef[0]) - 1 + len(F) - len(E)
+    nft = np.diff(ft[0])
+    assert set(nft.tolist()) <= {1, 2} and int((nft == 1).sum()) == cf["boundary_facets"]
+    sets = [set(r.tolist()) for r in T]
+    for rows, (off, idx), cols in ((E, et, sets), (F, ft, sets), (E, ef, [set(r.tolist()) for r in F])):
+        for r in (0, len(rows) // 3, len(rows) - 1):
+            want = [i for i, c in enumerate(cols) if set(rows[r].tolist()) <= c]
+            assert idx[off[r]:off[r + 1]].tolist() == want
+    tt = oracle.relations_global(3, nV, T, mask=4)["tt"]
+    pairs_tt = {(min(t, int(u)), max(t, int(u))) for t in range(nT) for u in tt[t] if u >= 0}
+    pairs_ft = {(int(ft[1][ft[0][f]]), int(ft[1][ft[0][f] + 1])) for f in range(len(F)) if nft[f] == 2}
+    assert pairs_tt == pairs_ft
