@@ -40,8 +40,14 @@ enum {
   GALE_REL_VT = 1, GALE_REL_VV = 2, GALE_REL_TT = 4,
   GALE_REL_ALL = 7,  /* the three relations of the hot path                                           */
   GALE_REL_VE = 8,   /* vertex -> incident edges; needs GALE_WITH_EDGES at create; also delivers VV   */
-  GALE_REL_VF = 16   /* vertex -> incident triangles (tetrahedral meshes); needs GALE_WITH_FACETS; also
+  GALE_REL_VF = 16,  /* vertex -> incident triangles (tetrahedral meshes); needs GALE_WITH_FACETS; also
                         delivers VT                                                                  */
+  /* the coboundary relations of edges and triangles (Table 1; MS complex :309), tetrahedral
+     meshes, need GALE_WITH_COBOUNDARY; rows = the edges / triangles internal to the requested clusters
+     (those whose lowest vertex belongs to the cluster), in id order; all deliver VT too  */
+  GALE_REL_EF = 32,  /* edge -> triangles                                                             */
+  GALE_REL_ET = 64,  /* edge -> simplices                                                             */
+  GALE_REL_FT = 128  /* triangle -> simplices (one or two)                                            */
 };
 
 enum {
@@ -69,6 +75,8 @@ enum {
                                   I_E (generated "only when the edge or triangle information
                                   is explicitly needed"); enables GALE_REL_VE                              */
   GALE_WITH_FACETS = 128u,     /* ... and the sorted triangle list F with I_F; enables GALE_REL_VF (dim = 3)  */
+  GALE_WITH_COBOUNDARY = 256u, /* with GALE_WITH_EDGES | GALE_WITH_FACETS (dim = 3): also size EF / ET / FT and reserve
+                                  room for them in the result slots; enables GALE_REL_EF / _ET / _FT          */
   GALE_STAGE_FROM_T = 32u,     /* dense kernel only (implies nothing for the walk kernel): stage the rows of T
                                   and T_ex themselves and derive the tile-local ids in the kernel instead of
                                   reading the create-time re-encoding; slower, kept for the A/B in DESIGN.md */
@@ -141,6 +149,14 @@ typedef struct {
   int64_t vf_nnz;
   const int32_t *vf_offsets;     /* [vt_rows+1] or NULL                                                */
   const int32_t *vf_indices;     /* [vf_nnz]                                                           */
+  /* EF / ET / FT: rows of the i-th requested cluster are [e_row_begin[i], e_row_begin[i+1]) (edges) resp.
+   * f_row_begin (triangles); the first row of cluster c is edge I_E[o[c]] resp. triangle I_F[o[c]]     */
+  const int32_t *e_row_begin;    /* HOST [n_clusters+1] or NULL                                        */
+  const int32_t *f_row_begin;    /* HOST [n_clusters+1] or NULL                                        */
+  int64_t ef_nnz, et_nnz, ft_nnz;
+  const int32_t *ef_offsets, *ef_indices;   /* [edge rows + 1], [ef_nnz]: triangle ids                 */
+  const int32_t *et_offsets, *et_indices;   /* [edge rows + 1], [et_nnz]: simplex ids                  */
+  const int32_t *ft_offsets, *ft_indices;   /* [triangle rows + 1], [ft_nnz]: simplex ids              */
 } gale_batch_view_t;
 
 /* Init statistics ("Initialization"), for reporting. */

@@ -16,8 +16,9 @@ from .build import LIB, build_library
 
 REL_VT, REL_VV, REL_TT, REL_ALL = 1, 2, 4, 7
 REL_VE, REL_VF = 8, 16
+REL_EF, REL_ET, REL_FT = 32, 64, 128
 VALIDATE, VALIDATE_MANIFOLD, STREAM_ORDERED, KERNEL_DENSE, KERNEL_WALK, STAGE_FROM_T = 1, 2, 4, 8, 16, 32
-WITH_EDGES, WITH_FACETS = 64, 128
+WITH_EDGES, WITH_FACETS, WITH_COBOUNDARY = 64, 128, 256
 OK, ERR_INVALID_ARG, ERR_NOT_CANONICAL, ERR_DEGENERATE, ERR_NONMANIFOLD, ERR_BAD_CLUSTER = 0, -1, -2, -3, -4, -5
 ERR_WOULD_BLOCK, ERR_EMPTY, ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -6, -7, -8, -9, -10
 
@@ -45,7 +46,12 @@ class gale_batch_view_t(ctypes.Structure):
                 ("prep_ms", ctypes.c_float), ("d2h_ms", ctypes.c_float), ("queue_ms", ctypes.c_float),
                 ("reserved", ctypes.c_int32),
                 ("ve_indices", ctypes.c_void_p), ("vf_nnz", ctypes.c_int64),
-                ("vf_offsets", ctypes.c_void_p), ("vf_indices", ctypes.c_void_p)]
+                ("vf_offsets", ctypes.c_void_p), ("vf_indices", ctypes.c_void_p),
+                ("e_row_begin", _i32p), ("f_row_begin", _i32p),
+                ("ef_nnz", ctypes.c_int64), ("et_nnz", ctypes.c_int64), ("ft_nnz", ctypes.c_int64),
+                ("ef_offsets", ctypes.c_void_p), ("ef_indices", ctypes.c_void_p),
+                ("et_offsets", ctypes.c_void_p), ("et_indices", ctypes.c_void_p),
+                ("ft_offsets", ctypes.c_void_p), ("ft_indices", ctypes.c_void_p)]
 
 
 class gale_mesh_info_t(ctypes.Structure):
@@ -329,6 +335,13 @@ class GaleMesh:
         if view.relation_mask & REL_VF:
             out["vf_offsets"] = self._array(view, view.vf_offsets, view.vt_rows + 1)
             out["vf_indices"] = self._array(view, view.vf_indices, view.vf_nnz)
+        if view.relation_mask & (REL_EF | REL_ET | REL_FT):
+            out["e_row_begin"] = np.ctypeslib.as_array(view.e_row_begin, shape=(n + 1,)).copy()
+            out["f_row_begin"] = np.ctypeslib.as_array(view.f_row_begin, shape=(n + 1,)).copy()
+            for key, bit, rb in (("ef", REL_EF, "e_row_begin"), ("et", REL_ET, "e_row_begin"), ("ft", REL_FT, "f_row_begin")):
+                if view.relation_mask & bit:
+                    out[key + "_offsets"] = self._array(view, getattr(view, key + "_offsets"), int(out[rb][-1]) + 1)
+                    out[key + "_indices"] = self._array(view, getattr(view, key + "_indices"), getattr(view, key + "_nnz"))
         return out
 
     def run_batch(self, cluster_ids, relation_mask: int = REL_ALL) -> dict:
@@ -379,5 +392,10 @@ def split_batch(host: dict, D: int) -> list:
             item["ve"] = ((off - off[0]).astype(np.int32), host["ve_indices"][off[0]:off[-1]])
         if "tt_indices" in host:
             item["tt"] = host["tt_indices"][t0 * D:t1 * D].reshape(-1, D)
+        for k, rb in (("ef", "e_row_begin"), ("et", "e_row_begin"), ("ft", "f_row_begin")):
+            if k + "_offsets" in host:                    # rows = the cluster's own edges / triangles
+                q0, q1 = int(host[rb][i]), int(host[rb][i + 1])
+                off = host[k + "_offsets"][q0:q1 + 1]
+                item[k] = ((off - off[0]).astype(np.int32), host[k + "_indices"][off[0]:off[-1]])
         res.append(item)
     return res

@@ -94,7 +94,9 @@ struct Plan {
 };
 
 struct SlotLayout {
-  size_t vt_off = 0, vt_idx = 0, vv_off = 0, vv_idx = 0, tt = 0, ve_idx = 0, vf_off = 0, vf_idx = 0, total = 0;
+  size_t vt_off = 0, vt_idx = 0, vv_off = 0, vv_idx = 0, tt = 0, ve_idx = 0, vf_off = 0, vf_idx = 0;
+  size_t cob_off[3] = {0, 0, 0}, cob_idx[3] = {0, 0, 0};  // ET, FT, EF (gale::sub::COB_*)
+  size_t total = 0;
 };
 SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
   const int D = p.dim + 1;
@@ -109,6 +111,16 @@ SlotLayout slot_capacity_layout(const Plan& p, int maxB) {
   if (p.flags & GALE_WITH_FACETS) {  // |VF(v)| <= 3 |VT(v)|: every triangle at v lies in a simplex of its star
     L.vf_off = o; o = up(o + (size_t(maxB) * p.max_rows + 1) * 4);
     L.vf_idx = o; o = up(o + size_t(maxB) * p.max_vt * 3 * 4);
+  }
+  if (p.flags & GALE_WITH_COBOUNDARY) {
+    // bounds known before E / F exist: an edge / triangle internal to a cluster has its lowest vertex a there and
+    // lies in a simplex of VT(a); a simplex has 3 edges and 3 triangles with a given lowest vertex
+    const size_t rows[3] = {size_t(p.max_vv), size_t(p.max_vt) * 3, size_t(p.max_vv)};
+    const size_t nnz[3] = {size_t(p.max_vt) * 3, size_t(p.max_vt) * 3, size_t(p.max_vt) * 6};
+    for (int k = 0; k < 3; ++k) {
+      L.cob_off[k] = o; o = up(o + (size_t(maxB) * rows[k] + 1) * 4);
+      L.cob_idx[k] = o; o = up(o + size_t(maxB) * nnz[k] * 4);
+    }
   }
   L.total = o;
   return L;
@@ -522,8 +534,9 @@ int check_desc(const gale_mesh_desc_t* d) {
   if (!d || (d->dim != 2 && d->dim != 3) || d->num_vertices < 0 || d->num_simplices < 0 || d->num_clusters < 0 ||
       !d->h_cluster_offsets || (d->num_simplices > 0 && !d->d_simplices) || d->max_batch_clusters < 1 ||
       d->queue_depth < 0 || d->device_ring < 0 || d->tile_vertices < 0 || d->num_simplices >= (1LL << 31) - 1 ||
-      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T | GALE_WITH_EDGES | GALE_WITH_FACETS)) ||
+      (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T | GALE_WITH_EDGES | GALE_WITH_FACETS | GALE_WITH_COBOUNDARY)) ||
       ((d->flags & GALE_WITH_FACETS) && d->dim != 3) ||
+      ((d->flags & GALE_WITH_COBOUNDARY) && (d->flags & (GALE_WITH_EDGES | GALE_WITH_FACETS)) != (GALE_WITH_EDGES | GALE_WITH_FACETS)) ||
       (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK))
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
@@ -581,6 +594,8 @@ struct Slot {
   uint32_t mask = 0;
   std::vector<int32_t> ids, row_begin, tt_row_begin;
   long long rows = 0, vt_nnz = 0, vv_nnz = 0, tt_rows = 0, vf_nnz = 0;
+  std::vector<int32_t> e_row_begin, f_row_begin;
+  long long cob_nnz[3] = {0, 0, 0};
   uint32_t eff_mask = 0;  // what the batch kernel computed (VE implies VV, VF implies VT)
   SlotLayout used;  // section offsets of this batch
   float prep_ms = 0.f;
@@ -619,6 +634,12 @@ struct gale_mesh {
   long long nE = 0, nF = 0;
   int vf_cap = 0;                       // candidate slots per vertex in k_vf (power of two)
   std::vector<long long> cl_vf;         // VF entries per cluster
+  // EF / ET / FT (GALE_WITH_COBOUNDARY), indexed by gale::sub::COB_*
+  DevMem d_tile_cob_rel[3];
+  std::vector<long long> cl_cob[3];     // entries per cluster
+  std::vector<int32_t> cl_e0, cl_f0;    // [nC+1] I_E / I_F at the cluster boundaries
+  int rows_cap_e = 0, rows_cap_f = 0, star_cap = 32;
+  bool cob_ready = false;
   gale::sub::SubIndex sub{};  // sample-batch time of the dense / walk kernel at create (0 = not timed)
 };
 
@@ -758,6 +779,7 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
     GALE_CUDA(cudaMemcpyAsync(&maxdeg, d_max.p, 4, cudaMemcpyDeviceToHost, st));
     GALE_CUDA(cudaStreamSynchronize(st));
     m->vf_cap = gi::pow2_ceil(std::max(3 * maxdeg, 32));
+    m->star_cap = gi::pow2_ceil(std::max(maxdeg, 32));
     const int vwarps = 8, vsm = (2 * ((p.tv + 4) & ~3) + vwarps * m->vf_cap) * 4;   // count mode keeps no results
     if ((2 * ((p.tv + 4) & ~3) + (vwarps + p.tv) * m->vf_cap) * 4 > kSmemLimit - 2048) { g_last_error = "a vertex star is too large for the VF kernel"; return GALE_ERR_UNSUPPORTED; }
     GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
@@ -793,6 +815,95 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
     }
     if ((rc = upload_vec(m->d_tile_vf_rel, rel, st))) return rc;
     GALE_CUDA(cudaStreamSynchronize(st));
+  }
+  if (p.flags & GALE_WITH_COBOUNDARY) {
+    // EF / ET / FT: rows per cluster and per tile from I_E / I_F at their boundaries, then exact entries per
+    // tile from a counting sweep over the VT rows (one launch per relation and batch)
+    std::vector<int32_t> tile_v(size_t(p.nTiles) + 1, p.nV), tile_e, tile_f;
+    for (int i = 0; i < p.nTiles; ++i) tile_v[size_t(i)] = p.tiles[size_t(i)].v_lo;
+    {
+      DevMem d_idx, d_out;
+      auto gather = [&](const std::vector<int32_t>& idx, const int32_t* src, std::vector<int32_t>& out) -> int {
+        int r2;
+        if ((r2 = upload_vec(d_idx, idx, st)) || (r2 = d_out.alloc(idx.size() * 4))) return r2;
+        gi::k_gather<<<blocks_for((long long)idx.size(), TB), TB, 0, st>>>(src, d_idx.as<int32_t>(), int(idx.size()), d_out.as<int32_t>());
+        return download_vec(out, d_out.p, idx.size(), st);
+      };
+      if ((rc = gather(p.cl_off, m->sub.e_first, m->cl_e0)) || (rc = gather(p.cl_off, m->sub.f_first, m->cl_f0)) ||
+          (rc = gather(tile_v, m->sub.e_first, tile_e)) || (rc = gather(tile_v, m->sub.f_first, tile_f)))
+        return rc;
+    }
+    // tiles are numbered cluster by cluster with ascending v_lo, but empty clusters own no tile: rows of tile i end
+    // where its vertices end
+    m->rows_cap_e = m->rows_cap_f = 4;
+    {
+      std::vector<int32_t> vend(size_t(p.nTiles));
+      for (int i = 0; i < p.nTiles; ++i) vend[size_t(i)] = p.tiles[size_t(i)].v_lo + p.tiles[size_t(i)].nrows;
+      std::vector<int32_t> e_end, f_end;
+      DevMem d_idx, d_out;
+      auto gather2 = [&](const int32_t* src, std::vector<int32_t>& out) -> int {
+        int r2;
+        if ((r2 = upload_vec(d_idx, vend, st)) || (r2 = d_out.alloc(std::max<size_t>(vend.size(), 1) * 4))) return r2;
+        if (!vend.empty()) gi::k_gather<<<blocks_for((long long)vend.size(), TB), TB, 0, st>>>(src, d_idx.as<int32_t>(), int(vend.size()), d_out.as<int32_t>());
+        return download_vec(out, d_out.p, vend.size(), st);
+      };
+      if ((rc = gather2(m->sub.e_first, e_end)) || (rc = gather2(m->sub.f_first, f_end))) return rc;
+      for (int i = 0; i < p.nTiles; ++i) {
+        m->rows_cap_e = std::max(m->rows_cap_e, e_end[size_t(i)] - tile_e[size_t(i)]);
+        m->rows_cap_f = std::max(m->rows_cap_f, f_end[size_t(i)] - tile_f[size_t(i)]);
+      }
+    }
+    const int warps = 8;
+    auto cob_smem = [&](int rows_cap) { return (((rows_cap + 4) & ~3) + ((p.tv + 4) & ~3)) * 4 + warps * m->star_cap * 16 + warps * 64 * 4; };
+    if (cob_smem(std::max(m->rows_cap_e, m->rows_cap_f)) > kSmemLimit - 2048) { g_last_error = "a tile has too many edges / triangles for the coboundary kernels"; return GALE_ERR_UNSUPPORTED; }
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_ET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_FT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_EF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_ET, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_FT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_EF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
+    DevMem d_stats[3];
+    for (int k = 0; k < 3; ++k)
+      if ((rc = d_stats[k].alloc(size_t(std::max(p.nTiles, 1)) * 4))) return rc;
+    rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int n) -> int {
+      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
+      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_idx);
+      for (int b = 0; b < n; b += gale::kMaxBatch) {
+        const int nb = std::min(gale::kMaxBatch, n - b);
+        gs::CobParams V{};
+        V.n_clusters = nb;
+        for (int i = 0; i < nb; ++i) {
+          const int c = s.ids[size_t(b + i)];
+          V.tile_prefix[i + 1] = V.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
+          V.cluster[i] = c;
+          V.vt_row_base[i] = s.row_begin[size_t(b + i)];
+        }
+        const int grid = V.tile_prefix[nb];
+        if (grid > 0) {
+          gs::k_cob<gs::COB_ET, true><<<grid, warps * 32, cob_smem(m->rows_cap_e), st>>>(m->dm, m->sub, V, m->rows_cap_e, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_ET].as<int32_t>());
+          gs::k_cob<gs::COB_FT, true><<<grid, warps * 32, cob_smem(m->rows_cap_f), st>>>(m->dm, m->sub, V, m->rows_cap_f, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_FT].as<int32_t>());
+          gs::k_cob<gs::COB_EF, true><<<grid, warps * 32, cob_smem(m->rows_cap_e), st>>>(m->dm, m->sub, V, m->rows_cap_e, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_EF].as<int32_t>());
+        }
+      }
+      GALE_CUDA(cudaGetLastError());
+      return int(GALE_OK);
+    });
+    if (rc != GALE_OK) return rc;
+    for (int k = 0; k < 3; ++k) {
+      std::vector<int32_t> stats, rel(size_t(std::max(p.nTiles, 1)), 0);
+      if ((rc = download_vec(stats, d_stats[k].p, size_t(p.nTiles), st))) return rc;
+      m->cl_cob[k].assign(size_t(p.nC), 0);
+      const long long cap_nnz = (k == gs::COB_EF ? 6LL : 3LL) * p.max_vt;  // the per-cluster bound of slot_capacity_layout
+      for (int c = 0; c < p.nC; ++c) {
+        long long acc = 0;
+        for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) { rel[size_t(i)] = int32_t(acc); acc += stats[size_t(i)]; }
+        if (acc > cap_nnz || acc >= (1LL << 31) - 1) { g_last_error = "coboundary relation exceeds its slot bound"; return GALE_ERR_UNSUPPORTED; }
+        m->cl_cob[k][size_t(c)] = acc;
+      }
+      if ((rc = upload_vec(m->d_tile_cob_rel[k], rel, st))) return rc;
+    }
+    GALE_CUDA(cudaStreamSynchronize(st));
+    m->cob_ready = true;
   }
   return GALE_OK;
 }
@@ -1035,14 +1146,17 @@ int32_t gale_mesh_triangles(const gale_mesh_t* m, const int32_t** d_first, const
 
 int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const int32_t* h_cluster_ids,
                                    int32_t n_clusters, void* cuda_stream) {
-  if (!m || (relation_mask & ~uint32_t(GALE_REL_ALL | GALE_REL_VE | GALE_REL_VF)) || relation_mask == 0 || n_clusters < 0 ||
+  constexpr uint32_t kCobMask = GALE_REL_EF | GALE_REL_ET | GALE_REL_FT;
+  if (!m || (relation_mask & ~uint32_t(GALE_REL_ALL | GALE_REL_VE | GALE_REL_VF | kCobMask)) || relation_mask == 0 || n_clusters < 0 ||
       (n_clusters > 0 && !h_cluster_ids))
     return GALE_ERR_INVALID_ARG;
   const uint32_t user_mask = relation_mask;
   if ((user_mask & GALE_REL_VE) && !m->sub.e_first) { g_last_error = "VE needs GALE_WITH_EDGES at create"; return GALE_ERR_UNSUPPORTED; }
   if ((user_mask & GALE_REL_VF) && !m->sub.f_first) { g_last_error = "VF needs GALE_WITH_FACETS at create"; return GALE_ERR_UNSUPPORTED; }
   // VE is a map over the VV rows, VF works on the VT rows: the batch kernel computes those too
-  relation_mask = (user_mask & GALE_REL_ALL) | ((user_mask & GALE_REL_VE) ? GALE_REL_VV : 0u) | ((user_mask & GALE_REL_VF) ? GALE_REL_VT : 0u);
+  if ((user_mask & kCobMask) && !m->cob_ready) { g_last_error = "EF / ET / FT need GALE_WITH_COBOUNDARY at create"; return GALE_ERR_UNSUPPORTED; }
+  relation_mask = (user_mask & GALE_REL_ALL) | ((user_mask & GALE_REL_VE) ? GALE_REL_VV : 0u) |
+                  ((user_mask & (GALE_REL_VF | kCobMask)) ? GALE_REL_VT : 0u);
   if (n_clusters > m->maxB) return GALE_ERR_BAD_CLUSTER;
   const Plan& p = *m->plan;
   for (int i = 0; i < n_clusters; ++i)
@@ -1089,6 +1203,25 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       if (s.vf_nnz >= (1LL << 31) - 1) return GALE_ERR_INVALID_ARG;
       s.used.vf_off = o; o = up(o + size_t(s.rows + 1) * 4, 16);
       s.used.vf_idx = o; o = up(o + size_t(s.vf_nnz) * 4, 16);
+    }
+    if (user_mask & kCobMask) {
+      s.e_row_begin.assign(size_t(n_clusters) + 1, 0);
+      s.f_row_begin.assign(size_t(n_clusters) + 1, 0);
+      for (int i = 0; i < n_clusters; ++i) {
+        const int c = s.ids[size_t(i)];
+        s.e_row_begin[size_t(i) + 1] = s.e_row_begin[size_t(i)] + (m->cl_e0[size_t(c) + 1] - m->cl_e0[size_t(c)]);
+        s.f_row_begin[size_t(i) + 1] = s.f_row_begin[size_t(i)] + (m->cl_f0[size_t(c) + 1] - m->cl_f0[size_t(c)]);
+      }
+      const uint32_t bit[3] = {GALE_REL_ET, GALE_REL_FT, GALE_REL_EF};
+      for (int k = 0; k < 3; ++k) {
+        s.cob_nnz[k] = 0;
+        if (!(user_mask & bit[k])) continue;
+        for (int i = 0; i < n_clusters; ++i) s.cob_nnz[k] += m->cl_cob[k][size_t(s.ids[size_t(i)])];
+        if (s.cob_nnz[k] >= (1LL << 31) - 1) return GALE_ERR_INVALID_ARG;
+        const long long rows = k == gale::sub::COB_FT ? s.f_row_begin[size_t(n_clusters)] : s.e_row_begin[size_t(n_clusters)];
+        s.used.cob_off[k] = o; o = up(o + size_t(rows + 1) * 4, 16);
+        s.used.cob_idx[k] = o; o = up(o + size_t(s.cob_nnz[k]) * 4, 16);
+      }
     }
     s.used.total = o;
     if (o > m->cap.total) return GALE_ERR_WORKSPACE;
@@ -1171,6 +1304,36 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
                                                            reinterpret_cast<int32_t*>(s.dev + s.used.vf_idx), nullptr);
       GALE_CUDA(cudaGetLastError());
     }
+    if (user_mask & kCobMask) {  // EF / ET / FT from the VT rows just written
+      namespace gs = gale::sub;
+      const uint32_t bit[3] = {GALE_REL_ET, GALE_REL_FT, GALE_REL_EF};
+      const int warps = 8;
+      for (int k = 0; k < 3; ++k) {
+        if (!(user_mask & bit[k])) continue;
+        const std::vector<int32_t>& rb = k == gs::COB_FT ? s.f_row_begin : s.e_row_begin;
+        gs::CobParams V{};
+        V.n_clusters = nb; V.total_rows = rb[size_t(n_clusters)]; V.total_nnz = int(s.cob_nnz[k]);
+        long long base = 0;
+        for (int i = 0; i < b; ++i) base += m->cl_cob[k][size_t(s.ids[size_t(i)])];
+        for (int i = 0; i < nb; ++i) {
+          V.tile_prefix[i + 1] = P.tile_prefix[i + 1];
+          V.cluster[i] = P.cluster[i];
+          V.vt_row_base[i] = P.row_base[i];
+          V.row_base[i] = rb[size_t(b + i)];
+          V.nnz_base[i] = int(base);
+          base += m->cl_cob[k][size_t(s.ids[size_t(b + i)])];
+        }
+        const int rows_cap = k == gs::COB_FT ? m->rows_cap_f : m->rows_cap_e;
+        const int csm = (((rows_cap + 4) & ~3) + ((p.tv + 4) & ~3)) * 4 + warps * m->star_cap * 16 + warps * 64 * 4;
+        int32_t* ooff = reinterpret_cast<int32_t*>(s.dev + s.used.cob_off[k]);
+        int32_t* oidx = reinterpret_cast<int32_t*>(s.dev + s.used.cob_idx[k]);
+        const int32_t* rel = m->d_tile_cob_rel[k].as<int32_t>();
+        if (k == gs::COB_ET) gs::k_cob<gs::COB_ET, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
+        else if (k == gs::COB_FT) gs::k_cob<gs::COB_FT, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
+        else gs::k_cob<gs::COB_EF, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
+        GALE_CUDA(cudaGetLastError());
+      }
+    }
   }
   GALE_CUDA(cudaEventRecord(s.ev_done, run));
   if (m->queue_depth > 0) {  // a7: D2H into the pinned slot on the side stream
@@ -1230,6 +1393,14 @@ int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_m
     out->tt_indices = reinterpret_cast<const int32_t*>(b + s.used.tt);
   }
   if (s.mask & GALE_REL_VE) out->ve_indices = reinterpret_cast<const int32_t*>(b + s.used.ve_idx);
+  if (s.mask & (GALE_REL_EF | GALE_REL_ET | GALE_REL_FT)) {
+    out->e_row_begin = s.e_row_begin.data();
+    out->f_row_begin = s.f_row_begin.data();
+    namespace gs = gale::sub;
+    if (s.mask & GALE_REL_ET) { out->et_nnz = s.cob_nnz[gs::COB_ET]; out->et_offsets = reinterpret_cast<const int32_t*>(b + s.used.cob_off[gs::COB_ET]); out->et_indices = reinterpret_cast<const int32_t*>(b + s.used.cob_idx[gs::COB_ET]); }
+    if (s.mask & GALE_REL_FT) { out->ft_nnz = s.cob_nnz[gs::COB_FT]; out->ft_offsets = reinterpret_cast<const int32_t*>(b + s.used.cob_off[gs::COB_FT]); out->ft_indices = reinterpret_cast<const int32_t*>(b + s.used.cob_idx[gs::COB_FT]); }
+    if (s.mask & GALE_REL_EF) { out->ef_nnz = s.cob_nnz[gs::COB_EF]; out->ef_offsets = reinterpret_cast<const int32_t*>(b + s.used.cob_off[gs::COB_EF]); out->ef_indices = reinterpret_cast<const int32_t*>(b + s.used.cob_idx[gs::COB_EF]); }
+  }
   if (s.mask & GALE_REL_VF) {
     out->vf_nnz = s.vf_nnz;
     out->vf_offsets = reinterpret_cast<const int32_t*>(b + s.used.vf_off);

@@ -286,12 +286,154 @@ __global__ void k_vf(const DeviceMesh M, const SubIndex X, const __grid_constant
     if (COUNT) stats[tile] = acc;
   }
   __syncthreads();
-  if (COUNT) return;
+  if constexpr (!COUNT) {
   for (int r = threadIdx.x; r < nrows; r += blockDim.x) vf_off[row0 + r] = deg[r];
   for (int r = w; r < nrows; r += nw) {  // write-out, one warp per row: the looked-up ids, then the own block
     const int nl = nlow[r], tot = deg[r + 1] - deg[r], own0 = X.f_first[v_lo + r];
     int32_t* out = vf_idx + deg[r];
     for (int i = lane; i < tot; i += 32) GALE_ST(out + i, i < nl ? keep[(size_t)r * cap + i] : own0 + (i - nl));
+  }
+  }
+}
+
+// ---- EF, ET, FT of a batch (PAPER.md:49, Table 1; the MS-complex set, :309) ----------------------------
+// Rows = the edges (E..) / triangles (F..) internal to the requested clusters, i.e. the blocks of E / F of
+// their vertices; the rows of a tile are contiguous ids. One block per tile, one warp per vertex a: the
+// simplices of VT(a) (just written by the batch kernel) are held in shared memory; row (a, b) of ET = those
+// that contain b, row (a, b, c) of FT = those that contain b and c — a ballot per 32 simplices, in VT's
+// ascending order; row (a, b) of EF = the triangles (a, b, x) of those simplices, looked up in F, sorted
+// and de-duplicated by the warp. COUNT (sizing at create): stats[tile] = entries of the tile.
+// Dynamic shared memory (ints): rows_cap + 4 (row counts -> offsets) | ((nrows + 4) & ~3) (vertex totals) |
+// warps * star_cap * 4 (the stars) | warps * 64 (EF candidates).
+enum { COB_ET = 0, COB_FT = 1, COB_EF = 2 };
+struct CobParams {
+  int n_clusters;
+  int total_rows, total_nnz;        // terminal offset
+  int tile_prefix[kMaxBatch + 1];
+  int cluster[kMaxBatch];
+  int vt_row_base[kMaxBatch];       // first VT row of slot i in the batch
+  int row_base[kMaxBatch];          // first edge / triangle row of slot i in the batch
+  int nnz_base[kMaxBatch];          // first entry of slot i in the batch
+};
+template <int KIND, bool COUNT>
+__global__ void k_cob(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P, int rows_cap, int star_cap,
+                      const int32_t* __restrict__ tile_rel, const int32_t* __restrict__ vt_off,
+                      const int32_t* __restrict__ vt_idx, int32_t* out_off, int32_t* out_idx, int32_t* stats) {
+  extern __shared__ int32_t shc[];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if (!COUNT && blockIdx.x == 0 && threadIdx.x == 0) { out_off[0] = 0; out_off[P.total_rows] = P.total_nnz; }
+  if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
+  int slot;
+  {
+    int lo = 0, hi = P.n_clusters;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
+    }
+    slot = lo;
+  }
+  const int tile = M.cluster_tile_begin[P.cluster[slot]] + ((int)blockIdx.x - P.tile_prefix[slot]);
+  const int nrows = M.tiles[tile].nrows, v_lo = M.tiles[tile].v_lo;
+  const int c_lo = v_lo - M.tiles[tile].row_rel;
+  const int32_t* first = KIND == COB_FT ? X.f_first : X.e_first;   // interval array of the ROW list
+  const int r_tile0 = first[v_lo], r_tile1 = first[v_lo + nrows];   // the tile's rows: contiguous ids
+  const int n_tile_rows = min(r_tile1 - r_tile0, rows_cap);
+  const int vrow0 = P.vt_row_base[slot] + M.tiles[tile].row_rel;
+  int32_t* rcnt = shc;                                   // [rows_cap + 1] counts, then offsets
+  int32_t* vtot = shc + ((rows_cap + 4) & ~3);           // [nrows + 1]
+  int4* star = reinterpret_cast<int4*>(vtot + ((nrows + 4) & ~3)) + (size_t)w * star_cap;
+  int32_t* cand = reinterpret_cast<int32_t*>(reinterpret_cast<int4*>(vtot + ((nrows + 4) & ~3)) + (size_t)nw * star_cap) + w * 64;
+  const int4* T4 = reinterpret_cast<const int4*>(M.T);
+  for (int pass = 0; pass < (COUNT ? 1 : 2); ++pass) {
+    for (int r = w; r < nrows; r += nw) {
+      const int a = v_lo + r;
+      const int t0 = vt_off[vrow0 + r];
+      const int deg = min(vt_off[vrow0 + r + 1] - t0, star_cap);
+      for (int i = lane; i < deg; i += 32) star[i] = __ldg(T4 + vt_idx[t0 + i]);
+      __syncwarp();
+      int tot = 0;
+      const int j0 = first[a], j1 = first[a + 1];
+      for (int j = j0; j < j1; ++j) {
+        const int jr = j - r_tile0;                       // row inside the tile
+        int b, c = -1;
+        if (KIND == COB_FT) { const int2 q = X.f_bc[j]; b = q.x; c = q.y; } else { b = X.e_hi[j]; }
+        const int wbase = (pass == 1 && jr < rows_cap) ? rcnt[jr] : 0;
+        int cnt = 0;
+        if (KIND != COB_EF) {
+          for (int i0 = 0; i0 < deg; i0 += 32) {
+            const int i = i0 + lane;
+            bool hit = false;
+            if (i < deg) {
+              const int4 q = star[i];
+              const bool hb = q.x == b || q.y == b || q.z == b || q.w == b;
+              hit = KIND == COB_FT ? (hb && (q.x == c || q.y == c || q.z == c || q.w == c)) : hb;
+            }
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
+            if (pass == 1 && hit) GALE_ST(out_idx + wbase + cnt + __popc(m & ((1u << lane) - 1u)), vt_idx[t0 + i]);
+            cnt += __popc(m);
+          }
+        } else {
+          int nc = 0;                                     // triangles (a, b, x) of the simplices that contain b
+          for (int i0 = 0; i0 < deg; i0 += 32) {
+            const int i = i0 + lane;
+            int id0 = INT_MAX, id1 = INT_MAX;
+            if (i < deg) {
+              const int4 q = star[i];
+              const int s[4] = {q.x, q.y, q.z, q.w};
+              if (s[0] == b || s[1] == b || s[2] == b || s[3] == b) {
+                int o[2] = {0, 0}, mm = 0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                  if (s[k] != a && s[k] != b && mm < 2) o[mm++] = s[k];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {               // sort (a, b, x): a < b
+                  const int x = o[u];
+                  const int p0 = x < a ? x : a, p2 = x > b ? x : b, p1 = a + b + x - p0 - p2;
+                  (u == 0 ? id0 : id1) = tri_id(X, p0, p1, p2);
+                }
+              }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+              const int id = u == 0 ? id0 : id1;
+              const unsigned m = __ballot_sync(0xFFFFFFFFu, id != INT_MAX);
+              if (id != INT_MAX && nc + __popc(m & ((1u << lane) - 1u)) < 64) cand[nc + __popc(m & ((1u << lane) - 1u))] = id;
+              nc = min(64, nc + __popc(m));
+            }
+          }
+          const int n2 = init::pow2_ceil(nc < 1 ? 1 : nc);
+          for (int i = nc + lane; i < n2; i += 32) cand[i] = INT_MAX;
+          __syncwarp();
+          warp_bitonic32(cand, n2, lane);
+          for (int i0 = 0; i0 < n2; i0 += 32) {
+            const int i = i0 + lane;
+            const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+            if (pass == 1 && head) GALE_ST(out_idx + wbase + cnt + __popc(m & ((1u << lane) - 1u)), cand[i]);
+            cnt += __popc(m);
+          }
+          __syncwarp();
+        }
+        if (pass == 0 && lane == 0 && jr < rows_cap) rcnt[jr] = cnt;
+        tot += cnt;
+      }
+      if (pass == 0 && lane == 0) vtot[r] = tot;
+      __syncwarp();
+    }
+    __syncthreads();
+    if (pass == 0) {
+      if (threadIdx.x == 0) {  // serial exclusive scan over the tile's rows (a few hundred)
+        int acc = COUNT ? 0 : P.nnz_base[slot] + tile_rel[tile];
+        for (int j = 0; j < n_tile_rows; ++j) { const int d = rcnt[j]; rcnt[j] = acc; acc += d; }
+        rcnt[n_tile_rows] = acc;
+        if (COUNT) stats[tile] = acc;
+      }
+      __syncthreads();
+      if (!COUNT) {
+        const int orow0 = P.row_base[slot] + (r_tile0 - first[c_lo]);
+        for (int j = threadIdx.x; j < n_tile_rows; j += blockDim.x) out_off[orow0 + j] = rcnt[j];
+      }
+    }
   }
 }
 

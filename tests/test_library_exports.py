@@ -39,7 +39,7 @@ def test_status_strings(lib):
 def test_struct_layout_matches_header():
     # sizes implied by include/gale.h on LP64
     assert ctypes.sizeof(gale.gale_mesh_desc_t) == 80
-    assert ctypes.sizeof(gale.gale_batch_view_t) == 184
+    assert ctypes.sizeof(gale.gale_batch_view_t) == 272
     assert ctypes.sizeof(gale.gale_mesh_info_t) == 112      # gcc sizeof(gale_mesh_info_t) of include/gale.h
 
 
