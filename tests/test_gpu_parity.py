@@ -222,7 +222,8 @@ def test_argument_errors_on_gpu():
     gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=4)
     for ids, mask, status in (([0, 8], 7, gale.ERR_BAD_CLUSTER), ([-1], 7, gale.ERR_BAD_CLUSTER),
                               ([0, 1, 2, 3, 4], 7, gale.ERR_BAD_CLUSTER), ([0], 0, gale.ERR_INVALID_ARG),
-                              ([0], 32, gale.ERR_INVALID_ARG), ([0], 8, gale.ERR_UNSUPPORTED)):     # 8 = VE: valid bit, no edge list
+                              ([0], 1 << 20, gale.ERR_INVALID_ARG),                          # not a relation bit
+                              ([0], gale.REL_VE, gale.ERR_UNSUPPORTED), ([0], gale.REL_EF, gale.ERR_UNSUPPORTED)):  # lists not built
         with pytest.raises(gale.GaleError) as e:
             gm.compute(ids, mask)
         assert e.value.status == status
