@@ -41,10 +41,11 @@ enum {
   GALE_REL_ALL = 7,  /* the three relations of the hot path                                           */
   GALE_REL_VE = 8,   /* vertex -> incident edges; needs GALE_WITH_EDGES at create; also delivers VV   */
   GALE_REL_VF = 16,  /* vertex -> incident triangles (tetrahedral meshes); needs GALE_WITH_FACETS; also
-                        delivers VT                                                                  */
+                        delivers VV (its source)                                                     */
   /* the coboundary relations of edges and triangles (Table 1; MS complex :309), tetrahedral
      meshes, need GALE_WITH_COBOUNDARY; rows = the edges / triangles internal to the requested clusters
-     (those whose lowest vertex belongs to the cluster), in id order; all deliver VT too  */
+     (those whose lowest vertex belongs to the cluster), in id order; EF also delivers VV,
+     ET and FT also deliver VT (the rows they are read off)                                            */
   GALE_REL_EF = 32,  /* edge -> triangles                                                             */
   GALE_REL_ET = 64,  /* edge -> simplices                                                             */
   GALE_REL_FT = 128  /* triangle -> simplices (one or two)                                            */
@@ -147,7 +148,7 @@ typedef struct {
    * edge between the row's vertex and vv_indices[i]. Edge / triangle ids = positions in the sorted lists E / F */
   const int32_t *ve_indices;     /* [vv_nnz] or NULL                                                   */
   int64_t vf_nnz;
-  const int32_t *vf_offsets;     /* [vt_rows+1] or NULL                                                */
+  const int32_t *vf_offsets;     /* [vt_row_begin[n_clusters]+1] (one row per vertex, like VT / VV) or NULL */
   const int32_t *vf_indices;     /* [vf_nnz]                                                           */
   /* EF / ET / FT: rows of the i-th requested cluster are [e_row_begin[i], e_row_begin[i+1]) (edges) resp.
    * f_row_begin (triangles); the first row of cluster c is edge I_E[o[c]] resp. triangle I_F[o[c]]     */

@@ -333,7 +333,7 @@ class GaleMesh:
         if view.relation_mask & REL_VE:
             out["ve_indices"] = self._array(view, view.ve_indices, view.vv_nnz)
         if view.relation_mask & REL_VF:
-            out["vf_offsets"] = self._array(view, view.vf_offsets, view.vt_rows + 1)
+            out["vf_offsets"] = self._array(view, view.vf_offsets, int(out["vt_row_begin"][-1]) + 1)
             out["vf_indices"] = self._array(view, view.vf_indices, view.vf_nnz)
         if view.relation_mask & (REL_EF | REL_ET | REL_FT):
             out["e_row_begin"] = np.ctypeslib.as_array(view.e_row_begin, shape=(n + 1,)).copy()

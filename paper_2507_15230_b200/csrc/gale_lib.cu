@@ -630,15 +630,15 @@ struct gale_mesh {
   double create_ms = 0;
   float tune_ms[2] = {0.f, 0.f};
   // edges / triangles (GALE_WITH_EDGES / GALE_WITH_FACETS): library-owned device memory
-  DevMem d_cl_off, d_e_first, d_e_hi, d_f_first, d_f_bc, d_tile_vf_rel;
+  DevMem d_cl_off, d_e_first, d_e_hi, d_f_first, d_f_bc;
   long long nE = 0, nF = 0;
-  int vf_cap = 0;                       // candidate slots per vertex in k_vf (power of two)
-  std::vector<long long> cl_vf;         // VF entries per cluster
-  // EF / ET / FT (GALE_WITH_COBOUNDARY), indexed by gale::sub::COB_*
-  DevMem d_tile_cob_rel[3];
-  std::vector<long long> cl_cob[3];     // entries per cluster
+  // VF (GALE_WITH_FACETS) and EF / ET / FT (GALE_WITH_COBOUNDARY), indexed by gale::sub::COB_* (VF = 3)
+  DevMem d_tile_cob_rel[4];             // first entry of a tile inside its cluster
+  std::vector<long long> cl_cob[4];     // entries per cluster
   std::vector<int32_t> cl_e0, cl_f0;    // [nC+1] I_E / I_F at the cluster boundaries
-  int rows_cap_e = 0, rows_cap_f = 0, star_cap = 32;
+  int rows_cap_e = 0, rows_cap_f = 0;   // most edges / triangles of a tile
+  int star_t = 1, star_f = 1;           // largest stars of k_star: |VT(v)|; triangles at a vertex
+  int fblock_max = 1, fstar_tile = 4;   // longest block of F; most triangles at the vertices of a tile
   bool cob_ready = false;
   gale::sub::SubIndex sub{};  // sample-batch time of the dense / walk kernel at create (0 = not timed)
 };
@@ -684,6 +684,121 @@ int sweep_batches(gale_mesh* m, uint32_t mask, cudaStream_t st, Fn&& per_batch) 
     if (rc2 != GALE_OK) return rc2;
   }
   m->submitted.store(0); m->popped.store(0);  // these batches were the library's own
+  return GALE_OK;
+}
+
+// ---- VF / EF / ET / FT launches (gale_sub.cuh: k_star) ---------------------------------------------------------
+constexpr int kStarWarps = 8;
+struct StarCfg { gale::sub::StarDims d; gale::sub::StarLayout lay; int smem; };
+StarCfg star_cfg(const gale_mesh* m, int kind) {
+  namespace gs = gale::sub;
+  const Plan& p = *m->plan;
+  const bool from_vt = kind == gs::COB_ET || kind == gs::COB_FT;
+  StarCfg c;
+  c.d.tv = p.tv;
+  c.d.rows_cap = kind == gs::COB_VF ? 0 : (kind == gs::COB_FT ? m->rows_cap_f : m->rows_cap_e);
+  c.d.src_cap = std::max(4, from_vt ? p.cfg.vt_max : p.cfg.vv_max);  // the tile capacities of the batch kernel
+  c.d.W = kind == gs::COB_VF ? 0 : ((from_vt ? m->star_t : m->star_f) + 31) / 32;
+  c.d.Wf = from_vt ? 0 : (m->fblock_max + 31) / 32;
+  c.d.fstar_cap = kind == gs::COB_EF ? m->fstar_tile : 0;
+  c.lay = gs::make_star_layout(kind, c.d);
+  c.smem = c.lay.total * 4;
+  return c;
+}
+// src = the batch's VT rows (ET, FT) or VV rows (EF, VF)
+template <bool COUNT>
+void launch_star(const gale_mesh* m, int kind, int grid, const gale::sub::CobParams& V, const int32_t* src_off,
+                 const int32_t* src_idx, int32_t* out_off, int32_t* out_idx, int32_t* stats, int32_t* stats_max, cudaStream_t st) {
+  namespace gs = gale::sub;
+  const StarCfg c = star_cfg(m, kind);
+  const int32_t* rel = COUNT ? nullptr : m->d_tile_cob_rel[kind].as<int32_t>();
+#define GALE_STAR(K) gs::k_star<K, COUNT><<<grid, kStarWarps * 32, c.smem, st>>>(m->dm, m->sub, V, c.d, c.lay, rel, src_off, src_idx, out_off, out_idx, stats, stats_max)
+  switch (kind) {
+    case gs::COB_ET: GALE_STAR(gs::COB_ET); break;
+    case gs::COB_FT: GALE_STAR(gs::COB_FT); break;
+    case gs::COB_EF: GALE_STAR(gs::COB_EF); break;
+    default: GALE_STAR(gs::COB_VF); break;
+  }
+#undef GALE_STAR
+}
+int star_allow_smem() {
+  namespace gs = gale::sub;
+  static bool done = false;
+  if (done) return GALE_OK;
+#define GALE_ATTR(K) GALE_CUDA(cudaFuncSetAttribute(gs::k_star<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048)); \
+                     GALE_CUDA(cudaFuncSetAttribute(gs::k_star<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048))
+  GALE_ATTR(gs::COB_ET); GALE_ATTR(gs::COB_FT); GALE_ATTR(gs::COB_EF); GALE_ATTR(gs::COB_VF);
+#undef GALE_ATTR
+  done = true;
+  return GALE_OK;
+}
+
+// Exact sizes of the relations in `kinds` (bits 1 << COB_*): one counting sweep over the batches with the source
+// relations `src_mask`; fills cl_cob, d_tile_cob_rel and (VF) the star sizes of EF.
+int size_star_relations(gale_mesh* m, cudaStream_t st, uint32_t kinds, uint32_t src_mask) {
+  namespace gs = gale::sub;
+  const Plan& p = *m->plan;
+  int rc;
+  if ((rc = star_allow_smem())) return rc;
+  DevMem d_stats[4], d_max;
+  if ((rc = d_max.alloc(16))) return rc;
+  GALE_CUDA(cudaMemsetAsync(d_max.p, 0, 16, st));
+  for (int k = 0; k < 4; ++k) {
+    if (!(kinds >> k & 1u)) continue;
+    if ((rc = d_stats[k].alloc(size_t(std::max(p.nTiles, 1)) * 4))) return rc;
+    if (star_cfg(m, k).smem > kSmemLimit - 2048) { g_last_error = "a vertex star or a tile is too large for the VF / EF / ET / FT kernels"; return GALE_ERR_UNSUPPORTED; }
+  }
+  rc = sweep_batches(m, src_mask, st, [&](const Slot& s, int, int n) -> int {
+    const int32_t* vt_off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
+    const int32_t* vt_idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_idx);
+    const int32_t* vv_off = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_off);
+    const int32_t* vv_idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vv_idx);
+    for (int b = 0; b < n; b += gale::kMaxBatch) {
+      const int nb = std::min(gale::kMaxBatch, n - b);
+      gs::CobParams V{};
+      V.n_clusters = nb;
+      for (int i = 0; i < nb; ++i) {
+        const int c = s.ids[size_t(b + i)];
+        V.tile_prefix[i + 1] = V.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
+        V.cluster[i] = c;
+        V.src_row_base[i] = s.row_begin[size_t(b + i)];
+      }
+      const int grid = V.tile_prefix[nb];
+      if (grid <= 0) continue;
+      for (int k = 0; k < 4; ++k) {
+        if (!(kinds >> k & 1u)) continue;
+        const bool from_vt = k == gs::COB_ET || k == gs::COB_FT;
+        launch_star<true>(m, k, grid, V, from_vt ? vt_off : vv_off, from_vt ? vt_idx : vv_idx, nullptr, nullptr,
+                          d_stats[k].as<int32_t>(), d_max.as<int32_t>() + k, st);
+      }
+    }
+    GALE_CUDA(cudaGetLastError());
+    return int(GALE_OK);
+  });
+  if (rc != GALE_OK) return rc;
+  int32_t vmax[4] = {0, 0, 0, 0};
+  GALE_CUDA(cudaMemcpyAsync(vmax, d_max.p, 16, cudaMemcpyDeviceToHost, st));
+  GALE_CUDA(cudaStreamSynchronize(st));
+  for (int k = 0; k < 4; ++k) {
+    if (!(kinds >> k & 1u)) continue;
+    std::vector<int32_t> stats, rel(size_t(std::max(p.nTiles, 1)), 0);
+    if ((rc = download_vec(stats, d_stats[k].p, size_t(p.nTiles), st))) return rc;
+    m->cl_cob[k].assign(size_t(p.nC), 0);
+    const long long per_vt = k == gs::COB_EF ? 6LL : 3LL;  // the per-cluster bounds of slot_capacity_layout
+    for (int c = 0; c < p.nC; ++c) {
+      long long acc = 0;
+      for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) { rel[size_t(i)] = int32_t(acc); acc += stats[size_t(i)]; }
+      if (acc > per_vt * (k == gs::COB_VF ? p.cl_vt[size_t(c)] : p.max_vt) || acc >= (1LL << 31) - 1) { g_last_error = "a relation exceeds its slot bound"; return GALE_ERR_UNSUPPORTED; }
+      m->cl_cob[k][size_t(c)] = acc;
+    }
+    if (k == gs::COB_VF) {  // the star of EF: the triangles at a vertex / at the vertices of a tile
+      m->star_f = std::max(1, int(vmax[k]));
+      m->fstar_tile = 4;
+      for (int i = 0; i < p.nTiles; ++i) m->fstar_tile = std::max(m->fstar_tile, int(stats[size_t(i)]));
+    }
+    if ((rc = upload_vec(m->d_tile_cob_rel[k], rel, st))) return rc;
+  }
+  GALE_CUDA(cudaStreamSynchronize(st));
   return GALE_OK;
 }
 
@@ -764,9 +879,9 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
     GALE_CUDA(cudaGetLastError());
     m->sub.f_first = first;
     m->sub.f_bc = m->d_f_bc.as<int2>();
-    // sizing of VF: the largest |VT(v)|, then the exact entries per tile
-    DevMem d_max, d_stats;
-    if ((rc = d_max.alloc(4)) || (rc = d_stats.alloc(size_t(std::max(p.nTiles, 1)) * 4))) return rc;
+    // sizing of VF: the largest |VT(v)| (star capacities), then the exact entries per tile
+    DevMem d_max;
+    if ((rc = d_max.alloc(4))) return rc;
     GALE_CUDA(cudaMemsetAsync(d_max.p, 0, 4, st));
     rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int) -> int {
       const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
@@ -778,47 +893,20 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
     int maxdeg = 0;
     GALE_CUDA(cudaMemcpyAsync(&maxdeg, d_max.p, 4, cudaMemcpyDeviceToHost, st));
     GALE_CUDA(cudaStreamSynchronize(st));
-    m->vf_cap = gi::pow2_ceil(std::max(3 * maxdeg, 32));
-    m->star_cap = gi::pow2_ceil(std::max(maxdeg, 32));
-    const int vwarps = 8, vsm = (2 * ((p.tv + 4) & ~3) + vwarps * m->vf_cap) * 4;   // count mode keeps no results
-    if ((2 * ((p.tv + 4) & ~3) + (vwarps + p.tv) * m->vf_cap) * 4 > kSmemLimit - 2048) { g_last_error = "a vertex star is too large for the VF kernel"; return GALE_ERR_UNSUPPORTED; }
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_vf<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int n) -> int {
-      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
-      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_idx);
-      for (int b = 0; b < n; b += gale::kMaxBatch) {
-        const int nb = std::min(gale::kMaxBatch, n - b);
-        gs::VFParams V{};
-        V.n_clusters = nb;
-        for (int i = 0; i < nb; ++i) {
-          const int c = s.ids[size_t(b + i)];
-          V.tile_prefix[i + 1] = V.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
-          V.cluster[i] = c;
-          V.row_base[i] = s.row_begin[size_t(b + i)];
-        }
-        if (V.tile_prefix[nb] > 0)
-          gs::k_vf<true><<<V.tile_prefix[nb], vwarps * 32, vsm, st>>>(m->dm, m->sub, V, m->vf_cap, nullptr, off, idx, nullptr, nullptr, d_stats.as<int32_t>());
-      }
-      GALE_CUDA(cudaGetLastError());
-      return int(GALE_OK);
-    });
-    if (rc != GALE_OK) return rc;
-    std::vector<int32_t> stats, rel(size_t(std::max(p.nTiles, 1)), 0);
-    if ((rc = download_vec(stats, d_stats.p, size_t(p.nTiles), st))) return rc;
-    m->cl_vf.assign(size_t(p.nC), 0);
-    for (int c = 0; c < p.nC; ++c) {
-      long long acc = 0;
-      for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) { rel[size_t(i)] = int32_t(acc); acc += stats[size_t(i)]; }
-      if (acc > 3 * p.cl_vt[size_t(c)] || acc >= (1LL << 31) - 1) return GALE_ERR_UNSUPPORTED;
-      m->cl_vf[size_t(c)] = acc;
+    m->star_t = std::max(maxdeg, 1);
+    {  // longest block of F
+      GALE_CUDA(cudaMemsetAsync(d_max.p, 0, 4, st));
+      if (p.nV) gs::k_max_row<<<blocks_for(p.nV, TB), TB, 0, st>>>(first, p.nV, d_max.as<int>());
+      int mx = 0;
+      GALE_CUDA(cudaMemcpyAsync(&mx, d_max.p, 4, cudaMemcpyDeviceToHost, st));
+      GALE_CUDA(cudaStreamSynchronize(st));
+      m->fblock_max = std::max(mx, 1);
     }
-    if ((rc = upload_vec(m->d_tile_vf_rel, rel, st))) return rc;
-    GALE_CUDA(cudaStreamSynchronize(st));
+    if ((rc = size_star_relations(m, st, 1u << gs::COB_VF, GALE_REL_VV))) return rc;
   }
   if (p.flags & GALE_WITH_COBOUNDARY) {
     // EF / ET / FT: rows per cluster and per tile from I_E / I_F at their boundaries, then exact entries per
-    // tile from a counting sweep over the VT rows (one launch per relation and batch)
+    // tile from a counting sweep over the VT / VV rows
     std::vector<int32_t> tile_v(size_t(p.nTiles) + 1, p.nV), tile_e, tile_f;
     for (int i = 0; i < p.nTiles; ++i) tile_v[size_t(i)] = p.tiles[size_t(i)].v_lo;
     {
@@ -853,56 +941,7 @@ int build_sub_index(gale_mesh* m, cudaStream_t st) {
         m->rows_cap_f = std::max(m->rows_cap_f, f_end[size_t(i)] - tile_f[size_t(i)]);
       }
     }
-    const int warps = 8;
-    auto cob_smem = [&](int rows_cap) { return (((rows_cap + 4) & ~3) + ((p.tv + 4) & ~3)) * 4 + warps * m->star_cap * 16 + warps * 64 * 4; };
-    if (cob_smem(std::max(m->rows_cap_e, m->rows_cap_f)) > kSmemLimit - 2048) { g_last_error = "a tile has too many edges / triangles for the coboundary kernels"; return GALE_ERR_UNSUPPORTED; }
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_ET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_FT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_EF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_ET, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_FT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    GALE_CUDA(cudaFuncSetAttribute(gs::k_cob<gs::COB_EF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048));
-    DevMem d_stats[3];
-    for (int k = 0; k < 3; ++k)
-      if ((rc = d_stats[k].alloc(size_t(std::max(p.nTiles, 1)) * 4))) return rc;
-    rc = sweep_batches(m, GALE_REL_VT, st, [&](const Slot& s, int, int n) -> int {
-      const int32_t* off = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_off);
-      const int32_t* idx = reinterpret_cast<const int32_t*>(s.dev + s.used.vt_idx);
-      for (int b = 0; b < n; b += gale::kMaxBatch) {
-        const int nb = std::min(gale::kMaxBatch, n - b);
-        gs::CobParams V{};
-        V.n_clusters = nb;
-        for (int i = 0; i < nb; ++i) {
-          const int c = s.ids[size_t(b + i)];
-          V.tile_prefix[i + 1] = V.tile_prefix[i] + (p.cl_tile_begin[c + 1] - p.cl_tile_begin[c]);
-          V.cluster[i] = c;
-          V.vt_row_base[i] = s.row_begin[size_t(b + i)];
-        }
-        const int grid = V.tile_prefix[nb];
-        if (grid > 0) {
-          gs::k_cob<gs::COB_ET, true><<<grid, warps * 32, cob_smem(m->rows_cap_e), st>>>(m->dm, m->sub, V, m->rows_cap_e, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_ET].as<int32_t>());
-          gs::k_cob<gs::COB_FT, true><<<grid, warps * 32, cob_smem(m->rows_cap_f), st>>>(m->dm, m->sub, V, m->rows_cap_f, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_FT].as<int32_t>());
-          gs::k_cob<gs::COB_EF, true><<<grid, warps * 32, cob_smem(m->rows_cap_e), st>>>(m->dm, m->sub, V, m->rows_cap_e, m->star_cap, nullptr, off, idx, nullptr, nullptr, d_stats[gs::COB_EF].as<int32_t>());
-        }
-      }
-      GALE_CUDA(cudaGetLastError());
-      return int(GALE_OK);
-    });
-    if (rc != GALE_OK) return rc;
-    for (int k = 0; k < 3; ++k) {
-      std::vector<int32_t> stats, rel(size_t(std::max(p.nTiles, 1)), 0);
-      if ((rc = download_vec(stats, d_stats[k].p, size_t(p.nTiles), st))) return rc;
-      m->cl_cob[k].assign(size_t(p.nC), 0);
-      const long long cap_nnz = (k == gs::COB_EF ? 6LL : 3LL) * p.max_vt;  // the per-cluster bound of slot_capacity_layout
-      for (int c = 0; c < p.nC; ++c) {
-        long long acc = 0;
-        for (int i = p.cl_tile_begin[c]; i < p.cl_tile_begin[c + 1]; ++i) { rel[size_t(i)] = int32_t(acc); acc += stats[size_t(i)]; }
-        if (acc > cap_nnz || acc >= (1LL << 31) - 1) { g_last_error = "coboundary relation exceeds its slot bound"; return GALE_ERR_UNSUPPORTED; }
-        m->cl_cob[k][size_t(c)] = acc;
-      }
-      if ((rc = upload_vec(m->d_tile_cob_rel[k], rel, st))) return rc;
-    }
-    GALE_CUDA(cudaStreamSynchronize(st));
+    if ((rc = size_star_relations(m, st, (1u << gs::COB_ET) | (1u << gs::COB_FT) | (1u << gs::COB_EF), GALE_REL_VT | GALE_REL_VV))) return rc;
     m->cob_ready = true;
   }
   return GALE_OK;
@@ -1155,8 +1194,9 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
   if ((user_mask & GALE_REL_VF) && !m->sub.f_first) { g_last_error = "VF needs GALE_WITH_FACETS at create"; return GALE_ERR_UNSUPPORTED; }
   // VE is a map over the VV rows, VF works on the VT rows: the batch kernel computes those too
   if ((user_mask & kCobMask) && !m->cob_ready) { g_last_error = "EF / ET / FT need GALE_WITH_COBOUNDARY at create"; return GALE_ERR_UNSUPPORTED; }
-  relation_mask = (user_mask & GALE_REL_ALL) | ((user_mask & GALE_REL_VE) ? GALE_REL_VV : 0u) |
-                  ((user_mask & (GALE_REL_VF | kCobMask)) ? GALE_REL_VT : 0u);
+  // sources: VE, VF and EF are read off the VV rows, ET and FT off the VT rows (gale_sub.cuh)
+  relation_mask = (user_mask & GALE_REL_ALL) | ((user_mask & (GALE_REL_VE | GALE_REL_VF | GALE_REL_EF)) ? GALE_REL_VV : 0u) |
+                  ((user_mask & (GALE_REL_ET | GALE_REL_FT)) ? GALE_REL_VT : 0u);
   if (n_clusters > m->maxB) return GALE_ERR_BAD_CLUSTER;
   const Plan& p = *m->plan;
   for (int i = 0; i < n_clusters; ++i)
@@ -1199,7 +1239,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
     s.used.ve_idx = o; if (user_mask & GALE_REL_VE) o = up(o + size_t(s.vv_nnz) * 4, 16);
     s.vf_nnz = 0;
     if (user_mask & GALE_REL_VF) {
-      for (int i = 0; i < n_clusters; ++i) s.vf_nnz += m->cl_vf[size_t(s.ids[i])];
+      for (int i = 0; i < n_clusters; ++i) s.vf_nnz += m->cl_cob[gale::sub::COB_VF][size_t(s.ids[i])];
       if (s.vf_nnz >= (1LL << 31) - 1) return GALE_ERR_INVALID_ARG;
       s.used.vf_off = o; o = up(o + size_t(s.rows + 1) * 4, 16);
       s.used.vf_idx = o; o = up(o + size_t(s.vf_nnz) * 4, 16);
@@ -1287,50 +1327,30 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
                                                                reinterpret_cast<int32_t*>(s.dev + s.used.ve_idx));
       GALE_CUDA(cudaGetLastError());
     }
-    if (user_mask & GALE_REL_VF) {  // VF from the VT rows just written
-      gale::sub::VFParams V{};
-      V.n_clusters = nb; V.total_rows = int(s.rows); V.total_vf = int(s.vf_nnz);
-      for (int i = 0; i < nb; ++i) {
-        V.tile_prefix[i + 1] = P.tile_prefix[i + 1];
-        V.cluster[i] = P.cluster[i];
-        V.row_base[i] = P.row_base[i];
-      }
-      long long base = 0;
-      for (int i = 0; i < b; ++i) base += m->cl_vf[size_t(s.ids[i])];
-      for (int i = 0; i < nb; ++i) { V.vf_base[i] = int(base); base += m->cl_vf[size_t(s.ids[b + i])]; }
-      const int warps = 8, vsm = (2 * ((p.tv + 4) & ~3) + (warps + p.tv) * m->vf_cap) * 4;
-      gale::sub::k_vf<false><<<grid, warps * 32, vsm, run>>>(m->dm, m->sub, V, m->vf_cap, m->d_tile_vf_rel.as<int32_t>(), O.vt_offsets,
-                                                           O.vt_indices, reinterpret_cast<int32_t*>(s.dev + s.used.vf_off),
-                                                           reinterpret_cast<int32_t*>(s.dev + s.used.vf_idx), nullptr);
-      GALE_CUDA(cudaGetLastError());
-    }
-    if (user_mask & kCobMask) {  // EF / ET / FT from the VT rows just written
+    if (user_mask & (GALE_REL_VF | kCobMask)) {  // VF / EF / ET / FT from the VT / VV rows just written
       namespace gs = gale::sub;
-      const uint32_t bit[3] = {GALE_REL_ET, GALE_REL_FT, GALE_REL_EF};
-      const int warps = 8;
-      for (int k = 0; k < 3; ++k) {
+      const uint32_t bit[4] = {GALE_REL_ET, GALE_REL_FT, GALE_REL_EF, GALE_REL_VF};
+      for (int k = 0; k < 4; ++k) {
         if (!(user_mask & bit[k])) continue;
-        const std::vector<int32_t>& rb = k == gs::COB_FT ? s.f_row_begin : s.e_row_begin;
         gs::CobParams V{};
-        V.n_clusters = nb; V.total_rows = rb[size_t(n_clusters)]; V.total_nnz = int(s.cob_nnz[k]);
+        V.n_clusters = nb;
+        if (k == gs::COB_VF) { V.total_rows = int(s.rows); V.total_nnz = int(s.vf_nnz); }
+        else { V.total_rows = (k == gs::COB_FT ? s.f_row_begin : s.e_row_begin)[size_t(n_clusters)]; V.total_nnz = int(s.cob_nnz[k]); }
         long long base = 0;
         for (int i = 0; i < b; ++i) base += m->cl_cob[k][size_t(s.ids[size_t(i)])];
         for (int i = 0; i < nb; ++i) {
           V.tile_prefix[i + 1] = P.tile_prefix[i + 1];
           V.cluster[i] = P.cluster[i];
-          V.vt_row_base[i] = P.row_base[i];
-          V.row_base[i] = rb[size_t(b + i)];
+          V.src_row_base[i] = P.row_base[i];
+          V.row_base[i] = k == gs::COB_VF ? P.row_base[i] : (k == gs::COB_FT ? s.f_row_begin : s.e_row_begin)[size_t(b + i)];
           V.nnz_base[i] = int(base);
           base += m->cl_cob[k][size_t(s.ids[size_t(b + i)])];
         }
-        const int rows_cap = k == gs::COB_FT ? m->rows_cap_f : m->rows_cap_e;
-        const int csm = (((rows_cap + 4) & ~3) + ((p.tv + 4) & ~3)) * 4 + warps * m->star_cap * 16 + warps * 64 * 4;
-        int32_t* ooff = reinterpret_cast<int32_t*>(s.dev + s.used.cob_off[k]);
-        int32_t* oidx = reinterpret_cast<int32_t*>(s.dev + s.used.cob_idx[k]);
-        const int32_t* rel = m->d_tile_cob_rel[k].as<int32_t>();
-        if (k == gs::COB_ET) gs::k_cob<gs::COB_ET, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
-        else if (k == gs::COB_FT) gs::k_cob<gs::COB_FT, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
-        else gs::k_cob<gs::COB_EF, false><<<grid, warps * 32, csm, run>>>(m->dm, m->sub, V, rows_cap, m->star_cap, rel, O.vt_offsets, O.vt_indices, ooff, oidx, nullptr);
+        int32_t* ooff = reinterpret_cast<int32_t*>(s.dev + (k == gs::COB_VF ? s.used.vf_off : s.used.cob_off[k]));
+        int32_t* oidx = reinterpret_cast<int32_t*>(s.dev + (k == gs::COB_VF ? s.used.vf_idx : s.used.cob_idx[k]));
+        const bool from_vt = k == gs::COB_ET || k == gs::COB_FT;
+        launch_star<false>(m, k, grid, V, from_vt ? O.vt_offsets : O.vv_offsets, from_vt ? O.vt_indices : O.vv_indices, ooff, oidx,
+                           nullptr, nullptr, run);
         GALE_CUDA(cudaGetLastError());
       }
     }

@@ -156,7 +156,7 @@ __global__ void k_ve(const __grid_constant__ BatchRows B, const SubIndex X, cons
   }
 }
 
-// largest row length of a CSR (sizes the candidate buffers of k_vf)
+// largest row length of a CSR (sizes the star buffers of k_star)
 __global__ void k_max_row(const int32_t* __restrict__ off, int n_rows, int* out) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   int d = r < n_rows ? off[r + 1] - off[r] : 0;
@@ -165,163 +165,106 @@ __global__ void k_max_row(const int32_t* __restrict__ off, int n_rows, int* out)
   if ((threadIdx.x & 31) == 0 && d > 0) atomicMax(out, d);
 }
 
-// ---- VF of a batch -------------------------------------------------------------------------------------
-// One block per tile (its rows), one warp per vertex in turn, over the VT rows the batch kernel has just
-// written. Candidates: for every simplex of VT(v) the three triangles that contain v; id of a triangle
-// (a, b, c) = position of (b, c) in a's block of F. COUNT (sizing at create): stats[tile] = entries of the
-// tile, nothing else is written. Dynamic shared memory (ints): 2 * ((rows + 4) & ~3) for the degrees +
-// warps * cap for the candidates + rows * cap for the rows' results (not in count mode), cap = power of
-// two >= 3 * the largest |VT(v)|.
-struct VFParams {
-  int n_clusters;
-  int total_rows, total_vf;         // terminal offset
-  int tile_prefix[kMaxBatch + 1];
-  int cluster[kMaxBatch];
-  int row_base[kMaxBatch];          // first VT row of slot i in the batch
-  int vf_base[kMaxBatch];           // first VF entry of slot i in the batch
-};
-__device__ __forceinline__ int tri_id(const SubIndex& X, int a, int b, int c) {
-  int lo = X.f_first[a], hi = X.f_first[a + 1];
-  while (lo < hi) {
-    const int mid = (lo + hi) >> 1;
-    const int2 q = X.f_bc[mid];
-    if (q.x < b || (q.x == b && q.y < c)) lo = mid + 1; else hi = mid;
-  }
-  return lo;
-}
-__device__ __forceinline__ void warp_bitonic32(int32_t* a, int n2, int lane) {
-  for (int k = 2; k <= n2; k <<= 1)
-    for (int j = k >> 1; j > 0; j >>= 1) {
-      for (int i = lane; i < n2; i += 32) {
-        const int p = i ^ j;
-        if (p > i) {
-          const int x = a[i], y = a[p];
-          const bool up = (i & k) == 0;
-          if ((x > y) == up) { a[i] = y; a[p] = x; }
-        }
-      }
-      __syncwarp();
-    }
-}
-template <bool COUNT>
-__global__ void k_vf(const DeviceMesh M, const SubIndex X, const __grid_constant__ VFParams P, int cap,
-                     const int32_t* __restrict__ tile_vf_rel, const int32_t* __restrict__ vt_off,
-                     const int32_t* __restrict__ vt_idx, int32_t* vf_off, int32_t* vf_idx, int32_t* stats) {
-  extern __shared__ int32_t shv[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  if (!COUNT && blockIdx.x == 0 && threadIdx.x == 0) { vf_off[0] = 0; vf_off[P.total_rows] = P.total_vf; }  // every launch of a batch writes the same two values
-  if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
-  int slot;
-  {
-    int lo = 0, hi = P.n_clusters;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (P.tile_prefix[mid] <= (int)blockIdx.x) lo = mid; else hi = mid;
-    }
-    slot = lo;
-  }
-  const int tile = M.cluster_tile_begin[P.cluster[slot]] + ((int)blockIdx.x - P.tile_prefix[slot]);
-  const int nrows = M.tiles[tile].nrows, v_lo = M.tiles[tile].v_lo;
-  const int row0 = P.row_base[slot] + M.tiles[tile].row_rel;
-  // shared memory: deg[nrows+1] | nlow[nrows] | cand[warps][cap] | keep[nrows][cap] (not in count mode)
-  const int pad = (nrows + 4) & ~3;
-  int32_t* deg = shv;
-  int32_t* nlow = shv + pad;
-  int32_t* cand = shv + 2 * pad + (size_t)w * cap;
-  int32_t* keep = shv + 2 * pad + (size_t)nw * cap;
-  const int4* T4 = reinterpret_cast<const int4*>(M.T);
-  // The triangles that have v as their LOWEST vertex are v's own block of F: contiguous ids, no look-up.
-  // The others lie in the blocks of lower vertices (smaller ids): they come from the simplices of VT(v) in
-  // which v is not the lowest vertex — each such triangle is found in at most two of them — and are
-  // looked up, sorted and de-duplicated by the warp.
-  for (int r = w; r < nrows; r += nw) {
-    const int v = v_lo + r;
-    const int t0 = vt_off[row0 + r], t1 = vt_off[row0 + r + 1];
-    const int n = min(3 * (t1 - t0), cap);
-    int nc = 0;  // candidates kept so far (compacted: the sort below is as small as the looked-up part)
-    for (int i0 = 0; i0 < n; i0 += 32) {
-      const int i = i0 + lane;
-      int id = INT_MAX;
-      if (i < n) {
-        const int4 q = __ldg(T4 + vt_idx[t0 + i / 3]);
-        if (q.x != v) {                                      // v is not the lowest vertex of this simplex
-          const int s[4] = {q.x, q.y, q.z, q.w};
-          int o[3] = {0, 0, 0}, m = 0;
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            if (s[k] != v && m < 3) o[m++] = s[k];          // the three other vertices, ascending
-          const int f = i % 3;                              // drop one of them: (v, o1, o2), (v, o0, o2), (v, o0, o1)
-          const int x = f == 0 ? o[1] : o[0], y = f == 2 ? o[1] : o[2];
-          if (x < v) {                                       // else v is the lowest vertex of the triangle: own block
-            int a = x, b = v, c = y;                         // x < v, x < y: sort (v, y)
-            if (b > c) { const int tt = b; b = c; c = tt; }
-            id = tri_id(X, a, b, c);
-          }
-        }
-      }
-      const unsigned mk = __ballot_sync(0xFFFFFFFFu, id != INT_MAX);
-      if (id != INT_MAX) cand[nc + __popc(mk & ((1u << lane) - 1u))] = id;
-      nc += __popc(mk);
-    }
-    const int n2 = init::pow2_ceil(nc < 1 ? 1 : nc);
-    for (int i = nc + lane; i < n2; i += 32) cand[i] = INT_MAX;
-    __syncwarp();
-    warp_bitonic32(cand, n2, lane);
-    int base = 0;
-    for (int i0 = 0; i0 < n2; i0 += 32) {
-      const int i = i0 + lane;
-      const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
-      const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
-      if (!COUNT && head) keep[(size_t)r * cap + base + __popc(m & ((1u << lane) - 1u))] = cand[i];
-      base += __popc(m);
-    }
-    __syncwarp();
-    if (lane == 0) { nlow[r] = base; deg[r] = base + (X.f_first[v + 1] - X.f_first[v]); }
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {  // a tile has few rows: serial exclusive scan
-    int acc = COUNT ? 0 : P.vf_base[slot] + tile_vf_rel[tile];
-    for (int r = 0; r < nrows; ++r) { const int d = deg[r]; deg[r] = acc; acc += d; }
-    deg[nrows] = acc;
-    if (COUNT) stats[tile] = acc;
-  }
-  __syncthreads();
-  if constexpr (!COUNT) {
-  for (int r = threadIdx.x; r < nrows; r += blockDim.x) vf_off[row0 + r] = deg[r];
-  for (int r = w; r < nrows; r += nw) {  // write-out, one warp per row: the looked-up ids, then the own block
-    const int nl = nlow[r], tot = deg[r + 1] - deg[r], own0 = X.f_first[v_lo + r];
-    int32_t* out = vf_idx + deg[r];
-    for (int i = lane; i < tot; i += 32) GALE_ST(out + i, i < nl ? keep[(size_t)r * cap + i] : own0 + (i - nl));
-  }
-  }
-}
 
-// ---- EF, ET, FT of a batch (PAPER.md:49, Table 1; the MS-complex set, :309) ----------------------------
-// Rows = the edges (E..) / triangles (F..) internal to the requested clusters, i.e. the blocks of E / F of
-// their vertices; the rows of a tile are contiguous ids. One block per tile, one warp per vertex a: the
-// simplices of VT(a) (just written by the batch kernel) are held in shared memory; row (a, b) of ET = those
-// that contain b, row (a, b, c) of FT = those that contain b and c — a ballot per 32 simplices, in VT's
-// ascending order; row (a, b) of EF = the triangles (a, b, x) of those simplices, looked up in F, sorted
-// and de-duplicated by the warp. COUNT (sizing at create): stats[tile] = entries of the tile.
-// Dynamic shared memory (ints): rows_cap + 4 (row counts -> offsets) | ((nrows + 4) & ~3) (vertex totals) |
-// warps * star_cap * 4 (the stars) | warps * 64 (EF candidates).
-enum { COB_ET = 0, COB_FT = 1, COB_EF = 2 };
+// ---- VF, EF, ET, FT of a batch (Table 1; DiscreteGradient :307, the MS-complex set :309) ----
+// Rows: VF = the vertices of the requested clusters; ET / EF = the edges, FT = the triangles internal to them,
+// i.e. the blocks of E / F of their vertices (the rows of a tile are contiguous ids). Every row of a vertex a
+// is a subset of one short, ascending list that belongs to a — its "star":
+//   ET (a, b)    = the simplices of VT(a) that contain b;  FT (a, b, c) = those that contain b and c;
+//   VF (a)       = the triangles at a: for every lower neighbour x of a (VV(a) ascends, so they come first and
+//                  in order) the entries of x's block of F that contain a, then a's own block — ids ascend
+//                  and every triangle is met once: no look-up, no sort, no duplicates;
+//   EF (a, b)    = the triangles at a that contain b.
+// One block per tile, everything flat (one thread per item, no warp-wide loops over short lists):
+//   A  one warp per vertex copies its source row into shared memory — the VT entries with the vertices of their
+//      simplices (ET, FT) or the VV entries with the F blocks of the lower neighbours (VF, EF) — and the
+//      descriptors (e_hi / f_bc) of its rows; all loads independent.
+//   B  VF, EF: one thread per (vertex a, lower neighbour x) scans x's block of F and keeps a bit per entry that
+//      contains a; a block scan over the pairs places the triangles of every vertex (the own blocks are
+//      contiguous ids, so their share of the offsets is a difference of I_F). VF writes them out; EF lists them
+//      in shared memory with their vertices above a: the star of a.
+//   C  ET, FT, EF: one thread per row scans the star of its vertex and keeps a bit per member (the rows come out
+//      sorted for free); sizes = popcounts, block scan, the thread writes the row's offset and entries.
+// COUNT (sizing at create): stats[tile] = entries of the tile; VF: *stats_max = the most triangles at a vertex.
+enum { COB_ET = 0, COB_FT = 1, COB_EF = 2, COB_VF = 3 };
 struct CobParams {
   int n_clusters;
   int total_rows, total_nnz;        // terminal offset
   int tile_prefix[kMaxBatch + 1];
   int cluster[kMaxBatch];
-  int vt_row_base[kMaxBatch];       // first VT row of slot i in the batch
-  int row_base[kMaxBatch];          // first edge / triangle row of slot i in the batch
+  int src_row_base[kMaxBatch];      // first VT / VV row of slot i in the batch
+  int row_base[kMaxBatch];          // first output row of slot i in the batch (VF: its vertex rows)
   int nnz_base[kMaxBatch];          // first entry of slot i in the batch
 };
+struct StarDims {
+  int tv;         // vertices of a tile
+  int rows_cap;   // rows of a tile: edges (ET, EF), triangles (FT); VF: 0
+  int src_cap;    // entries of the tile's source rows: VT (ET, FT) or VV (EF, VF)
+  int W;          // words of a row mask: ceil(largest star / 32); VF: 0
+  int Wf;         // EF, VF: words of a pair mask: ceil(longest block of F / 32)
+  int fstar_cap;  // EF: triangles at the vertices of a tile
+};
+struct StarLayout {  // offsets in ints, every section a multiple of 4
+  int wsum, soff, rfirst, ofirst, fo, s0, s1, s2, pcnt, pmask, desc, rown, rloc, rmask, fid, ftup, total;
+};
+__host__ __device__ inline StarLayout make_star_layout(int kind, const StarDims& d) {
+  auto pad = [](int n) { return (n + 3) & ~3; };
+  const bool from_vt = kind == COB_ET || kind == COB_FT, rows = kind != COB_VF;
+  StarLayout L;
+  int o = 0;
+  L.wsum = o;   o += 32;                    // scratch of the block scans
+  L.soff = o;   o += pad(d.tv + 1);         // offsets of the source rows
+  L.rfirst = o; o += pad(d.tv + 1);         // I_E / I_F of the tile's vertices (rows)
+  L.ofirst = o; o += pad(d.tv + 1);         // I_F of the tile's vertices (EF, VF: own blocks)
+  L.fo = o;     o += pad(d.tv + 1);         // EF, VF: first triangle at every vertex, inside the tile
+  L.s0 = o;     o += pad(d.src_cap);                                 // simplex ids | first entry of x's F block
+  L.s1 = o;     o += from_vt ? 3 * pad(d.src_cap) : pad(d.src_cap);  // their 2nd, 3rd, 4th vertices (one array each: rows of different vertices
+                                                                     // read different banks) | length of the block (0: x is not below a)
+  L.s2 = o;     o += from_vt ? 0 : pad(d.src_cap);                   // | owner a of the pair
+  L.pcnt = o;   o += from_vt ? 0 : pad(d.src_cap + 1);               // hits of the pair, then their prefix
+  L.pmask = o;  o += from_vt ? 0 : pad(d.src_cap * d.Wf);
+  L.desc = o;   o += rows ? pad(d.rows_cap * (kind == COB_FT ? 2 : 1)) : 0;
+  L.rown = o;   o += rows ? pad(d.rows_cap) : 0;                     // vertex of the row
+  L.rloc = o;   o += rows ? pad(d.rows_cap + 1) : 0;                 // row sizes, then offsets inside the tile
+  L.rmask = o;  o += rows ? pad(d.rows_cap * d.W) : 0;
+  L.fid = o;    o += kind == COB_EF ? pad(d.fstar_cap) : 0;          // EF: the triangles at the tile's vertices ...
+  L.ftup = o;   o += kind == COB_EF ? 2 * pad(d.fstar_cap) : 0;      // ... and their vertices above a (-1: none)
+  L.total = o;
+  return L;
+}
+// In-place exclusive scan of v[0, n) in shared memory by the whole block; v[n] = total (also returned). The
+// values must be complete (barrier) before the call; wsum = 32 ints of scratch.
+__device__ __forceinline__ int block_scan_smem(int32_t* v, int n, int32_t* wsum) {
+  const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, w = tid >> 5, nw = NT >> 5;
+  const int per = (n + NT - 1) / NT;
+  const int j0 = min(tid * per, n), j1 = min(j0 + per, n);
+  int sum = 0;
+  for (int j = j0; j < j1; ++j) sum += v[j];
+  int incl = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int y = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= d) incl += y;
+  }
+  if (lane == 31) wsum[w] = incl;
+  __syncthreads();
+  int before = 0, total = 0;
+  for (int k = 0; k < nw; ++k) { const int t = wsum[k]; if (k < w) before += t; total += t; }
+  int acc = before + incl - sum;
+  for (int j = j0; j < j1; ++j) { const int c = v[j]; v[j] = acc; acc += c; }
+  if (tid == 0) v[n] = total;
+  __syncthreads();
+  return total;
+}
 template <int KIND, bool COUNT>
-__global__ void k_cob(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P, int rows_cap, int star_cap,
-                      const int32_t* __restrict__ tile_rel, const int32_t* __restrict__ vt_off,
-                      const int32_t* __restrict__ vt_idx, int32_t* out_off, int32_t* out_idx, int32_t* stats) {
-  extern __shared__ int32_t shc[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  if (!COUNT && blockIdx.x == 0 && threadIdx.x == 0) { out_off[0] = 0; out_off[P.total_rows] = P.total_nnz; }
+__global__ void __launch_bounds__(256)
+k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P, const StarDims Dm, const StarLayout L,
+       const int32_t* __restrict__ tile_rel, const int32_t* __restrict__ src_off, const int32_t* __restrict__ src_idx,
+       int32_t* out_off, int32_t* out_idx, int32_t* stats, int32_t* stats_max) {
+  extern __shared__ __align__(16) int32_t shs[];
+  constexpr bool FROM_VT = KIND == COB_ET || KIND == COB_FT, ROWS = KIND != COB_VF;
+  const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, w = tid >> 5, nw = NT >> 5;
+  if (!COUNT && blockIdx.x == 0 && tid == 0) { out_off[0] = 0; out_off[P.total_rows] = P.total_nnz; }  // every launch of a batch writes the same two values
   if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
   int slot;
   {
@@ -333,105 +276,193 @@ __global__ void k_cob(const DeviceMesh M, const SubIndex X, const __grid_constan
     slot = lo;
   }
   const int tile = M.cluster_tile_begin[P.cluster[slot]] + ((int)blockIdx.x - P.tile_prefix[slot]);
-  const int nrows = M.tiles[tile].nrows, v_lo = M.tiles[tile].v_lo;
-  const int c_lo = v_lo - M.tiles[tile].row_rel;
-  const int32_t* first = KIND == COB_FT ? X.f_first : X.e_first;   // interval array of the ROW list
-  const int r_tile0 = first[v_lo], r_tile1 = first[v_lo + nrows];   // the tile's rows: contiguous ids
-  const int n_tile_rows = min(r_tile1 - r_tile0, rows_cap);
-  const int vrow0 = P.vt_row_base[slot] + M.tiles[tile].row_rel;
-  int32_t* rcnt = shc;                                   // [rows_cap + 1] counts, then offsets
-  int32_t* vtot = shc + ((rows_cap + 4) & ~3);           // [nrows + 1]
-  int4* star = reinterpret_cast<int4*>(vtot + ((nrows + 4) & ~3)) + (size_t)w * star_cap;
-  int32_t* cand = reinterpret_cast<int32_t*>(reinterpret_cast<int4*>(vtot + ((nrows + 4) & ~3)) + (size_t)nw * star_cap) + w * 64;
-  const int4* T4 = reinterpret_cast<const int4*>(M.T);
-  for (int pass = 0; pass < (COUNT ? 1 : 2); ++pass) {
-    for (int r = w; r < nrows; r += nw) {
-      const int a = v_lo + r;
-      const int t0 = vt_off[vrow0 + r];
-      const int deg = min(vt_off[vrow0 + r + 1] - t0, star_cap);
-      for (int i = lane; i < deg; i += 32) star[i] = __ldg(T4 + vt_idx[t0 + i]);
-      __syncwarp();
-      int tot = 0;
-      const int j0 = first[a], j1 = first[a + 1];
-      for (int j = j0; j < j1; ++j) {
-        const int jr = j - r_tile0;                       // row inside the tile
-        int b, c = -1;
-        if (KIND == COB_FT) { const int2 q = X.f_bc[j]; b = q.x; c = q.y; } else { b = X.e_hi[j]; }
-        const int wbase = (pass == 1 && jr < rows_cap) ? rcnt[jr] : 0;
-        int cnt = 0;
-        if (KIND != COB_EF) {
-          for (int i0 = 0; i0 < deg; i0 += 32) {
-            const int i = i0 + lane;
-            bool hit = false;
-            if (i < deg) {
-              const int4 q = star[i];
-              const bool hb = q.x == b || q.y == b || q.z == b || q.w == b;
-              hit = KIND == COB_FT ? (hb && (q.x == c || q.y == c || q.z == c || q.w == c)) : hb;
-            }
-            const unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
-            if (pass == 1 && hit) GALE_ST(out_idx + wbase + cnt + __popc(m & ((1u << lane) - 1u)), vt_idx[t0 + i]);
-            cnt += __popc(m);
-          }
-        } else {
-          int nc = 0;                                     // triangles (a, b, x) of the simplices that contain b
-          for (int i0 = 0; i0 < deg; i0 += 32) {
-            const int i = i0 + lane;
-            int id0 = INT_MAX, id1 = INT_MAX;
-            if (i < deg) {
-              const int4 q = star[i];
-              const int s[4] = {q.x, q.y, q.z, q.w};
-              if (s[0] == b || s[1] == b || s[2] == b || s[3] == b) {
-                int o[2] = {0, 0}, mm = 0;
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                  if (s[k] != a && s[k] != b && mm < 2) o[mm++] = s[k];
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {               // sort (a, b, x): a < b
-                  const int x = o[u];
-                  const int p0 = x < a ? x : a, p2 = x > b ? x : b, p1 = a + b + x - p0 - p2;
-                  (u == 0 ? id0 : id1) = tri_id(X, p0, p1, p2);
-                }
-              }
-            }
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-              const int id = u == 0 ? id0 : id1;
-              const unsigned m = __ballot_sync(0xFFFFFFFFu, id != INT_MAX);
-              if (id != INT_MAX && nc + __popc(m & ((1u << lane) - 1u)) < 64) cand[nc + __popc(m & ((1u << lane) - 1u))] = id;
-              nc = min(64, nc + __popc(m));
-            }
-          }
-          const int n2 = init::pow2_ceil(nc < 1 ? 1 : nc);
-          for (int i = nc + lane; i < n2; i += 32) cand[i] = INT_MAX;
-          __syncwarp();
-          warp_bitonic32(cand, n2, lane);
-          for (int i0 = 0; i0 < n2; i0 += 32) {
-            const int i = i0 + lane;
-            const bool head = i < n2 && cand[i] != INT_MAX && (i == 0 || cand[i] != cand[i - 1]);
-            const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
-            if (pass == 1 && head) GALE_ST(out_idx + wbase + cnt + __popc(m & ((1u << lane) - 1u)), cand[i]);
-            cnt += __popc(m);
-          }
-          __syncwarp();
-        }
-        if (pass == 0 && lane == 0 && jr < rows_cap) rcnt[jr] = cnt;
-        tot += cnt;
+  const int nrows = min(M.tiles[tile].nrows, Dm.tv), v_lo = M.tiles[tile].v_lo, row_rel = M.tiles[tile].row_rel;
+  const int srow0 = P.src_row_base[slot] + row_rel;
+  const int W = Dm.W, Wf = Dm.Wf;
+  const int32_t* first = KIND == COB_FT ? X.f_first : X.e_first;  // interval array of the ROW list (not VF)
+  int32_t* wsum = shs + L.wsum;
+  int32_t* soff = shs + L.soff;
+  int32_t* rfirst = shs + L.rfirst;
+  int32_t* ofirst = shs + L.ofirst;
+  int32_t* fo = shs + L.fo;
+  int32_t* sid = shs + L.s0;                                   // ET / FT: simplex ids
+  const int sp = (Dm.src_cap + 3) & ~3;
+  int32_t* ty = shs + L.s1;                                    // ET / FT: 2nd, 3rd, 4th vertex of those simplices (the lowest is never asked for)
+  int32_t* tz = ty + sp;
+  int32_t* tw = tz + sp;
+  int32_t* nf0 = shs + L.s0;                                   // EF / VF: F block of the lower neighbour x of the pair ...
+  int32_t* nlen = shs + L.s1;                                  // ... its length (0: x is not below a) ...
+  int32_t* nown = shs + L.s2;                                  // ... and a
+  int32_t* pcnt = shs + L.pcnt;
+  uint32_t* pmask = reinterpret_cast<uint32_t*>(shs + L.pmask);
+  int32_t* desc = shs + L.desc;
+  int32_t* rown = shs + L.rown;
+  int32_t* rloc = shs + L.rloc;
+  uint32_t* rmask = reinterpret_cast<uint32_t*>(shs + L.rmask);
+  int32_t* fid = shs + L.fid;
+  int32_t* fp1 = shs + L.ftup;                                 // EF: the (up to two) vertices above a of the triangles at a, -1: none
+  int32_t* fp2 = fp1 + ((Dm.fstar_cap + 3) & ~3);
+  // ---- A1: offsets of the tile's vertices ------------------------------------------------------------------
+  for (int r = tid; r <= nrows; r += NT) {
+    soff[r] = src_off[srow0 + r];
+    if constexpr (ROWS) rfirst[r] = first[v_lo + r];
+    if constexpr (!FROM_VT) ofirst[r] = X.f_first[v_lo + r];
+  }
+  __syncthreads();
+  const int s_base = soff[0];
+  const int n_src = min(soff[nrows] - s_base, Dm.src_cap);
+  const int r_tile0 = ROWS ? rfirst[0] : 0;
+  const int n_tile_rows = ROWS ? min(rfirst[nrows] - r_tile0, Dm.rows_cap) : 0;
+  // ---- A2: one warp per vertex: its source row and the descriptors of its rows ---------------------------
+  for (int r = w; r < nrows; r += nw) {
+    const int a = v_lo + r;
+    const int i0 = min(soff[r] - s_base, n_src), i1 = min(soff[r + 1] - s_base, n_src);
+    for (int i = i0 + lane; i < i1; i += 32) {
+      const int e = src_idx[s_base + i];
+      if constexpr (FROM_VT) {
+        sid[i] = e;
+        const int4 q = __ldg(reinterpret_cast<const int4*>(M.T) + e);
+        ty[i] = q.y; tz[i] = q.z; tw[i] = q.w;
+      } else {
+        int f0 = 0, len = 0;
+        if (e < a) { f0 = X.f_first[e]; len = X.f_first[e + 1] - f0; }
+        nf0[i] = f0;
+        nlen[i] = len;
+        nown[i] = r;
       }
-      if (pass == 0 && lane == 0) vtot[r] = tot;
-      __syncwarp();
+    }
+    if constexpr (ROWS) {
+      const int j0 = min(rfirst[r] - r_tile0, n_tile_rows), j1 = min(rfirst[r + 1] - r_tile0, n_tile_rows);
+      for (int j = j0 + lane; j < j1; j += 32) {
+        if constexpr (KIND == COB_FT) { const int2 q = X.f_bc[r_tile0 + j]; desc[2 * j] = q.x; desc[2 * j + 1] = q.y; }
+        else desc[j] = X.e_hi[r_tile0 + j];
+        rown[j] = r;
+      }
+    }
+  }
+  __syncthreads();
+  const int base0 = COUNT ? 0 : P.nnz_base[slot] + tile_rel[tile];
+  // ---- B: the triangles at the tile's vertices (VF, EF) -----------------------------------------------------
+  if constexpr (!FROM_VT) {
+    for (int i = tid; i < n_src; i += NT) {  // one thread per pair (a, lower neighbour x): a bit per entry of x's block that contains a
+      const int len = min(nlen[i], 32 * Wf), f0 = nf0[i], a = v_lo + nown[i];
+      int cnt = 0;
+      for (int k = 0; k < Wf; ++k) {
+        uint32_t bits = 0u;
+        const int e1 = min(32, len - 32 * k);
+        for (int e = 0; e < e1; ++e) {
+          const int2 q = X.f_bc[f0 + 32 * k + e];
+          bits |= (uint32_t)(q.x == a || q.y == a) << e;
+        }
+        pmask[i * Wf + k] = bits;
+        cnt += __popc(bits);
+      }
+      pcnt[i] = cnt;
     }
     __syncthreads();
-    if (pass == 0) {
-      if (threadIdx.x == 0) {  // serial exclusive scan over the tile's rows (a few hundred)
-        int acc = COUNT ? 0 : P.nnz_base[slot] + tile_rel[tile];
-        for (int j = 0; j < n_tile_rows; ++j) { const int d = rcnt[j]; rcnt[j] = acc; acc += d; }
-        rcnt[n_tile_rows] = acc;
-        if (COUNT) stats[tile] = acc;
+    block_scan_smem(pcnt, n_src, wsum);
+    const int ob = ofirst[0];
+    for (int r = tid; r <= nrows; r += NT) fo[r] = pcnt[min(soff[r] - s_base, n_src)] + (ofirst[r] - ob);  // own blocks: contiguous ids
+    __syncthreads();
+    if constexpr (KIND == COB_VF) {
+      if (COUNT) {
+        if (tid == 0) stats[tile] = fo[nrows];
+        int vmax = 0;
+        for (int r = tid; r < nrows; r += NT) vmax = max(vmax, fo[r + 1] - fo[r]);
+        if (vmax > 0) atomicMax(stats_max, vmax);
+      } else {
+        const int orow0 = P.row_base[slot] + row_rel;
+        for (int r = tid; r < nrows; r += NT) out_off[orow0 + r] = base0 + fo[r];
       }
-      __syncthreads();
-      if (!COUNT) {
-        const int orow0 = P.row_base[slot] + (r_tile0 - first[c_lo]);
-        for (int j = threadIdx.x; j < n_tile_rows; j += blockDim.x) out_off[orow0 + j] = rcnt[j];
+    }
+    if (!COUNT || KIND == COB_EF) {
+      for (int i = tid; i < n_src; i += NT) {  // the pair's triangles, in place
+        const int r = nown[i], a = v_lo + r, f0 = nf0[i];
+        int pos = fo[r] + (pcnt[i] - pcnt[min(soff[r] - s_base, n_src)]);
+        for (int k = 0; k < Wf; ++k) {
+          uint32_t bits = pmask[i * Wf + k];
+          while (bits) {
+            const int j = f0 + 32 * k + __ffs(bits) - 1;
+            bits &= bits - 1;
+            if constexpr (KIND == COB_VF) {
+              GALE_ST(out_idx + base0 + pos, j);
+            } else if (pos < Dm.fstar_cap) {
+              const int2 q = X.f_bc[j];
+              fid[pos] = j;
+              fp1[pos] = q.x == a ? q.y : -1;  // (x, a, y): y is above a; (x, y, a): no vertex above a
+              fp2[pos] = -1;
+            }
+            ++pos;
+          }
+        }
+      }
+      for (int r = w; r < nrows; r += nw) {  // the own blocks
+        const int o0 = ofirst[r], n_own = ofirst[r + 1] - o0, at = fo[r + 1] - n_own;
+        for (int t = lane; t < n_own; t += 32) {
+          if constexpr (KIND == COB_VF) {
+            GALE_ST(out_idx + base0 + at + t, o0 + t);
+          } else if (at + t < Dm.fstar_cap) {
+            fid[at + t] = o0 + t;
+            const int2 q = X.f_bc[o0 + t];
+            fp1[at + t] = q.x;
+            fp2[at + t] = q.y;
+          }
+        }
+      }
+    }
+    if constexpr (KIND == COB_EF) __syncthreads();
+  }
+  // ---- C: one thread per row: members of the star, sizes -> offsets, write-out --------------------------
+  if constexpr (ROWS) {
+    for (int j = tid; j < n_tile_rows; j += NT) {
+      const int r = rown[j];
+      int st0, n;
+      if constexpr (FROM_VT) { st0 = min(soff[r] - s_base, n_src); n = min(soff[r + 1] - s_base, n_src) - st0; }
+      else { st0 = min(fo[r], Dm.fstar_cap); n = min(fo[r + 1], Dm.fstar_cap) - st0; }
+      n = min(n, 32 * W);
+      const int b = desc[KIND == COB_FT ? 2 * j : j];
+      const int c = KIND == COB_FT ? desc[2 * j + 1] : 0;
+      int cnt = 0;
+      for (int k = 0; k < W; ++k) {
+        uint32_t bits = 0u;
+        const int e1 = min(32, n - 32 * k);
+        for (int e = 0; e < e1; ++e) {
+          bool hit;
+          if constexpr (KIND == COB_EF) {
+            hit = fp1[st0 + 32 * k + e] == b || fp2[st0 + 32 * k + e] == b;
+          } else {
+            const int at = st0 + 32 * k + e;         // a < b (< c): b is not the lowest vertex, c not one of the two lowest
+            const int qy = ty[at], qz = tz[at], qw = tw[at];
+            if constexpr (KIND == COB_ET) hit = qy == b || qz == b || qw == b;
+            else hit = (qy == b || qz == b) && (qz == c || qw == c);
+          }
+          bits |= (uint32_t)hit << e;
+        }
+        rmask[j * W + k] = bits;
+        cnt += __popc(bits);
+      }
+      rloc[j] = cnt;
+    }
+    __syncthreads();
+    const int total = block_scan_smem(rloc, n_tile_rows, wsum);
+    if (COUNT) {
+      if (tid == 0) stats[tile] = total;
+    } else {
+      const int orow0 = P.row_base[slot] + (r_tile0 - first[v_lo - row_rel]);
+      for (int j = tid; j < n_tile_rows; j += NT) {
+        int off = base0 + rloc[j];
+        out_off[orow0 + j] = off;
+        const int r = rown[j];
+        const int32_t* ids = KIND == COB_EF ? fid + min(fo[r], Dm.fstar_cap) : sid + min(soff[r] - s_base, n_src);
+        for (int k = 0; k < W; ++k) {
+          uint32_t bits = rmask[j * W + k];
+          while (bits) {
+            const int bpos = __ffs(bits) - 1;
+            bits &= bits - 1;
+            GALE_ST(out_idx + off, ids[k * 32 + bpos]);
+            ++off;
+          }
+        }
       }
     }
   }
