@@ -210,8 +210,9 @@ def main():
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--streams", type=int, default=1,
                     help="CUDA streams the batches are submitted on in turn (consecutive batches overlap)")
-    ap.add_argument("--mask", type=int, default=7, help="relation mask of the device-timed pass (1 VT, 2 VV, 4 TT); "
-                    "the bench line of record uses 7, other values are for per-relation diagnosis")
+    ap.add_argument("--mask", type=int, default=7, help="relation mask of the device-timed pass (1 VT, 2 VV, 4 TT; 8 VE, 16 VF, 32 EF, "
+                    "64 ET, 128 FT build the edge / triangle lists at create); the bench line of record uses 7, other "
+                    "values are for per-relation diagnosis (the roofline figures then still count the VT+VV+TT bytes)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "dense", "walk"],
                     help="kernel variant: auto = gale_mesh_create times both on a sample batch and keeps the faster")
     ap.add_argument("--stage-from-t", action="store_true",
@@ -251,7 +252,10 @@ def main():
     gm = gale.GaleMesh(mesh.dim, mesh.num_vertices, mesh.simplices, mesh.cluster_offsets, max_batch_clusters=B,
                        queue_depth=0, device_ring=args.ring, tile_vertices=args.tile,
                        flags={"auto": 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[args.kernel] |
-                       (gale.STAGE_FROM_T if args.stage_from_t else 0))
+                       (gale.STAGE_FROM_T if args.stage_from_t else 0) |
+                       (gale.WITH_EDGES if args.mask & (gale.REL_VE | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
+                       (gale.WITH_FACETS if args.mask & (gale.REL_VF | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
+                       (gale.WITH_COBOUNDARY if args.mask & (gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0))
     create_s = time.time() - t0
     info = gm.info
     stream = torch.cuda.current_stream()
