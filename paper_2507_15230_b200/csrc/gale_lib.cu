@@ -765,6 +765,12 @@ int size_star_relations(gale_mesh* m, cudaStream_t st, uint32_t kinds, uint32_t 
       }
       const int grid = V.tile_prefix[nb];
       if (grid <= 0) continue;
+      {
+        const int per = V.tile_prefix[1];
+        bool uniform = per > 0;
+        for (int i = 0; i < nb && uniform; ++i) uniform = V.tile_prefix[i + 1] - V.tile_prefix[i] == per;
+        V.uniform_tiles = uniform ? per : 0;
+      }
       for (int k = 0; k < 4; ++k) {
         if (!(kinds >> k & 1u)) continue;
         const bool from_vt = k == gs::COB_ET || k == gs::COB_FT;
@@ -1334,6 +1340,7 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
         if (!(user_mask & bit[k])) continue;
         gs::CobParams V{};
         V.n_clusters = nb;
+        V.uniform_tiles = P.uniform_tiles;
         if (k == gs::COB_VF) { V.total_rows = int(s.rows); V.total_nnz = int(s.vf_nnz); }
         else { V.total_rows = (k == gs::COB_FT ? s.f_row_begin : s.e_row_begin)[size_t(n_clusters)]; V.total_nnz = int(s.cob_nnz[k]); }
         long long base = 0;

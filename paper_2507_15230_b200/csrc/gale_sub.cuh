@@ -190,6 +190,7 @@ enum { COB_ET = 0, COB_FT = 1, COB_EF = 2, COB_VF = 3 };
 struct CobParams {
   int n_clusters;
   int total_rows, total_nnz;        // terminal offset
+  int uniform_tiles;                // > 0: every cluster of the batch has this many tiles (slot = block / it)
   int tile_prefix[kMaxBatch + 1];
   int cluster[kMaxBatch];
   int src_row_base[kMaxBatch];      // first VT / VV row of slot i in the batch
@@ -267,7 +268,9 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
   if (!COUNT && blockIdx.x == 0 && tid == 0) { out_off[0] = 0; out_off[P.total_rows] = P.total_nnz; }  // every launch of a batch writes the same two values
   if ((int)blockIdx.x >= P.tile_prefix[P.n_clusters]) return;
   int slot;
-  {
+  if (P.uniform_tiles > 0) {  // every cluster of the batch has this many tiles
+    slot = (int)blockIdx.x / P.uniform_tiles;
+  } else {
     int lo = 0, hi = P.n_clusters;
     while (hi - lo > 1) {
       const int mid = (lo + hi) >> 1;
