@@ -316,6 +316,15 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
   const int n_src = min(soff[nrows] - s_base, Dm.src_cap);
   const int r_tile0 = ROWS ? rfirst[0] : 0;
   const int n_tile_rows = ROWS ? min(rfirst[nrows] - r_tile0, Dm.rows_cap) : 0;
+#if GALE_CHECK_BOUNDS
+  // the capacities fixed at create hold for this tile (the clamps above and below never bite)
+  if (tid == 0) {
+    bool ok = M.tiles[tile].nrows <= Dm.tv && soff[nrows] - s_base <= Dm.src_cap;
+    if (ROWS) ok = ok && rfirst[nrows] - r_tile0 <= Dm.rows_cap;
+    if (KIND == COB_EF) ok = ok && ofirst[nrows] - ofirst[0] <= Dm.fstar_cap;
+    (void)GALE_IN_BOUNDS(M.err, ok);
+  }
+#endif
   // ---- A2: one warp per vertex: its source row and the descriptors of its rows ---------------------------
   for (int r = w; r < nrows; r += nw) {
     const int a = v_lo + r;
@@ -349,6 +358,7 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
   if constexpr (!FROM_VT) {
     for (int i = tid; i < n_src; i += NT) {  // one thread per pair (a, lower neighbour x): a bit per entry of x's block that contains a
       const int len = min(nlen[i], 32 * Wf), f0 = nf0[i], a = v_lo + nown[i];
+      (void)GALE_IN_BOUNDS(M.err, nlen[i] <= 32 * Wf && nown[i] >= 0 && nown[i] < nrows);
       int cnt = 0;
       for (int k = 0; k < Wf; ++k) {
         uint32_t bits = 0u;
@@ -388,8 +398,8 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
             const int j = f0 + 32 * k + __ffs(bits) - 1;
             bits &= bits - 1;
             if constexpr (KIND == COB_VF) {
-              GALE_ST(out_idx + base0 + pos, j);
-            } else if (pos < Dm.fstar_cap) {
+              if (GALE_IN_BOUNDS(M.err, pos >= fo[r] && pos < fo[r + 1])) GALE_ST(out_idx + base0 + pos, j);
+            } else if (GALE_IN_BOUNDS(M.err, pos < Dm.fstar_cap) && pos < Dm.fstar_cap) {
               const int2 q = X.f_bc[j];
               fid[pos] = j;
               fp1[pos] = q.x == a ? q.y : -1;  // (x, a, y): y is above a; (x, y, a): no vertex above a
@@ -422,6 +432,7 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
       int st0, n;
       if constexpr (FROM_VT) { st0 = min(soff[r] - s_base, n_src); n = min(soff[r + 1] - s_base, n_src) - st0; }
       else { st0 = min(fo[r], Dm.fstar_cap); n = min(fo[r + 1], Dm.fstar_cap) - st0; }
+      (void)GALE_IN_BOUNDS(M.err, n >= 0 && n <= 32 * W && r >= 0 && r < nrows);
       n = min(n, 32 * W);
       const int b = desc[KIND == COB_FT ? 2 * j : j];
       const int c = KIND == COB_FT ? desc[2 * j + 1] : 0;
@@ -462,7 +473,7 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
           while (bits) {
             const int bpos = __ffs(bits) - 1;
             bits &= bits - 1;
-            GALE_ST(out_idx + off, ids[k * 32 + bpos]);
+            if (GALE_IN_BOUNDS(M.err, off < base0 + rloc[j + 1])) GALE_ST(out_idx + off, ids[k * 32 + bpos]);
             ++off;
           }
         }

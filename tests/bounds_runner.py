@@ -60,4 +60,32 @@ for (name, make, batch, tv, mask), kernel in RUNS:
             assert np.array_equal(g["tt"], r["tt"]), (name, "tt", r["cluster"])
     print(f"ok {name}: tiles {gm.info.num_tiles}, tile {gm.info.tile_vertices}, {gm.info.local_id_bytes}-byte ids")
     gm.destroy()
+# VE / VF / EF / ET / FT (k_star and the list builders) through the checked build, against the oracle
+SUB_CASES = [
+    ("cfg1 sub", lambda: meshgen.make_config(1), 3),
+    ("holes3d sub", lambda: meshgen.make_mesh(3, 16, clustering="octree", capacity=400, permute=True, drop_frac=0.15, seed=15), 5),
+    ("delaunay3d sub", lambda: meshgen.make_delaunay(3, 3000, seed=44, capacity=400), 4),
+]
+if not os.environ.get("GALE_CHECK_SELFTEST"):
+    for name, make, batch in SUB_CASES:
+        m = make()
+        T, nV = m.simplices, m.num_vertices
+        gm = gale.GaleMesh(3, nV, T, m.cluster_offsets, max_batch_clusters=batch, device_ring=2,
+                           flags=gale.VALIDATE | gale.WITH_EDGES | gale.WITH_FACETS | gale.WITH_COBOUNDARY)
+        E, F = oracle.sub_simplices(3, nV, T, 2), oracle.sub_simplices(3, nV, T, 3)
+        ref = {k: oracle.coboundary(3, nV, T, k.upper()) for k in ("ef", "et", "ft")}
+        first = {"ef": E["first"], "et": E["first"], "ft": F["first"]}
+        ids = list(range(m.num_clusters))
+        mask = gale.REL_ALL | gale.REL_VE | gale.REL_VF | gale.REL_EF | gale.REL_ET | gale.REL_FT
+        for b in range(0, len(ids), batch):
+            for g in gale.split_batch(gm.run_batch(ids[b:b + batch], mask), 4):
+                lo, hi = int(m.cluster_offsets[g["cluster"]]), int(m.cluster_offsets[g["cluster"] + 1])
+                for k in ("ef", "et", "ft"):
+                    off = ref[k][0][int(first[k][lo]):int(first[k][hi]) + 1]
+                    assert np.array_equal(g[k][0], (off - off[0]).astype(np.int32)), (name, k, g["cluster"])
+                    assert np.array_equal(g[k][1], ref[k][1][off[0]:off[-1]]), (name, k, g["cluster"])
+                off = F["v_off"][lo:hi + 1]
+                assert np.array_equal(g["vf"][1], F["v_idx"][off[0]:off[-1]]), (name, "vf", g["cluster"])
+        print(f"ok {name}: E {gm.info.num_edges}, F {gm.info.num_triangles}")
+        gm.destroy()
 print("ALL CHECKED CASES PASSED")
