@@ -28,10 +28,16 @@ struct WalkLayout {
   int total;
 };
 
-// Capacities come in a SmemCfg; `hs` = table slots per tile vertex (even, so the row stride hs+1 is odd).
+// Rows per block of the instantiation that runs tiles of `tv` vertices (NT / 2, a multiple of 32).
+__host__ __device__ inline int walk_rows_for_tile(int tv) { return tv > 128 ? 256 : (tv > 64 ? 128 : (tv > 32 ? 64 : 32)); }
+
+// Capacities come in a SmemCfg; `hs` = table slots per tile vertex. The structures a thread owns alone (VV
+// bitmap row, facet table of vertex p) are stored word-interleaved over the rows — word w of row p at
+// [w * TV + p] — so that lane p always works in bank p and the serial walks meet no bank conflict.
 template <int D>
 __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   WalkLayout L;
+  const int tvp = walk_rows_for_tile(c.tv);
   int o = 0;
   L.mbar = o;   o = align16(o + 8);
   L.ctx = o;    o = align16(o + 112);
@@ -51,9 +57,9 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
     const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
     o += bm > reuse ? bm : reuse;
   }
-  L.bmV = o;    o = align16(o + c.tv * c.WV * 4);
+  L.bmV = o;    o = align16(o + tvp * c.WV * 4);
   L.bm_end = o;
-  L.tbl = o;    o = align16(o + (c.hs ? c.tv * (c.hs + 1) * 4 : 0));
+  L.tbl = o;    o = align16(o + (c.hs ? tvp * c.hs * 4 : 0));
   L.ttrow = o;  o = align16(o + (c.hs ? c.sint * D * 2 : 0));
   L.ext0 = o;   o = align16(o + (c.hs ? c.sext * 2 : 0));
   L.tt_end = o;
@@ -76,7 +82,7 @@ __device__ __forceinline__ void named_barrier(int id, int count) {
 __device__ __forceinline__ uint32_t bit_of(int l) { return 1u << (l & 31); }
 
 struct GroupCtx {
-  uint32_t* tbl;       // this vertex's table, hs slots
+  uint32_t* tbl;       // this vertex's table, hs slots, slot h at tbl[h * TV]
   uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
   uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
   uint16_t* ext0;      // entry 0 of the external simplices, same encoding
@@ -86,25 +92,25 @@ struct GroupCtx {
 
 // Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
 // holds the same key (the other coface) and write both TT entries. The thread owns the table.
-template <int D>
+template <int D, int TV>
 __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
   using FB = FacetBits<D>;
   uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
-  uint32_t cur = g.tbl[h];
+  uint32_t cur = g.tbl[h * TV];
 #if GALE_CHECK_BOUNDS
   uint32_t probe = 0;
 #endif
   // a table has more slots than its group has records, so an empty slot or the key is always met
   while (cur != kEmpty32 && (cur & FB::kKeyMask) != key) {  // probe loop kept minimal: lanes diverge here
     h = h + 1 == g.hs ? 0u : h + 1;
-    cur = g.tbl[h];
+    cur = g.tbl[h * TV];
 #if GALE_CHECK_BOUNDS
     if (++probe >= g.hs) { raise_err(err, ERR_TT_TABLE_FULL); return; }
 #endif
   }
   if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
   if (cur == kEmpty32) {
-    g.tbl[h] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
+    g.tbl[h * TV] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
   } else {
     const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
     if (!GALE_IN_BOUNDS(err, s < g.s_all && s2 < g.s_all && k2 < D)) return;
@@ -320,7 +326,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
 
   // ---- P3: A walks the bits of row p, B walks the run of p ------------------------------------
   if (live) {
-    uint32_t* vvrow = bmV + p * WV;
+    uint32_t* vvrow = bmV + p;  // word w of the row at vvrow[w * TV]
     if (!isB) {
       const uint32_t* row = bmT + p * WT;
       int pos = off, sbase = -32;
@@ -335,14 +341,14 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
           st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
         if (do_vv) {
 #pragma unroll
-          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));  // self bit cleared in P4
+          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5) * TV, bit_of(l[k]));  // self bit cleared in P4
         }
       }
     } else {
       GroupCtx g;
       if (do_tt) {
         const int hs = C.hs;
-        g.tbl = tbl + p * (hs + 1);
+        g.tbl = tbl + p;
         g.hs = (uint32_t)hs;
         g.ttrow = ttrow; g.ext0 = ext0;
         g.s_ext = s_ext; g.s_all = S;
@@ -356,12 +362,12 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= s_ext && s < S)) st_vt[pos++] = (uint16_t)s;
         if (do_vv) {
 #pragma unroll
-          for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5), bit_of(l[k]));
+          for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5) * TV, bit_of(l[k]));
         }
         if (do_tt) {
-          group_place<D>(g, facet_key<D, 1>(l), s, 1, M.err);
-          group_place<D>(g, facet_key<D, 2>(l), s, 2, M.err);
-          if constexpr (D == 4) group_place<D>(g, facet_key<D, 3>(l), s, 3, M.err);
+          group_place<D, TV>(g, facet_key<D, 1>(l), s, 1, M.err);
+          group_place<D, TV>(g, facet_key<D, 2>(l), s, 2, M.err);
+          if constexpr (D == 4) group_place<D, TV>(g, facet_key<D, 3>(l), s, 3, M.err);
         }
       }
     }
@@ -374,7 +380,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     if (do_tt && live) {
       GroupCtx g;
       const int hs = C.hs;
-      g.tbl = tbl + p * (hs + 1);
+      g.tbl = tbl + p;
       g.hs = (uint32_t)hs;
       g.ttrow = ttrow; g.ext0 = ext0;
       g.s_ext = s_ext; g.s_all = S;
@@ -388,17 +394,17 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         const int s = (int)(e & 0x7FFFu);
         int l[4];
         load_local<LB>(tets, s, l);
-        group_place<D>(g, facet_key<D, 0>(l), s, 0, M.err);
+        group_place<D, TV>(g, facet_key<D, 0>(l), s, 0, M.err);
       }
     }
   } else if (do_vv) {
     const int wV = (td.nloc + 31) >> 5;
-    uint32_t* row = bmV + p * WV;
+    uint32_t* row = bmV + p;
     int nbv = 0;
     if (live) {
-      row[ploc >> 5] &= ~bit_of(ploc);  // a vertex is not its own neighbour
+      row[(ploc >> 5) * TV] &= ~bit_of(ploc);  // a vertex is not its own neighbour
 #pragma unroll 4
-      for (int w = 0; w < wV; ++w) nbv += __popc(row[w]);
+      for (int w = 0; w < wV; ++w) nbv += __popc(row[w * TV]);
     }
     uint32_t tot;
     const int offv = (int)half_exclusive_scan<NT>((uint32_t)nbv, scan, &tot);
@@ -408,7 +414,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       int pos = offv, lbase = -32;
       uint32_t bits = 0u;
       for (int n = 0; n < nbv; ++n) {
-        while (bits == 0u) { bits = *row++; lbase += 32; }
+        while (bits == 0u) { bits = *row; row += TV; lbase += 32; }
         if (GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vv_max && lbase + __ffs(bits) - 1 < td.nloc))
           st_vv[pos++] = (uint16_t)(lbase + __ffs(bits) - 1);
         bits &= bits - 1;
