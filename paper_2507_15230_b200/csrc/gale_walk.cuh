@@ -325,6 +325,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   if (do_vt && live && !isB) O.vt_offsets[row0 + p] = vt0 + off;
 
   // ---- P3: A walks the bits of row p, B walks the run of p ------------------------------------
+  uint32_t fmask = 0u;  // A: which of the first 32 entries of the row have p as second vertex (their facets 0 join p's group in P4)
   if (live) {
     uint32_t* vvrow = bmV + p;  // word w of the row at vvrow[w * TV]
     if (!isB) {
@@ -337,8 +338,10 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         bits &= bits - 1;
         int l[4];
         load_local<LB>(tets, s, l);
+        const bool second = l[1] == ploc;
+        if (n < 32) fmask |= (uint32_t)second << n;
         if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= 0 && s < S))
-          st_vt[pos++] = (uint16_t)(s | (l[1] == ploc ? 0x8000 : 0));
+          st_vt[pos++] = (uint16_t)(s | (second ? 0x8000 : 0));
         if (do_vv) {
 #pragma unroll
           for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5) * TV, bit_of(l[k]));  // self bit cleared in P4
@@ -384,7 +387,14 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       g.hs = (uint32_t)hs;
       g.ttrow = ttrow; g.ext0 = ext0;
       g.s_ext = s_ext; g.s_all = S;
-      int i = off;
+      // the flagged entries among the first 32 come from the walk's mask, longer rows are scanned for the rest
+      for (uint32_t fm = fmask; fm != 0u; fm &= fm - 1u) {
+        const int s = (int)(st_vt[off + __ffs(fm) - 1] & 0x7FFFu);
+        int l[4];
+        load_local<LB>(tets, s, l);
+        group_place<D, TV>(g, facet_key<D, 0>(l), s, 0, M.err);
+      }
+      int i = off + 32;
       const int end = off + nb;
       for (;;) {
         uint32_t e = 0u;
