@@ -223,6 +223,8 @@ def main():
                     help="> 0: also run CriticalPoints (VV + VT) over the whole mesh through the pinned queue with "
                          "this many consumer threads and report the paper's per-stage waiting times (PAPER.md:411)")
     ap.add_argument("--impl", default="gale", choices=["gale", "reference"])
+    ap.add_argument("--canonicalize", action="store_true",
+                    help="also time gale_canonicalize (SURVEY §8(f)-1) on a device-scrambled copy of the simplices; reported in config")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-depth", type=int, default=3, help="pinned queue slots per handle in the e2e leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -247,6 +249,21 @@ def main():
     D = mesh.dim + 1
     nC, B = mesh.num_clusters, args.batch
     batches = [np.arange(b, min(nC, b + B), dtype=np.int32) for b in range(0, nC, B)]
+
+    canon = None
+    if args.canonicalize:   # the step before the initialization: rows + vertex order scrambled on the device, best of 3
+        Tc = torch.from_numpy(mesh.simplices).cuda()
+        S = Tc[torch.randperm(Tc.shape[0], device="cuda", generator=torch.Generator(device="cuda").manual_seed(5))].flip(1).contiguous()
+        best = float("inf")
+        for _ in range(3):
+            torch.cuda.synchronize()
+            t0 = time.time()
+            out, perm = gale.canonicalize(mesh.dim, mesh.num_vertices, S)
+            torch.cuda.synchronize()
+            best = min(best, time.time() - t0)
+        canon = {"canonicalize_s": best, "rows_per_s": mesh.num_simplices / best, "restored": bool(torch.equal(out, Tc))}
+        del Tc, S, out, perm
+        torch.cuda.empty_cache()
 
     t0 = time.time()
     gm = gale.GaleMesh(mesh.dim, mesh.num_vertices, mesh.simplices, mesh.cluster_offsets, max_batch_clusters=B,
@@ -491,7 +508,8 @@ def main():
                                                        "create_sample_ms": {"dense": info.tune_dense_ms, "walk": info.tune_walk_ms},
                                                        "block_threads": info.block_threads, "relation_mask": args.mask,
                                                        "index_bytes": info.index_bytes, "workspace_used": info.workspace_used,
-                                                       "mesh_bytes": int(mesh.simplices.nbytes)}),
+                                                       "mesh_bytes": int(mesh.simplices.nbytes),
+                                                       **({"canonicalize": canon} if canon else {})}),
                 "clocks": clocks, "sustained": sustained, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu}
         if cons is not None:

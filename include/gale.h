@@ -55,7 +55,7 @@ enum {
   GALE_OK = 0,
   GALE_ERR_INVALID_ARG = -1,   /* null pointer, bad dim, relation_mask == 0, ...                      */
   GALE_ERR_NOT_CANONICAL = -2, /* C1-C3 violated (checked when GALE_VALIDATE is set)                  */
-  GALE_ERR_DEGENERATE = -3,    /* reserved                                                            */
+  GALE_ERR_DEGENERATE = -3,    /* gale_canonicalize: a simplex repeats a vertex or names one out of range */
   GALE_ERR_NONMANIFOLD = -4,   /* C4 violated (checked when GALE_VALIDATE_MANIFOLD is set)            */
   GALE_ERR_BAD_CLUSTER = -5,   /* cluster id out of range, or n_clusters > max_batch_clusters         */
   GALE_ERR_WOULD_BLOCK = -6,   /* every queue slot is un-released (compute), or timeout (pop)         */
@@ -180,6 +180,23 @@ typedef struct {
   float tune_dense_ms, tune_walk_ms; /* sample-batch times behind that choice (0 = not timed)           */
   int32_t reserved;
 } gale_mesh_info_t;
+
+/* Canonical form of a simplex list, on the device (the form gale_plan_create expects,
+ * DESIGN.md §2 reading 2): every row ascending, rows in ascending lexicographic order — the order in which
+ * the simplices internal to a segment (lowest vertex in the segment) are one contiguous range,
+ * which is what the interval array I_T of the paper's initialization records.
+ *   d_simplices_in   DEVICE int32[num_simplices * (dim + 1)], vertex ids in any order inside a row, rows in any
+ *                    order; valid in stream order on cuda_stream; not modified
+ *   d_simplices_out  DEVICE int32[num_simplices * (dim + 1)], caller-owned, must not alias the input
+ *   d_perm_out       DEVICE int32[num_simplices] or NULL: output row i is input row d_perm_out[i]. The sort is
+ *                    stable (equal rows keep their input order), so the permutation is unique
+ * dim is 2 or 3; num_vertices bounds the ids (it fixes the number of radix passes). Temporary device memory
+ * (one more copy of the rows and of the permutation, 1 KB of counters per 2,048 rows) is the library's and is
+ * released before return; the call synchronises cuda_stream. Errors: GALE_ERR_INVALID_ARG (NULL / aliased
+ * arrays, bad dim or sizes), GALE_ERR_DEGENERATE (a row repeats a vertex or names one outside
+ * [0, num_vertices); the output is then unspecified), GALE_ERR_CUDA, GALE_ERR_UNSUPPORTED (no sm_100 device). */
+int32_t gale_canonicalize(int32_t dim, int64_t num_simplices, int32_t num_vertices, const int32_t *d_simplices_in,
+                          int32_t *d_simplices_out, int32_t *d_perm_out, void *cuda_stream);
 
 /* Initialization analysis ("Initialization": I_T, the external lists T_ex, interval
  * arrays): reads the simplices from the DEVICE array desc->d_simplices — they must be valid in stream

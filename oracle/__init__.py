@@ -281,6 +281,20 @@ def coboundary(dim: int, num_vertices: int, simplices: np.ndarray, name: str) ->
         lib.go_cob_release(h)
 
 
+def canonical_form(simplices: np.ndarray) -> tuple:
+    """The canonical form the path expects (DESIGN.md §2 reading 2; the simplices internal to a
+    segment — lowest vertex in the segment — must be one contiguous range, which the interval array I_T records):
+    every row ascending, rows in ascending lexicographic order, equal rows in input order. Plain definition:
+    sort each row, then a stable lexicographic sort of the rows (numpy's lexsort is stable). Returns
+    (canonical rows, perm) with canonical row i = sorted(input row perm[i]).
+    Pins (tests/test_oracle_pins.py): the generator's own canonicalisation (independent C++), a pure-Python
+    sorted() of tuples, the oracle's C1 / C2 check, stability on duplicated rows."""
+    rows = np.sort(np.ascontiguousarray(simplices, dtype=np.int32), axis=1)
+    D = rows.shape[1]
+    order = np.lexsort(tuple(rows[:, k] for k in range(D - 1, -1, -1)))  # last key = primary = column 0
+    return np.ascontiguousarray(rows[order]), order.astype(np.int64)
+
+
 def brute_force(dim: int, num_vertices: int, simplices: np.ndarray) -> dict:
     """Brute-force enumeration of VT, VV, TT for tiny meshes (membership scans only)."""
     lib = _load()

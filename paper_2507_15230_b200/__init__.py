@@ -72,7 +72,7 @@ class gale_tile_view_t(ctypes.Structure):
                 ("d_external", ctypes.c_void_p), ("d_local_to_global", ctypes.c_void_p)]
 
 
-EXPORTS = ["gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+EXPORTS = ["gale_canonicalize", "gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
            "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
@@ -99,6 +99,8 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
                            "`python -c 'import __graft_entry__ as g; g.build()'`")
     lib = ctypes.CDLL(path)
     vp = ctypes.c_void_p
+    lib.gale_canonicalize.restype = ctypes.c_int32
+    lib.gale_canonicalize.argtypes = [ctypes.c_int32, ctypes.c_int64, ctypes.c_int32, vp, vp, vp, vp]
     lib.gale_plan_create.restype = ctypes.c_int32
     lib.gale_plan_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
     lib.gale_plan_workspace_bytes.restype = ctypes.c_int32
@@ -147,6 +149,29 @@ def _check(status: int, where: str):
 
 
 # ---- the C-ABI calls, same names, marshalling only ----------------------------------------------------
+def gale_canonicalize(dim: int, num_simplices: int, num_vertices: int, d_in: int, d_out: int, d_perm: int = 0,
+                      cuda_stream: int = 0) -> None:
+    """DEVICE pointers in, DEVICE pointers out (include/gale.h); d_perm = 0 skips the permutation."""
+    _check(load_library().gale_canonicalize(dim, num_simplices, num_vertices, ctypes.c_void_p(d_in), ctypes.c_void_p(d_out),
+                                            ctypes.c_void_p(d_perm or None), ctypes.c_void_p(cuda_stream)), "gale_canonicalize")
+
+
+def canonicalize(dim: int, num_vertices: int, simplices, want_perm: bool = True):
+    """Argument marshalling for gale_canonicalize: `simplices` is a CUDA int32 tensor [n, dim+1] (or anything
+    torch.as_tensor takes, uploaded first); returns (canonical simplices, permutation or None) as CUDA tensors."""
+    import torch
+
+    t = torch.as_tensor(simplices, dtype=torch.int32)
+    if t.device.type != "cuda":
+        t = t.cuda()
+    t = t.contiguous().reshape(-1, dim + 1)
+    out = torch.empty_like(t)
+    perm = torch.empty(t.shape[0], dtype=torch.int32, device=t.device) if want_perm else None
+    gale_canonicalize(dim, t.shape[0], num_vertices, t.data_ptr(), out.data_ptr(), perm.data_ptr() if want_perm else 0,
+                      torch.cuda.current_stream().cuda_stream)
+    return out, perm
+
+
 def gale_plan_create(desc: gale_mesh_desc_t, cuda_stream: int = 0) -> ctypes.c_void_p:
     h = ctypes.c_void_p()
     _check(load_library().gale_plan_create(ctypes.byref(desc), ctypes.c_void_p(cuda_stream), ctypes.byref(h)),

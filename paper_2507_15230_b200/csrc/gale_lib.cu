@@ -8,6 +8,7 @@
 #include "gale_walk.cuh"
 #include "gale_init.cuh"
 #include "gale_sub.cuh"
+#include "gale_canon.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -1078,6 +1079,37 @@ const char* gale_status_string(int32_t s) {
   }
 }
 const char* gale_last_error(void) { return g_last_error.c_str(); }
+
+int32_t gale_canonicalize(int32_t dim, int64_t num_simplices, int32_t num_vertices, const int32_t* d_simplices_in,
+                          int32_t* d_simplices_out, int32_t* d_perm_out, void* cuda_stream) {
+  namespace gc = gale::canon;
+  if ((dim != 2 && dim != 3) || num_simplices < 0 || num_simplices > 0x7FFFFFFFll || num_vertices <= 0) return GALE_ERR_INVALID_ARG;
+  if (num_simplices > 0 && (!d_simplices_in || !d_simplices_out || d_simplices_in == d_simplices_out)) return GALE_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc != GALE_OK) return rc;
+  if (num_simplices == 0) return GALE_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int D = dim + 1;
+  const long long n = num_simplices;
+  const int nseg = (int)((n + gc::kSeg - 1) / gc::kSeg);
+  const size_t n_counts = size_t(gc::kDigits) * nseg;
+  DevMem d_T1, d_p0, d_p1, d_counts, d_scratch, d_bad;
+  if ((rc = d_T1.alloc(size_t(n) * D * 4)) || (rc = d_p1.alloc(size_t(n) * 4)) || (rc = d_counts.alloc(n_counts * 4)) ||
+      (rc = d_scratch.alloc((n_counts / gale::init::kScanChunk + 2) * 4)) || (rc = d_bad.alloc(4)))
+    return rc;
+  if (!d_perm_out && (rc = d_p0.alloc(size_t(n) * 4))) return rc;
+  gc::Buffers B;
+  B.T[0] = d_simplices_out; B.T[1] = d_T1.as<int32_t>();
+  B.perm[0] = d_perm_out ? d_perm_out : d_p0.as<int32_t>(); B.perm[1] = d_p1.as<int32_t>();
+  B.counts = d_counts.as<int32_t>(); B.scratch = d_scratch.as<int32_t>(); B.bad = d_bad.as<int>();
+  GALE_CUDA(cudaMemsetAsync(B.bad, 0, 4, st));
+  GALE_CUDA(dim == 3 ? gc::canonicalize<4>(d_simplices_in, n, num_vertices, B, st) : gc::canonicalize<3>(d_simplices_in, n, num_vertices, B, st));
+  int bad = 0;
+  GALE_CUDA(cudaMemcpyAsync(&bad, B.bad, 4, cudaMemcpyDeviceToHost, st));
+  GALE_CUDA(cudaStreamSynchronize(st));  // the temporaries are released on return
+  if (bad) { g_last_error = "a simplex names a vertex outside [0, num_vertices) or repeats one"; return GALE_ERR_DEGENERATE; }
+  return GALE_OK;
+}
 
 int32_t gale_plan_create(const gale_mesh_desc_t* desc, void* cuda_stream, gale_plan_t** out) {
   if (!out) return GALE_ERR_INVALID_ARG;

@@ -384,3 +384,41 @@ def test_ef_et_ft_counts_brute_force_and_tt_consistency(n):
     pairs_tt = {(min(t, int(u)), max(t, int(u))) for t in range(nT) for u in tt[t] if u >= 0}
     pairs_ft = {(int(ft[1][ft[0][f]]), int(ft[1][ft[0][f] + 1])) for f in range(len(F)) if nft[f] == 2}
     assert pairs_tt == pairs_ft
+
+
+# ---- canonical form (SURVEY.md §8(f)-1 "canonicalisation itself"; DESIGN.md §2 reading 2) ------------------
+def _scramble(T, seed):
+    """Rows in random order, vertices in random order inside every row (seeded)."""
+    rng = np.random.default_rng(seed)
+    rows = T[rng.permutation(len(T))]
+    cols = np.argsort(rng.random(rows.shape), axis=1)
+    return np.take_along_axis(rows, cols, axis=1)
+
+
+@pytest.mark.parametrize("make", [lambda: meshgen.make_config(1), lambda: meshgen.make_mesh(2, 40, clustering="morton", block=8),
+                                  lambda: meshgen.make_delaunay(3, 800, seed=9, capacity=200)],
+                         ids=["kuhn3d", "grid2d", "delaunay3d"])
+def test_canonical_form_pins(make):
+    m = make()
+    T = m.simplices
+    S = _scramble(T, 17)
+    got, perm = oracle.canonical_form(S)
+    # (1) the generator canonicalises with its own C++ code: a scrambled copy must come back to exactly its output
+    assert np.array_equal(got, T)
+    # (2) plain Python: sorted tuples of sorted rows
+    assert [tuple(r) for r in got] == sorted(tuple(sorted(r)) for r in S.tolist())
+    # (3) the permutation leads back to the input rows, and a canonical list is a fixed point
+    assert np.array_equal(np.sort(S[perm], axis=1), got) and sorted(perm.tolist()) == list(range(len(S)))
+    again, p2 = oracle.canonical_form(T)
+    assert np.array_equal(again, T) and np.array_equal(p2, np.arange(len(T)))
+    # (4) the oracle's own C1 / C2 check (its C++ input contract) accepts it and rejects the scrambled list
+    oracle.relations_global(m.dim, m.num_vertices, got, mask=1)
+    with pytest.raises(oracle.OracleError):
+        oracle.relations_global(m.dim, m.num_vertices, S, mask=1)
+
+
+def test_canonical_form_is_stable_on_equal_rows():
+    S = np.array([[5, 1, 3, 2], [0, 9, 4, 7], [2, 5, 1, 3], [3, 2, 1, 5], [7, 9, 0, 4]], dtype=np.int32)
+    got, perm = oracle.canonical_form(S)
+    assert got.tolist() == [[0, 4, 7, 9], [0, 4, 7, 9], [1, 2, 3, 5], [1, 2, 3, 5], [1, 2, 3, 5]]
+    assert perm.tolist() == [1, 4, 0, 2, 3]   # equal rows keep their input order
