@@ -485,9 +485,11 @@ int analyse_device(Plan& p, const gale_mesh_desc_t& d, cudaStream_t st) {
     if (last) { g_last_error = "a single vertex star exceeds the kernels' shared-memory limits"; return GALE_ERR_UNSUPPORTED; }
   }
   {  // can the walk kernel run these tiles?
-    // load <= 3/4 even if no facet of a group is shared; every interior facet is recorded twice, so the
-    // usual load is about 0.4 (measured: at 0.54 the re-probes cost 3 warp-instructions per tet)
-    p.cfg.hs = std::max(8, (p.gmax + p.gmax / 3 + 1) & ~1);
+    // as many slots as the largest group has records: when a record is placed at most gmax - 1 slots are
+    // taken, so the probe always meets an empty slot or its key; every interior facet is recorded twice, so
+    // the usual load is about 0.5 (the tables are bank-conflict free, re-probes are cheap; the 1 KB saved
+    // per block buys two more resident blocks)
+    p.cfg.hs = std::max(8, p.gmax);
     p.w_NT = walk_threads_for_tile(p.tv);
     p.w_smem = walk_layout_for(D, walk_cfg_for_mask(p.cfg, 7)).total;
     p.walk_ok = p.tv <= 256 && p.w_smem <= kSmemLimit && p.cfg.smax < 32768 && p.cfg.vt_max < 65536;

@@ -44,14 +44,14 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
-  L.ft = o;     o = align16(o + (c.tv + 1) * 4);
+  L.ft = o;     // (the slice of I_T is read straight from global memory)
   L.cnt = o;    o = align16(o + c.tv * 4);
   L.scan = o;   o = align16(o + 48 * 4);
   // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
   // fallback queue (written in P5)
   L.bmT = o;
   {
-    const int bm = align16(c.tv * c.WT * 4);
+    const int bm = align16(tvp * ((c.smax + 31) / 32) * 4);  // word w of row p at [w * TV + p], like the VV rows
     L.st_vv = o;
     L.fbq = o + align16(c.vv_max * 2);
     const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
@@ -225,11 +225,11 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   const TileDesc& td = ctx->td;
   const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
   const int S = s_int + s_ext;
-  const int WT = C.WT, WV = C.WV;
+  const int WV = C.WV;
 #if GALE_CHECK_BOUNDS
   {
     bool ok = nrows >= 0 && nrows <= C.tv && NT >= 2 * C.tv && S >= 0 && S <= C.smax && s_ext <= C.sext &&
-              td.nloc <= C.nloc && nlo >= 0 && nlo + nrows <= td.nloc && ((S + 31) >> 5) <= WT;
+              td.nloc <= C.nloc && nlo >= 0 && nlo + nrows <= td.nloc;
     if (mask & REL_VV) ok = ok && ((td.nloc + 31) >> 5) <= WV;
     if (mask & REL_TT) ok = ok && s_int <= C.sint && C.hs >= 2;
     if (mask & (REL_VT | REL_TT)) ok = ok && td.vt_nnz <= C.vt_max;
@@ -244,7 +244,6 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   unsigned char* tets = smem + L.tets;
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
-  int32_t* ft = reinterpret_cast<int32_t*>(smem + L.ft);        // first_tet[v_lo .. v_lo+nrows] (I_T)
   uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
   uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [36] queue length, [38] n_vv
@@ -257,9 +256,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
 
   const int row0 = ctx->row0, vt0 = ctx->vt0, vv0 = ctx->vv0, tt0 = ctx->tt0;
-  for (int i = tid; i <= nrows; i += NT) ft[i] = __ldg(M.first_tet + td.v_lo + i);
   mbar_wait(bar, 0);
-  __syncthreads();  // ft
 
   // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
   for (int s = tid; s < S; s += NT) {
@@ -270,12 +267,12 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       if (!GALE_IN_BOUNDS(M.err, l[k] >= 0 && l[k] < td.nloc)) l[k] = nlo;  // keep later indexing inside the row
     if (s >= s_ext) (void)GALE_IN_BOUNDS(M.err, (unsigned)(l[0] - nlo) < (unsigned)nrows);  // internal: lowest vertex in the tile
 #endif
-    uint32_t* col = bmT + (s >> 5);
+    uint32_t* col = bmT + (s >> 5) * TV;
     const uint32_t bit = bit_of(s);
 #pragma unroll
     for (int k = 1; k < D; ++k) {
       const int r = l[k] - nlo;
-      if ((unsigned)r < (unsigned)nrows) atomicOr(col + r * WT, bit);
+      if ((unsigned)r < (unsigned)nrows) atomicOr(col + r, bit);
     }
   }
   __syncthreads();
@@ -288,11 +285,11 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   const int wT = (S + 31) >> 5;
   if (live) {
     const int half = (wT + 1) >> 1;
-    const uint32_t* row = bmT + p * WT;
+    const uint32_t* row = bmT + p;
     int c = 0;
     const int w0 = isB ? half : 0, w1 = isB ? wT : half;
 #pragma unroll 4
-    for (int w = w0; w < w1; ++w) c += __popc(row[w]);
+    for (int w = w0; w < w1; ++w) c += __popc(row[w * TV]);
     cnt[(isB ? C.tv : 0) + p] = (uint16_t)c;
   }
   __syncthreads();
@@ -302,7 +299,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     uint32_t deg = 0u, tot;
     if (live) {
       nb = (int)cnt[p] + (int)cnt[C.tv + p];
-      run_lo = ft[p]; run_hi = ft[p + 1];
+      run_lo = __ldg(M.first_tet + td.v_lo + p); run_hi = __ldg(M.first_tet + td.v_lo + p + 1);
       deg = (uint32_t)(nb + run_hi - run_lo);
     }
     if constexpr (NT == 64) {
@@ -329,11 +326,11 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   if (live) {
     uint32_t* vvrow = bmV + p;  // word w of the row at vvrow[w * TV]
     if (!isB) {
-      const uint32_t* row = bmT + p * WT;
+      const uint32_t* row = bmT + p;
       int pos = off, sbase = -32;
       uint32_t bits = 0u;
       for (int n = 0; n < nb; ++n) {
-        while (bits == 0u) { bits = *row++; sbase += 32; }
+        while (bits == 0u) { bits = *row; row += TV; sbase += 32; }
         const int s = sbase + __ffs(bits) - 1;
         bits &= bits - 1;
         int l[4];
