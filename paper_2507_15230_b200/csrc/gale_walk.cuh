@@ -23,7 +23,7 @@ namespace gale {
 
 struct WalkLayout {
   int mbar, ctx, tets, texid, gid, ft, cnt, fbq, scan, bmT, bmV, bm_end;
-  int tbl, ttrow, ext0, tt_end;
+  int tbl, ttrow, tt_end;
   int st_vt, st_vv;
   int total;
 };
@@ -45,8 +45,9 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.texid = o;  o = align16(o + c.sext * 4);
   L.gid = o;    o = align16(o + c.nloc * 4);
   L.ft = o;     // (the slice of I_T is read straight from global memory)
-  L.cnt = o;    o = align16(o + c.tv * 4);
-  L.scan = o;   o = align16(o + 48 * 4);
+  L.scan = o;   o = align16(o + 36 * 4);   // [0..33) scan scratch, [33] a5 queue length, [34] n_vv
+  // the 64-thread instantiation scans inside its warps and leaves scan[0..32) unused: the row counts live there
+  if (tvp == 32) { L.cnt = L.scan; } else { L.cnt = o; o = align16(o + c.tv * 4); }
   // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
   // fallback queue (written in P5)
   L.bmT = o;
@@ -57,11 +58,10 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
     const int reuse = align16(c.vv_max * 2) + align16(c.sint * 2);
     o += bm > reuse ? bm : reuse;
   }
-  L.bmV = o;    o = align16(o + tvp * c.WV * 4);
+  L.bmV = o;    o = align16(o + (c.WV ? tvp * ((c.nloc + 31) / 32) * 4 : 0));  // interleaved rows need no odd stride
   L.bm_end = o;
   L.tbl = o;    o = align16(o + (c.hs ? tvp * c.hs * 4 : 0));
   L.ttrow = o;  o = align16(o + (c.hs ? c.sint * D * 2 : 0));
-  L.ext0 = o;   o = align16(o + (c.hs ? c.sext * 2 : 0));
   L.tt_end = o;
   L.st_vt = o;  o = align16(o + c.vt_max * 2);
   L.total = o;
@@ -85,14 +85,32 @@ struct GroupCtx {
   uint32_t* tbl;       // this vertex's table, hs slots, slot h at tbl[h * TV]
   uint32_t hs;         // slots (any size >= the group's records: a group never overflows its table)
   uint16_t* ttrow;     // TT rows of the tile's internal simplices as staged indices, 0xFFFF = none
-  uint16_t* ext0;      // entry 0 of the external simplices, same encoding
   int s_ext;
   int s_all;           // staged simplices of the tile (bounds-checked build)
+  // entry 0 of an external simplex of this cluster goes straight to the output (its row belongs to another tile)
+  const unsigned char* tets;
+  const int32_t* texid;
+  const int32_t* gid;
+  int32_t* tt;         // O.tt_indices
+  int t_lo, tt_slot, c_lo, c_tlo;
 };
+
+// TT entry 0 of the external simplex s (its facet 0 has this tile's vertex p as lowest vertex, so only this tile
+// can match it): written when s belongs to this tile's cluster (else the cluster of s resolves it itself, a5).
+// partner = staged index of the coface, -1 = none so far: the first arrival of a facet writes -1 and the same
+// thread overwrites it if the coface turns up later (same thread, same address: program order).
+template <int D, int LB>
+__device__ __forceinline__ void ext_entry0(const GroupCtx& g, int s, int partner) {
+  const int l0 = LB == 2 ? (int)reinterpret_cast<const uint16_t*>(g.tets)[s * 4] : (int)g.tets[s * 4];
+  if (g.gid[l0] >= g.c_lo) {
+    const int val = partner < 0 ? -1 : (partner < g.s_ext ? g.texid[partner] : g.t_lo + (partner - g.s_ext));
+    GALE_ST(g.tt + (long long)(g.tt_slot + (g.texid[s] - g.c_tlo)) * D, val);
+  }
+}
 
 // Place facet k of staged simplex s with key `key`: claim an empty slot, or meet the record that
 // holds the same key (the other coface) and write both TT entries. The thread owns the table.
-template <int D, int TV>
+template <int D, int TV, int LB>
 __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int s, int k, int32_t* err) {
   using FB = FacetBits<D>;
   uint32_t h = __umulhi(key * 0x9E3779B1u, g.hs);
@@ -111,12 +129,13 @@ __device__ __forceinline__ void group_place(const GroupCtx& g, uint32_t key, int
   if (!GALE_IN_BOUNDS(err, h < g.hs && (uint32_t)s <= FB::kIdxMask && key <= FB::kKeyMask && k >= 0 && k < D)) return;
   if (cur == kEmpty32) {
     g.tbl[h * TV] = key | ((uint32_t)s << FB::kKeyBits) | ((uint32_t)k << 30);
+    if (s < g.s_ext) ext_entry0<D, LB>(g, s, -1);
   } else {
     const int s2 = (int)((cur >> FB::kKeyBits) & FB::kIdxMask), k2 = (int)(cur >> 30);
     if (!GALE_IN_BOUNDS(err, s < g.s_all && s2 < g.s_all && k2 < D)) return;
     // an external simplex only ever records its facet 0
-    if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2; else g.ext0[s] = (uint16_t)s2;
-    if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s; else g.ext0[s2] = (uint16_t)s;
+    if (s >= g.s_ext) g.ttrow[(s - g.s_ext) * D + k] = (uint16_t)s2; else ext_entry0<D, LB>(g, s, s2);
+    if (s2 >= g.s_ext) g.ttrow[(s2 - g.s_ext) * D + k2] = (uint16_t)s; else ext_entry0<D, LB>(g, s2, s);
   }
 }
 
@@ -220,7 +239,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     const int n16 = (L.tt_end - L.tbl) >> 4;
     for (int i = tid; i < n16; i += NT) z[i] = make_int4(-1, -1, -1, -1);
   }
-  if (tid == 0) { reinterpret_cast<uint32_t*>(smem + L.scan)[36] = 0u; reinterpret_cast<uint32_t*>(smem + L.scan)[38] = 0u; }
+  if (tid == 0) { reinterpret_cast<uint32_t*>(smem + L.scan)[33] = 0u; reinterpret_cast<uint32_t*>(smem + L.scan)[34] = 0u; }
   __syncthreads();
   const TileDesc& td = ctx->td;
   const int nrows = td.nrows, t_lo = td.t_lo, s_int = td.s_int, s_ext = td.s_ext, nlo = td.nlo;
@@ -246,12 +265,11 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
   uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
-  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [36] queue length, [38] n_vv
+  uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [33] queue length, [34] n_vv
   uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
   uint32_t* bmV = reinterpret_cast<uint32_t*>(smem + L.bmV);
   uint32_t* tbl = reinterpret_cast<uint32_t*>(smem + L.tbl);
   uint16_t* ttrow = reinterpret_cast<uint16_t*>(smem + L.ttrow);
-  uint16_t* ext0 = reinterpret_cast<uint16_t*>(smem + L.ext0);
   uint16_t* st_vt = reinterpret_cast<uint16_t*>(smem + L.st_vt);
   uint16_t* st_vv = reinterpret_cast<uint16_t*>(smem + L.st_vv);
 
@@ -350,7 +368,9 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         const int hs = C.hs;
         g.tbl = tbl + p;
         g.hs = (uint32_t)hs;
-        g.ttrow = ttrow; g.ext0 = ext0;
+        g.ttrow = ttrow;
+        g.tets = tets; g.texid = texid; g.gid = gid; g.tt = O.tt_indices;
+        g.t_lo = t_lo; g.tt_slot = ctx->tt_slot; g.c_lo = td.v_lo - td.row_rel; g.c_tlo = t_lo - td.tt_rel;
         g.s_ext = s_ext; g.s_all = S;
       }
       int pos = off + nb;
@@ -365,9 +385,9 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
           for (int k = 1; k < D; ++k) atomicOr(vvrow + (l[k] >> 5) * TV, bit_of(l[k]));
         }
         if (do_tt) {
-          group_place<D, TV>(g, facet_key<D, 1>(l), s, 1, M.err);
-          group_place<D, TV>(g, facet_key<D, 2>(l), s, 2, M.err);
-          if constexpr (D == 4) group_place<D, TV>(g, facet_key<D, 3>(l), s, 3, M.err);
+          group_place<D, TV, LB>(g, facet_key<D, 1>(l), s, 1, M.err);
+          group_place<D, TV, LB>(g, facet_key<D, 2>(l), s, 2, M.err);
+          if constexpr (D == 4) group_place<D, TV, LB>(g, facet_key<D, 3>(l), s, 3, M.err);
         }
       }
     }
@@ -382,14 +402,16 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
       const int hs = C.hs;
       g.tbl = tbl + p;
       g.hs = (uint32_t)hs;
-      g.ttrow = ttrow; g.ext0 = ext0;
+      g.ttrow = ttrow;
+      g.tets = tets; g.texid = texid; g.gid = gid; g.tt = O.tt_indices;
+      g.t_lo = t_lo; g.tt_slot = ctx->tt_slot; g.c_lo = td.v_lo - td.row_rel; g.c_tlo = t_lo - td.tt_rel;
       g.s_ext = s_ext; g.s_all = S;
       // the flagged entries among the first 32 come from the walk's mask, longer rows are scanned for the rest
       for (uint32_t fm = fmask; fm != 0u; fm &= fm - 1u) {
         const int s = (int)(st_vt[off + __ffs(fm) - 1] & 0x7FFFu);
         int l[4];
         load_local<LB>(tets, s, l);
-        group_place<D, TV>(g, facet_key<D, 0>(l), s, 0, M.err);
+        group_place<D, TV, LB>(g, facet_key<D, 0>(l), s, 0, M.err);
       }
       int i = off + 32;
       const int end = off + nb;
@@ -401,7 +423,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         const int s = (int)(e & 0x7FFFu);
         int l[4];
         load_local<LB>(tets, s, l);
-        group_place<D, TV>(g, facet_key<D, 0>(l), s, 0, M.err);
+        group_place<D, TV, LB>(g, facet_key<D, 0>(l), s, 0, M.err);
       }
     }
   } else if (do_vv) {
@@ -415,7 +437,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     }
     uint32_t tot;
     const int offv = (int)half_exclusive_scan<NT>((uint32_t)nbv, scan, &tot);
-    if (tid == TV) scan[38] = tot;
+    if (tid == TV) scan[34] = tot;
     if (live) {
       O.vv_offsets[row0 + p] = vv0 + offv;
       int pos = offv, lbase = -32;
@@ -429,14 +451,13 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     }
   }
   __syncthreads();
-  n_vv = (int)scan[38];
+  n_vv = (int)scan[34];
   if (tid == 0 && ((do_vt && n_vt != td.vt_nnz) || (do_vv && n_vv != td.vv_nnz)))
     raise_err(M.err, ERR_SIZE_MISMATCH);  // the sizes fixed at create must be reproduced exactly
 
   // ---- P5: translate to global ids, coalesced write-out ----------------------------------------
   if (do_tt) {
     const int c_lo = td.v_lo - td.row_rel, c_hi = c_lo + td.c_rows;  // the cluster's vertex range
-    const int c_tlo = t_lo - td.tt_rel;                               // its first internal simplex
     for (int i = tid; i < s_int; i += NT) {
       bool need_fb = false;
       {
@@ -475,19 +496,8 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         }
       }
       if (need_fb) {  // rare (cross-cluster facets only): a plain atomic per facet
-        const uint32_t pos = atomicAdd(&scan[36], 1u);
+        const uint32_t pos = atomicAdd(&scan[33], 1u);
         if (GALE_IN_BOUNDS(M.err, (int)pos < C.sint)) fbq[pos] = (uint16_t)i;
-      }
-    }
-    // entry 0 of the external simplices of this cluster whose second vertex is a vertex of this tile
-    for (int s = tid; s < s_ext; s += NT) {
-      int l[4];
-      load_local<LB>(tets, s, l);
-      if ((unsigned)(l[1] - nlo) < (unsigned)nrows && gid[l[0]] >= c_lo) {
-        const int e = ext0[s];
-        const int v = e == 0xFFFF ? -1 : (e < s_ext ? texid[e] : t_lo + (e - s_ext));
-        const long long row = (long long)ctx->tt_slot + (texid[s] - c_tlo);
-        GALE_ST(O.tt_indices + row * D, v);
       }
     }
   }
@@ -502,7 +512,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   if (do_tt) {
     __syncthreads();  // queue complete, TT rows stored
     // ---- a5: one queued facet per thread, resolved from global memory -------------------------
-    const int nq = (int)scan[36];
+    const int nq = (int)scan[33];
     for (int q = tid; q < nq; q += NT) {
       const int i = fbq[q];
       int l[4];
