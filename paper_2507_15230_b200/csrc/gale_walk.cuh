@@ -358,8 +358,14 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
         if (entries && GALE_IN_BOUNDS(M.err, pos >= 0 && pos < C.vt_max && s >= 0 && s < S))
           st_vt[pos++] = (uint16_t)(s | (second ? 0x8000 : 0));
         if (do_vv) {
-#pragma unroll
-          for (int k = 0; k < D; ++k) atomicOr(vvrow + (l[k] >> 5) * TV, bit_of(l[k]));  // self bit cleared in P4
+          // p is not the lowest vertex here: mark l[0] and the D-2 vertices among l[1..D-1] other than p itself
+          atomicOr(vvrow + (l[0] >> 5) * TV, bit_of(l[0]));
+          const int m1 = second ? l[2] : l[1];
+          atomicOr(vvrow + (m1 >> 5) * TV, bit_of(m1));
+          if constexpr (D == 4) {
+            const int m2 = l[3] == ploc ? l[2] : l[3];
+            atomicOr(vvrow + (m2 >> 5) * TV, bit_of(m2));
+          }
         }
       }
     } else {
@@ -431,7 +437,7 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
     uint32_t* row = bmV + p;
     int nbv = 0;
     if (live) {
-      row[(ploc >> 5) * TV] &= ~bit_of(ploc);  // a vertex is not its own neighbour
+      // (p itself is never marked: a vertex is not its own neighbour)
 #pragma unroll 4
       for (int w = 0; w < wV; ++w) nbv += __popc(row[w * TV]);
     }
