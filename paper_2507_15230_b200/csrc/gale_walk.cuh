@@ -46,8 +46,7 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.gid = o;    o = align16(o + c.nloc * 4);
   L.ft = o;     // (the slice of I_T is read straight from global memory)
   L.scan = o;   o = align16(o + 36 * 4);   // [0..33) scan scratch, [33] a5 queue length, [34] n_vv
-  // the 64-thread instantiation scans inside its warps and leaves scan[0..32) unused: the row counts live there
-  if (tvp == 32) { L.cnt = L.scan; } else { L.cnt = o; o = align16(o + c.tv * 4); }
+  L.cnt = o;    // (unused: every thread counts its own row)
   // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
   // fallback queue (written in P5)
   L.bmT = o;
@@ -263,7 +262,6 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   unsigned char* tets = smem + L.tets;
   int32_t* texid = reinterpret_cast<int32_t*>(smem + L.texid);
   int32_t* gid = reinterpret_cast<int32_t*>(smem + L.gid);
-  uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);    // [2][tv] set bits of the row halves
   uint16_t* fbq = reinterpret_cast<uint16_t*>(smem + L.fbq);
   uint32_t* scan = reinterpret_cast<uint32_t*>(smem + L.scan);  // [0..33) scans, [33] queue length, [34] n_vv
   uint32_t* bmT = reinterpret_cast<uint32_t*>(smem + L.bmT);
@@ -301,22 +299,22 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   const bool live = p < nrows;
   const int ploc = nlo + p;
   const int wT = (S + 31) >> 5;
+  // every thread counts its whole row (conflict-free reads, 12 words on config 5) :
+  // no exchange between the halves, no barrier
+  int row_bits = 0;
   if (live) {
-    const int half = (wT + 1) >> 1;
     const uint32_t* row = bmT + p;
-    int c = 0;
-    const int w0 = isB ? half : 0, w1 = isB ? wT : half;
 #pragma unroll 4
-    for (int w = w0; w < w1; ++w) c += __popc(row[w * TV]);
-    cnt[(isB ? C.tv : 0) + p] = (uint16_t)c;
+    for (int w = 0; w < wT; ++w) {
+      row_bits += __popc(row[w * TV]);
+    }
   }
-  __syncthreads();
   int nb = 0, off = 0, n_vt;
   int run_lo = 0, run_hi = 0;  // run of p: simplices [run_lo, run_hi) have p as lowest vertex (I_T)
   {
     uint32_t deg = 0u, tot;
     if (live) {
-      nb = (int)cnt[p] + (int)cnt[C.tv + p];
+      nb = row_bits;
       run_lo = __ldg(M.first_tet + td.v_lo + p); run_hi = __ldg(M.first_tet + td.v_lo + p + 1);
       deg = (uint32_t)(nb + run_hi - run_lo);
     }
