@@ -281,6 +281,29 @@ def coboundary(dim: int, num_vertices: int, simplices: np.ndarray, name: str) ->
         lib.go_cob_release(h)
 
 
+def boundary(dim: int, num_vertices: int, simplices: np.ndarray, name: str) -> np.ndarray:
+    """Boundary relations FE, TE, TF (Table 1 :53-58; the look-up of :186-192) over the whole mesh as a
+    fixed-width array: row i = ids (positions in the sorted lists E / F) of the edges / triangles on
+    the boundary of triangle i of F (FE) or of simplex i of T (TE, TF), in the lexicographic order of their vertex
+    combinations — the order of the paper's example, FE(f5) = [(v0,v3), (v0,v4), (v3,v4)] (:192). Plain definition:
+    every combination is looked up in a dictionary of the whole list (no interval array involved).
+    Pins (tests/test_oracle_pins.py): FE / TE / TF are the transposes of the coboundary relations EF / ET / FT (a
+    different routine of the oracle, itself pinned), the paper's e2 and e9 for the triangle (v0, v3, v4) of the
+    Fig. 4 fixture, row-wise vertex sets."""
+    import itertools
+
+    T = _canon(simplices)
+    frm, to = {"FE": (3, 2), "TE": (dim + 1, 2), "TF": (dim + 1, 3)}[name]
+    rows = T if frm == dim + 1 and name != "FE" else sub_simplices(dim, num_vertices, T, 3)["list"]
+    ids = {tuple(r): i for i, r in enumerate(sub_simplices(dim, num_vertices, T, to)["list"].tolist())}
+    combos = list(itertools.combinations(range(rows.shape[1]), to))   # lexicographic
+    out = np.empty((rows.shape[0], len(combos)), dtype=np.int32)
+    for i, r in enumerate(rows.tolist()):
+        for j, c in enumerate(combos):
+            out[i, j] = ids[tuple(r[k] for k in c)]
+    return out
+
+
 def canonical_form(simplices: np.ndarray) -> tuple:
     """The canonical form the path expects (DESIGN.md §2 reading 2; the simplices internal to a
     segment — lowest vertex in the segment — must be one contiguous range, which the interval array I_T records):

@@ -422,3 +422,40 @@ def test_canonical_form_is_stable_on_equal_rows():
     got, perm = oracle.canonical_form(S)
     assert got.tolist() == [[0, 4, 7, 9], [0, 4, 7, 9], [1, 2, 3, 5], [1, 2, 3, 5], [1, 2, 3, 5]]
     assert perm.tolist() == [1, 4, 0, 2, 3]   # equal rows keep their input order
+
+
+# ---- boundary relations FE / TE / TF (Table 1 :53-58; look-up :186-192) ---------------------------
+def test_fig4_fe_example(golden_dir):
+    """FE of the triangle (v0, v3, v4) ('f5'): edges (v0,v3), (v0,v4), (v3,v4) in this order; the
+    paper prints e2, e6, e9 — e2 and e9 are reproduced, e6 cannot be (DESIGN.md §2 reading 18)."""
+    T, S, exp = _fig4(golden_dir)
+    F = oracle.sub_simplices(3, 6, T, 3)["list"].tolist()
+    fe = oracle.boundary(3, 6, T, "FE")
+    row = fe[F.index([0, 3, 4])].tolist()
+    assert row[0] == 2 and row[2] == 9
+    E = oracle.sub_simplices(3, 6, T, 2)["list"].tolist()
+    assert [E[e] for e in row] == [[0, 3], [0, 4], [3, 4]]
+
+
+@pytest.mark.parametrize("make", [lambda: meshgen.make_mesh(3, 6, clustering="octree", capacity=60, permute=True, seed=21),
+                                  lambda: meshgen.make_mesh(3, 7, clustering="octree", capacity=80, drop_frac=0.2, seed=4),
+                                  lambda: meshgen.make_delaunay(3, 300, seed=12, capacity=80)], ids=["kuhn", "holes", "delaunay"])
+def test_boundary_relations_are_transposes_of_the_coboundary_relations(make):
+    m = make()
+    T, nV = m.simplices, m.num_vertices
+    for bnd, cob in (("FE", "EF"), ("TE", "ET"), ("TF", "FT")):
+        B = oracle.boundary(3, nV, T, bnd)
+        off, idx = oracle.coboundary(3, nV, T, cob)      # rows = sub-simplices, entries = containing simplices
+        pairs_b = {(int(x), r) for r, row in enumerate(B.tolist()) for x in row}
+        pairs_c = {(r, int(x)) for r in range(len(off) - 1) for x in idx[off[r]:off[r + 1]]}
+        assert pairs_b == pairs_c, bnd
+        assert all(len(set(row)) == B.shape[1] for row in B.tolist())    # distinct faces
+    assert oracle.boundary(3, nV, T, "TE").shape == (len(T), 6) and oracle.boundary(3, nV, T, "TF").shape == (len(T), 4)
+
+
+def test_boundary_te_2d():
+    m = meshgen.make_mesh(2, 9, clustering="octree", capacity=30, seed=2)
+    te = oracle.boundary(2, m.num_vertices, m.simplices, "TE")
+    E = oracle.sub_simplices(2, m.num_vertices, m.simplices, 2)["list"]
+    for t, row in zip(m.simplices.tolist(), te.tolist()):   # brute force: position of each pair in the sorted edge list
+        assert [E[e].tolist() for e in row] == [[t[0], t[1]], [t[0], t[2]], [t[1], t[2]]]
