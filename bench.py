@@ -225,6 +225,8 @@ def main():
     ap.add_argument("--impl", default="gale", choices=["gale", "reference"])
     ap.add_argument("--canonicalize", action="store_true",
                     help="also time gale_canonicalize (SURVEY §8(f)-1) on a device-scrambled copy of the simplices; reported in config")
+    ap.add_argument("--boundary", action="store_true",
+                    help="also time the boundary look-ups FE / TE / TF over the whole mesh (builds E and F at create); reported in config")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-depth", type=int, default=3, help="pinned queue slots per handle in the e2e leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -270,11 +272,27 @@ def main():
                        queue_depth=0, device_ring=args.ring, tile_vertices=args.tile,
                        flags={"auto": 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[args.kernel] |
                        (gale.STAGE_FROM_T if args.stage_from_t else 0) |
-                       (gale.WITH_EDGES if args.mask & (gale.REL_VE | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
-                       (gale.WITH_FACETS if args.mask & (gale.REL_VF | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
+                       (gale.WITH_EDGES if args.boundary or args.mask & (gale.REL_VE | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
+                       (gale.WITH_FACETS if (args.boundary and mesh.dim == 3) or args.mask & (gale.REL_VF | gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0) |
                        (gale.WITH_COBOUNDARY if args.mask & (gale.REL_EF | gale.REL_ET | gale.REL_FT) else 0))
     create_s = time.time() - t0
     info = gm.info
+    bnd = None
+    if args.boundary:   # PAPER.md:186-192 look-ups in bulk: one call per relation over every row, CUDA events, best of 3
+        bnd = {}
+        for name, rel, rows in (("TE", gale.BND_TE, mesh.num_simplices),) + ((("TF", gale.BND_TF, mesh.num_simplices),
+                                                                               ("FE", gale.BND_FE, int(info.num_triangles))) if mesh.dim == 3 else ()):
+            best = float("inf")
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                out = gm.boundary(rel, 0, rows)
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+            bnd[name] = {"rows": rows, "ms": best, "entries_per_s": rows * out.shape[1] / (best * 1e-3)}
+            del out
+        torch.cuda.empty_cache()
     stream = torch.cuda.current_stream()
     # batches are independent (disjoint result slots): submitting them on several streams in turn lets the
     # draining tail of one launch (8,192 blocks = 3.7 waves of resident blocks) overlap the next launch
@@ -509,7 +527,8 @@ def main():
                                                        "block_threads": info.block_threads, "relation_mask": args.mask,
                                                        "index_bytes": info.index_bytes, "workspace_used": info.workspace_used,
                                                        "mesh_bytes": int(mesh.simplices.nbytes),
-                                                       **({"canonicalize": canon} if canon else {})}),
+                                                       **({"canonicalize": canon} if canon else {}),
+                                                       **({"boundary": bnd} if bnd else {})}),
                 "clocks": clocks, "sustained": sustained, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu}
         if cons is not None:

@@ -251,6 +251,21 @@ int32_t gale_mesh_tile(const gale_mesh_t *mesh, int32_t tile, gale_tile_view_t *
  * [I[lo], I[hi]). */
 int32_t gale_mesh_interval_array(const gale_mesh_t *mesh, const int32_t **d_first_simplex);
 
+/* Boundary relations FE, TE, TF (Table 1 :53-58) by the look-up of PAPER.md:186-192: "retrieve the
+ * boundary vertices ... locate edge indices through the edge list E with limiting the search range by the edge
+ * interval array I_E" — one interval-bounded binary search per face, on the device, for a range of rows:
+ *   GALE_BND_FE  rows = triangles [first_id, first_id + count) of F, 3 edge ids each          (dim 3, E and F built)
+ *   GALE_BND_TE  rows = simplices of T, 6 edge ids each (3 for a triangle mesh)               (E built)
+ *   GALE_BND_TF  rows = simplices of T, 4 triangle ids each                                   (dim 3, F built)
+ * Entry j of a row is the j-th vertex combination in lexicographic order ((v0,v1), (v0,v2), .. — the order of the
+ * paper's example FE(f5) = (v0,v3), (v0,v4), (v3,v4)). The remaining boundary relations are the lists themselves
+ * (EV = gale_mesh_edges, FV = gale_mesh_triangles, TV = the caller's simplices).
+ *   d_out  DEVICE int32[count * width], caller-owned; written in stream order on cuda_stream (asynchronous)
+ * Errors: GALE_ERR_INVALID_ARG (relation, range), GALE_ERR_UNSUPPORTED (list not built), GALE_ERR_CUDA. */
+enum { GALE_BND_FE = 1, GALE_BND_TE = 2, GALE_BND_TF = 3 };
+int32_t gale_boundary_lookup(gale_mesh_t *mesh, int32_t relation, int64_t first_id, int64_t count, int32_t *d_out,
+                             void *cuda_stream);
+
 /* The sorted edge list E with its interval array, when built: the edges whose lowest vertex
  * is a are the ids [d_first[a], d_first[a+1]) and d_upper[id] is their other vertex (ascending). DEVICE
  * memory owned by the library, valid as long as the handle. GALE_ERR_UNSUPPORTED when not built. */

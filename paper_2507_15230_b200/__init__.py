@@ -72,7 +72,7 @@ class gale_tile_view_t(ctypes.Structure):
                 ("d_external", ctypes.c_void_p), ("d_local_to_global", ctypes.c_void_p)]
 
 
-EXPORTS = ["gale_canonicalize", "gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+EXPORTS = ["gale_canonicalize", "gale_boundary_lookup", "gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
            "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
@@ -101,6 +101,8 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
     vp = ctypes.c_void_p
     lib.gale_canonicalize.restype = ctypes.c_int32
     lib.gale_canonicalize.argtypes = [ctypes.c_int32, ctypes.c_int64, ctypes.c_int32, vp, vp, vp, vp]
+    lib.gale_boundary_lookup.restype = ctypes.c_int32
+    lib.gale_boundary_lookup.argtypes = [vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, vp, vp]
     lib.gale_plan_create.restype = ctypes.c_int32
     lib.gale_plan_create.argtypes = [ctypes.POINTER(gale_mesh_desc_t), vp, ctypes.POINTER(vp)]
     lib.gale_plan_workspace_bytes.restype = ctypes.c_int32
@@ -170,6 +172,14 @@ def canonicalize(dim: int, num_vertices: int, simplices, want_perm: bool = True)
     gale_canonicalize(dim, t.shape[0], num_vertices, t.data_ptr(), out.data_ptr(), perm.data_ptr() if want_perm else 0,
                       torch.cuda.current_stream().cuda_stream)
     return out, perm
+
+
+BND_FE, BND_TE, BND_TF = 1, 2, 3
+
+
+def gale_boundary_lookup(handle, relation: int, first_id: int, count: int, d_out: int, cuda_stream: int = 0) -> None:
+    _check(load_library().gale_boundary_lookup(handle, relation, first_id, count, ctypes.c_void_p(d_out or None),
+                                               ctypes.c_void_p(cuda_stream)), "gale_boundary_lookup")
 
 
 def gale_plan_create(desc: gale_mesh_desc_t, cuda_stream: int = 0) -> ctypes.c_void_p:
@@ -388,6 +398,15 @@ class GaleMesh:
                 host[k] = v
         self.release(view)
         return host
+
+    def boundary(self, relation: int, first_id: int, count: int):
+        """FE / TE / TF rows [first_id, first_id + count) as a CUDA int32 tensor [count, width] (marshalling only)."""
+        import torch
+
+        width = 4 if relation == BND_TF else (3 if relation == BND_FE or self.dim == 2 else 6)
+        out = torch.empty((count, width), dtype=torch.int32, device="cuda")
+        gale_boundary_lookup(self.handle, relation, first_id, count, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        return out
 
     def destroy(self) -> None:
         if getattr(self, "handle", None):

@@ -1223,6 +1223,32 @@ int32_t gale_mesh_triangles(const gale_mesh_t* m, const int32_t** d_first, const
   return GALE_OK;
 }
 
+int32_t gale_boundary_lookup(gale_mesh_t* m, int32_t relation, int64_t first_id, int64_t count, int32_t* d_out, void* cuda_stream) {
+  namespace gs = gale::sub;
+  if (!m || count < 0 || first_id < 0 || (count > 0 && !d_out)) return GALE_ERR_INVALID_ARG;
+  if (relation != GALE_BND_FE && relation != GALE_BND_TE && relation != GALE_BND_TF) return GALE_ERR_INVALID_ARG;
+  const bool need_e = relation != GALE_BND_TF, need_f = relation != GALE_BND_TE;
+  if ((need_e && !m->sub.e_first) || (need_f && !m->sub.f_first)) {
+    g_last_error = "the boundary relation needs the edge / triangle list (GALE_WITH_EDGES / GALE_WITH_FACETS at create)";
+    return GALE_ERR_UNSUPPORTED;
+  }
+  const long long rows = relation == GALE_BND_FE ? m->nF : m->plan->nT;
+  if (first_id + count > rows) return GALE_ERR_INVALID_ARG;
+  if (count == 0) return GALE_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int W = gs::boundary_width(relation, m->D);
+  const long long n = count * W;
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  const int32_t* T = m->dm.T;
+  const int nV = m->plan->nV;
+  if (relation == GALE_BND_FE) gs::k_boundary<gs::BND_FE, 4><<<blocks, 256, 0, st>>>(m->sub, T, nV, first_id, count, d_out);
+  else if (relation == GALE_BND_TF) gs::k_boundary<gs::BND_TF, 4><<<blocks, 256, 0, st>>>(m->sub, T, nV, first_id, count, d_out);
+  else if (m->D == 4) gs::k_boundary<gs::BND_TE, 4><<<blocks, 256, 0, st>>>(m->sub, T, nV, first_id, count, d_out);
+  else gs::k_boundary<gs::BND_TE, 3><<<blocks, 256, 0, st>>>(m->sub, T, nV, first_id, count, d_out);
+  GALE_CUDA(cudaGetLastError());
+  return GALE_OK;
+}
+
 int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const int32_t* h_cluster_ids,
                                    int32_t n_clusters, void* cuda_stream) {
   constexpr uint32_t kCobMask = GALE_REL_EF | GALE_REL_ET | GALE_REL_FT;

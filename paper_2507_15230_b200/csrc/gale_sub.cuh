@@ -482,5 +482,74 @@ k_star(const DeviceMesh M, const SubIndex X, const __grid_constant__ CobParams P
   }
 }
 
+// ---- boundary relations FE / TE / TF by look-up --------------------------------------
+// "Locate edge indices ... through the edge list E with limiting the search range by the edge interval array
+// I_E": the edge (x, y), x < y, lies in the block [e_first[x], e_first[x+1]) of its lower vertex, which ascends
+// with y; likewise a triangle (x, y, z) in the block of x of F, which ascends with (y, z). -1 = not in the list.
+__device__ __forceinline__ int edge_id(const SubIndex& X, int x, int y) {
+  int lo = __ldg(X.e_first + x), hi = __ldg(X.e_first + x + 1);
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(X.e_hi + mid) < y) lo = mid + 1; else hi = mid;
+  }
+  return (lo < __ldg(X.e_first + x + 1) && __ldg(X.e_hi + lo) == y) ? lo : -1;
+}
+__device__ __forceinline__ int triangle_id(const SubIndex& X, int x, int y, int z) {
+  int lo = __ldg(X.f_first + x), hi = __ldg(X.f_first + x + 1);
+  const int end = hi;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    const int2 q = __ldg(X.f_bc + mid);
+    if (q.x < y || (q.x == y && q.y < z)) lo = mid + 1; else hi = mid;
+  }
+  if (lo >= end) return -1;
+  const int2 q = __ldg(X.f_bc + lo);
+  return (q.x == y && q.y == z) ? lo : -1;
+}
+
+enum { BND_FE = 1, BND_TE = 2, BND_TF = 3 };
+__host__ __device__ inline int boundary_width(int kind, int D) { return kind == BND_TF ? 4 : (kind == BND_FE ? 3 : (D == 4 ? 6 : 3)); }
+
+// One thread per output entry: entry j of row r = the j-th vertex combination (lexicographic) of triangle
+// first + r of F (FE) or of simplex first + r of T (TE, TF). out[r * width + j]; coalesced.
+template <int KIND, int D>
+__global__ void k_boundary(const SubIndex X, const int32_t* __restrict__ T, int nV, long long first, long long count, int32_t* out) {
+  constexpr int W = KIND == BND_TF ? 4 : (KIND == BND_FE ? 3 : (D == 4 ? 6 : 3));
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count * W) return;
+  const long long r = e / W;
+  const int j = (int)(e - r * W);
+  const long long id = first + r;
+  int v[4];
+  if constexpr (KIND == BND_FE) {
+    // lowest vertex of triangle id: the vertex whose block of F holds it (last a with f_first[a] <= id)
+    int lo = 0, hi = nV;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if ((long long)__ldg(X.f_first + mid) <= id) lo = mid; else hi = mid;
+    }
+    const int2 q = __ldg(X.f_bc + id);
+    v[0] = lo; v[1] = q.x; v[2] = q.y; v[3] = 0;
+  } else {
+#pragma unroll
+    for (int k = 0; k < D; ++k) v[k] = __ldg(T + id * D + k);
+  }
+  int res;
+  if constexpr (KIND == BND_TF) {
+    // (0,1,2) (0,1,3) (0,2,3) (1,2,3)
+    const int a = j == 3 ? v[1] : v[0], b = j >= 2 ? v[2] : v[1], c = j == 0 ? v[2] : v[3];
+    res = triangle_id(X, a, b, c);
+  } else if (W == 3) {
+    // (0,1) (0,2) (1,2)
+    res = edge_id(X, j == 2 ? v[1] : v[0], j == 0 ? v[1] : v[2]);
+  } else {
+    // (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)
+    const int a = j < 3 ? v[0] : (j < 5 ? v[1] : v[2]);
+    const int b = j == 0 ? v[1] : ((j == 1 || j == 3) ? v[2] : v[3]);
+    res = edge_id(X, a, b);
+  }
+  out[e] = res;
+}
+
 }  // namespace sub
 }  // namespace gale

@@ -152,3 +152,50 @@ def test_ef_et_ft(name, make, batch):
             if b == 0:
                 assert "tt" in g and "ve" in g and "vf" in g
     gm.destroy()
+
+
+BND_CASES = [
+    ("cfg1", lambda: meshgen.make_config(1)),
+    ("holes3d", lambda: meshgen.make_mesh(3, 12, clustering="octree", capacity=200, permute=True, drop_frac=0.15, seed=8)),
+    ("delaunay3d", lambda: meshgen.make_delaunay(3, 1500, seed=41, capacity=300)),
+]
+
+
+@pytest.mark.parametrize("name,make", BND_CASES, ids=[c[0] for c in BND_CASES])
+def test_boundary_relations_fe_te_tf(name, make):
+    """FE / TE / TF by the interval-bounded look-up on the device against the oracle's dictionary
+    look-up in the whole list, every row, plus a ragged sub-range."""
+    import paper_2507_15230_b200 as gale
+
+    m = make()
+    gm = gale.GaleMesh(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=4,
+                       flags=gale.WITH_EDGES | gale.WITH_FACETS)
+    nF = len(oracle.sub_simplices(3, m.num_vertices, m.simplices, 3)["list"])
+    for rel, key, rows in ((gale.BND_FE, "FE", nF), (gale.BND_TE, "TE", len(m.simplices)), (gale.BND_TF, "TF", len(m.simplices))):
+        ref = oracle.boundary(3, m.num_vertices, m.simplices, key)
+        got = gm.boundary(rel, 0, rows).cpu().numpy()
+        assert np.array_equal(got, ref), f"{name}: {key}"
+        lo, n = rows // 3 + 1, min(777, rows - rows // 3 - 1)
+        assert np.array_equal(gm.boundary(rel, lo, n).cpu().numpy(), ref[lo:lo + n])
+        assert gm.boundary(rel, rows, 0).shape[0] == 0
+        with pytest.raises(gale.GaleError) as e:
+            gm.boundary(rel, rows - 1, 2)
+        assert e.value.status == gale.ERR_INVALID_ARG
+    gm.destroy()
+
+
+def test_boundary_te_2d_and_missing_lists():
+    import paper_2507_15230_b200 as gale
+
+    tri = meshgen.make_mesh(2, 30, clustering="octree", capacity=150, drop_frac=0.1, seed=3)
+    gm = gale.GaleMesh(2, tri.num_vertices, tri.simplices, tri.cluster_offsets, max_batch_clusters=4, flags=gale.WITH_EDGES)
+    ref = oracle.boundary(2, tri.num_vertices, tri.simplices, "TE")
+    assert np.array_equal(gm.boundary(gale.BND_TE, 0, len(tri.simplices)).cpu().numpy(), ref)
+    for rel in (gale.BND_FE, gale.BND_TF):
+        with pytest.raises(gale.GaleError) as e:
+            gm.boundary(rel, 0, 1)
+        assert e.value.status == gale.ERR_UNSUPPORTED
+    with pytest.raises(gale.GaleError) as e:
+        gm.boundary(7, 0, 1)
+    assert e.value.status == gale.ERR_INVALID_ARG
+    gm.destroy()
