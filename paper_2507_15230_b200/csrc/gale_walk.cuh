@@ -275,7 +275,11 @@ gale_walk_kernel(const DeviceMesh M, const __grid_constant__ BatchParams P, cons
   mbar_wait(bar, 0);
 
   // ---- P1: VT incidence bits (rows = tile vertices, columns = staged simplices) ---------------
-  for (int s = tid; s < S; s += NT) {
+  // thread t takes the simplices t*K .. t*K+K-1: the lanes of a warp then work K apart in the sorted list, where
+  // simplices rarely share a row — neighbouring simplices (same word of the bitmap, same vertices) would hit
+  // the same address in one atomic instruction
+  const int K1 = (S + NT - 1) / NT;
+  for (int s = tid * K1, s_end = min(S, s + K1); s < s_end; ++s) {
     int l[4];
     load_local<LB>(tets, s, l);
 #if GALE_CHECK_BOUNDS
