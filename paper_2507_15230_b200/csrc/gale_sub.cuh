@@ -522,6 +522,7 @@ __global__ void k_boundary(const SubIndex X, const int32_t* __restrict__ T, int 
   const long long id = first + r;
   int v[4];
   if constexpr (KIND == BND_FE) {
+    // (the three entries of a row repeat this search: the loads of the second and third hit the first's lines)
     // lowest vertex of triangle id: the vertex whose block of F holds it (last a with f_first[a] <= id)
     int lo = 0, hi = nV;
     while (hi - lo > 1) {
