@@ -399,17 +399,28 @@ def main():
         peak, peak_kind = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_kind = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-    traffic = None
+    traffic, issue = None, None
     tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        tj = json.load(open(tpath))
+        traffic = tj.get("dram_bytes_per_launch")
+        # secondary view (the kernel is limited by instruction issue, not by HBM): warp-instructions per
+        # launch from the committed ncu capture of this build / the measured launch time, against 4 issue slots per
+        # SM per cycle at the SM clock sampled during the timed region
+        wi = tj.get("warp_instructions_per_launch")
+        if wi and info.kernel_variant == 1 and args.config == 5 and args.mask == 7 and args.n is None and args.batch == 64 and args.tile in (0, 32):
+            sms = torch.cuda.get_device_properties(0).multi_processor_count
+            mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+            peak_i = sms * 4 * mhz * 1e6
+            issue = {"warp_inst_per_launch": wi, "achieved_ginst_s": wi / (avg_launch_ms * 1e-3) / 1e9,
+                     "peak_ginst_s": peak_i / 1e9, "frac": wi / (avg_launch_ms * 1e-3) / peak_i}
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "kernel": ("gale_walk_kernel" if info.kernel_variant == 1 else "gale_batch_kernel") + f"<{D}>", "peak_kind": peak_kind,
                 "bytes_per_launch": alg_bytes / len(batches), "avg_launch_ms": avg_launch_ms,
                 "avg_launch_ms_is": "CUDA-event time of the timed region / launches in it (2 launches overlap)",
                 "event_launch_ms": event_launch_ms,
                 "step_gbs": alg_bytes / (ms_per_step * 1e-3) / 1e9,
-                "frac_of_8TBs_nominal": achieved / 8000.0}
+                "frac_of_8TBs_nominal": achieved / 8000.0, "issue": issue}
     gm.destroy()
     del gm
 
