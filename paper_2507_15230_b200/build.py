@@ -8,7 +8,7 @@ CSRC = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
 LIB = os.path.join(CSRC, "libgale.so")
 LIB_CHECKED = os.path.join(CSRC, "libgale_checked.so")   # -DGALE_CHECK_BOUNDS=1 (tests/test_gpu_bounds.py)
 SOURCES = ["gale_lib.cu"]
-DEPS = SOURCES + ["gale_kernels.cuh", "gale_walk.cuh", "gale_init.cuh", "gale_sub.cuh", os.path.join("..", "..", "include", "gale.h")]
+DEPS = SOURCES + ["gale_kernels.cuh", "gale_walk.cuh", "gale_init.cuh", "gale_sub.cuh", "gale_canon.cuh", os.path.join("..", "..", "include", "gale.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "170"]
