@@ -198,6 +198,36 @@ typedef struct {
 int32_t gale_canonicalize(int32_t dim, int64_t num_simplices, int32_t num_vertices, const int32_t *d_simplices_in,
                           int32_t *d_simplices_out, int32_t *d_perm_out, void *cuda_stream);
 
+/* gale_canonicalize for callers that must not allocate device memory. Same operation, same arguments, same
+ * results and error codes as gale_canonicalize above — but this entry
+ * never calls cudaMalloc / cudaFree or any library routine that allocates.
+ *
+ * Who needs it: an analysis that runs in situ next to a simulation which has handed all of the GPU's memory to
+ * its own pool (a cudaMalloc from a guest library fails there with out-of-memory although the pool could spare
+ * the room), and a service loop that cannot afford the device-wide synchronisation cudaMalloc / cudaFree imply.
+ * Such callers bring their input and output arrays; what the radix sort needs besides them (the second copy of
+ * the rows, two permutation buffers, the per-segment digit counters, the error flag) lives in ONE array that is
+ * part of the library image itself:
+ *   - it is GALE_CANON_STATIC_SCRATCH_BYTES (about 25 MiB) of device memory on EVERY GPU on which this library's
+ *     kernels get loaded, taken when the library's code is loaded there and held until the process exits, whether
+ *     or not this entry is ever called;
+ *   - it bounds the problem: num_simplices > GALE_CANON_STATIC_MAX_SIMPLICES returns GALE_ERR_WORKSPACE (with a
+ *     text in gale_last_error) before anything is launched; larger lists need gale_canonicalize;
+ *   - every call on a device uses the same array. Two calls whose kernels could overlap on the GPU would corrupt
+ *     each other's sort, so the library holds a process-wide lock from entry until cuda_stream has drained; do not
+ *     call it from a callback that this very stream waits on. The array keeps whatever the last call left in it;
+ *     the one word that has to start at zero (the error flag) is cleared by every call, all other parts are
+ *     fully overwritten before they are read.
+ * The first call on each device (with that device current) looks up the device address of the array and checks the
+ * device's compute capability; make that first call at set-up time, outside any CUDA stream capture. The call
+ * synchronises cuda_stream, like gale_canonicalize. */
+#define GALE_CANON_STATIC_MAX_SIMPLICES (1 << 20)
+#define GALE_CANON_STATIC_SCRATCH_BYTES                                                                             \
+  ((size_t)GALE_CANON_STATIC_MAX_SIMPLICES * (16 + 4 + 4) /* rows, two permutations */                              \
+   + (size_t)(GALE_CANON_STATIC_MAX_SIMPLICES / 2048) * 1024 /* digit counters */ + 512 /* scan sums, error flag */)
+int32_t gale_canonicalize_static(int32_t dim, int64_t num_simplices, int32_t num_vertices, const int32_t *d_simplices_in,
+                                 int32_t *d_simplices_out, int32_t *d_perm_out, void *cuda_stream);
+
 /* Initialization analysis ("Initialization": I_T, the external lists T_ex, interval
  * arrays): reads the simplices from the DEVICE array desc->d_simplices — they must be valid in stream
  * order on cuda_stream — validates them and builds the index on the host side of the library. This is

@@ -72,7 +72,7 @@ class gale_tile_view_t(ctypes.Structure):
                 ("d_external", ctypes.c_void_p), ("d_local_to_global", ctypes.c_void_p)]
 
 
-EXPORTS = ["gale_canonicalize", "gale_boundary_lookup", "gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
+EXPORTS = ["gale_canonicalize", "gale_canonicalize_static", "gale_boundary_lookup", "gale_mesh_edges", "gale_mesh_triangles", "gale_mesh_tile", "gale_mesh_interval_array", "gale_plan_create", "gale_plan_workspace_bytes", "gale_plan_destroy", "gale_mesh_create_planned",
            "gale_mesh_workspace_bytes", "gale_mesh_create", "gale_mesh_info", "gale_cluster_batch_compute",
            "gale_queue_pop", "gale_queue_release", "gale_destroy", "gale_status_string", "gale_last_error"]
 
@@ -101,6 +101,8 @@ def load_library(build_if_missing: bool = False) -> ctypes.CDLL:
     vp = ctypes.c_void_p
     lib.gale_canonicalize.restype = ctypes.c_int32
     lib.gale_canonicalize.argtypes = [ctypes.c_int32, ctypes.c_int64, ctypes.c_int32, vp, vp, vp, vp]
+    lib.gale_canonicalize_static.restype = ctypes.c_int32
+    lib.gale_canonicalize_static.argtypes = [ctypes.c_int32, ctypes.c_int64, ctypes.c_int32, vp, vp, vp, vp]
     lib.gale_boundary_lookup.restype = ctypes.c_int32
     lib.gale_boundary_lookup.argtypes = [vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, vp, vp]
     lib.gale_plan_create.restype = ctypes.c_int32
@@ -171,6 +173,36 @@ def canonicalize(dim: int, num_vertices: int, simplices, want_perm: bool = True)
     perm = torch.empty(t.shape[0], dtype=torch.int32, device=t.device) if want_perm else None
     gale_canonicalize(dim, t.shape[0], num_vertices, t.data_ptr(), out.data_ptr(), perm.data_ptr() if want_perm else 0,
                       torch.cuda.current_stream().cuda_stream)
+    return out, perm
+
+
+CANON_STATIC_MAX_SIMPLICES = 1 << 20   # GALE_CANON_STATIC_MAX_SIMPLICES of include/gale.h
+
+
+def gale_canonicalize_static(dim: int, num_simplices: int, num_vertices: int, d_in: int, d_out: int, d_perm: int = 0,
+                             cuda_stream: int = 0) -> None:
+    """gale_canonicalize for callers that may not allocate device memory (include/gale.h): the library makes no
+    cudaMalloc / cudaFree here, its temporaries sit in a fixed array inside the library image, which limits the
+    call to CANON_STATIC_MAX_SIMPLICES rows (ERR_WORKSPACE beyond). Same pointers, results and errors otherwise."""
+    _check(load_library().gale_canonicalize_static(dim, num_simplices, num_vertices, ctypes.c_void_p(d_in), ctypes.c_void_p(d_out),
+                                                   ctypes.c_void_p(d_perm or None), ctypes.c_void_p(cuda_stream)),
+           "gale_canonicalize_static")
+
+
+def canonicalize_static(dim: int, num_vertices: int, simplices, want_perm: bool = True):
+    """Argument marshalling for gale_canonicalize_static, same shape as `canonicalize`. Note that this helper itself
+    creates the output tensors with torch (the caller's side of the contract: inputs and outputs are the caller's);
+    a caller that really cannot allocate passes pointers it already owns to gale_canonicalize_static directly."""
+    import torch
+
+    t = torch.as_tensor(simplices, dtype=torch.int32)
+    if t.device.type != "cuda":
+        t = t.cuda()
+    t = t.contiguous().reshape(-1, dim + 1)
+    out = torch.empty_like(t)
+    perm = torch.empty(t.shape[0], dtype=torch.int32, device=t.device) if want_perm else None
+    gale_canonicalize_static(dim, t.shape[0], num_vertices, t.data_ptr(), out.data_ptr(), perm.data_ptr() if want_perm else 0,
+                             torch.cuda.current_stream().cuda_stream)
     return out, perm
 
 

@@ -1062,6 +1062,71 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
 }
 }  // namespace
 
+// ---- scratch of gale_canonicalize_static (include/gale.h) ----------------------------------------------------
+// Everything the radix sort of gale_canon.cuh needs besides the caller's input and output, for callers that
+// cannot allocate device memory (an in-situ analysis inside a host application whose pool owns the whole GPU,
+// a loop that cannot take cudaMalloc's device-wide synchronisation). The array is part of the library image:
+// every GPU that loads this library's code holds these ~25 MiB until the process exits. It is never
+// initialised by the library beyond what a call writes, and it keeps the previous call's contents.
+// NOTE for host code in this file: `g_canon_static_scratch` names a host-side stand-in of the symbol, not device
+// memory — kernels must be given the address canon_static_base() obtains with cudaGetSymbolAddress.
+namespace {
+constexpr long long kCanonStaticMaxN = GALE_CANON_STATIC_MAX_SIMPLICES;
+constexpr int kCanonStaticMaxSeg = (int)(kCanonStaticMaxN / gale::canon::kSeg);
+constexpr size_t kCsT1 = 0;                                                   // int32[maxN * 4]  second row buffer
+constexpr size_t kCsP0 = kCsT1 + size_t(kCanonStaticMaxN) * 16;               // int32[maxN]      permutation (no d_perm_out)
+constexpr size_t kCsP1 = kCsP0 + size_t(kCanonStaticMaxN) * 4;                // int32[maxN]      permutation, other side
+constexpr size_t kCsCounts = kCsP1 + size_t(kCanonStaticMaxN) * 4;            // int32[256 * maxSeg]
+constexpr size_t kCsScan = kCsCounts + size_t(gale::canon::kDigits) * kCanonStaticMaxSeg * 4;   // chunk sums of the scan
+constexpr size_t kCsBad = kCsScan + 256;                                      // int: the error flag, cleared per call
+constexpr size_t kCsTotal = kCsBad + 256;
+static_assert(kCanonStaticMaxN % gale::canon::kSeg == 0, "whole segments");
+static_assert((size_t(gale::canon::kDigits) * kCanonStaticMaxSeg / gale::init::kScanChunk + 2) * 4 <= 256, "scan sums fit their slot");
+static_assert(kCsTotal == GALE_CANON_STATIC_SCRATCH_BYTES, "gale.h states the size of the static scratch");
+static_assert(kCsP0 % 256 == 0 && kCsP1 % 256 == 0 && kCsCounts % 256 == 0 && kCsScan % 256 == 0, "256-byte aligned parts");
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_canon_static_scratch[kCsTotal];
+
+namespace {
+constexpr int kCanonStaticMaxDevices = 64;
+std::mutex g_canon_static_mutex;                                  // set-up table AND the calls themselves (one array per device)
+unsigned char* g_canon_static_ptr[kCanonStaticMaxDevices] = {};   // device address of the array, per device ordinal
+
+// Device address of the scratch array on the CURRENT device; resolved once per device (the caller holds the
+// mutex). No allocation: cudaGetSymbolAddress only reports where the module's global lives.
+int canon_static_base(unsigned char** out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    g_last_error = "no CUDA device";
+    return GALE_ERR_UNSUPPORTED;
+  }
+  if (dev < 0 || dev >= kCanonStaticMaxDevices) {
+    g_last_error = "gale_canonicalize_static: device ordinal " + std::to_string(dev) + " beyond the " +
+                   std::to_string(kCanonStaticMaxDevices) + " this entry keeps addresses for";
+    return GALE_ERR_UNSUPPORTED;
+  }
+  if (!g_canon_static_ptr[dev]) {
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
+      cudaGetLastError();
+      g_last_error = "device is not sm_100";
+      return GALE_ERR_UNSUPPORTED;
+    }
+    unsigned char* p = nullptr;
+    GALE_CUDA(cudaGetSymbolAddress((void**)&p, g_canon_static_scratch));
+    if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) {
+      g_last_error = "gale_canonicalize_static: the scratch array has no usable device address";
+      return GALE_ERR_CUDA;
+    }
+    g_canon_static_ptr[dev] = p;
+  }
+  *out = g_canon_static_ptr[dev];
+  return GALE_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char* gale_status_string(int32_t s) {
@@ -1109,6 +1174,44 @@ int32_t gale_canonicalize(int32_t dim, int64_t num_simplices, int32_t num_vertic
   int bad = 0;
   GALE_CUDA(cudaMemcpyAsync(&bad, B.bad, 4, cudaMemcpyDeviceToHost, st));
   GALE_CUDA(cudaStreamSynchronize(st));  // the temporaries are released on return
+  if (bad) { g_last_error = "a simplex names a vertex outside [0, num_vertices) or repeats one"; return GALE_ERR_DEGENERATE; }
+  return GALE_OK;
+}
+
+// The same sort with its temporaries in g_canon_static_scratch instead of cudaMalloc'ed buffers (include/gale.h):
+// for callers that cannot allocate. No cudaMalloc / cudaFree / allocating library call on this path. The first
+// call on a device resolves the array's device address (canon_static_base) — do it before any stream capture.
+int32_t gale_canonicalize_static(int32_t dim, int64_t num_simplices, int32_t num_vertices, const int32_t* d_simplices_in,
+                                 int32_t* d_simplices_out, int32_t* d_perm_out, void* cuda_stream) {
+  namespace gc = gale::canon;
+  if ((dim != 2 && dim != 3) || num_simplices < 0 || num_vertices <= 0) return GALE_ERR_INVALID_ARG;
+  if (num_simplices > kCanonStaticMaxN) {   // checked before any pointer or device is looked at
+    g_last_error = "gale_canonicalize_static: num_simplices " + std::to_string((long long)num_simplices) +
+                   " exceeds GALE_CANON_STATIC_MAX_SIMPLICES (" + std::to_string(kCanonStaticMaxN) +
+                   "), the capacity of the library's built-in scratch; use gale_canonicalize";
+    return GALE_ERR_WORKSPACE;
+  }
+  if (num_simplices > 0 && (!d_simplices_in || !d_simplices_out || d_simplices_in == d_simplices_out)) return GALE_ERR_INVALID_ARG;
+  // one array per device shared by every call: nobody else may be sorting in it while this call's kernels run
+  std::lock_guard<std::mutex> lock(g_canon_static_mutex);
+  unsigned char* base = nullptr;
+  int rc = canon_static_base(&base);
+  if (rc != GALE_OK) return rc;
+  if (num_simplices == 0) return GALE_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const long long n = num_simplices;
+  gc::Buffers B;
+  B.T[0] = d_simplices_out; B.T[1] = reinterpret_cast<int32_t*>(base + kCsT1);
+  B.perm[0] = d_perm_out ? d_perm_out : reinterpret_cast<int32_t*>(base + kCsP0);
+  B.perm[1] = reinterpret_cast<int32_t*>(base + kCsP1);
+  B.counts = reinterpret_cast<int32_t*>(base + kCsCounts);   // every (digit, segment) counter is written by k_count
+  B.scratch = reinterpret_cast<int32_t*>(base + kCsScan);    // every chunk sum is written by k_scan_sums
+  B.bad = reinterpret_cast<int*>(base + kCsBad);             // only ever set by the kernels: must start at zero
+  GALE_CUDA(cudaMemsetAsync(B.bad, 0, 4, st));
+  GALE_CUDA(dim == 3 ? gc::canonicalize<4>(d_simplices_in, n, num_vertices, B, st) : gc::canonicalize<3>(d_simplices_in, n, num_vertices, B, st));
+  int bad = 0;
+  GALE_CUDA(cudaMemcpyAsync(&bad, B.bad, 4, cudaMemcpyDeviceToHost, st));
+  GALE_CUDA(cudaStreamSynchronize(st));  // the scratch is free for the next call once this returns
   if (bad) { g_last_error = "a simplex names a vertex outside [0, num_vertices) or repeats one"; return GALE_ERR_DEGENERATE; }
   return GALE_OK;
 }
