@@ -42,6 +42,7 @@ class RelationServer:
         self.store_cap = int(store_clusters)
         self.cv = threading.Condition()
         self.stop = False
+        self.error = None                                                  # the exception that ended the leader, if any
         self.stats = dict(requests=0, hits=0, launches=0, clusters_computed=0, lookahead_used=0,
                           queue_lengths=[], enqueue_ms=0.0, in_queue_ms=0.0, prep_ms=0.0, kernel_ms=0.0, d2h_ms=0.0,
                           integrate_ms=0.0)
@@ -68,21 +69,45 @@ class RelationServer:
             self.queues[relation].append(req)                               # push under the lock
             self.stats["enqueue_ms"] += 1e3 * (time.perf_counter() - t0)
             self.cv.notify_all()
-            while req["result"] is None and not self.stop:                  # the semaphore of the paper
+            while req["result"] is None and req.get("error") is None and not self.stop:   # the semaphore of the paper
                 self.cv.wait(0.05)
             if req["result"] is None:
+                err = req.get("error") or self.error
+                if err is not None:                                         # the leader producer failed: every waiter learns why
+                    raise RuntimeError(f"RelationServer: the leader producer failed: {err!r}") from err
                 raise RuntimeError("RelationServer stopped")
             return req["result"]
 
     # ---- leader producer -------------------------------------------------------------------------------
     def _lead(self):
+        """Leader thread: serves until close(). A failing backend (a GaleError from compute / pop, anything else) must
+        not leave consumers asleep: the exception is handed to every pending request, the server stops, and get()
+        re-raises it in the consumers' threads."""
+        work = {}
+        try:
+            self._serve(work)
+        except BaseException as e:   # noqa: BLE001 - handed over to the consumers, not swallowed
+            with self.cv:
+                self.error = e
+                self.stop = True
+                for reqs in work.values():
+                    for rq in reqs:
+                        if rq["result"] is None:
+                            rq["error"] = e
+                for q in self.queues.values():
+                    for rq in q:
+                        rq["error"] = e
+                    q.clear()
+                self.cv.notify_all()
+
+    def _serve(self, work):
         while True:
+            work.clear()
             with self.cv:
                 while not self.stop and not any(self.queues.values()):
                     self.cv.wait(0.05)
                 if self.stop:
                     return
-                work = {}
                 for r, q in self.queues.items():                            # pop ALL pending requests (PAPER.md:224)
                     if q:
                         self.stats["queue_lengths"].append(len(q))
@@ -114,12 +139,20 @@ class RelationServer:
                         self.store[r][c] = res
                         if c not in asked:
                             self._lookahead_pending[r].add(c)
+                    # hand the results over BEFORE discarding: a requested cluster that an earlier look-ahead had
+                    # already cached is not in `results`, and a small store may evict it in this very pass
+                    for rq in reqs:
+                        c = rq["cluster"]
+                        res = results.get(c)
+                        if res is None:
+                            res = self.store[r].get(c)
+                        if res is None:
+                            raise RuntimeError(f"no result for relation {r} of cluster {c}")
+                        rq["result"] = res
+                        self.stats["in_queue_ms"] += 1e3 * (now - rq["t_push"])
                     while len(self.store[r]) > self.store_cap:               # compute and discard
                         old, _ = self.store[r].popitem(last=False)
                         self._lookahead_pending[r].discard(old)
-                    for rq in reqs:
-                        rq["result"] = results.get(rq["cluster"], self.store[r].get(rq["cluster"]))
-                        self.stats["in_queue_ms"] += 1e3 * (now - rq["t_push"])
                     self.cv.notify_all()
 
     def close(self):

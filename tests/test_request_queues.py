@@ -77,6 +77,83 @@ def test_leader_pops_all_pending_requests():
     srv.close()
 
 
+def test_failing_backend_wakes_every_consumer_with_the_error():
+    """A backend error (e.g. a GaleError from compute / pop) ends the leader; nobody may stay asleep in get()."""
+    import time
+
+    class Boom(RuntimeError):
+        pass
+
+    def backend(mask, ids):
+        time.sleep(0.2)                                  # let more requests pile up behind the one being served
+        raise Boom("device guard fired")
+
+    srv = RelationServer(backend, 16, lookahead=2)
+    errors = {}
+
+    def consumer(c):
+        try:
+            srv.get(1, c)
+        except RuntimeError as e:
+            errors[c] = e
+
+    ts = [threading.Thread(target=consumer, args=(c,), daemon=True) for c in (0, 5, 9)]
+    ts[0].start()
+    time.sleep(0.05)
+    for t in ts[1:]:
+        t.start()
+    for t in ts:
+        t.join(10)
+        assert not t.is_alive()                          # the served request AND the queued ones woke up
+    assert sorted(errors) == [0, 5, 9]
+    for e in errors.values():
+        assert isinstance(e.__cause__, Boom) and "device guard fired" in str(e)
+    with pytest.raises(RuntimeError, match="device guard fired"):   # later requests fail at once, too
+        srv.get(2, 1)
+    srv.close()
+
+
+def test_store_smaller_than_the_lookahead_window():
+    """store_clusters < lookahead x consumers: a request whose cluster an earlier look-ahead cached while it waited
+    in the queue is served from the store — and must be served before that pass evicts the cluster again."""
+    import time
+
+    m = meshgen.make_config(3, n=24)
+    nC = m.num_clusters
+    assert nC >= 6
+    log, gate = [], threading.Event()
+
+    def slow_backend(mask, ids):
+        gate.wait(5)
+        return _oracle_backend(m, log)(mask, ids)
+
+    srv = RelationServer(slow_backend, nC, lookahead=2, store_clusters=1)
+    ref = oracle.cluster_results(m.dim, m.num_vertices, m.simplices, m.cluster_offsets, range(nC), mask=1)
+    out = {}
+
+    def consumer(c):
+        out[c] = srv.get(1, c)
+
+    first = threading.Thread(target=consumer, args=(0,), daemon=True)
+    first.start()
+    time.sleep(0.2)                                      # the leader is computing clusters 0, 1 for request 0
+    rest = [threading.Thread(target=consumer, args=(c,), daemon=True) for c in (1, 4)]   # 1 is not in the store yet: queued
+    for t in rest:
+        t.start()
+    time.sleep(0.2)
+    gate.set()
+    for t in [first] + rest:
+        t.join(10)
+        assert not t.is_alive()
+    # second pass: 1 was cached by the first (the store keeps {1}), so only its look-ahead and 4's window are
+    # computed; storing those three evicts 1 in the same pass
+    assert [ids for _, ids in log] == [[0, 1], [2, 4, 5]]
+    assert 1 not in srv.store[1] and len(srv.store[1]) == 1
+    for c in (0, 1, 4):
+        assert _same(out[c], ref[c]["vt"])
+    srv.close()
+
+
 @pytest.mark.gpu
 def test_request_queues_over_the_c_abi():
     import paper_2507_15230_b200 as gale
