@@ -78,9 +78,10 @@ enum {
   GALE_WITH_FACETS = 128u,     /* ... and the sorted triangle list F with I_F; enables GALE_REL_VF (dim = 3)  */
   GALE_WITH_COBOUNDARY = 256u, /* with GALE_WITH_EDGES | GALE_WITH_FACETS (dim = 3): also size EF / ET / FT and reserve
                                   room for them in the result slots; enables GALE_REL_EF / _ET / _FT          */
-  GALE_STAGE_FROM_T = 32u,     /* dense kernel only (implies nothing for the walk kernel): stage the rows of T
-                                  and T_ex themselves and derive the tile-local ids in the kernel instead of
-                                  reading the create-time re-encoding; slower, kept for the A/B in DESIGN.md */
+  GALE_STAGE_FROM_T = 32u,     /* stage the rows of T and T_ex themselves and derive the tile-local ids in the
+                                  kernel instead of reading the create-time re-encoding; only the dense kernel
+                                  can, so the flag selects it (as GALE_KERNEL_DENSE does; with GALE_KERNEL_WALK:
+                                  GALE_ERR_INVALID_ARG); slower, kept for the A/B in DESIGN.md              */
   GALE_STREAM_ORDERED = 4u     /* run every batch kernel on the cuda_stream passed to compute itself
                                   (plain stream order: work the caller enqueues afterwards runs after
                                   the batch) instead of on the library's two overlapping launch streams */
@@ -91,7 +92,9 @@ typedef struct {
   int32_t num_vertices;
   int64_t num_simplices;            /* every simplex id must fit int32                                */
   const int32_t *d_simplices;       /* DEVICE, [num_simplices*(dim+1)], canonical, 16-byte aligned;
-                                       caller-owned, must outlive the handle, never written          */
+                                       caller-owned, must outlive the handle, never written by the
+                                       library; its CONTENTS must not change while the handle lives
+                                       (see gale_plan_create)                                         */
   int32_t num_clusters;
   const int32_t *h_cluster_offsets; /* HOST, [num_clusters+1], I_V: 0 = o[0] <= ... <= o[nC] = nV;
                                        read during create only                                       */
@@ -230,10 +233,16 @@ int32_t gale_canonicalize_static(int32_t dim, int64_t num_simplices, int32_t num
 
 /* Initialization analysis ("Initialization": I_T, the external lists T_ex, interval
  * arrays): reads the simplices from the DEVICE array desc->d_simplices — they must be valid in stream
- * order on cuda_stream — validates them and builds the index on the host side of the library. This is
- * the expensive part of creating a handle (seconds on a 100 M-tet mesh); d_workspace / workspace_bytes of
- * the descriptor are ignored. *out is owned by the caller until it is passed to
- * gale_mesh_create_planned or gale_plan_destroy. */
+ * order on cuda_stream — validates them and builds the index with device kernels (csrc/gale_init.cuh) in
+ * memory the library allocates and owns until the plan is consumed; the simplices never leave the GPU
+ * (exception: GALE_VALIDATE_MANIFOLD checks C4 on a host copy). This is the expensive part of creating a
+ * handle (about a third of a second for a 100 M-tet mesh on a warm context; the first CUDA call of a process
+ * adds its context and module load); d_workspace / workspace_bytes of the descriptor are ignored. *out is
+ * owned by the caller until it is passed to gale_mesh_create_planned or gale_plan_destroy.
+ * The index is a digest of the VALUES of d_simplices at this moment: from here until gale_destroy the
+ * array's contents are frozen. The batch kernels read the index, not the array (only the cross-cluster TT
+ * look-ups and gale_boundary_lookup read it), so overwriting it with another mesh is not detected and
+ * yields results of the old mesh, or garbage; a new mesh needs a new plan and a new handle. */
 int32_t gale_plan_create(const gale_mesh_desc_t *desc, void *cuda_stream, gale_plan_t **out);
 
 /* Exact device workspace (index + result slots) a handle built from this plan needs. Cheap. */
@@ -315,13 +324,17 @@ int32_t gale_mesh_triangles(const gale_mesh_t *mesh, const int32_t **d_first, co
  * before the batches using them have been popped (gale_destroy drains them).
  * With GALE_STREAM_ORDERED in desc->flags the kernels run on cuda_stream itself: plain stream order,
  * later work on that stream sees the device slot complete (no overlap between consecutive batches).
- * Asynchronous w.r.t. the host. Returns GALE_ERR_WOULD_BLOCK when all slots are un-released. */
+ * Asynchronous w.r.t. the host. Returns GALE_ERR_WOULD_BLOCK when all slots are un-released.
+ * The results describe the mesh as it was at create: the simplex array must still hold the same values. */
 int32_t gale_cluster_batch_compute(gale_mesh_t *mesh, uint32_t relation_mask, const int32_t *h_cluster_ids,
                                    int32_t n_clusters, void *cuda_stream);
 
 /* Consumer side (PAPER.md:158 "signals the consumer", :194: the consumer blocks until its relation is
  * there): wait (up to timeout_ms; < 0 = forever) for the oldest submitted batch and describe it in *out. Batches pop in submission order. GALE_ERR_EMPTY if nothing is in flight,
- * GALE_ERR_WOULD_BLOCK on timeout, GALE_ERR_WORKSPACE if a device-side capacity guard fired. */
+ * GALE_ERR_WOULD_BLOCK on timeout. GALE_ERR_WORKSPACE: a device-side capacity guard fired in this or another batch
+ * of the handle; the batch IS popped and *out describes it (contents unspecified) — release it like any other view.
+ * The condition is latched: every later pop of the handle reports it the same way, so a consumer loop must treat
+ * any status other than GALE_OK / GALE_ERR_WOULD_BLOCK / GALE_ERR_EMPTY as fatal, drain and destroy the handle. */
 int32_t gale_queue_pop(gale_mesh_t *mesh, gale_batch_view_t *out, int32_t timeout_ms);
 
 /* Give a popped slot back to the queue (the relation buffers are pre-allocated and reused,

@@ -299,11 +299,16 @@ def gale_cluster_batch_compute(handle, relation_mask: int, cluster_ids, cuda_str
 
 
 def gale_queue_pop(handle, timeout_ms: int = -1):
-    """Returns (status, view); status is OK, ERR_EMPTY or ERR_WOULD_BLOCK; other errors raise."""
+    """Returns (status, view); status is OK, ERR_EMPTY or ERR_WOULD_BLOCK; other errors raise. ERR_WORKSPACE (a device
+    capacity guard fired, include/gale.h) still pops the batch: its slot is given back here before raising."""
     view = gale_batch_view_t()
-    st = load_library().gale_queue_pop(handle, ctypes.byref(view), timeout_ms)
+    lib = load_library()
+    st = lib.gale_queue_pop(handle, ctypes.byref(view), timeout_ms)
     if st not in (OK, ERR_EMPTY, ERR_WOULD_BLOCK):
-        _check(st, "gale_queue_pop")
+        detail = lib.gale_last_error().decode()
+        if st == ERR_WORKSPACE:
+            lib.gale_queue_release(handle, ctypes.byref(view))
+        raise GaleError(st, "gale_queue_pop", detail)
     return st, view
 
 

@@ -85,10 +85,22 @@ def run_critical_points(mesh, scalar: np.ndarray, *, consumers: int = 4, batch: 
     lock, pop_lock = threading.Lock(), threading.Lock()
     state = dict(submitted=0, done=False, popped=0)
 
+    failed = []                                         # first exception of any thread: everybody stops, the caller gets it
+
+    def guarded(body):
+        def run():
+            try:
+                body()
+            except BaseException as e:   # noqa: BLE001 - re-raised in the calling thread after the join
+                failed.append(e)
+        return run
+
     def producer():
         for ids in batches:
             t0 = time.perf_counter()
             while gm.compute(ids, gale.REL_VT | gale.REL_VV) == gale.ERR_WOULD_BLOCK:
+                if failed:
+                    return
                 time.sleep(0.0002)                      # bounded queue: back-pressure until a consumer releases
             with lock:
                 stage["enqueue_ms"] += 1e3 * (time.perf_counter() - t0)
@@ -97,10 +109,12 @@ def run_critical_points(mesh, scalar: np.ndarray, *, consumers: int = 4, batch: 
 
     def consumer():
         while True:
+            if failed:
+                return
             with pop_lock:                              # one popping thread at a time (boundary contract)
                 if state["done"] and state["popped"] >= len(batches):
                     return
-                st, v = gm.pop(20)
+                st, v = gm.pop(20)                      # OK / WOULD_BLOCK / EMPTY; anything else raises (fatal)
                 if st == gale.OK:
                     state["popped"] += 1
             if st != gale.OK:
@@ -125,13 +139,18 @@ def run_critical_points(mesh, scalar: np.ndarray, *, consumers: int = 4, batch: 
             gm.release(v)
 
     t0 = time.perf_counter()
-    th = [threading.Thread(target=producer)] + [threading.Thread(target=consumer) for _ in range(max(1, consumers))]
+    th = [threading.Thread(target=guarded(producer))] + [threading.Thread(target=guarded(consumer)) for _ in range(max(1, consumers))]
     for t in th:
         t.start()
     for t in th:
         t.join()
     wall = time.perf_counter() - t0
     info = gm.info
+    if failed:
+        try:
+            gm.destroy()
+        finally:
+            raise failed[0]
     gm.destroy()
     hist = np.bincount(types, minlength=4)
     return dict(minima=int(hist[MINIMUM]), maxima=int(hist[MAXIMUM]), saddles=int(hist[SADDLE]), regular=int(hist[REGULAR]),

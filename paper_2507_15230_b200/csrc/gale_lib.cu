@@ -540,7 +540,8 @@ int check_desc(const gale_mesh_desc_t* d) {
       (d->flags & ~uint32_t(GALE_VALIDATE | GALE_VALIDATE_MANIFOLD | GALE_STREAM_ORDERED | GALE_KERNEL_DENSE | GALE_KERNEL_WALK | GALE_STAGE_FROM_T | GALE_WITH_EDGES | GALE_WITH_FACETS | GALE_WITH_COBOUNDARY)) ||
       ((d->flags & GALE_WITH_FACETS) && d->dim != 3) ||
       ((d->flags & GALE_WITH_COBOUNDARY) && (d->flags & (GALE_WITH_EDGES | GALE_WITH_FACETS)) != (GALE_WITH_EDGES | GALE_WITH_FACETS)) ||
-      (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK))
+      (d->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK)) == (GALE_KERNEL_DENSE | GALE_KERNEL_WALK) ||
+      (d->flags & (GALE_STAGE_FROM_T | GALE_KERNEL_WALK)) == (GALE_STAGE_FROM_T | GALE_KERNEL_WALK))  // the walk kernel cannot stage from T
     return GALE_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d->d_simplices) % 16) return GALE_ERR_INVALID_ARG;
   return GALE_OK;
@@ -725,14 +726,13 @@ void launch_star(const gale_mesh* m, int kind, int grid, const gale::sub::CobPar
 #undef GALE_STAR
 }
 int star_allow_smem() {
+  // set on every create, for the device that is current: a cached "done" would leave a second device (or a new
+  // context) without the attribute, and k_star launches with more than 48 KB would fail there
   namespace gs = gale::sub;
-  static bool done = false;
-  if (done) return GALE_OK;
 #define GALE_ATTR(K) GALE_CUDA(cudaFuncSetAttribute(gs::k_star<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048)); \
                      GALE_CUDA(cudaFuncSetAttribute(gs::k_star<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit - 2048))
   GALE_ATTR(gs::COB_ET); GALE_ATTR(gs::COB_FT); GALE_ATTR(gs::COB_EF); GALE_ATTR(gs::COB_VF);
 #undef GALE_ATTR
-  done = true;
   return GALE_OK;
 }
 
@@ -1024,7 +1024,8 @@ int build_mesh(std::unique_ptr<Plan> p, void* d_workspace, size_t workspace_byte
     GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb, false), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
     GALE_CUDA(cudaFuncSetAttribute(walk_kernel_for(m->D, p->w_NT, p->cfg.lb, true), cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit));
   }
-  const uint32_t force = p->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK);
+  uint32_t force = p->flags & (GALE_KERNEL_DENSE | GALE_KERNEL_WALK);
+  if (p->flags & GALE_STAGE_FROM_T) force = GALE_KERNEL_DENSE;  // only the dense kernel can stage from T: the flag selects it
   const bool may_walk = p->walk_ok;
   m->plan = std::move(p);
   if (force == GALE_KERNEL_WALK && !may_walk) { g_last_error = "the walk kernel cannot run these tiles (capacity limits)"; return GALE_ERR_UNSUPPORTED; }
@@ -1461,8 +1462,8 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
     GALE_CUDA(cudaStreamWaitEvent(run, s.ev_submit, 0));
   }
   GALE_CUDA(cudaEventRecord(s.ev_start, run));
-  for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
-    gale::BatchParams P{};
+  // descriptor of the launch that covers the clusters [b, b + nb) of the batch (<= kMaxBatch per launch)
+  auto fill_params = [&](int b, gale::BatchParams& P) -> int {
     const int nb = std::max(0, std::min(gale::kMaxBatch, n_clusters - b));
     P.n_clusters = nb; P.mask = relation_mask;
     P.total_rows = int(s.rows); P.total_vt_nnz = int(s.vt_nnz); P.total_vv_nnz = int(s.vv_nnz);
@@ -1481,10 +1482,23 @@ int32_t gale_cluster_batch_compute(gale_mesh_t* m, uint32_t relation_mask, const
       for (int i = 0; i < nb && uniform; ++i) uniform = P.tile_prefix[i + 1] - P.tile_prefix[i] == per;
       P.uniform_tiles = uniform ? per : 0;
     }
+    return nb;
+  };
+  // First the VT / VV / TT rows of the WHOLE batch, launch by launch; only then the relations read off them. A row's
+  // end is the next row's offset, and the next row may belong to the following launch: a VE / VF / EF / ET / FT launch
+  // issued right after "its" batch-kernel launch would read the offset at the seam before anybody has written it.
+  for (int b = 0; b < std::max(1, n_clusters); b += gale::kMaxBatch) {
+    gale::BatchParams P{};
+    const int nb = fill_params(b, P);
     const int grid = std::max(1, P.tile_prefix[nb]);
     if (walk) walk_kernel_for(D, p.w_NT, p.cfg.lb, relation_mask == GALE_REL_ALL)<<<grid, p.w_NT, smem, run>>>(m->dm, P, cfg, wlay, O);
     else kernel_for(D, p.NT, false, p.cfg.lb)<<<grid, p.NT, smem, run>>>(m->dm, P, cfg, lay, O);
     GALE_CUDA(cudaGetLastError());
+  }
+  for (int b = 0; (user_mask & (GALE_REL_VE | GALE_REL_VF | kCobMask)) && b < std::max(1, n_clusters); b += gale::kMaxBatch) {
+    gale::BatchParams P{};
+    const int nb = fill_params(b, P);
+    const int grid = std::max(1, P.tile_prefix[nb]);
     if (nb > 0 && (user_mask & GALE_REL_VE)) {  // VE: a map over the VV rows just written (gale_sub.cuh)
       gale::sub::BatchRows B{};
       B.n_clusters = nb;
@@ -1557,10 +1571,11 @@ int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_m
       std::this_thread::yield();
     }
   }
-  if (*static_cast<volatile int32_t*>(m->h_err) != 0) {
-    g_last_error = "device capacity guard fired: code " + std::to_string(*m->h_err);
-    return GALE_ERR_WORKSPACE;
-  }
+  // A fired capacity guard is latched for the life of the handle (the flag is shared by all batches in flight, so
+  // it cannot be pinned on one of them): the batch is popped all the same — its view must be released like any
+  // other, its contents are unspecified — and this and every later pop report GALE_ERR_WORKSPACE. The queue keeps
+  // moving, nobody spins on a slot that never frees.
+  const int32_t guard = *static_cast<volatile int32_t*>(m->h_err);
   const char* b = m->queue_depth > 0 ? s.pinned : s.dev;
   std::memset(out, 0, sizeof(*out));
   out->sequence = s.seq; out->n_clusters = s.n; out->relation_mask = s.mask; out->dim = m->dim;
@@ -1607,6 +1622,10 @@ int32_t gale_queue_pop(gale_mesh_t* m, gale_batch_view_t* out, int32_t timeout_m
   out->slot = int32_t(seq % (long long)m->slots.size());
   s.state.store(SLOT_POPPED, std::memory_order_release);
   m->popped.store(seq + 1);
+  if (guard != 0) {
+    g_last_error = "device capacity guard fired: code " + std::to_string(guard);
+    return GALE_ERR_WORKSPACE;
+  }
   return GALE_OK;
 }
 

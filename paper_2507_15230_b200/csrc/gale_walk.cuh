@@ -26,7 +26,7 @@
 namespace gale {
 
 struct WalkLayout {
-  int mbar, ctx, tets, texid, gid, ft, cnt, fbq, scan, bmT, bmV, bm_end;
+  int mbar, ctx, tets, texid, gid, fbq, scan, bmT, bmV, bm_end;
   int tbl, ttrow, tt_end;
   int st_vt, st_vv;
   int total;
@@ -47,10 +47,8 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.ctx = o;    o = align16(o + 112);
   L.tets = o;   o = align16(o + c.smax * 4 * c.lb);
   L.texid = o;  o = align16(o + c.sext * 4);
-  L.gid = o;    o = align16(o + c.nloc * 4);
-  L.ft = o;     // (the slice of I_T is read straight from global memory)
-  L.scan = o;   o = align16(o + 36 * 4);   // [0..33) scan scratch, [33] a5 queue length, [34] n_vv
-  L.cnt = o;    // (unused: every thread counts its own row)
+  L.gid = o;    o = align16(o + c.nloc * 4);  // (the slice of I_T is read straight from global memory)
+  L.scan = o;   o = align16(o + 36 * 4);   // [0..33) scan scratch, [33] a5 queue length, [34] n_vv; every thread counts its own row
   // VT bitmap (P1-P3); afterwards the same bytes hold the VV staging area (written in P4) and the
   // fallback queue (written in P5)
   L.bmT = o;
@@ -70,12 +68,6 @@ __host__ __device__ inline WalkLayout make_walk_layout(const SmemCfg& c) {
   L.total = o;
   return L;
 }
-
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
 // Barrier among the `count` threads that name the same id (ids 1..15; 0 is __syncthreads).
 __device__ __forceinline__ void named_barrier(int id, int count) {

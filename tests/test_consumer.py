@@ -94,6 +94,55 @@ def test_linear_function_on_a_convex_grid_has_one_minimum_one_maximum_no_saddle(
     assert got[np.argmin(f)] == consumer.MINIMUM and got[np.argmax(f)] == consumer.MAXIMUM
 
 
+def test_run_critical_points_stops_and_raises_when_the_queue_fails(monkeypatch):
+    """A fatal pop status (e.g. GALE_ERR_WORKSPACE after a device guard fired) must end the run with the error,
+    not leave the producer spinning on back-pressure and the other consumers polling an empty queue (no GPU:
+    the handle is a stand-in whose queue fails after the second submitted batch)."""
+    import threading
+
+    import paper_2507_15230_b200 as gale
+
+    made = []
+
+    class FailingMesh:
+        info = None
+
+        def __init__(self, *a, **k):
+            self.lock, self.submitted, self.destroyed = threading.Lock(), 0, False
+            made.append(self)
+
+        def compute(self, ids, mask):
+            with self.lock:
+                if self.submitted >= 2:
+                    return gale.ERR_WOULD_BLOCK          # the bounded queue is full and nothing is ever released
+                self.submitted += 1
+                return gale.OK
+
+        def pop(self, timeout_ms=-1):
+            if self.submitted < 2:
+                return gale.ERR_EMPTY, None
+            raise gale.GaleError(gale.ERR_WORKSPACE, "gale_queue_pop", "device capacity guard fired: code 3")
+
+        def destroy(self):
+            self.destroyed = True
+
+    monkeypatch.setattr(gale, "GaleMesh", FailingMesh)
+    m = meshgen.make_config(1, keep_fields=True)
+    result = {}
+
+    def run():
+        try:
+            consumer.run_critical_points(m, m.scalar, consumers=3, batch=2)
+        except gale.GaleError as e:
+            result["error"] = e
+
+    t = threading.Thread(target=run, daemon=True)
+    t.start()
+    t.join(30)
+    assert not t.is_alive()                              # nobody spins forever
+    assert result["error"].status == gale.ERR_WORKSPACE and made[0].destroyed
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("consumers", [1, 3])
 def test_critical_points_through_the_queue(consumers):

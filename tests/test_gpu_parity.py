@@ -256,3 +256,13 @@ def test_parity_staging_from_t(name, make, batch):
     got, ref, info = _run_all(m, batch, flags=gale.VALIDATE | gale.KERNEL_DENSE | gale.STAGE_FROM_T)
     assert info.kernel_variant == 0
     _compare(got, ref, f"{name} [stage from T]")
+
+
+def test_staging_from_t_selects_the_dense_kernel():
+    """GALE_STAGE_FROM_T alone (no GALE_KERNEL_DENSE): the flag must not become a silent no-op when the create-time
+    timing would have picked the walk kernel (which cannot stage from T)."""
+    gale = _gale()
+    m = meshgen.make_config(1)                      # a regular grid: the walk kernel's home ground
+    got, ref, info = _run_all(m, 8, flags=gale.VALIDATE | gale.STAGE_FROM_T)
+    assert info.kernel_variant == 0 and info.tune_walk_ms == 0.0
+    _compare(got, ref, "cfg1 [stage from T, kernel not named]")

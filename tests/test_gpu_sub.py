@@ -154,6 +154,63 @@ def test_ef_et_ft(name, make, batch):
     gm.destroy()
 
 
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
+def test_batches_larger_than_one_launch(kernel):
+    """A batch of 200 clusters is split over two kernel launches (128 clusters per batch descriptor, gale_lib.cu):
+    the per-launch row / nnz bases of every relation (VT / VV / TT, VE, VF, EF / ET / FT) must continue where the
+    previous launch stopped. 587 small clusters, one of them empty, duplicated ids in the batch, all eight relations
+    at once, three batches (200 + 200 + a ragged one), against the oracle."""
+    import paper_2507_15230_b200 as gale
+
+    m = meshgen.make_mesh(3, 18, clustering="octree", capacity=16, permute=True, drop_frac=0.1, seed=9)
+    T, nV = m.simplices, m.num_vertices
+    off = np.asarray(m.cluster_offsets)
+    off = np.insert(off, 100, off[100]).astype(np.int32)            # cluster 100 owns no vertex
+    nC = len(off) - 1
+    assert nC > 260 and off[100] == off[101]
+    batch = 200
+    flags = gale.VALIDATE | gale.WITH_EDGES | gale.WITH_FACETS | gale.WITH_COBOUNDARY
+    flags |= gale.KERNEL_WALK if kernel == "walk" else gale.KERNEL_DENSE
+    try:
+        gm = gale.GaleMesh(3, nV, T, off, max_batch_clusters=batch, device_ring=2, flags=flags)
+    except gale.GaleError as e:
+        if kernel == "walk" and e.status == gale.ERR_UNSUPPORTED:
+            pytest.skip("walk kernel does not admit this mesh")
+        raise
+    assert gm.info.kernel_variant == (1 if kernel == "walk" else 0)
+    rng = np.random.default_rng(4)
+    ids = [int(c) for c in rng.permutation(nC)]
+    ids[10] = ids[150] = 100                                         # the empty cluster, in both launches of batch 0
+    ids[140] = ids[3]                                                # a duplicate across the launch boundary
+    ids[199] = ids[198]                                              # and inside the second launch
+    E = oracle.sub_simplices(3, nV, T, 2)
+    F = oracle.sub_simplices(3, nV, T, 3)
+    cob = {k: oracle.coboundary(3, nV, T, k.upper()) for k in ("ef", "et", "ft")}
+    first = {"ef": E["first"], "et": E["first"], "ft": F["first"]}
+    mask = gale.REL_ALL | gale.REL_VE | gale.REL_VF | gale.REL_EF | gale.REL_ET | gale.REL_FT
+    for b in range(0, len(ids), batch):
+        chunk = ids[b:b + batch]
+        ref = oracle.cluster_results(3, nV, T, off, chunk)
+        got = gale.split_batch(gm.run_batch(chunk, mask), 4)
+        assert [g["cluster"] for g in got] == chunk
+        for g, r in zip(got, ref):
+            c = g["cluster"]
+            lo, hi = int(off[c]), int(off[c + 1])
+            for k in ("vt", "vv"):
+                assert np.array_equal(g[k][0], r[k][0]) and np.array_equal(g[k][1], r[k][1]), f"{k} of cluster {c}"
+            assert np.array_equal(g["tt"], r["tt"]), f"tt of cluster {c}"
+            o, i = _rows(E, lo, hi)
+            assert np.array_equal(g["ve"][0], o) and np.array_equal(g["ve"][1], i), f"ve of cluster {c}"
+            o, i = _rows(F, lo, hi)
+            assert np.array_equal(g["vf"][0], o) and np.array_equal(g["vf"][1], i), f"vf of cluster {c}"
+            for k in ("ef", "et", "ft"):
+                r0, r1 = int(first[k][lo]), int(first[k][hi])
+                o = cob[k][0][r0:r1 + 1]
+                assert np.array_equal(g[k][0], (o - o[0]).astype(np.int32)), f"{k} offsets of cluster {c}"
+                assert np.array_equal(g[k][1], cob[k][1][o[0]:o[-1]]), f"{k} of cluster {c}"
+    gm.destroy()
+
+
 BND_CASES = [
     ("cfg1", lambda: meshgen.make_config(1)),
     ("holes3d", lambda: meshgen.make_mesh(3, 12, clustering="octree", capacity=200, permute=True, drop_frac=0.15, seed=8)),

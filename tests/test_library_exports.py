@@ -52,6 +52,14 @@ def test_argument_errors_without_gpu(lib):
     assert lib.gale_mesh_workspace_bytes(ctypes.byref(d), None, ctypes.byref(out)) == gale.ERR_INVALID_ARG
     assert lib.gale_destroy(None) == gale.ERR_INVALID_ARG
     assert lib.gale_queue_pop(None, None, 0) == gale.ERR_INVALID_ARG
+    # GALE_STAGE_FROM_T selects the dense kernel; asking for the walk kernel as well is a contradiction
+    import numpy as np
+    off = np.array([0, 5], np.int32)
+    d = gale.gale_mesh_desc_t()
+    d.dim, d.num_vertices, d.num_simplices, d.num_clusters, d.max_batch_clusters = 3, 5, 0, 1, 1
+    d.h_cluster_offsets = off.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+    d.flags = gale.STAGE_FROM_T | gale.KERNEL_WALK
+    assert lib.gale_mesh_workspace_bytes(ctypes.byref(d), None, ctypes.byref(out)) == gale.ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback(lib):
