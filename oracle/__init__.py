@@ -345,3 +345,49 @@ def neighbour_sum(num_vertices: int, vv_off: np.ndarray, vv_idx: np.ndarray, sca
         for u in vv_idx[vv_off[v]:vv_off[v + 1]]:
             out[v] += float(scalar[u])
     return out
+
+
+CP_REGULAR, CP_MINIMUM, CP_SADDLE, CP_MAXIMUM = "regular", "minimum", "saddle", "maximum"
+
+
+def critical_points(dim: int, num_vertices: int, simplices: np.ndarray, scalar: np.ndarray) -> list:
+    """PL critical points of a scalar field on the vertices (the paper's CriticalPoints consumer: it
+    needs VV and VT), written out as the definition: order the vertices by (scalar, id) (ties broken by id); the
+    link of v is spanned by its VV neighbours, two of them adjacent when they share a simplex of VT(v); the lower
+    (upper) link is the part on neighbours below (above) v. v is a minimum when its lower link is empty, a maximum
+    when its upper link is empty, regular when both have exactly one connected component, a saddle otherwise.
+    Components by flood fill over python sets, relations from the oracle's own global VV / VT. Slow on purpose.
+    Pinned in tests/test_consumer.py: a hand-derived example on Fig. 1's two tetrahedra and the closed form for a
+    linear function on a convex grid (one minimum, one maximum, no saddle).
+    Returns a list of CP_* strings, one per vertex."""
+    g = relations_global(dim, num_vertices, simplices, mask=3)
+    T = np.asarray(simplices)
+    f = [float(x) for x in np.asarray(scalar)]
+    out = []
+    for v in range(num_vertices):
+        nb = [int(u) for u in g["vv_idx"][g["vv_off"][v]:g["vv_off"][v + 1]]]
+        lower = {u for u in nb if (f[u], u) < (f[v], v)}
+        adj = {u: set() for u in nb}
+        for t in g["vt_idx"][g["vt_off"][v]:g["vt_off"][v + 1]]:
+            others = [int(u) for u in T[int(t)] if int(u) != v]
+            for a in others:
+                for b in others:
+                    if a != b and ((a in lower) == (b in lower)):
+                        adj[a].add(b)
+        comps = {True: 0, False: 0}
+        seen = set()
+        for u in nb:
+            if u in seen:
+                continue
+            comps[u in lower] += 1
+            seen.add(u)
+            stack = [u]
+            while stack:
+                x = stack.pop()
+                for y in adj[x]:
+                    if y not in seen:
+                        seen.add(y)
+                        stack.append(y)
+        lo, up = comps[True], comps[False]
+        out.append(CP_MINIMUM if lo == 0 else CP_MAXIMUM if up == 0 else CP_REGULAR if (lo, up) == (1, 1) else CP_SADDLE)
+    return out

@@ -37,37 +37,41 @@ def test_neighbour_sum_closed_form_and_oracle():
                        oracle.neighbour_sum(m.num_vertices, g["vv_off"], g["vv_idx"], f), rtol=1e-6)
 
 
-def _naive_types(m, g, f):
-    """Independent classification: components of the lower / upper link by flood fill over python sets."""
-    out = np.zeros(m.num_vertices, np.uint8)
-    T = m.simplices
-    for v in range(m.num_vertices):
-        nb = g["vv_idx"][g["vv_off"][v]:g["vv_off"][v + 1]].tolist()
-        low = {u for u in nb if (f[u], u) < (f[v], v)}
-        adj = {u: set() for u in nb}
-        for t in g["vt_idx"][g["vt_off"][v]:g["vt_off"][v + 1]]:
-            others = [int(u) for u in T[t] if u != v]
-            for a in others:
-                for b in others:
-                    if a != b and ((a in low) == (b in low)):
-                        adj[a].add(b)
-        comps = {True: 0, False: 0}
-        seen = set()
-        for u in nb:
-            if u in seen:
-                continue
-            comps[u in low] += 1
-            stack = [u]
-            seen.add(u)
-            while stack:
-                x = stack.pop()
-                for y in adj[x]:
-                    if y not in seen:
-                        seen.add(y)
-                        stack.append(y)
-        lo, up = comps[True], comps[False]
-        out[v] = consumer.MINIMUM if lo == 0 else consumer.MAXIMUM if up == 0 else consumer.REGULAR if (lo, up) == (1, 1) else consumer.SADDLE
-    return out
+_CODE = {oracle.CP_REGULAR: consumer.REGULAR, oracle.CP_MINIMUM: consumer.MINIMUM, oracle.CP_SADDLE: consumer.SADDLE,
+         oracle.CP_MAXIMUM: consumer.MAXIMUM}
+
+
+def _oracle_types(m, f):
+    """oracle.critical_points (the plain definition: lower / upper link components by flood fill) as the consumer's codes"""
+    return np.array([_CODE[c] for c in oracle.critical_points(m.dim, m.num_vertices, m.simplices, f)], np.uint8)
+
+
+def test_oracle_critical_points_hand_derived_example():
+    """Pin of oracle.critical_points on Fig. 1's mesh (tetrahedra (v0 v1 v2 v3), (v1 v2 v3 v4)) with
+    f = (5, 1, 2, 4, 8), derived by hand:
+      v0 (5): neighbours v1 v2 v3 all lower, one triangle -> upper link empty                      -> maximum
+      v1 (1): neighbours v0 v2 v3 v4 all higher -> lower link empty                                 -> minimum
+      v2 (2): lower {v1}; upper {v0, v3, v4}, v0-v3 share the first simplex, v3-v4 the second: 1+1   -> regular
+      v3 (4): lower {v1, v2} (adjacent); upper {v0, v4}: v0 and v4 share no simplex: 1 + 2          -> saddle
+      v4 (8): neighbours v1 v2 v3 all lower                                                        -> maximum"""
+    m = meshgen.toy_two_tets()
+    got = oracle.critical_points(3, 5, m.simplices, np.array([5.0, 1.0, 2.0, 4.0, 8.0]))
+    assert got == [oracle.CP_MAXIMUM, oracle.CP_MINIMUM, oracle.CP_REGULAR, oracle.CP_SADDLE, oracle.CP_MAXIMUM]
+    # ties are broken by vertex id: with a constant field the order is the id order
+    flat = oracle.critical_points(3, 5, m.simplices, np.zeros(5))
+    assert flat[0] == oracle.CP_MINIMUM and flat[4] == oracle.CP_MAXIMUM and oracle.CP_SADDLE not in flat
+
+
+@pytest.mark.parametrize("dim,n", [(3, 7), (2, 16)])
+def test_oracle_critical_points_linear_function_closed_form(dim, n):
+    """Pin of oracle.critical_points: a linear function on a triangulated convex box has exactly one minimum, one
+    maximum and no saddle (sub-level sets of a linear function on a convex set are convex, hence connected)."""
+    m = meshgen.make_mesh(dim, n, clustering="octree", capacity=200, permute=True, seed=12)
+    pos = np.rint(m.coords).astype(np.float64)
+    f = pos @ np.array([1.0, np.pi, np.e][:dim])
+    got = oracle.critical_points(dim, m.num_vertices, m.simplices, f)
+    assert got.count(oracle.CP_MINIMUM) == 1 and got.count(oracle.CP_MAXIMUM) == 1 and got.count(oracle.CP_SADDLE) == 0
+    assert got[int(np.argmin(f))] == oracle.CP_MINIMUM and got[int(np.argmax(f))] == oracle.CP_MAXIMUM
 
 
 @pytest.mark.parametrize("dim,n", [(3, 6), (2, 9)])
@@ -76,7 +80,7 @@ def test_critical_points_against_naive_enumeration(dim, n):
     g = _global(m)
     f = m.scalar.astype(np.float32)
     got = consumer.critical_points(0, dim + 1, g["vt_off"], g["vt_idx"], g["vv_off"], g["vv_idx"], m.simplices, f)
-    assert np.array_equal(got, _naive_types(m, g, f))
+    assert np.array_equal(got, _oracle_types(m, f))
     assert (got == consumer.SADDLE).any() and (got == consumer.MINIMUM).any()
 
 
