@@ -51,6 +51,18 @@ def _compare(got, ref, what):
 
 @pytest.mark.parametrize("cfg", [2, 3, 4, 5])
 def test_full_size_in_bench_configuration(cfg):
+    _full_size(cfg, None)
+
+
+@pytest.mark.parametrize("kernel", ["dense", "walk"])
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_with_each_kernel(cfg, kernel):
+    """The create-time choice checks one of the two shipped kernels per mesh; here both are forced at full size on the
+    permuted grid (config 3) and on the graded one (config 4, the most diverse tiles), same comparison."""
+    _full_size(cfg, kernel)
+
+
+def _full_size(cfg, kernel):
     import torch
     import paper_2507_15230_b200 as gale
 
@@ -61,7 +73,10 @@ def test_full_size_in_bench_configuration(cfg):
     assert nT == cf["T"] and nV == GRID_N[cfg] ** m.dim
 
     gm = gale.GaleMesh(m.dim, nV, m.simplices, m.cluster_offsets, max_batch_clusters=BATCH, queue_depth=0,
-                       device_ring=4, tile_vertices=0, flags=0)          # exactly bench.py's handle
+                       device_ring=4, tile_vertices=0,                   # exactly bench.py's handle (kernel None)
+                       flags={None: 0, "dense": gale.KERNEL_DENSE, "walk": gale.KERNEL_WALK}[kernel])
+    if kernel is not None:
+        assert gm.info.kernel_variant == (1 if kernel == "walk" else 0)
     assert gm.info.vt_nnz == D * nT                                      # sizes fixed at create
     assert gm.info.vv_nnz == 2 * cf["E"]
 
@@ -169,4 +184,71 @@ def test_edges_triangles_ve_vf_full_size():
         tot_vf += a["vf_indices"].numel()
         gm.release(v)
     assert tot_ve == 2 * nE_cf and tot_vf == 3 * nF_cf
+    gm.destroy()
+
+
+def test_coboundary_and_boundary_relations_full_size():
+    """The rest of SURVEY §8(f)-2 at full size (PAPER.md:309: the relation set of the MS complex; :186-192: the boundary
+    look-up). Config 3 (12.3 M tets, 14.5 M edges, 24.7 M triangles):
+      * EF / ET / FT of EVERY cluster, element by element against oracle.coboundary (batches of 64, capacities
+        rows_cap / star sizes / slot bounds as create derives them at this size);
+      * FE / TE / TF of every row against the oracle's sorted lists E and F: entry j of a row must be the id of the row's
+        j-th vertex combination in lexicographic order, i.e. list[id] == that combination (ids are unique per
+        combination, so this fixes every entry).
+    Config 5 (99.5 M tets): the closed forms sum |ET| = 6 T, sum |FT| = 4 T, sum |EF| = 3 F over a complete pass."""
+    import itertools
+
+    import paper_2507_15230_b200 as gale
+
+    m = meshgen.make_config(3)
+    nV, T, off = m.num_vertices, m.simplices, m.cluster_offsets
+    gm = gale.GaleMesh(3, nV, T, off, max_batch_clusters=BATCH, device_ring=2,
+                       flags=gale.WITH_EDGES | gale.WITH_FACETS | gale.WITH_COBOUNDARY)
+    E = oracle.sub_simplices(3, nV, T, 2)
+    F = oracle.sub_simplices(3, nV, T, 3)
+    # boundary look-ups, every row
+    for rel, rows, lst, width in ((gale.BND_TE, T, E["list"], 2), (gale.BND_TF, T, F["list"], 3), (gale.BND_FE, F["list"], E["list"], 2)):
+        got = gm.boundary(rel, 0, len(rows)).cpu().numpy()
+        combos = list(itertools.combinations(range(rows.shape[1]), width))
+        assert got.shape == (len(rows), len(combos))
+        assert got.min() >= 0 and got.max() < len(lst)
+        for j, c in enumerate(combos):
+            assert np.array_equal(lst[got[:, j]], rows[:, list(c)]), f"boundary relation {rel}, entry {j}"
+        del got
+    first = {"ef": E["first"], "et": E["first"], "ft": F["first"]}
+    for name, bit in (("et", gale.REL_ET), ("ft", gale.REL_FT), ("ef", gale.REL_EF)):   # one oracle relation in memory at a time
+        r_off, r_idx = oracle.coboundary(3, nV, T, name.upper())
+        for b in range(0, m.num_clusters, BATCH):
+            ids = list(range(b, min(m.num_clusters, b + BATCH)))
+            for g in gale.split_batch(gm.run_batch(ids, bit), 4):
+                c = g["cluster"]
+                r0, r1 = int(first[name][off[c]]), int(first[name][off[c + 1]])
+                o = r_off[r0:r1 + 1]
+                assert np.array_equal(g[name][0], (o - o[0]).astype(np.int32)), f"{name} offsets of cluster {c}"
+                assert np.array_equal(g[name][1], r_idx[o[0]:o[-1]]), f"{name} of cluster {c}"
+        del r_off, r_idx
+    gm.destroy()
+    del E, F, m, T
+
+    m = meshgen.make_config(5)
+    mm = GRID_N[5] - 1
+    nT, nF_cf = 6 * mm ** 3, 12 * mm ** 3 + 6 * mm * mm
+    gm = gale.GaleMesh(3, m.num_vertices, m.simplices, m.cluster_offsets, max_batch_clusters=BATCH, device_ring=2,
+                       flags=gale.WITH_EDGES | gale.WITH_FACETS | gale.WITH_COBOUNDARY)
+    assert gm.info.num_triangles == nF_cf
+    tot = dict(et=0, ft=0, ef=0)
+    for b in range(0, m.num_clusters, BATCH):
+        ids = np.arange(b, min(m.num_clusters, b + BATCH), dtype=np.int32)
+        assert gm.compute(ids, gale.REL_ET | gale.REL_FT | gale.REL_EF) == gale.OK
+        st, v = gm.pop(-1)
+        assert st == gale.OK
+        tot["et"] += int(v.et_nnz); tot["ft"] += int(v.ft_nnz); tot["ef"] += int(v.ef_nnz)
+        a = gm.view_arrays(v)
+        for k in ("et", "ft", "ef"):
+            o = a[k + "_offsets"]
+            assert int(o[0]) == 0 and int(o[-1]) == a[k + "_indices"].numel() == int(getattr(v, k + "_nnz"))
+            assert bool((o[1:] > o[:-1]).all())                       # every edge / triangle has a coface
+        assert int(a["ft_indices"].max()) < nT and int(a["ef_indices"].max()) < nF_cf
+        gm.release(v)
+    assert tot["et"] == 6 * nT and tot["ft"] == 4 * nT and tot["ef"] == 3 * nF_cf
     gm.destroy()
